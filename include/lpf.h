@@ -1,0 +1,200 @@
+/* lpf.h -- C-ABI of the B200-native LPF hot path ("Live Pulse Finder").
+ *
+ * The per-time-step source-detection and flux-measurement stage of Ruhe et al.,
+ * arXiv 2103.15418, over a streaming image cube X_t in R^{B x D x D}:
+ *
+ *   lpf_cube_qc        quality control            App. A, eq. A.1
+ *   lpf_detect_sources peak detection/localisation  eqs. 2-7
+ *                      + cross-frequency duplicate filter
+ *   lpf_associate      match to the t-1 catalogue, monitoring
+ *   lpf_measure_flux   max pixel in a box, all frequencies
+ *   lpf_append_dynspec dynamic spectra (frequency x time)           (Fig. 1 :23)
+ *
+ * Conventions
+ *   - Every pointer named d_* is DEVICE memory (sm_100a, one GPU); h_* is HOST
+ *     memory.  The caller owns the cube and every output buffer; the context owns
+ *     its scratch (one set per lane), the candidate table, the slot map and the
+ *     rings.  The cube is never written (a rejected band is expressed by band_ok).
+ *   - `stream` is a cudaStream_t passed as void*.  Every call only enqueues work
+ *     on it; counts live in device memory; nothing on the hot path synchronises
+ *     with the host (lpf_create, lpf_destroy, lpf_get_counters and the *_host
+ *     entry point do).
+ *   - Layout: cube [B][Dy][Dx] float32, x fastest; pix = y*Dx + x; plane p < B is
+ *     band p, plane B is the sum over accepted bands.
+ *   - lpf_associate / lpf_append_dynspec must be issued in increasing t.  A lane
+ *     (0 <= lane < n_lanes) is a set of scratch buffers; two frames in flight at
+ *     the same time must use different lanes (BASELINE.json config 4: 4 lanes).
+ *   - Return value: 0 = LPF_OK; negative = error (nothing was enqueued).
+ *     Capacity overflow (max_det, n_cand_max) is not undefined behaviour: the list
+ *     is truncated and a device counter is incremented (lpf_get_counters).
+ *   - There is no CPU fallback: without a CUDA device lpf_create returns
+ *     LPF_E_CUDA.
+ *
+ * Definitions O1..O10 and readings R1..R24 referenced below are in DESIGN.md.
+ */
+#ifndef LPF_H_
+#define LPF_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LPF_OK 0
+#define LPF_E_ARG (-1)   /* bad argument / unsupported parameter value */
+#define LPF_E_CUDA (-2)  /* a CUDA runtime call failed (see lpf_last_cuda_error) */
+#define LPF_E_STATE (-3) /* call order / lane misuse */
+#define LPF_E_NOMEM (-4)
+
+#define LPF_MAX_BANDS 64  /* band_ok bits are kept in one 64-bit word per time step */
+#define LPF_MAX_RADIUS 16 /* k_mf, k_bg <= 16 ; k_max, r_flux, r_dedupe, r_assoc <= 8 */
+#define LPF_STATS_PER_BAND 8
+
+typedef struct lpf_ctx lpf_ctx; /* opaque */
+
+/* Plain-old-data parameter block, copied at lpf_create. */
+typedef struct {
+  int32_t B, Dy, Dx;        /* cube shape; 1 <= B <= 64 */
+  float kappa;              /* eq. 5 threshold */
+  int32_t k_max;            /* eq. 6 max-filter half width (window 2k+1) */
+  float eps_rel;            /* rounding guard S_eff = max(S, (eps_rel |C|)^2) (R8); 1e-5 */
+  float sigma_mf;           /* matched-filter Gaussian sigma [px]; <= 0: F = X (paper-literal) */
+  int32_t k_mf;             /* matched-filter half width */
+  int32_t bg_kernel;        /* background kernel G of eqs. 3-4: 0 = Gaussian (eq. 2), 1 = uniform box */
+  float s_bg;               /* Gaussian s of eq. 2 (ignored for the box) */
+  int32_t k_bg;             /* half width of G */
+  int32_t n_iter;           /* sigma-clip iterations, >= 1 */
+  int32_t detect_sum_plane; /* also run eqs. 2-7 on the channel-summed plane (north_star; R5) */
+  float qc_tau;             /* eq. A.1 threshold, "e.g. 5" */
+  float qc_clip;            /* sigma of the one clip round behind the clipped mean/rms (R13) */
+  int32_t r_flux;           /* flux box half width (R15) */
+  int32_t r_dedupe;         /* duplicate-filter radius [px] (R17) */
+  int32_t r_assoc;          /* association radius [px] (R16) */
+  int32_t n_forget;         /* retire after this many accepted frames without a detection */
+  int32_t T_ring;           /* dynamic-spectrum ring length [time steps] */
+  int32_t n_cand_max;       /* candidate-table capacity */
+  int32_t max_det;          /* capacity of the per-plane record list, per frame */
+  int32_t n_lanes;          /* frames in flight */
+} lpf_params;
+
+/* One peak (eq. 7: p = q and y) of one plane.  24 bytes. */
+typedef struct {
+  int32_t pix;   /* y*Dx + x */
+  int16_t plane; /* 0..B-1 band, B = sum plane */
+  int16_t iter;  /* sigma-clip iteration of first detection, 1-based */
+  float f;       /* matched-filtered value F at the peak */
+  float c;       /* local centre C (eq. 3) at first detection */
+  float s;       /* local spread S_eff (eq. 4 + guard R8) at first detection */
+  float snr;     /* (F - C) / sqrt(S_eff) */
+} lpf_det;
+
+/* Device-side views of what lpf_process_frame left in a lane (valid until the lane is reused). */
+typedef struct {
+  const float* d_stats;      /* [B][8] n, mean, rms, n_clip, clipped mean, clipped rms, z_mean, z_rms */
+  const uint8_t* d_band_ok;  /* [B+1], last = frame_ok */
+  const lpf_det* d_dets;     /* [<= max_det] unordered */
+  const int32_t* d_ndets;    /* [1] number of records found (may exceed max_det: truncated) */
+  const int32_t* d_upos;     /* unique detections, ascending pix */
+  const int16_t* d_uplane;   /* plane of the largest snr at that pixel */
+  const float* d_usnr;       /* that snr */
+  const int32_t* d_nu;       /* [1] */
+  const int32_t* d_cand_idx; /* [nu] candidate slot of each unique detection (-1: dropped / rejected frame) */
+  const int32_t* d_act_slots;/* [npos] active slots after this frame, ascending */
+  const int32_t* d_act_pix;  /* [npos] their pixels */
+  const int32_t* d_npos;     /* [1] */
+  const float* d_flux;       /* [npos][B] */
+} lpf_frame_view;
+
+/* Host-side result sizes / pointers for lpf_process_frame_host (all HOST memory, caller-owned). */
+typedef struct {
+  float* h_stats;        /* [B][8] */
+  uint8_t* h_band_ok;    /* [B+1] */
+  int32_t* h_upos;       /* [cap_u] */
+  int16_t* h_uplane;     /* [cap_u] */
+  float* h_usnr;         /* [cap_u] */
+  int32_t* h_cand_idx;   /* [cap_u] */
+  int32_t cap_u;         /* capacity of the four arrays above */
+  int32_t* h_act_slots;  /* [cap_pos] */
+  float* h_flux;         /* [cap_pos][B] */
+  int32_t cap_pos;
+  int32_t nu, npos, ndets; /* written by the call */
+} lpf_host_result;
+
+/* -- life cycle ------------------------------------------------------------ */
+/* d_valid_mask: device uint8 [Dy][Dx] (1 = valid pixel W, R7/R14) or NULL (all valid); copied.
+ * Synchronises.  Precomputes the static normalised-convolution denominators (R7). */
+int lpf_create(lpf_ctx** out, const lpf_params* p, const uint8_t* d_valid_mask);
+int lpf_destroy(lpf_ctx* ctx);
+
+/* -- S1+S2: quality control (App. A; O1, O2) --------------------------------
+ * d_stats [B][8] float32, d_band_ok [B+1] uint8 (band_ok[B] = frame_ok).
+ * Per band over valid pixels: n, mean b (the paper's b), rms, and after one
+ * qc_clip-sigma clip round n_clip, clipped mean, clipped rms; then eq. A.1 z-scores of the mean
+ * and of the rms across bands (median / median-absolute-deviation, SE floor; R10-R13);
+ * band_ok = |z_mean| <= tau and |z_rms| <= tau; frame_ok = #ok >= ceil(B/2). */
+int lpf_cube_qc(lpf_ctx* ctx, int lane, const float* d_cube, int64_t t, float* d_stats,
+                uint8_t* d_band_ok, void* stream);
+
+/* -- S3-S9: detection (eqs. 2-7; O3-O7) -------------------------------------
+ * For every accepted plane: F = g_mf (*)_W X; n_iter rounds of C = G (*)_W' F,
+ * S = G (*)_W' (F-C)^2, y = [F-C > 0 and (F-C)^2 > kappa^2 S_eff]; q = local max of F over the
+ * (2 k_max+1)^2 window; p = q and y.  Records (unordered) go to d_dets / d_ndets; then the
+ * cross-plane duplicate filter writes the unique positions sorted by pix.
+ * Capacities: d_dets [max_det]; d_upos/d_uplane/d_usnr [max_det].
+ * A rejected frame (band_ok[B] = 0) yields ndets = nu = 0. */
+int lpf_detect_sources(lpf_ctx* ctx, int lane, const float* d_cube, const uint8_t* d_band_ok,
+                       lpf_det* d_dets, int32_t* d_ndets, int32_t* d_upos, int16_t* d_uplane,
+                       float* d_usnr, int32_t* d_nu, void* stream);
+
+/* -- S10: association + monitoring (O8) -----------------------
+ * d_cand_idx [nu]; d_act_slots / d_act_pix [n_cand_max]; d_npos [1]. */
+int lpf_associate(lpf_ctx* ctx, int lane, const int32_t* d_upos, const int32_t* d_nu,
+                  const uint8_t* d_band_ok, int64_t t, int32_t* d_cand_idx, int32_t* d_act_slots,
+                  int32_t* d_act_pix, int32_t* d_npos, void* stream);
+
+/* Pre-load n forced positions (monitored for ever, BASELINE.json config 5) into the lowest free
+ * slots; d_slots_out [n] (may be NULL).  Synchronises.  Returns LPF_E_STATE if the table is full. */
+int lpf_add_candidates(lpf_ctx* ctx, const int32_t* d_pix, int32_t n, int32_t* d_slots_out, void* stream);
+
+/* -- S11: forced peak flux (O9) --------------------------------
+ * d_flux [npos][B] = max of the raw cube over the (2 r_flux+1)^2 box, valid in-image pixels;
+ * rejected band or frame -> 0.  d_pos is any pixel list (normally d_act_pix). */
+int lpf_measure_flux(lpf_ctx* ctx, const float* d_cube, const uint8_t* d_band_ok, const int32_t* d_pos,
+                     const int32_t* d_npos, float* d_flux, void* stream);
+
+/* -- S12: ring append (O10) ------------------------------------
+ * ring[slot][t mod T_ring][b] = flux; a slot born at t is pre-filled with NaN first. */
+int lpf_append_dynspec(lpf_ctx* ctx, const int32_t* d_slots, const int32_t* d_n, const float* d_flux,
+                       const uint8_t* d_band_ok, int64_t t, void* stream);
+
+/* d_out [B][T_ring], time ordered oldest -> newest, ending at t_last (frequency x time, Fig. 1). */
+int lpf_get_dynspec(lpf_ctx* ctx, int32_t slot, int64_t t_last, float* d_out, void* stream);
+
+/* -- whole step --------------------------------------------------------------
+ * qc -> detect -> associate -> flux -> append for one cube on one lane, results in lane-owned
+ * buffers (lpf_frame_view).  Frames on different lanes/streams overlap; the association chain is
+ * ordered across lanes with an event.  Issue in increasing t. */
+int lpf_process_frame(lpf_ctx* ctx, int lane, const float* d_cube, int64_t t, void* stream);
+int lpf_get_frame_view(lpf_ctx* ctx, int lane, lpf_frame_view* out);
+
+/* Same step from HOST memory: copies h_cube (pinned for full speed) to the lane's device cube
+ * buffer, runs the chain, copies the results back into `res`.  Synchronises `stream`. */
+int lpf_process_frame_host(lpf_ctx* ctx, int lane, const float* h_cube, int64_t t, lpf_host_result* res,
+                           void* stream);
+
+/* h_out[0] = records dropped (max_det), h_out[1] = detections dropped (n_cand_max full),
+ * h_out[2] = kernels launched by this context so far, h_out[3] = active candidates.  Synchronises. */
+int lpf_get_counters(lpf_ctx* ctx, int64_t* h_out);
+
+/* Convenience for bindings: synchronous copy of `bytes` from device to host memory. */
+int lpf_memcpy_d2h(void* h_dst, const void* d_src, int64_t bytes);
+
+const char* lpf_strerror(int code);
+const char* lpf_last_cuda_error(void);
+int lpf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LPF_H_ */

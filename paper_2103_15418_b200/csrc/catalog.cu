@@ -1,0 +1,408 @@
+// S9-S12: duplicate filter, association + monitoring, forced flux, dynamic-spectrum rings.
+// (O7-O10.)  All integer / compare work: results are exact.
+#include <math_constants.h>
+
+#include "lpf_internal.cuh"
+
+namespace {
+
+constexpr int CAT_BLOCKS = 64, CAT_THREADS = 256;
+
+// key: larger snr wins, equal snr -> lower plane wins.  snr > 0 so its bit pattern is monotone.
+__device__ __forceinline__ unsigned long long dd_key(float snr, int plane) {
+  return ((unsigned long long)__float_as_uint(snr) << 32) | (unsigned)(0x7fff - plane);
+}
+
+__global__ void __launch_bounds__(CAT_THREADS)
+k_dedupe_scatter(const lpf_det* __restrict__ dets, const int32_t* __restrict__ ndets, int max_det,
+                 unsigned long long* __restrict__ M, int32_t* __restrict__ tmp_n) {
+  const int n = min(*ndets, max_det);
+  if (blockIdx.x == 0 && threadIdx.x == 0) *tmp_n = 0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+    atomicMax(&M[dets[i].pix], dd_key(dets[i].snr, dets[i].plane));
+}
+
+__global__ void __launch_bounds__(CAT_THREADS)
+k_dedupe_select(const lpf_det* __restrict__ dets, const int32_t* __restrict__ ndets, int max_det,
+                const unsigned long long* __restrict__ M, int Dy, int Dx, int r,
+                int32_t* __restrict__ tmp_pos, int16_t* __restrict__ tmp_plane, float* __restrict__ tmp_snr,
+                int32_t* __restrict__ tmp_n) {
+  const int n = min(*ndets, max_det);
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const lpf_det d = dets[i];
+    const unsigned long long key = dd_key(d.snr, d.plane);
+    if (M[d.pix] != key) continue;  // not the best plane at this pixel
+    const int y = d.pix / Dx, x = d.pix - y * Dx;
+    bool keep = true;
+    for (int j = -r; j <= r && keep; ++j) {
+      const int yy = y + j;
+      if (yy < 0 || yy >= Dy) continue;
+      for (int k = -r; k <= r; ++k) {
+        const int xx = x + k;
+        if (xx < 0 || xx >= Dx || (j == 0 && k == 0) || j * j + k * k > r * r) continue;
+        const int q = yy * Dx + xx;
+        const unsigned long long kq = M[q];
+        if (!kq) continue;
+        const unsigned sq = (unsigned)(kq >> 32), si = (unsigned)(key >> 32);
+        if (sq > si || (sq == si && q < d.pix)) { keep = false; break; }
+      }
+    }
+    if (keep) {
+      const int o = atomicAdd(tmp_n, 1);
+      tmp_pos[o] = d.pix; tmp_plane[o] = d.plane; tmp_snr[o] = d.snr;
+    }
+  }
+}
+
+// rank sort by pixel (pixels are distinct) + reset of the touched map entries
+__global__ void __launch_bounds__(CAT_THREADS)
+k_dedupe_sort(const lpf_det* __restrict__ dets, const int32_t* __restrict__ ndets, int max_det,
+              unsigned long long* __restrict__ M, const int32_t* __restrict__ tmp_pos,
+              const int16_t* __restrict__ tmp_plane, const float* __restrict__ tmp_snr,
+              const int32_t* __restrict__ tmp_n, int32_t* __restrict__ upos, int16_t* __restrict__ uplane,
+              float* __restrict__ usnr, int32_t* __restrict__ nu) {
+  const int n = min(*ndets, max_det);
+  const int m = *tmp_n;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < m; i += gridDim.x * blockDim.x) {
+    const int mine = tmp_pos[i];
+    int rank = 0;
+    for (int j = 0; j < m; ++j) rank += (tmp_pos[j] < mine);
+    upos[rank] = mine; uplane[rank] = tmp_plane[i]; usnr[rank] = tmp_snr[i];
+  }
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) M[dets[i].pix] = 0ull;
+  if (blockIdx.x == 0 && threadIdx.x == 0) *nu = m;
+}
+
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(CAT_THREADS)
+k_assoc_match(const int32_t* __restrict__ upos, const int32_t* __restrict__ nu, const uint8_t* __restrict__ band_ok,
+              int B, const int32_t* __restrict__ slotmap, const int32_t* __restrict__ cpix, int Dy, int Dx, int r,
+              long long t, long long* __restrict__ matched_t, int32_t* __restrict__ cand_idx) {
+  const int n = *nu;
+  const bool frame_ok = band_ok[B] != 0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    int best = -1;
+    if (frame_ok) {
+      const int pix = upos[i];
+      const int y = pix / Dx, x = pix - y * Dx;
+      int best_d = 0x7fffffff;
+      for (int j = -r; j <= r; ++j) {
+        const int yy = y + j;
+        if (yy < 0 || yy >= Dy) continue;
+        for (int k = -r; k <= r; ++k) {
+          const int xx = x + k;
+          const int d2 = j * j + k * k;
+          if (xx < 0 || xx >= Dx || d2 > r * r) continue;
+          const int s = slotmap[yy * Dx + xx];
+          if (s < 0) continue;
+          if (d2 < best_d || (d2 == best_d && s < best)) { best_d = d2; best = s; }
+        }
+      }
+      if (best >= 0) matched_t[best] = t;
+    }
+    cand_idx[i] = best;
+  }
+}
+
+// exclusive block scan of one int per thread (1024 threads)
+__device__ __forceinline__ int block_excl_scan(int v, int* s_warp /*[33]*/, int& total) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  int inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int u = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += u; }
+  __syncthreads();
+  if (lane == 31) s_warp[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    int x = lane < (int)(blockDim.x >> 5) ? s_warp[lane] : 0;
+    int xi = x;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int u = __shfl_up_sync(0xffffffffu, xi, o); if (lane >= o) xi += u; }
+    s_warp[lane] = xi - x;
+    if (lane == 31) s_warp[32] = xi;
+  }
+  __syncthreads();
+  total = s_warp[32];
+  return s_warp[w] + inc - v;
+}
+
+struct AssocArgs {
+  uint8_t* active; uint8_t* forced; int32_t* cpix; int32_t* miss; long long* born; const long long* matched_t;
+  int32_t* slotmap; int32_t* free_list; int n_cand_max, n_forget;
+  const int32_t* upos; const int32_t* nu; const uint8_t* band_ok; int B; long long t;
+  int32_t* cand_idx; int32_t* act_slots; int32_t* act_pix; int32_t* npos; int32_t* counters;
+};
+
+// Single block: age / retire, rebuild the slot map around retired pixels, hand the lowest free
+// slots to the unmatched detections in ascending pix, compact the active list.
+__global__ void __launch_bounds__(1024)
+k_assoc_update(const AssocArgs a) {
+  __shared__ int s_warp[33];
+  const int T = blockDim.x;
+  const int tid = threadIdx.x;
+  const bool frame_ok = a.band_ok[a.B] != 0;
+  const int per = (a.n_cand_max + T - 1) / T;
+  const int s0 = tid * per, s1 = min(s0 + per, a.n_cand_max);
+  if (frame_ok) {
+    // 1. age and retire
+    for (int s = s0; s < s1; ++s) {
+      if (!a.active[s]) continue;
+      if (a.matched_t[s] == a.t) a.miss[s] = 0;
+      else {
+        const int m = a.miss[s] + 1;
+        a.miss[s] = m;
+        if (!a.forced[s] && m >= a.n_forget) { a.active[s] = 0; a.slotmap[a.cpix[s]] = -1; }
+      }
+    }
+    __syncthreads();
+    // 2. another (forced) candidate may share a retired pixel: restore the lowest active slot there
+    for (int s = s0; s < s1; ++s)
+      if (a.active[s]) atomicMin(reinterpret_cast<unsigned*>(&a.slotmap[a.cpix[s]]), (unsigned)s);
+    // 3. free list (ascending)
+    int nfree_mine = 0;
+    for (int s = s0; s < s1; ++s) nfree_mine += a.active[s] ? 0 : 1;
+    int n_free;
+    int off = block_excl_scan(nfree_mine, s_warp, n_free);
+    for (int s = s0; s < s1; ++s) if (!a.active[s]) a.free_list[off++] = s;
+    __syncthreads();
+    // 4. unmatched detections, ascending pix (upos is sorted)
+    const int nu = *a.nu;
+    const int peru = (nu + T - 1) / T;
+    const int u0 = min(tid * peru, nu), u1 = min(u0 + peru, nu);
+    int nun_mine = 0;
+    for (int i = u0; i < u1; ++i) nun_mine += (a.cand_idx[i] < 0);
+    int n_un;
+    int uo = block_excl_scan(nun_mine, s_warp, n_un);
+    for (int i = u0; i < u1; ++i) {
+      if (a.cand_idx[i] >= 0) continue;
+      const int k = uo++;
+      if (k < n_free) {
+        const int s = a.free_list[k];
+        const int pix = a.upos[i];
+        a.active[s] = 1; a.forced[s] = 0; a.cpix[s] = pix; a.miss[s] = 0; a.born[s] = a.t;
+        atomicMin(reinterpret_cast<unsigned*>(&a.slotmap[pix]), (unsigned)s);
+        a.cand_idx[i] = s;
+      } else {
+        atomicAdd(&a.counters[1], 1);
+      }
+    }
+    __syncthreads();
+  }
+  // 5. active list, ascending slot
+  int na_mine = 0;
+  for (int s = s0; s < s1; ++s) na_mine += a.active[s] ? 1 : 0;
+  int n_act;
+  int ao = block_excl_scan(na_mine, s_warp, n_act);
+  for (int s = s0; s < s1; ++s)
+    if (a.active[s]) { a.act_slots[ao] = s; a.act_pix[ao] = a.cpix[s]; ++ao; }
+  if (tid == 0) { *a.npos = n_act; a.counters[2] = n_act; }
+}
+
+struct AddArgs {
+  uint8_t* active; uint8_t* forced; int32_t* cpix; int32_t* miss; long long* born; int32_t* slotmap;
+  int32_t* free_list; int n_cand_max; const int32_t* pix; int n; int32_t* slots_out; int32_t* status;
+};
+
+__global__ void __launch_bounds__(1024)
+k_add_candidates(const AddArgs a) {
+  __shared__ int s_warp[33];
+  const int T = blockDim.x, tid = threadIdx.x;
+  const int per = (a.n_cand_max + T - 1) / T;
+  const int s0 = tid * per, s1 = min(s0 + per, a.n_cand_max);
+  int nfree_mine = 0;
+  for (int s = s0; s < s1; ++s) nfree_mine += a.active[s] ? 0 : 1;
+  int n_free;
+  int off = block_excl_scan(nfree_mine, s_warp, n_free);
+  for (int s = s0; s < s1; ++s) if (!a.active[s]) a.free_list[off++] = s;
+  __syncthreads();
+  if (n_free < a.n) { if (tid == 0) *a.status = 1; return; }
+  for (int i = tid; i < a.n; i += T) {
+    const int s = a.free_list[i];
+    a.active[s] = 1; a.forced[s] = 1; a.cpix[s] = a.pix[i]; a.miss[s] = 0; a.born[s] = -1;
+    atomicMin(reinterpret_cast<unsigned*>(&a.slotmap[a.pix[i]]), (unsigned)s);
+    if (a.slots_out) a.slots_out[i] = s;
+  }
+  if (tid == 0) *a.status = 0;
+}
+
+// NaN rows for freshly added forced slots (slots_out list)
+__global__ void __launch_bounds__(256)
+k_ring_nan_slots(float* __restrict__ ring, const int32_t* __restrict__ free_list, int n, long long per_slot) {
+  for (int i = blockIdx.y; i < n; i += gridDim.y) {
+    float* r = ring + (long long)free_list[i] * per_slot;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < per_slot; q += (long long)gridDim.x * blockDim.x)
+      r[q] = CUDART_NAN_F;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_measure_flux(const float* __restrict__ cube, const uint8_t* __restrict__ band_ok, const uint8_t* __restrict__ W,
+               int B, int Dy, int Dx, int r, const int32_t* __restrict__ pos, const int32_t* __restrict__ npos,
+               float* __restrict__ flux) {
+  const long long N = (long long)Dy * Dx;
+  const long long total = (long long)(*npos) * B;
+  const bool frame_ok = band_ok[B] != 0;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+    const int ip = (int)(i / B), b = (int)(i - (long long)ip * B);
+    float best = 0.f;
+    if (frame_ok && band_ok[b]) {
+      const int pix = pos[ip];
+      const int y = pix / Dx, x = pix - y * Dx;
+      const float* X = cube + (long long)b * N;
+      bool any = false;
+      for (int j = -r; j <= r; ++j) {
+        const int yy = y + j;
+        if (yy < 0 || yy >= Dy) continue;
+        for (int k = -r; k <= r; ++k) {
+          const int xx = x + k;
+          if (xx < 0 || xx >= Dx) continue;
+          const long long q = (long long)yy * Dx + xx;
+          if (!W[q]) continue;
+          const float v = __ldg(X + q);
+          if (!any || v > best) { best = v; any = true; }
+        }
+      }
+      if (!any) best = 0.f;
+    }
+    flux[i] = best;
+  }
+}
+
+// one warp per position: NaN prefill of a slot born at t, then this step's column
+__global__ void __launch_bounds__(256)
+k_append(float* __restrict__ ring, long long* __restrict__ meta_t, unsigned long long* __restrict__ meta_ok,
+         const long long* __restrict__ born, int T_ring, int B, const int32_t* __restrict__ slots,
+         const int32_t* __restrict__ n, const float* __restrict__ flux, const uint8_t* __restrict__ band_ok, long long t) {
+  const int tau = (int)(t % T_ring);
+  const int lane = threadIdx.x & 31;
+  const int wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+  const int cnt = *n;
+  for (int i = wid; i < cnt; i += nw) {
+    const int s = slots[i];
+    float* r = ring + (long long)s * T_ring * B;
+    if (born[s] == t) {
+      for (int q = lane; q < T_ring * B; q += 32) r[q] = CUDART_NAN_F;
+      __syncwarp();
+    }
+    for (int b = lane; b < B; b += 32) r[(long long)tau * B + b] = flux[(long long)i * B + b];
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    meta_t[tau] = t;
+    unsigned long long bits = 0;
+    if (band_ok[B]) for (int b = 0; b < B; ++b) if (band_ok[b]) bits |= (1ull << b);
+    meta_ok[tau] = bits;
+  }
+}
+
+__global__ void __launch_bounds__(256)
+k_get_dynspec(const float* __restrict__ ring, const long long* __restrict__ meta_t, int T_ring, int B, int slot,
+              long long t_last, float* __restrict__ out) {
+  const float* r = ring + (long long)slot * T_ring * B;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < B * T_ring; i += gridDim.x * blockDim.x) {
+    const int b = i / T_ring, j = i - b * T_ring;
+    const long long tt = t_last - T_ring + 1 + j;
+    const int tau = (int)(((tt % T_ring) + T_ring) % T_ring);
+    const bool have = tt >= 0 && meta_t[tau] == tt;
+    out[i] = have ? r[(long long)tau * B + b] : CUDART_NAN_F;
+  }
+}
+
+__global__ void k_fill_f32(float* p, long long n, float v) {
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) p[i] = v;
+}
+__global__ void k_fill_i32(int32_t* p, long long n, int32_t v) {
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) p[i] = v;
+}
+
+}  // namespace
+
+int lpf_launch_dedupe(lpf_ctx* c, LpfLane& L, const lpf_det* d_dets, const int32_t* d_ndets, int32_t* d_upos,
+                      int16_t* d_uplane, float* d_usnr, int32_t* d_nu, cudaStream_t st) {
+  const lpf_params& p = c->p;
+  k_dedupe_scatter<<<CAT_BLOCKS, CAT_THREADS, 0, st>>>(d_dets, d_ndets, p.max_det, L.M, L.tmp_n);
+  LPF_LAUNCH_CHECK(c);
+  k_dedupe_select<<<CAT_BLOCKS, CAT_THREADS, 0, st>>>(d_dets, d_ndets, p.max_det, L.M, p.Dy, p.Dx, p.r_dedupe,
+                                                       L.tmp_pos, L.tmp_plane, L.tmp_snr, L.tmp_n);
+  LPF_LAUNCH_CHECK(c);
+  k_dedupe_sort<<<CAT_BLOCKS, CAT_THREADS, 0, st>>>(d_dets, d_ndets, p.max_det, L.M, L.tmp_pos, L.tmp_plane, L.tmp_snr,
+                                                     L.tmp_n, d_upos, d_uplane, d_usnr, d_nu);
+  LPF_LAUNCH_CHECK(c);
+  return LPF_OK;
+}
+
+int lpf_launch_associate(lpf_ctx* c, const int32_t* d_upos, const int32_t* d_nu, const uint8_t* d_band_ok,
+                         long long t, int32_t* d_cand_idx, int32_t* d_act_slots, int32_t* d_act_pix,
+                         int32_t* d_npos, cudaStream_t st) {
+  const lpf_params& p = c->p;
+  k_assoc_match<<<CAT_BLOCKS, CAT_THREADS, 0, st>>>(d_upos, d_nu, d_band_ok, p.B, c->slotmap, c->cpix, p.Dy, p.Dx,
+                                                     p.r_assoc, t, c->matched_t, d_cand_idx);
+  LPF_LAUNCH_CHECK(c);
+  AssocArgs a{};
+  a.active = c->active; a.forced = c->forced; a.cpix = c->cpix; a.miss = c->miss; a.born = c->born;
+  a.matched_t = c->matched_t; a.slotmap = c->slotmap; a.free_list = c->free_list;
+  a.n_cand_max = p.n_cand_max; a.n_forget = p.n_forget;
+  a.upos = d_upos; a.nu = d_nu; a.band_ok = d_band_ok; a.B = p.B; a.t = t;
+  a.cand_idx = d_cand_idx; a.act_slots = d_act_slots; a.act_pix = d_act_pix; a.npos = d_npos; a.counters = c->counters;
+  k_assoc_update<<<1, 1024, 0, st>>>(a);
+  LPF_LAUNCH_CHECK(c);
+  return LPF_OK;
+}
+
+int lpf_launch_add_candidates(lpf_ctx* c, const int32_t* d_pix, int n, int32_t* d_slots_out, cudaStream_t st) {
+  const lpf_params& p = c->p;
+  int32_t* d_status = c->counters + 3;
+  AddArgs a{};
+  a.active = c->active; a.forced = c->forced; a.cpix = c->cpix; a.miss = c->miss; a.born = c->born;
+  a.slotmap = c->slotmap; a.free_list = c->free_list; a.n_cand_max = p.n_cand_max;
+  a.pix = d_pix; a.n = n; a.slots_out = d_slots_out; a.status = d_status;
+  k_add_candidates<<<1, 1024, 0, st>>>(a);
+  LPF_LAUNCH_CHECK(c);
+  int32_t status = -1;
+  LPF_CUDA(cudaMemcpyAsync(&status, d_status, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  LPF_CUDA(cudaStreamSynchronize(st));
+  if (status != 0) return LPF_E_STATE;
+  if (n > 0) {
+    const long long per_slot = (long long)p.T_ring * p.B;
+    const long long gx = (per_slot + 255) / 256;
+    const dim3 grid((unsigned)(gx < 64 ? gx : 64), (unsigned)(n < 4096 ? n : 4096));
+    k_ring_nan_slots<<<grid, 256, 0, st>>>(c->ring, c->free_list, n, per_slot);
+    LPF_LAUNCH_CHECK(c);
+    LPF_CUDA(cudaStreamSynchronize(st));
+  }
+  return LPF_OK;
+}
+
+int lpf_launch_measure_flux(lpf_ctx* c, const float* d_cube, const uint8_t* d_band_ok, const int32_t* d_pos,
+                            const int32_t* d_npos, float* d_flux, cudaStream_t st) {
+  const lpf_params& p = c->p;
+  k_measure_flux<<<c->n_sm * 2, 256, 0, st>>>(d_cube, d_band_ok, c->W, p.B, p.Dy, p.Dx, p.r_flux, d_pos, d_npos, d_flux);
+  LPF_LAUNCH_CHECK(c);
+  return LPF_OK;
+}
+
+int lpf_launch_append(lpf_ctx* c, const int32_t* d_slots, const int32_t* d_n, const float* d_flux,
+                      const uint8_t* d_band_ok, long long t, cudaStream_t st) {
+  const lpf_params& p = c->p;
+  k_append<<<c->n_sm, 256, 0, st>>>(c->ring, c->meta_t, c->meta_ok, c->born, p.T_ring, p.B, d_slots, d_n, d_flux, d_band_ok, t);
+  LPF_LAUNCH_CHECK(c);
+  return LPF_OK;
+}
+
+int lpf_launch_get_dynspec(lpf_ctx* c, int slot, long long t_last, float* d_out, cudaStream_t st) {
+  const lpf_params& p = c->p;
+  k_get_dynspec<<<8, 256, 0, st>>>(c->ring, c->meta_t, p.T_ring, p.B, slot, t_last, d_out);
+  LPF_LAUNCH_CHECK(c);
+  return LPF_OK;
+}
+
+int lpf_launch_fill_nan(lpf_ctx* c, float* d, int64_t n, cudaStream_t st) {
+  k_fill_f32<<<c->n_sm * 4, 256, 0, st>>>(d, n, nanf(""));
+  LPF_LAUNCH_CHECK(c);
+  return LPF_OK;
+}
+int lpf_launch_fill_i32(lpf_ctx* c, int32_t* d, int64_t n, int32_t v, cudaStream_t st) {
+  k_fill_i32<<<c->n_sm * 4, 256, 0, st>>>(d, n, v);
+  LPF_LAUNCH_CHECK(c);
+  return LPF_OK;
+}

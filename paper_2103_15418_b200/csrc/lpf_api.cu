@@ -1,0 +1,336 @@
+// C-ABI entry points (include/lpf.h): argument checks, context life cycle, step chaining.
+#include <climits>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "lpf_internal.cuh"
+
+thread_local char g_lpf_cuda_err[256] = "";
+
+int lpf_cuda_fail(cudaError_t e, const char* what) {
+  snprintf(g_lpf_cuda_err, sizeof(g_lpf_cuda_err), "%s: %s", what, cudaGetErrorString(e));
+  (void)cudaGetLastError();
+  return LPF_E_CUDA;
+}
+
+namespace {
+
+// eq. 2 taps, R1: g_i = exp(-i^2 / 2 s^2) / sum ; uniform: 1/(2k+1) ; s <= 0: identity.
+void make_taps(int kind, double s, int k, LpfTaps* t) {
+  t->R = k;
+  const int n = 2 * k + 1;
+  double e[LPF_NTAPS];
+  double sum = 0;
+  for (int i = -k; i <= k; ++i) {
+    double v;
+    if (kind == 1) v = 1.0;
+    else if (s <= 0) v = (i == 0) ? 1.0 : 0.0;
+    else v = std::exp(-(double)(i * i) / (2.0 * s * s));
+    e[i + k] = v; sum += v;
+  }
+  for (int i = 0; i < LPF_NTAPS; ++i) t->g[i] = i < n ? (float)(e[i] / sum) : 0.f;
+}
+
+template <typename T>
+int dalloc(T** p, size_t n) {
+  cudaError_t e = cudaMalloc((void**)p, n * sizeof(T));
+  if (e != cudaSuccess) { lpf_cuda_fail(e, "cudaMalloc"); return LPF_E_NOMEM; }
+  return LPF_OK;
+}
+
+#define TRY(x) do { int rc__ = (x); if (rc__ != LPF_OK) return rc__; } while (0)
+
+int check_params(const lpf_params* p) {
+  if (!p) return LPF_E_ARG;
+  if (p->B < 1 || p->B > LPF_MAX_BANDS || p->Dy < 1 || p->Dx < 1) return LPF_E_ARG;
+  if ((long long)p->Dy * p->Dx > (1ll << 30)) return LPF_E_ARG;
+  if (!(p->kappa > 0) || p->k_max < 0 || p->k_max > 8) return LPF_E_ARG;
+  if (p->k_mf < 0 || p->k_mf > LPF_MAX_RADIUS || p->k_bg < 1 || p->k_bg > LPF_MAX_RADIUS) return LPF_E_ARG;
+  if (p->bg_kernel != 0 && p->bg_kernel != 1) return LPF_E_ARG;
+  if (p->bg_kernel == 0 && !(p->s_bg > 0)) return LPF_E_ARG;
+  if (p->n_iter < 1 || p->n_iter > 255) return LPF_E_ARG;
+  if (p->r_flux < 0 || p->r_flux > 8 || p->r_dedupe < 0 || p->r_dedupe > 8 || p->r_assoc < 0 || p->r_assoc > 8) return LPF_E_ARG;
+  if (p->n_forget < 1 || p->T_ring < 1 || p->n_cand_max < 1 || p->max_det < 1 || p->n_lanes < 1 || p->n_lanes > 64) return LPF_E_ARG;
+  if (!(p->eps_rel >= 0) || !(p->qc_tau > 0) || !(p->qc_clip > 0)) return LPF_E_ARG;
+  return LPF_OK;
+}
+
+int alloc_lane(lpf_ctx* c, LpfLane& L) {
+  const lpf_params& p = c->p;
+  const size_t N = (size_t)c->N, P = (size_t)p.B + 1;
+  TRY(dalloc(&L.qc_part1, (size_t)p.B * c->qc_nblk * 3));
+  TRY(dalloc(&L.qc_part2, (size_t)p.B * c->qc_nblk * 3));
+  TRY(dalloc(&L.sum_plane, N));
+  TRY(dalloc(&L.F, P * N));
+  TRY(dalloc(&L.C, P * N));
+  TRY(dalloc(&L.S, P * N));
+  if (p.n_iter > 1) { TRY(dalloc(&L.Y, P * N)); TRY(dalloc(&L.normp, P * N)); }
+  TRY(dalloc(&L.M, N));
+  LPF_CUDA(cudaMemset(L.M, 0, N * sizeof(unsigned long long)));
+  TRY(dalloc(&L.tmp_pos, (size_t)p.max_det));
+  TRY(dalloc(&L.tmp_plane, (size_t)p.max_det));
+  TRY(dalloc(&L.tmp_snr, (size_t)p.max_det));
+  TRY(dalloc(&L.tmp_n, 1));
+  TRY(dalloc(&L.stats, (size_t)p.B * LPF_STATS_PER_BAND));
+  TRY(dalloc(&L.band_ok, (size_t)p.B + 1));
+  TRY(dalloc(&L.dets, (size_t)p.max_det));
+  TRY(dalloc(&L.ndets, 1));
+  TRY(dalloc(&L.upos, (size_t)p.max_det));
+  TRY(dalloc(&L.uplane, (size_t)p.max_det));
+  TRY(dalloc(&L.usnr, (size_t)p.max_det));
+  TRY(dalloc(&L.nu, 1));
+  TRY(dalloc(&L.cand_idx, (size_t)p.max_det));
+  TRY(dalloc(&L.act_slots, (size_t)p.n_cand_max));
+  TRY(dalloc(&L.act_pix, (size_t)p.n_cand_max));
+  TRY(dalloc(&L.npos, 1));
+  TRY(dalloc(&L.flux, (size_t)p.n_cand_max * p.B));
+  LPF_CUDA(cudaMemset(L.ndets, 0, sizeof(int32_t)));
+  LPF_CUDA(cudaMemset(L.nu, 0, sizeof(int32_t)));
+  LPF_CUDA(cudaMemset(L.npos, 0, sizeof(int32_t)));
+  LPF_CUDA(cudaMallocHost((void**)&L.h_counts, 4 * sizeof(int32_t)));
+  return LPF_OK;
+}
+
+void free_lane(LpfLane& L) {
+  void* ptrs[] = {L.qc_part1, L.qc_part2, L.sum_plane, L.F, L.C, L.S, L.Y, L.normp, L.M, L.tmp_pos, L.tmp_plane,
+                  L.tmp_snr, L.tmp_n, L.stats, L.band_ok, L.dets, L.ndets, L.upos, L.uplane, L.usnr, L.nu,
+                  L.cand_idx, L.act_slots, L.act_pix, L.npos, L.flux, L.cube};
+  for (void* q : ptrs) if (q) cudaFree(q);
+  if (L.h_counts) cudaFreeHost(L.h_counts);
+  L = LpfLane();
+}
+
+int lane_ok(lpf_ctx* c, int lane) { return (c && lane >= 0 && lane < (int)c->lanes.size()) ? LPF_OK : LPF_E_ARG; }
+
+}  // namespace
+
+extern "C" {
+
+int lpf_create(lpf_ctx** out, const lpf_params* p, const uint8_t* d_valid_mask) {
+  if (!out) return LPF_E_ARG;
+  *out = nullptr;
+  TRY(check_params(p));
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return lpf_cuda_fail(cudaErrorNoDevice, "cudaGetDeviceCount");
+  lpf_ctx* c = new (std::nothrow) lpf_ctx();
+  if (!c) return LPF_E_NOMEM;
+  c->p = *p;
+  c->N = (int64_t)p->Dy * p->Dx;
+  c->n_planes = p->B + (p->detect_sum_plane ? 1 : 0);
+  {
+    long long nb = c->N / 8192;
+    c->qc_nblk = (int)(nb < 1 ? 1 : (nb > 64 ? 64 : nb));
+  }
+  int dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { delete c; return lpf_cuda_fail(cudaErrorUnknown, "cudaGetDeviceProperties"); }
+  c->n_sm = prop.multiProcessorCount;
+  make_taps(0, p->sigma_mf, p->k_mf, &c->g_mf);
+  make_taps(p->bg_kernel, p->s_bg, p->k_bg, &c->g_bg);
+
+  auto fail = [&](int rc) { lpf_destroy(c); return rc; };
+#define TRYC(x) do { int rc__ = (x); if (rc__ != LPF_OK) return fail(rc__); } while (0)
+#define CUDAC(x) do { cudaError_t e__ = (x); if (e__ != cudaSuccess) return fail(lpf_cuda_fail(e__, #x)); } while (0)
+  const size_t N = (size_t)c->N;
+  TRYC(dalloc(&c->W, N));
+  if (d_valid_mask) CUDAC(cudaMemcpy(c->W, d_valid_mask, N, cudaMemcpyDeviceToDevice));
+  else CUDAC(cudaMemset(c->W, 1, N));
+  {  // first valid pixel: pivot of the band statistics
+    std::vector<uint8_t> hW(N);
+    CUDAC(cudaMemcpy(hW.data(), c->W, N, cudaMemcpyDeviceToHost));
+    c->first_valid = 0;
+    for (size_t i = 0; i < N; ++i) if (hW[i]) { c->first_valid = (int)i; break; }
+    // normalise to {0,1}
+    bool dirty = false;
+    for (size_t i = 0; i < N; ++i) if (hW[i] > 1) { hW[i] = 1; dirty = true; }
+    if (dirty) CUDAC(cudaMemcpy(c->W, hW.data(), N, cudaMemcpyHostToDevice));
+  }
+  TRYC(dalloc(&c->norm_mf, N));
+  TRYC(dalloc(&c->norm_bg, N));
+  TRYC(lpf_launch_static_norm(c, c->g_mf, c->norm_mf, nullptr, 0));
+  TRYC(lpf_launch_static_norm(c, c->g_bg, c->norm_bg, nullptr, 0));
+
+  const size_t nc = (size_t)p->n_cand_max;
+  TRYC(dalloc(&c->active, nc)); TRYC(dalloc(&c->forced, nc)); TRYC(dalloc(&c->cpix, nc)); TRYC(dalloc(&c->miss, nc));
+  TRYC(dalloc(&c->born, nc)); TRYC(dalloc(&c->matched_t, nc)); TRYC(dalloc(&c->free_list, nc));
+  TRYC(dalloc(&c->slotmap, N));
+  TRYC(dalloc(&c->ring, nc * p->T_ring * p->B));
+  TRYC(dalloc(&c->meta_t, (size_t)p->T_ring)); TRYC(dalloc(&c->meta_ok, (size_t)p->T_ring));
+  TRYC(dalloc(&c->counters, 8));
+  CUDAC(cudaMemset(c->active, 0, nc)); CUDAC(cudaMemset(c->forced, 0, nc));
+  CUDAC(cudaMemset(c->cpix, 0, nc * 4)); CUDAC(cudaMemset(c->miss, 0, nc * 4));
+  CUDAC(cudaMemset(c->born, 0xff, nc * 8));       // -1
+  CUDAC(cudaMemset(c->matched_t, 0x80, nc * 8));  // very negative
+  CUDAC(cudaMemset(c->slotmap, 0xff, N * 4));     // -1
+  CUDAC(cudaMemset(c->meta_t, 0xff, (size_t)p->T_ring * 8));
+  CUDAC(cudaMemset(c->meta_ok, 0, (size_t)p->T_ring * 8));
+  CUDAC(cudaMemset(c->counters, 0, 8 * 4));
+  TRYC(lpf_launch_fill_nan(c, c->ring, (int64_t)(nc * p->T_ring * p->B), 0));
+  CUDAC(cudaEventCreateWithFlags(&c->chain_ev, cudaEventDisableTiming));
+  c->lanes.resize(p->n_lanes);
+  for (auto& L : c->lanes) TRYC(alloc_lane(c, L));
+  CUDAC(cudaDeviceSynchronize());
+  CUDAC(cudaGetLastError());
+#undef TRYC
+#undef CUDAC
+  *out = c;
+  return LPF_OK;
+}
+
+int lpf_destroy(lpf_ctx* c) {
+  if (!c) return LPF_E_ARG;
+  cudaDeviceSynchronize();
+  for (auto& L : c->lanes) free_lane(L);
+  void* ptrs[] = {c->W, c->norm_mf, c->norm_bg, c->active, c->forced, c->cpix, c->miss, c->born, c->matched_t,
+                  c->slotmap, c->free_list, c->ring, c->meta_t, c->meta_ok, c->counters};
+  for (void* q : ptrs) if (q) cudaFree(q);
+  if (c->chain_ev) cudaEventDestroy(c->chain_ev);
+  delete c;
+  return LPF_OK;
+}
+
+int lpf_cube_qc(lpf_ctx* c, int lane, const float* d_cube, int64_t t, float* d_stats, uint8_t* d_band_ok, void* stream) {
+  (void)t;
+  TRY(lane_ok(c, lane));
+  if (!d_cube || !d_stats || !d_band_ok) return LPF_E_ARG;
+  return lpf_launch_qc(c, c->lanes[lane], d_cube, d_stats, d_band_ok, (cudaStream_t)stream);
+}
+
+int lpf_detect_sources(lpf_ctx* c, int lane, const float* d_cube, const uint8_t* d_band_ok, lpf_det* d_dets,
+                       int32_t* d_ndets, int32_t* d_upos, int16_t* d_uplane, float* d_usnr, int32_t* d_nu, void* stream) {
+  TRY(lane_ok(c, lane));
+  if (!d_cube || !d_band_ok || !d_dets || !d_ndets || !d_upos || !d_uplane || !d_usnr || !d_nu) return LPF_E_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  LpfLane& L = c->lanes[lane];
+  TRY(lpf_launch_detect_general(c, L, d_cube, d_band_ok, d_dets, d_ndets, st));
+  return lpf_launch_dedupe(c, L, d_dets, d_ndets, d_upos, d_uplane, d_usnr, d_nu, st);
+}
+
+int lpf_associate(lpf_ctx* c, int lane, const int32_t* d_upos, const int32_t* d_nu, const uint8_t* d_band_ok, int64_t t,
+                  int32_t* d_cand_idx, int32_t* d_act_slots, int32_t* d_act_pix, int32_t* d_npos, void* stream) {
+  TRY(lane_ok(c, lane));
+  if (!d_upos || !d_nu || !d_band_ok || !d_cand_idx || !d_act_slots || !d_act_pix || !d_npos || t < 0) return LPF_E_ARG;
+  return lpf_launch_associate(c, d_upos, d_nu, d_band_ok, (long long)t, d_cand_idx, d_act_slots, d_act_pix, d_npos,
+                              (cudaStream_t)stream);
+}
+
+int lpf_add_candidates(lpf_ctx* c, const int32_t* d_pix, int32_t n, int32_t* d_slots_out, void* stream) {
+  if (!c || n < 0 || (n > 0 && !d_pix)) return LPF_E_ARG;
+  if (n == 0) return LPF_OK;
+  if (n > c->p.n_cand_max) return LPF_E_STATE;
+  return lpf_launch_add_candidates(c, d_pix, n, d_slots_out, (cudaStream_t)stream);
+}
+
+int lpf_measure_flux(lpf_ctx* c, const float* d_cube, const uint8_t* d_band_ok, const int32_t* d_pos,
+                     const int32_t* d_npos, float* d_flux, void* stream) {
+  if (!c || !d_cube || !d_band_ok || !d_pos || !d_npos || !d_flux) return LPF_E_ARG;
+  return lpf_launch_measure_flux(c, d_cube, d_band_ok, d_pos, d_npos, d_flux, (cudaStream_t)stream);
+}
+
+int lpf_append_dynspec(lpf_ctx* c, const int32_t* d_slots, const int32_t* d_n, const float* d_flux,
+                       const uint8_t* d_band_ok, int64_t t, void* stream) {
+  if (!c || !d_slots || !d_n || !d_flux || !d_band_ok || t < 0) return LPF_E_ARG;
+  return lpf_launch_append(c, d_slots, d_n, d_flux, d_band_ok, (long long)t, (cudaStream_t)stream);
+}
+
+int lpf_get_dynspec(lpf_ctx* c, int32_t slot, int64_t t_last, float* d_out, void* stream) {
+  if (!c || !d_out || slot < 0 || slot >= c->p.n_cand_max) return LPF_E_ARG;
+  return lpf_launch_get_dynspec(c, slot, (long long)t_last, d_out, (cudaStream_t)stream);
+}
+
+int lpf_process_frame(lpf_ctx* c, int lane, const float* d_cube, int64_t t, void* stream) {
+  TRY(lane_ok(c, lane));
+  if (!d_cube || t < 0) return LPF_E_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  LpfLane& L = c->lanes[lane];
+  TRY(lpf_launch_qc(c, L, d_cube, L.stats, L.band_ok, st));
+  TRY(lpf_launch_detect_general(c, L, d_cube, L.band_ok, L.dets, L.ndets, st));
+  TRY(lpf_launch_dedupe(c, L, L.dets, L.ndets, L.upos, L.uplane, L.usnr, L.nu, st));
+  // the candidate table and the rings are shared by all lanes: order the chain across streams
+  if (c->chain_valid) LPF_CUDA(cudaStreamWaitEvent(st, c->chain_ev, 0));
+  TRY(lpf_launch_associate(c, L.upos, L.nu, L.band_ok, (long long)t, L.cand_idx, L.act_slots, L.act_pix, L.npos, st));
+  TRY(lpf_launch_measure_flux(c, d_cube, L.band_ok, L.act_pix, L.npos, L.flux, st));
+  TRY(lpf_launch_append(c, L.act_slots, L.npos, L.flux, L.band_ok, (long long)t, st));
+  LPF_CUDA(cudaEventRecord(c->chain_ev, st));
+  c->chain_valid = true;
+  return LPF_OK;
+}
+
+int lpf_get_frame_view(lpf_ctx* c, int lane, lpf_frame_view* v) {
+  TRY(lane_ok(c, lane));
+  if (!v) return LPF_E_ARG;
+  const LpfLane& L = c->lanes[lane];
+  v->d_stats = L.stats; v->d_band_ok = L.band_ok; v->d_dets = L.dets; v->d_ndets = L.ndets;
+  v->d_upos = L.upos; v->d_uplane = L.uplane; v->d_usnr = L.usnr; v->d_nu = L.nu; v->d_cand_idx = L.cand_idx;
+  v->d_act_slots = L.act_slots; v->d_act_pix = L.act_pix; v->d_npos = L.npos; v->d_flux = L.flux;
+  return LPF_OK;
+}
+
+int lpf_process_frame_host(lpf_ctx* c, int lane, const float* h_cube, int64_t t, lpf_host_result* res, void* stream) {
+  TRY(lane_ok(c, lane));
+  if (!h_cube || !res) return LPF_E_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  LpfLane& L = c->lanes[lane];
+  const lpf_params& p = c->p;
+  const size_t cube_bytes = (size_t)p.B * c->N * sizeof(float);
+  if (!L.cube) TRY(dalloc(&L.cube, (size_t)p.B * c->N));
+  LPF_CUDA(cudaMemcpyAsync(L.cube, h_cube, cube_bytes, cudaMemcpyHostToDevice, st));
+  TRY(lpf_process_frame(c, lane, L.cube, t, st));
+  LPF_CUDA(cudaMemcpyAsync(&L.h_counts[0], L.nu, 4, cudaMemcpyDeviceToHost, st));
+  LPF_CUDA(cudaMemcpyAsync(&L.h_counts[1], L.npos, 4, cudaMemcpyDeviceToHost, st));
+  LPF_CUDA(cudaMemcpyAsync(&L.h_counts[2], L.ndets, 4, cudaMemcpyDeviceToHost, st));
+  if (res->h_stats) LPF_CUDA(cudaMemcpyAsync(res->h_stats, L.stats, (size_t)p.B * LPF_STATS_PER_BAND * 4, cudaMemcpyDeviceToHost, st));
+  if (res->h_band_ok) LPF_CUDA(cudaMemcpyAsync(res->h_band_ok, L.band_ok, (size_t)p.B + 1, cudaMemcpyDeviceToHost, st));
+  LPF_CUDA(cudaStreamSynchronize(st));
+  res->nu = L.h_counts[0]; res->npos = L.h_counts[1]; res->ndets = L.h_counts[2];
+  const size_t nu = (size_t)(res->nu < res->cap_u ? res->nu : res->cap_u);
+  const size_t np = (size_t)(res->npos < res->cap_pos ? res->npos : res->cap_pos);
+  if (nu) {
+    if (res->h_upos) LPF_CUDA(cudaMemcpyAsync(res->h_upos, L.upos, nu * 4, cudaMemcpyDeviceToHost, st));
+    if (res->h_uplane) LPF_CUDA(cudaMemcpyAsync(res->h_uplane, L.uplane, nu * 2, cudaMemcpyDeviceToHost, st));
+    if (res->h_usnr) LPF_CUDA(cudaMemcpyAsync(res->h_usnr, L.usnr, nu * 4, cudaMemcpyDeviceToHost, st));
+    if (res->h_cand_idx) LPF_CUDA(cudaMemcpyAsync(res->h_cand_idx, L.cand_idx, nu * 4, cudaMemcpyDeviceToHost, st));
+  }
+  if (np) {
+    if (res->h_act_slots) LPF_CUDA(cudaMemcpyAsync(res->h_act_slots, L.act_slots, np * 4, cudaMemcpyDeviceToHost, st));
+    if (res->h_flux) LPF_CUDA(cudaMemcpyAsync(res->h_flux, L.flux, np * p.B * 4, cudaMemcpyDeviceToHost, st));
+  }
+  LPF_CUDA(cudaStreamSynchronize(st));
+  return LPF_OK;
+}
+
+int lpf_get_counters(lpf_ctx* c, int64_t* h_out) {
+  if (!c || !h_out) return LPF_E_ARG;
+  int32_t h[4];
+  LPF_CUDA(cudaDeviceSynchronize());
+  LPF_CUDA(cudaMemcpy(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost));
+  h_out[0] = h[0]; h_out[1] = h[1]; h_out[2] = c->launches; h_out[3] = h[2];
+  return LPF_OK;
+}
+
+int lpf_memcpy_d2h(void* h_dst, const void* d_src, int64_t bytes) {
+  if (bytes < 0 || (bytes > 0 && (!h_dst || !d_src))) return LPF_E_ARG;
+  if (bytes == 0) return LPF_OK;
+  LPF_CUDA(cudaMemcpy(h_dst, d_src, (size_t)bytes, cudaMemcpyDeviceToHost));
+  return LPF_OK;
+}
+
+const char* lpf_strerror(int code) {
+  switch (code) {
+    case LPF_OK: return "ok";
+    case LPF_E_ARG: return "bad argument or unsupported parameter";
+    case LPF_E_CUDA: return "CUDA runtime error";
+    case LPF_E_STATE: return "bad state (call order, capacity)";
+    case LPF_E_NOMEM: return "out of device memory";
+    default: return "unknown";
+  }
+}
+
+const char* lpf_last_cuda_error(void) { return g_lpf_cuda_err; }
+
+int lpf_version(void) { return 100; }
+
+}  // extern "C"

@@ -1,0 +1,133 @@
+// Internal declarations of the LPF CUDA library (sm_100a).  Not part of the C-ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/lpf.h"
+
+#define LPF_NTAPS (2 * LPF_MAX_RADIUS + 1)
+
+struct LpfTaps {
+  int R;
+  float g[LPF_NTAPS];
+};
+
+// Scratch and owned outputs of one frame in flight.
+struct LpfLane {
+  double* qc_part1 = nullptr;  // [B][nblk][3]  n, sum(x-p), sum(x-p)^2
+  double* qc_part2 = nullptr;  // [B][nblk][3]  clipped
+  float* sum_plane = nullptr;  // [N]
+  float* F = nullptr;          // [(B+1)][N] matched-filtered planes (general path)
+  float* C = nullptr;          // [(B+1)][N]
+  float* S = nullptr;          // [(B+1)][N]
+  uint8_t* Y = nullptr;        // [(B+1)][N] iteration of first detection (n_iter > 1 only)
+  float* normp = nullptr;      // [(B+1)][N] per-plane normaliser for iterations > 1
+  unsigned long long* M = nullptr;  // [N] dedupe key map, all zero between frames
+  int32_t* tmp_pos = nullptr;
+  int16_t* tmp_plane = nullptr;
+  float* tmp_snr = nullptr;
+  int32_t* tmp_n = nullptr;
+  // lane-owned results of lpf_process_frame
+  float* stats = nullptr;
+  uint8_t* band_ok = nullptr;
+  lpf_det* dets = nullptr;
+  int32_t* ndets = nullptr;
+  int32_t* upos = nullptr;
+  int16_t* uplane = nullptr;
+  float* usnr = nullptr;
+  int32_t* nu = nullptr;
+  int32_t* cand_idx = nullptr;
+  int32_t* act_slots = nullptr;
+  int32_t* act_pix = nullptr;
+  int32_t* npos = nullptr;
+  float* flux = nullptr;
+  float* cube = nullptr;       // device cube for the *_host entry (lazy)
+  int32_t* h_counts = nullptr; // pinned [4]
+};
+
+struct lpf_ctx {
+  lpf_params p;
+  int64_t N;        // Dy*Dx
+  int n_planes;     // B + detect_sum_plane
+  int qc_nblk;
+  int first_valid;  // first valid pixel (pivot of the statistics)
+  int n_sm;
+  LpfTaps g_mf, g_bg;
+  uint8_t* W = nullptr;      // [N] valid mask (always materialised)
+  float* norm_mf = nullptr;  // [N] W / (g_mf (*) W)
+  float* norm_bg = nullptr;  // [N] W / (g_bg (*) W)
+  // candidate table
+  uint8_t* active = nullptr;
+  uint8_t* forced = nullptr;
+  int32_t* cpix = nullptr;
+  int32_t* miss = nullptr;
+  long long* born = nullptr;
+  long long* matched_t = nullptr;
+  int32_t* slotmap = nullptr;  // [N] lowest active slot at that pixel, -1 none
+  int32_t* free_list = nullptr;
+  float* ring = nullptr;       // [n_cand_max][T_ring][B]
+  long long* meta_t = nullptr; // [T_ring]
+  unsigned long long* meta_ok = nullptr;
+  int32_t* counters = nullptr; // [0] dropped records, [1] dropped detections, [2] active candidates
+  cudaEvent_t chain_ev = nullptr;
+  bool chain_valid = false;
+  int64_t launches = 0;
+  std::vector<LpfLane> lanes;
+};
+
+extern thread_local char g_lpf_cuda_err[256];
+int lpf_cuda_fail(cudaError_t e, const char* what);
+
+#define LPF_CUDA(call)                                        \
+  do {                                                        \
+    cudaError_t e__ = (call);                                 \
+    if (e__ != cudaSuccess) return lpf_cuda_fail(e__, #call); \
+  } while (0)
+
+#define LPF_LAUNCH_CHECK(ctx)                                     \
+  do {                                                            \
+    (ctx)->launches++;                                            \
+    cudaError_t e__ = cudaPeekAtLastError();                      \
+    if (e__ != cudaSuccess) return lpf_cuda_fail(e__, "launch");  \
+  } while (0)
+
+// ---- launchers implemented in the kernel translation units ---------------------------------
+int lpf_launch_qc(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, cudaStream_t st);
+
+int lpf_launch_sum_plane(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, cudaStream_t st);
+int lpf_launch_detect_general(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok,
+                              lpf_det* d_dets, int32_t* d_ndets, cudaStream_t st);
+int lpf_launch_static_norm(lpf_ctx* c, const LpfTaps& g, float* d_norm, float* d_tmp, cudaStream_t st);
+
+int lpf_launch_dedupe(lpf_ctx* c, LpfLane& L, const lpf_det* d_dets, const int32_t* d_ndets, int32_t* d_upos,
+                      int16_t* d_uplane, float* d_usnr, int32_t* d_nu, cudaStream_t st);
+int lpf_launch_associate(lpf_ctx* c, const int32_t* d_upos, const int32_t* d_nu, const uint8_t* d_band_ok,
+                         long long t, int32_t* d_cand_idx, int32_t* d_act_slots, int32_t* d_act_pix,
+                         int32_t* d_npos, cudaStream_t st);
+int lpf_launch_add_candidates(lpf_ctx* c, const int32_t* d_pix, int n, int32_t* d_slots_out, cudaStream_t st);
+int lpf_launch_measure_flux(lpf_ctx* c, const float* d_cube, const uint8_t* d_band_ok, const int32_t* d_pos,
+                            const int32_t* d_npos, float* d_flux, cudaStream_t st);
+int lpf_launch_append(lpf_ctx* c, const int32_t* d_slots, const int32_t* d_n, const float* d_flux,
+                      const uint8_t* d_band_ok, long long t, cudaStream_t st);
+int lpf_launch_get_dynspec(lpf_ctx* c, int slot, long long t_last, float* d_out, cudaStream_t st);
+int lpf_launch_fill_nan(lpf_ctx* c, float* d, int64_t n, cudaStream_t st);
+int lpf_launch_fill_i32(lpf_ctx* c, int32_t* d, int64_t n, int32_t v, cudaStream_t st);
+
+// ---- small device helpers --------------------------------------------------------------------
+__device__ __forceinline__ float lpf_warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ double lpf_warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ int lpf_warp_sum(int v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}

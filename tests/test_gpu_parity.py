@@ -1,0 +1,274 @@
+"""-m gpu: the CUDA path (through the C-ABI) against the CPU oracle, element by element,
+on the five BASELINE.json configs (SURVEY.md 8(d) parity scope, sized to finish in minutes)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle as O
+from paper_2103_15418_b200 import synth
+import parity
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+def _make(cfg, torch, **kw):
+    from paper_2103_15418_b200.binding import LPF
+    s = synth.CubeStream(cfg)
+    bg = kw.pop("bg", "box"); n_iter = kw.pop("n_iter", 1)
+    p = synth.default_params(cfg, bg=bg, n_iter=n_iter)
+    p.update(kw)
+    return s, p, LPF(p, s.mask)
+
+
+def _run_chain(torch, s, p, lpf, frames, direct=False, via="calls", tag=""):
+    pipe = O.OraclePipeline(p, s.mask, direct=direct)
+    worst_z = 0.0; ties = 0
+    for t in frames:
+        cube = s.frame(t)
+        cube_d = torch.from_numpy(cube).cuda()
+        o = pipe.step(cube, t)
+        if via == "calls":
+            g = parity.gpu_step_by_calls(lpf, cube_d, t)
+        else:
+            lpf.process_frame(cube_d, t)
+            g = lpf.frame_view(0)
+        r = parity.check_frame(g, o, pipe, cube, f"{tag} t={t}")
+        assert r["in_sync"], f"{tag} t={t}: chain lost sync after a tie: {parity.TIES[-3:]}"
+        worst_z = max(worst_z, r["zerr"]); ties += r["n_ties"]
+    return pipe, worst_z, ties
+
+
+# ------------------------------------------------------------------ config 1
+@pytest.mark.parametrize("bg,n_iter", [("box", 1), ("gauss", 1), ("box", 3), ("gauss", 3)])
+def test_config1_all_frames(torch_cuda, bg, n_iter):
+    s, p, lpf = _make(1, torch_cuda, bg=bg, n_iter=n_iter)
+    pipe, wz, ties = _run_chain(torch_cuda, s, p, lpf, range(32), direct=True, via="calls", tag=f"cfg1 {bg} it{n_iter}")
+    assert ties == 0
+    # dynamic spectrum of the source's candidate: bit-exact, time ordered
+    ds_g = lpf.get_dynspec(0, 31).cpu().numpy()
+    ds_o = pipe.table.dynspec(0, 31)
+    assert np.array_equal(np.isnan(ds_g), np.isnan(ds_o))
+    assert np.array_equal(ds_g[~np.isnan(ds_g)], ds_o[~np.isnan(ds_o)])
+    assert lpf.counters()["dropped_records"] == 0
+    lpf.close()
+
+
+def test_config1_process_frame_entry(torch_cuda):
+    s, p, lpf = _make(1, torch_cuda)
+    _run_chain(torch_cuda, s, p, lpf, range(8), via="frame", tag="cfg1 process_frame")
+    lpf.close()
+
+
+# ------------------------------------------------------------------ config 2
+def test_config2_chain_box(torch_cuda):
+    s, p, lpf = _make(2, torch_cuda)
+    pipe, wz, ties = _run_chain(torch_cuda, s, p, lpf, range(40), via="frame", tag="cfg2 box")
+    assert ties == 0
+    # every active candidate's dynamic spectrum is bit-exact
+    act = np.flatnonzero(pipe.table.active)
+    assert act.size > 50
+    for slot in act[:: max(1, act.size // 25)]:
+        ds_g = lpf.get_dynspec(int(slot), 39).cpu().numpy(); ds_o = pipe.table.dynspec(int(slot), 39)
+        assert np.array_equal(np.isnan(ds_g), np.isnan(ds_o)) and np.array_equal(ds_g[~np.isnan(ds_g)], ds_o[~np.isnan(ds_o)])
+    lpf.close()
+
+
+@pytest.mark.parametrize("bg,n_iter", [("gauss", 1), ("box", 3), ("gauss", 3)])
+def test_config2_variants(torch_cuda, bg, n_iter):
+    s, p, lpf = _make(2, torch_cuda, bg=bg, n_iter=n_iter)
+    _run_chain(torch_cuda, s, p, lpf, range(4), via="calls", tag=f"cfg2 {bg} it{n_iter}")
+    lpf.close()
+
+
+def test_config2_direct_definition_one_frame(torch_cuda):
+    # the oracle's direct 2-D window form (no factorisation) on a full config-2 frame
+    s, p, lpf = _make(2, torch_cuda)
+    _run_chain(torch_cuda, s, p, lpf, [0], direct=True, tag="cfg2 direct")
+    lpf.close()
+
+
+# ------------------------------------------------------------------ config 3
+def test_config3_frames_with_rfi(torch_cuda):
+    s, p, lpf = _make(3, torch_cuda)
+    t_bad = next(t for t in range(600) if s.rfi(t))
+    frames = [0, t_bad, t_bad + 1] if t_bad > 0 else [0, 1]
+    pipe = O.OraclePipeline(p, s.mask, direct=False)
+    for t in frames:
+        cube = s.frame(t)
+        o = pipe.step(cube, t)
+        lpf.process_frame(torch_cuda.from_numpy(cube).cuda(), t)
+        g = lpf.frame_view(0)
+        r = parity.check_frame(g, o, pipe, cube, f"cfg3 t={t}")
+        assert r["in_sync"]
+        if t == t_bad:   # QC must flag every injected band (and nothing else)
+            bad = s.truth_rfi_bands(t)
+            assert [b for b in range(p["B"]) if not o["band_ok"][b]] == bad
+            assert [b for b in range(p["B"]) if not g["band_ok"][b]] == bad
+    lpf.close()
+
+
+def test_config3_gauss_one_frame(torch_cuda):
+    s, p, lpf = _make(3, torch_cuda, bg="gauss")
+    _run_chain(torch_cuda, s, p, lpf, [0], via="frame", tag="cfg3 gauss")
+    lpf.close()
+
+
+# ------------------------------------------------------------------ config 4
+def test_config4_four_lanes(torch_cuda):
+    torch = torch_cuda
+    s, p, lpf = _make(4, torch)
+    assert p["n_lanes"] == 4
+    cubes = [s.frame(t) for t in range(4)]
+    dcubes = [torch.from_numpy(c).cuda() for c in cubes]
+    streams = [torch.cuda.Stream() for _ in range(4)]
+    torch.cuda.synchronize()
+    for t in range(4):   # four frames in flight on separate CUDA streams
+        lpf.process_frame(dcubes[t], t, lane=t, stream=streams[t])
+    torch.cuda.synchronize()
+    views = [lpf.frame_view(t) for t in range(4)]
+    pipe = O.OraclePipeline(p, s.mask, direct=False)
+    o0 = pipe.step(cubes[0], 0)
+    r = parity.check_frame(views[0], o0, pipe, cubes[0], "cfg4 t=0")
+    assert r["in_sync"]
+    # frames 1..3: the association chain must have run in t order across lanes: same result as a
+    # fresh single-lane context fed sequentially
+    from paper_2103_15418_b200.binding import LPF
+    p1 = dict(p); p1["n_lanes"] = 1
+    seq = LPF(p1, s.mask)
+    for t in range(4):
+        seq.process_frame(dcubes[t], t)
+        v = seq.frame_view(0)
+        for k in ("band_ok", "upos", "cand_idx", "act_slots", "act_pix", "flux"):
+            assert np.array_equal(v[k], views[t][k]), (t, k)
+    seq.close(); lpf.close()
+
+
+# ------------------------------------------------------------------ config 5
+def test_config5_forced_flux_and_detection(torch_cuda):
+    torch = torch_cuda
+    s, p, lpf = _make(5, torch)
+    slots = lpf.add_candidates(s.forced_pix).cpu().numpy()
+    assert np.array_equal(slots, np.arange(10000))
+    pipe = O.OraclePipeline(p, s.mask, direct=False)
+    pipe.table.add_forced(s.forced_pix)
+    cube = s.frame(0)
+    o = pipe.step(cube, 0)
+    lpf.process_frame(torch.from_numpy(cube).cuda(), 0)
+    g = lpf.frame_view(0)
+    r = parity.check_frame(g, o, pipe, cube, "cfg5 t=0")
+    assert r["in_sync"] and g["flux"].shape[0] >= 10000 and g["flux"].shape[1] == 64
+    lpf.close()
+
+
+def test_config5_ring_wraparound(torch_cuda):
+    # 64-channel rings with forced positions; T_ring shortened so that the wrap-around is reached in 20 frames
+    torch = torch_cuda
+    s = synth.CubeStream(5)
+    p = synth.default_params(5); p["T_ring"] = 16
+    from paper_2103_15418_b200.binding import LPF
+    lpf = LPF(p, s.mask)
+    n_forced = 2000
+    fp = s.forced_pix[:n_forced]
+    lpf.add_candidates(fp)
+    tb = O.CandidateTable(p["n_cand_max"], 16, 64, p["Dx"], p["r_assoc"], p["n_forget"])
+    slots = tb.add_forced(fp)
+    pos_d = torch.from_numpy(fp.astype(np.int32)).cuda(); slots_d = torch.from_numpy(slots).cuda()
+    n_d = torch.tensor([n_forced], dtype=torch.int32, device="cuda")
+    rng = np.random.default_rng(0)
+    for t in range(20):
+        cube = s.frame(t)
+        ok = np.ones(65, np.uint8)
+        if t == 7:
+            ok[5] = 0
+        if t == 9:
+            ok[64] = 0
+        ok_d = torch.from_numpy(ok).cuda()
+        cube_d = torch.from_numpy(cube).cuda()
+        flux_d = lpf.measure_flux(cube_d, ok_d, pos_d, n_d)
+        lpf.append_dynspec(slots_d, n_d, flux_d, ok_d, t)
+        flux_o = O.measure_flux(cube, ok, s.mask, fp, p["r_flux"])
+        tb.append(slots, flux_o, ok, t)
+        assert np.array_equal(flux_d.cpu().numpy(), flux_o), t
+    for slot in rng.choice(n_forced, 40, replace=False):
+        a = lpf.get_dynspec(int(slot), 19).cpu().numpy(); b = tb.dynspec(int(slot), 19)
+        assert np.array_equal(np.isnan(a), np.isnan(b)) and np.array_equal(a[~np.isnan(a)], b[~np.isnan(b)])
+        assert not np.isnan(a).any()
+    lpf.close()
+
+
+# ------------------------------------------------------------------ edge cases
+def test_edge_cases(torch_cuda):
+    torch = torch_cuda
+    from paper_2103_15418_b200.binding import LPF, LpfError
+    # ragged sizes (not multiples of the tile, odd row length -> scalar load path), run-time radii
+    rng = np.random.default_rng(21)
+    Dy, Dx, B = 77, 93, 3
+    p = synth.default_params(1); p.update(B=B, Dy=Dy, Dx=Dx, k_mf=2, k_bg=5, kappa=3.5, n_iter=2, n_cand_max=256, T_ring=4)
+    W = (rng.random((Dy, Dx)) > 0.1).astype(np.uint8); W[:9, :11] = 0
+    cube = rng.standard_normal((B, Dy, Dx)).astype(np.float32)
+    cube[:, 40, 50] += 9.0; cube[:, 41, 50] += 6.0; cube[:, 5, 88] += 9.0
+    cube *= W
+    lpf = LPF(p, W)
+    pipe = O.OraclePipeline(p, W, direct=True)
+    for t in range(3):
+        o = pipe.step(cube, t)
+        g = parity.gpu_step_by_calls(lpf, torch.from_numpy(cube).cuda(), t)
+        assert parity.check_frame(g, o, pipe, cube, f"ragged t={t}")["in_sync"]
+    lpf.close()
+    # constant cube: zero detections; all bands ok
+    p = synth.default_params(1)
+    lpf = LPF(p, None)
+    for c in (0.0, 3.25, -1e6):
+        cube = np.full((4, 64, 64), c, np.float32)
+        g = parity.gpu_step_by_calls(lpf, torch.from_numpy(cube).cuda(), 0)
+        assert g["ndets"] == 0 and g["upos"].size == 0 and g["band_ok"].all()
+    # non-finite band is rejected, the rest of the frame is processed
+    s = synth.CubeStream(1)
+    cube = s.frame(0); cube[2, 10, 10] = np.nan
+    pipe = O.OraclePipeline(p, None, direct=False)
+    o = pipe.step(cube, 0)
+    g = parity.gpu_step_by_calls(lpf, torch.from_numpy(cube).cuda(), 1)
+    assert g["band_ok"].tolist() == [1, 1, 0, 1, 1] == o["band_ok"].tolist()
+    assert np.array_equal(g["upos"], o["upos"]) and np.array_equal(g["flux"][:, 2], np.zeros(g["flux"].shape[0], np.float32))
+    # rejected frame (majority of bands bad): no detections, zero fluxes, table unchanged
+    cube = s.frame(1); cube[0] *= 50; cube[1] += 30; cube[3] *= 0.01
+    o = pipe.step(cube, 2)
+    g = parity.gpu_step_by_calls(lpf, torch.from_numpy(cube).cuda(), 2)
+    assert o["band_ok"][4] == 0 and g["band_ok"].tolist() == o["band_ok"].tolist()
+    assert g["upos"].size == 0 and np.all(g["flux"] == 0) and np.array_equal(g["act_slots"], o["act_slots"])
+    lpf.close()
+    # capacity overflow is counted, not UB
+    p2 = synth.default_params(1); p2["max_det"] = 2; p2["kappa"] = 1.0
+    lpf = LPF(p2, None)
+    g = parity.gpu_step_by_calls(lpf, torch.from_numpy(s.frame(0)).cuda(), 0)
+    assert g["ndets"] > 2 and len(g["rec"]) == 2 and lpf.counters()["dropped_records"] == g["ndets"] - 2
+    lpf.close()
+    # argument errors
+    bad = synth.default_params(1); bad["k_bg"] = 40
+    with pytest.raises(LpfError):
+        LPF(bad, None)
+
+
+def test_host_entry_point(torch_cuda):
+    torch = torch_cuda
+    from paper_2103_15418_b200.binding import HostResult
+    s, p, lpf = _make(2, torch)
+    pipe = O.OraclePipeline(p, s.mask, direct=False)
+    res = HostResult(p)
+    for t in range(3):
+        cube = s.frame(t)
+        h = torch.from_numpy(cube).pin_memory()
+        lpf.process_frame_host(h, t, res)
+        o = pipe.step(cube, t)
+        assert np.array_equal(res.band_ok.numpy(), o["band_ok"])
+        assert np.array_equal(res.upos[:res.nu].numpy(), o["upos"])
+        assert np.array_equal(res.cand_idx[:res.nu].numpy(), o["cand_idx"])
+        assert np.array_equal(res.act_slots[:res.npos].numpy(), o["act_slots"])
+        assert np.array_equal(res.flux[:res.npos].numpy(), o["flux"])
+    lpf.close()
