@@ -47,15 +47,20 @@ void orc_band_stats(const float* cube, int B, int Dy, int Dx, const uint8_t* W,
     for (int64_t i = 0; i < N; ++i)
       if (!W || W[i]) { double d = (double)X[i] - mean; ss += d * d; }
     const double rms = std::sqrt(ss / n);
+    // membership of the clip round is a floating-point DECISION: it is taken in the kernel's precision
+    // (float32: |x - (float)mean| <= (float)(qc_clip rms)), reading R25; the moments of the
+    // selected pixels are float64 as everywhere else.
+    const float meanf = (float)mean, thrf = (float)(qc_clip * rms);
+    auto inside = [&](float x) { const float d = x - meanf; return std::fabs(d) <= thrf; };
     double nc = 0, sc = 0;
     for (int64_t i = 0; i < N; ++i)
-      if (!W || W[i]) { double d = (double)X[i] - mean; if (std::fabs(d) <= qc_clip * rms) { nc += 1; sc += (double)X[i]; } }
+      if ((!W || W[i]) && inside(X[i])) { nc += 1; sc += (double)X[i]; }
     double cmean = 0, crms = 0;
     if (nc > 0) {
       cmean = sc / nc;
       double ssc = 0;
       for (int64_t i = 0; i < N; ++i)
-        if (!W || W[i]) { double d = (double)X[i] - mean; if (std::fabs(d) <= qc_clip * rms) { double e = (double)X[i] - cmean; ssc += e * e; } }
+        if ((!W || W[i]) && inside(X[i])) { double e = (double)X[i] - cmean; ssc += e * e; }
       crms = std::sqrt(ssc / nc);
     }
     o[0] = n; o[1] = mean; o[2] = rms; o[3] = nc; o[4] = cmean; o[5] = crms;
