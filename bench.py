@@ -1,0 +1,364 @@
+#!/usr/bin/env python
+"""bench.py -- frames/s of the LPF hot path (qc -> detect -> associate -> flux -> append) on
+seeded synthetic AARTFAAC-shaped cubes (BASELINE.json: 1024x1024x16 fp32 = config 3).
+
+    python bench.py --gpus N --steps K --warmup W            # our CUDA path
+    python bench.py --impl reference --gpus N --steps K ...  # the CPU oracle, as it stands
+
+One JSON line on stdout (rank 0).  A "step" is one cube through the whole path.  The pool of
+distinct device-resident frames is larger than L2 and cycled, so every step reads its cube from HBM.
+Timing: CUDA events on a main stream that all lane streams fork from / join to; max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "image-cube frames/s (whole path: qc+detect+associate+flux+dynspec)"
+UNIT = "frames/s"
+FALLBACK_HBM_GBS = 6650.0           # /opt/skills/guides/B200_PROFILING.md fallback
+N_SM, FP32_LANES, SM_MAX_GHZ = 148, 128, 1.965
+ALU_PEAK_TFLOPS = N_SM * FP32_LANES * 2 * SM_MAX_GHZ / 1e3   # 74.4 TFLOP/s fp32 FMA
+
+
+def env_rank():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        d = json.load(open(path))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)", d
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)", {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the GPU is under load."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def mark(self):
+        return time.time()
+
+    def stop(self, t0=None, t1=None):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons, pw = [], [], set(), []
+        for (ts, ln) in self.rows:
+            if t0 is not None and not (t0 <= ts <= t1 + 0.2):
+                continue
+            f = [x.strip() for x in ln.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except Exception:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples in timed region"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+# algorithmic bytes / flops per launch of each kernel
+def kernel_model(name: str, p: dict, n_valid: int):
+    B, N = p["B"], p["Dy"] * p["Dx"]
+    P = B + (1 if p["detect_sum_plane"] else 0)
+    kmf, kbg = p["k_mf"], p["k_bg"]
+    m = {
+        "qc_pass1": (4 * B * N, 6 * B * N),
+        "qc_pass2": (4 * B * N, 6 * B * N),
+        "sum_plane": (4 * B * N + 4 * N, B * N),
+        "conv_mf": (8 * P * N, 2 * 2 * (2 * kmf + 1) * P * N),
+        "conv_c": (8 * P * N, 2 * 2 * (2 * kbg + 1) * P * N),
+        "conv_s": (12 * P * N, 2 * 2 * (2 * kbg + 1) * P * N),
+        "conv_den": (5 * P * N, 2 * 2 * (2 * kbg + 1) * P * N),
+        "threshold_peaks": (12 * P * N, 8 * P * N),
+        # fused path: reads the cube (and the sum plane) once; flops = defined arithmetic per plane-voxel
+        "fused_detect": (4 * P * N, (2 * 2 * (2 * kmf + 1) + 30) * P * N),
+    }
+    return m.get(name, (0, 0))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2103_15418_b200 import synth
+    from paper_2103_15418_b200.binding import LPF, HostResult
+
+    rank, world, local = env_rank()
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    cfg = args.config
+    s = synth.CubeStream(cfg, seed=rank)           # every rank: its own independent stream (weak scaling)
+    p = synth.default_params(cfg, bg=args.bg, n_iter=args.n_iter)
+    p["n_lanes"] = args.lanes
+    B, D = p["B"], p["Dy"]
+    N = D * D
+    cube_bytes = 4 * B * N
+    n_pool = args.pool
+    n_valid = int(s.mask.sum()) if s.mask is not None else N
+
+    pool_h = torch.empty((n_pool, B, D, D), dtype=torch.float32, pin_memory=True)
+    for i in range(n_pool):
+        pool_h[i] = torch.from_numpy(s.frame(i))
+    pool_d = pool_h.to(dev)
+    lpf = LPF(p, s.mask, device=f"cuda:{local}")
+    if s.forced_pix.size:
+        lpf.add_candidates(s.forced_pix)
+    lanes = args.lanes
+    streams = [torch.cuda.Stream(device=dev) for _ in range(lanes)]
+    main = torch.cuda.current_stream()
+
+    def run_steps(t0, k):
+        ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+        ev0.record(main)
+        for st in streams:
+            st.wait_event(ev0)
+        for i in range(k):
+            t = t0 + i
+            lpf.process_frame(pool_d[t % n_pool], t, lane=t % lanes, stream=streams[t % lanes])
+        for st in streams:
+            e = torch.cuda.Event(); e.record(st); main.wait_event(e)
+        ev1.record(main)
+        return ev0, ev1
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    run_steps(0, args.warmup)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    l0 = lpf.counters()["launches"]
+    ts0 = sampler.mark()
+    ev0, ev1 = run_steps(args.warmup, args.steps)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ts1 = sampler.mark()
+    ms = ev0.elapsed_time(ev1)
+    launches = lpf.counters()["launches"] - l0
+    if world > 1:
+        tms = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+        ms = float(tms.item())
+        tl = torch.tensor([launches], device=dev, dtype=torch.int64)
+        dist.all_reduce(tl, op=dist.ReduceOp.SUM)
+        launches = int(tl.item())
+    t_next = args.warmup + args.steps
+
+    # keep the GPU under the same load until nvidia-smi has had time to sample it
+    tload = time.time()
+    while ms < 1500.0 and time.time() - tload < 1.6 - ms / 1e3:
+        run_steps(t_next, 64); t_next += 64
+        torch.cuda.synchronize()
+    ts1b = sampler.mark()
+    clocks = sampler.stop(ts0, max(ts1, ts1b))
+
+    # per-kernel CUDA-event profile over the same step mix -> roofline of the dominant kernel
+    kp = min(args.steps, 200)
+    lpf.profile_begin()
+    run_steps(t_next, kp); t_next += kp
+    prof = lpf.profile_end()
+    kernels = {k: {"launches_per_step": c / kp, "us_per_launch": 1e3 * tm / c, "us_per_step": 1e3 * tm / kp}
+               for k, (c, tm) in prof.items()}
+    step_kernel_us = sum(v["us_per_step"] for v in kernels.values())
+    dom = max(kernels, key=lambda k: kernels[k]["us_per_step"])
+    hbm_peak, peak_src, _ = load_peaks()
+    abytes, aflops = kernel_model(dom, p, n_valid)
+    dur_s = kernels[dom]["us_per_launch"] * 1e-6
+    gbs = abytes / dur_s / 1e9
+    tfl = aflops / dur_s / 1e12
+    t_hbm, t_alu = abytes / (hbm_peak * 1e9), aflops / (ALU_PEAK_TFLOPS * 1e12)
+    if t_hbm >= t_alu:
+        roof = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak}
+    else:
+        roof = {"bound": "alu", "achieved": tfl, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": tfl / ALU_PEAK_TFLOPS}
+    roof.update({"kernel": dom, "us_per_launch": kernels[dom]["us_per_launch"], "share_of_step": kernels[dom]["us_per_step"] / step_kernel_us,
+                 "algorithmic_bytes": abytes, "algorithmic_flops": aflops, "hbm_gbs": gbs, "hbm_frac": gbs / hbm_peak,
+                 "peak_source": peak_src, "alu_peak_source": "148 SM x 128 fp32 lanes x 2 x 1.965 GHz", "traffic": args.traffic})
+
+    frames_s = world * args.steps / (ms / 1e3)
+    step_gbs = cube_bytes * frames_s / 1e9 / world
+
+    # end to end through the host entry point: pinned host cube -> H2D -> path -> D2H of the results
+    e2e = None
+    if not args.no_e2e:
+        res = HostResult(p)
+        ke = max(3, min(args.steps, args.e2e_steps))
+        for i in range(3):
+            lpf.process_frame_host(pool_h[i % n_pool], t_next, res, lane=0, stream=streams[0]); t_next += 1
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        w0 = time.perf_counter(); d2h = 0
+        for i in range(ke):
+            lpf.process_frame_host(pool_h[i % n_pool], t_next, res, lane=0, stream=streams[0]); t_next += 1
+            d2h += res.d2h_bytes
+        torch.cuda.synchronize()
+        w1 = time.perf_counter()
+        dt = w1 - w0
+        if world > 1:
+            tt = torch.tensor([dt], device=dev, dtype=torch.float64)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            dt = float(tt.item())
+        e2e = {"value": world * ke / dt, "unit": UNIT, "h2d_bytes_per_step": cube_bytes, "d2h_bytes_per_step": d2h // ke,
+               "steps": ke, "api": "lpf_process_frame_host (pinned host cube in, results out, 1 lane)"}
+
+    out = {
+        "metric": METRIC, "value": frames_s, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": s.c.name, "cube": [B, D, D], "bg_kernel": args.bg, "n_iter": args.n_iter, "lanes": lanes,
+                   "pool_frames": n_pool, "pool_bytes": n_pool * cube_bytes,
+                   "l2": "inputs larger than L2 (pool cycled, %d MB)" % (n_pool * cube_bytes >> 20),
+                   "parallelism": "independent streams per GPU, no data-path collective" if world > 1 else "1 GPU"},
+        "voxels_per_s": frames_s * B * N, "cube_gbs_per_gpu": step_gbs, "hbm_frac_step": step_gbs / hbm_peak,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "kernels": kernels, "roofline": roof,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu:
+        out["cpu_baseline"] = cpu_baseline(cfg, args, seconds=args.cpu_seconds)
+    lpf.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return out if rank == 0 else None
+
+
+# ------------------------------------------------------------------------------------------------
+def oracle_step_factory(cfg, bg, n_iter, crop):
+    """One bounded sample of the workload for the CPU oracle: the whole chain on a centred crop of each frame
+    (all bands).  Returns (step_fn, fraction_of_a_frame)."""
+    import oracle as O
+    from paper_2103_15418_b200 import synth
+    s = synth.CubeStream(cfg)
+    p = synth.default_params(cfg, bg=bg, n_iter=n_iter)
+    D = p["Dy"]
+    c = min(crop, D)
+    y0 = (D - c) // 2
+    p["Dy"] = p["Dx"] = c
+    mask = None if s.mask is None else np.ascontiguousarray(s.mask[y0:y0 + c, y0:y0 + c])
+    pipe = O.OraclePipeline(p, mask, direct=False)
+    frames = [np.ascontiguousarray(s.frame(t)[:, y0:y0 + c, y0:y0 + c]) for t in range(2)]
+    state = {"t": 0}
+
+    def step():
+        t = state["t"]; state["t"] += 1
+        pipe.step(frames[t % len(frames)], t)
+    return step, (c * c) / float(D * D), s.c.name, p
+
+
+def cpu_baseline(cfg, args, seconds=12.0):
+    step, frac, name, p = oracle_step_factory(cfg, args.bg, args.n_iter, args.cpu_crop)
+    step()
+    n = 0; t0 = time.perf_counter()
+    while True:
+        step(); n += 1
+        dt = time.perf_counter() - t0
+        if dt >= seconds or n >= 64:
+            break
+    return {"value": n * frac / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "%d steps of the whole chain on a centred %dx%d crop of %s (all %d bands), float64 oracle "
+                      "(row-then-column form of the window sums), scaled by crop/frame voxels" % (n, p["Dy"], p["Dx"], name, p["B"]),
+            "host_cpus": os.cpu_count()}
+
+
+def run_reference(args):
+    rank, world, _ = env_rank()
+    if rank != 0:
+        return None
+    # bounded sample: the crop is sized so that K steps of the (untuned) oracle end within ~2.5 minutes
+    # (0.46 s per 256x256x16 crop measured on the build container, cost ~ pixels)
+    per_step = 150.0 / max(1, args.steps + min(args.warmup, 3))
+    crop = int(256.0 * (per_step / 0.5) ** 0.5) // 32 * 32
+    crop = max(64, min(512, crop, args.cpu_crop if args.cpu_crop != 256 else 512))
+    step, frac, name, p = oracle_step_factory(args.config, args.bg, args.n_iter, crop)
+    for _ in range(min(args.warmup, 3)):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    v = args.steps * frac / dt
+    sample = ("each step = whole chain on a centred %dx%d crop of %s (all %d bands) with the float64 CPU oracle, "
+              "1 thread; value scaled by crop/frame voxels" % (p["Dy"], p["Dx"], name, p["B"]))
+    return {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": name, "cube": [p["B"], CONFIG_D(args.config), CONFIG_D(args.config)], "bg_kernel": args.bg,
+                       "n_iter": args.n_iter},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+
+
+def CONFIG_D(cfg):
+    from paper_2103_15418_b200 import synth
+    return synth.CONFIGS[cfg].D
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); 3 = 1024x1024x16")
+    ap.add_argument("--bg", default="box", choices=["box", "gauss"])
+    ap.add_argument("--n-iter", dest="n_iter", type=int, default=1)
+    ap.add_argument("--lanes", type=int, default=4)
+    ap.add_argument("--pool", type=int, default=16)
+    ap.add_argument("--e2e-steps", type=int, default=64)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--cpu-crop", type=int, default=256)
+    ap.add_argument("--traffic", type=float, default=None, help="dram bytes/launch of the dominant kernel from ncu (profiles/)")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    out = run_reference(args) if args.impl == "reference" else run_ours(args)
+    if out is not None:
+        print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    main()

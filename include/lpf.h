@@ -187,6 +187,15 @@ int lpf_process_frame_host(lpf_ctx* ctx, int lane, const float* h_cube, int64_t 
  * h_out[2] = kernels launched by this context so far, h_out[3] = active candidates.  Synchronises. */
 int lpf_get_counters(lpf_ctx* ctx, int64_t* h_out);
 
+/* Optional per-kernel timing with CUDA events recorded on the launching stream, around every kernel
+ * this context launches between lpf_profile_begin and lpf_profile_end (both synchronise).
+ * h_count[k] / h_ms[k]: launches and summed milliseconds of kernel id k, n >= lpf_profile_kernel_count().
+ * Used by bench.py for the roofline of the dominant kernel; off by default (no events recorded). */
+int lpf_profile_begin(lpf_ctx* ctx);
+int lpf_profile_end(lpf_ctx* ctx, int32_t* h_count, float* h_ms, int32_t n);
+int lpf_profile_kernel_count(void);
+const char* lpf_profile_kernel_name(int kid);
+
 /* Convenience for bindings: synchronous copy of `bytes` from device to host memory. */
 int lpf_memcpy_d2h(void* h_dst, const void* d_src, int64_t bytes);
 

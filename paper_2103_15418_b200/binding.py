@@ -54,7 +54,7 @@ EXPORTS = [
     "lpf_create", "lpf_destroy", "lpf_cube_qc", "lpf_detect_sources", "lpf_associate", "lpf_add_candidates",
     "lpf_measure_flux", "lpf_append_dynspec", "lpf_get_dynspec", "lpf_process_frame", "lpf_get_frame_view",
     "lpf_process_frame_host", "lpf_get_counters", "lpf_memcpy_d2h", "lpf_strerror", "lpf_last_cuda_error",
-    "lpf_version",
+    "lpf_version", "lpf_profile_begin", "lpf_profile_end", "lpf_profile_kernel_count", "lpf_profile_kernel_name",
 ]
 
 
@@ -90,8 +90,12 @@ def load_library(path: Optional[str] = None):
     lib.lpf_strerror.argtypes = [C.c_int]
     lib.lpf_strerror.restype = C.c_char_p
     lib.lpf_last_cuda_error.restype = C.c_char_p
+    lib.lpf_profile_begin.argtypes = [vp]
+    lib.lpf_profile_end.argtypes = [vp, vp, vp, i32]
+    lib.lpf_profile_kernel_name.argtypes = [C.c_int]
+    lib.lpf_profile_kernel_name.restype = C.c_char_p
     for n in EXPORTS:
-        if n not in ("lpf_strerror", "lpf_last_cuda_error"):
+        if n not in ("lpf_strerror", "lpf_last_cuda_error", "lpf_profile_kernel_name"):
             getattr(lib, n).restype = C.c_int
     if path == LIB_PATH:
         _lib = lib
@@ -245,6 +249,16 @@ class LPF:
         _check(self.lib, self.lib.lpf_process_frame_host(self.h, lane, ptr, t, C.byref(res.c), _stream(stream)),
                "lpf_process_frame_host")
         return res
+
+    def profile_begin(self):
+        _check(self.lib, self.lib.lpf_profile_begin(self.h), "lpf_profile_begin")
+
+    def profile_end(self) -> dict:
+        """{kernel name: (launches, total ms)} for every kernel launched since profile_begin."""
+        n = self.lib.lpf_profile_kernel_count()
+        cnt = (C.c_int32 * n)(); ms = (C.c_float * n)()
+        _check(self.lib, self.lib.lpf_profile_end(self.h, cnt, ms, n), "lpf_profile_end")
+        return {self.lib.lpf_profile_kernel_name(i).decode(): (int(cnt[i]), float(ms[i])) for i in range(n) if cnt[i]}
 
     def counters(self) -> dict:
         h = (C.c_int64 * 4)()

@@ -320,14 +320,12 @@ __global__ void k_fill_i32(int32_t* p, long long n, int32_t v) {
 int lpf_launch_dedupe(lpf_ctx* c, LpfLane& L, const lpf_det* d_dets, const int32_t* d_ndets, int32_t* d_upos,
                       int16_t* d_uplane, float* d_usnr, int32_t* d_nu, cudaStream_t st) {
   const lpf_params& p = c->p;
-  k_dedupe_scatter<<<CAT_BLOCKS, CAT_THREADS, 0, st>>>(d_dets, d_ndets, p.max_det, L.M, L.tmp_n);
-  LPF_LAUNCH_CHECK(c);
-  k_dedupe_select<<<CAT_BLOCKS, CAT_THREADS, 0, st>>>(d_dets, d_ndets, p.max_det, L.M, p.Dy, p.Dx, p.r_dedupe,
-                                                       L.tmp_pos, L.tmp_plane, L.tmp_snr, L.tmp_n);
-  LPF_LAUNCH_CHECK(c);
-  k_dedupe_sort<<<CAT_BLOCKS, CAT_THREADS, 0, st>>>(d_dets, d_ndets, p.max_det, L.M, L.tmp_pos, L.tmp_plane, L.tmp_snr,
-                                                     L.tmp_n, d_upos, d_uplane, d_usnr, d_nu);
-  LPF_LAUNCH_CHECK(c);
+  LPF_KLAUNCH(c, KID_DEDUPE_SCATTER, st, k_dedupe_scatter<<<CAT_BLOCKS, CAT_THREADS, 0, st>>>(
+      d_dets, d_ndets, p.max_det, L.M, L.tmp_n));
+  LPF_KLAUNCH(c, KID_DEDUPE_SELECT, st, k_dedupe_select<<<CAT_BLOCKS, CAT_THREADS, 0, st>>>(
+      d_dets, d_ndets, p.max_det, L.M, p.Dy, p.Dx, p.r_dedupe, L.tmp_pos, L.tmp_plane, L.tmp_snr, L.tmp_n));
+  LPF_KLAUNCH(c, KID_DEDUPE_SORT, st, k_dedupe_sort<<<CAT_BLOCKS, CAT_THREADS, 0, st>>>(
+      d_dets, d_ndets, p.max_det, L.M, L.tmp_pos, L.tmp_plane, L.tmp_snr, L.tmp_n, d_upos, d_uplane, d_usnr, d_nu));
   return LPF_OK;
 }
 
@@ -335,17 +333,15 @@ int lpf_launch_associate(lpf_ctx* c, const int32_t* d_upos, const int32_t* d_nu,
                          long long t, int32_t* d_cand_idx, int32_t* d_act_slots, int32_t* d_act_pix,
                          int32_t* d_npos, cudaStream_t st) {
   const lpf_params& p = c->p;
-  k_assoc_match<<<CAT_BLOCKS, CAT_THREADS, 0, st>>>(d_upos, d_nu, d_band_ok, p.B, c->slotmap, c->cpix, p.Dy, p.Dx,
-                                                     p.r_assoc, t, c->matched_t, d_cand_idx);
-  LPF_LAUNCH_CHECK(c);
+  LPF_KLAUNCH(c, KID_ASSOC_MATCH, st, k_assoc_match<<<CAT_BLOCKS, CAT_THREADS, 0, st>>>(
+      d_upos, d_nu, d_band_ok, p.B, c->slotmap, c->cpix, p.Dy, p.Dx, p.r_assoc, t, c->matched_t, d_cand_idx));
   AssocArgs a{};
   a.active = c->active; a.forced = c->forced; a.cpix = c->cpix; a.miss = c->miss; a.born = c->born;
   a.matched_t = c->matched_t; a.slotmap = c->slotmap; a.free_list = c->free_list;
   a.n_cand_max = p.n_cand_max; a.n_forget = p.n_forget;
   a.upos = d_upos; a.nu = d_nu; a.band_ok = d_band_ok; a.B = p.B; a.t = t;
   a.cand_idx = d_cand_idx; a.act_slots = d_act_slots; a.act_pix = d_act_pix; a.npos = d_npos; a.counters = c->counters;
-  k_assoc_update<<<1, 1024, 0, st>>>(a);
-  LPF_LAUNCH_CHECK(c);
+  LPF_KLAUNCH(c, KID_ASSOC_UPDATE, st, k_assoc_update<<<1, 1024, 0, st>>>(a));
   return LPF_OK;
 }
 
@@ -356,8 +352,7 @@ int lpf_launch_add_candidates(lpf_ctx* c, const int32_t* d_pix, int n, int32_t* 
   a.active = c->active; a.forced = c->forced; a.cpix = c->cpix; a.miss = c->miss; a.born = c->born;
   a.slotmap = c->slotmap; a.free_list = c->free_list; a.n_cand_max = p.n_cand_max;
   a.pix = d_pix; a.n = n; a.slots_out = d_slots_out; a.status = d_status;
-  k_add_candidates<<<1, 1024, 0, st>>>(a);
-  LPF_LAUNCH_CHECK(c);
+  LPF_KLAUNCH(c, KID_MISC, st, k_add_candidates<<<1, 1024, 0, st>>>(a));
   int32_t status = -1;
   LPF_CUDA(cudaMemcpyAsync(&status, d_status, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   LPF_CUDA(cudaStreamSynchronize(st));
@@ -366,8 +361,7 @@ int lpf_launch_add_candidates(lpf_ctx* c, const int32_t* d_pix, int n, int32_t* 
     const long long per_slot = (long long)p.T_ring * p.B;
     const long long gx = (per_slot + 255) / 256;
     const dim3 grid((unsigned)(gx < 64 ? gx : 64), (unsigned)(n < 4096 ? n : 4096));
-    k_ring_nan_slots<<<grid, 256, 0, st>>>(c->ring, c->free_list, n, per_slot);
-    LPF_LAUNCH_CHECK(c);
+    LPF_KLAUNCH(c, KID_MISC, st, k_ring_nan_slots<<<grid, 256, 0, st>>>(c->ring, c->free_list, n, per_slot));
     LPF_CUDA(cudaStreamSynchronize(st));
   }
   return LPF_OK;
@@ -376,33 +370,30 @@ int lpf_launch_add_candidates(lpf_ctx* c, const int32_t* d_pix, int n, int32_t* 
 int lpf_launch_measure_flux(lpf_ctx* c, const float* d_cube, const uint8_t* d_band_ok, const int32_t* d_pos,
                             const int32_t* d_npos, float* d_flux, cudaStream_t st) {
   const lpf_params& p = c->p;
-  k_measure_flux<<<c->n_sm * 2, 256, 0, st>>>(d_cube, d_band_ok, c->W, p.B, p.Dy, p.Dx, p.r_flux, d_pos, d_npos, d_flux);
-  LPF_LAUNCH_CHECK(c);
+  LPF_KLAUNCH(c, KID_MEASURE_FLUX, st, k_measure_flux<<<c->n_sm * 2, 256, 0, st>>>(
+      d_cube, d_band_ok, c->W, p.B, p.Dy, p.Dx, p.r_flux, d_pos, d_npos, d_flux));
   return LPF_OK;
 }
 
 int lpf_launch_append(lpf_ctx* c, const int32_t* d_slots, const int32_t* d_n, const float* d_flux,
                       const uint8_t* d_band_ok, long long t, cudaStream_t st) {
   const lpf_params& p = c->p;
-  k_append<<<c->n_sm, 256, 0, st>>>(c->ring, c->meta_t, c->meta_ok, c->born, p.T_ring, p.B, d_slots, d_n, d_flux, d_band_ok, t);
-  LPF_LAUNCH_CHECK(c);
+  LPF_KLAUNCH(c, KID_APPEND, st, k_append<<<c->n_sm, 256, 0, st>>>(
+      c->ring, c->meta_t, c->meta_ok, c->born, p.T_ring, p.B, d_slots, d_n, d_flux, d_band_ok, t));
   return LPF_OK;
 }
 
 int lpf_launch_get_dynspec(lpf_ctx* c, int slot, long long t_last, float* d_out, cudaStream_t st) {
   const lpf_params& p = c->p;
-  k_get_dynspec<<<8, 256, 0, st>>>(c->ring, c->meta_t, p.T_ring, p.B, slot, t_last, d_out);
-  LPF_LAUNCH_CHECK(c);
+  LPF_KLAUNCH(c, KID_MISC, st, k_get_dynspec<<<8, 256, 0, st>>>(c->ring, c->meta_t, p.T_ring, p.B, slot, t_last, d_out));
   return LPF_OK;
 }
 
 int lpf_launch_fill_nan(lpf_ctx* c, float* d, int64_t n, cudaStream_t st) {
-  k_fill_f32<<<c->n_sm * 4, 256, 0, st>>>(d, n, nanf(""));
-  LPF_LAUNCH_CHECK(c);
+  LPF_KLAUNCH(c, KID_MISC, st, k_fill_f32<<<c->n_sm * 4, 256, 0, st>>>(d, n, nanf("")));
   return LPF_OK;
 }
 int lpf_launch_fill_i32(lpf_ctx* c, int32_t* d, int64_t n, int32_t v, cudaStream_t st) {
-  k_fill_i32<<<c->n_sm * 4, 256, 0, st>>>(d, n, v);
-  LPF_LAUNCH_CHECK(c);
+  LPF_KLAUNCH(c, KID_MISC, st, k_fill_i32<<<c->n_sm * 4, 256, 0, st>>>(d, n, v));
   return LPF_OK;
 }

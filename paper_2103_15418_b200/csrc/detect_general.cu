@@ -152,13 +152,13 @@ int launch_sepconv(lpf_ctx* c, const ConvArgs& a, cudaStream_t st) {
   const int R = a.g.R;
   const dim3 grid((a.Dx + TX - 1) / TX, (a.Dy + TY - 1) / TY, a.n_planes);
   const size_t smem = (size_t)((TY + 2 * R) * (((TX + 2 * R) | 1) + (TX + 1))) * sizeof(float);
+  const int kid = MODE == MODE_MF ? KID_CONV_MF : MODE == MODE_C ? KID_CONV_C : MODE == MODE_S ? KID_CONV_S : KID_CONV_DEN;
   switch (R) {
-    case 3: k_sepconv<MODE, 3><<<grid, CT, smem, st>>>(a); break;
-    case 12: k_sepconv<MODE, 12><<<grid, CT, smem, st>>>(a); break;
-    case 16: k_sepconv<MODE, 16><<<grid, CT, smem, st>>>(a); break;
-    default: k_sepconv<MODE, 0><<<grid, CT, smem, st>>>(a); break;
+    case 3: LPF_KLAUNCH(c, kid, st, k_sepconv<MODE, 3><<<grid, CT, smem, st>>>(a)); break;
+    case 12: LPF_KLAUNCH(c, kid, st, k_sepconv<MODE, 12><<<grid, CT, smem, st>>>(a)); break;
+    case 16: LPF_KLAUNCH(c, kid, st, k_sepconv<MODE, 16><<<grid, CT, smem, st>>>(a)); break;
+    default: LPF_KLAUNCH(c, kid, st, k_sepconv<MODE, 0><<<grid, CT, smem, st>>>(a)); break;
   }
-  LPF_LAUNCH_CHECK(c);
   return LPF_OK;
 }
 
@@ -249,14 +249,11 @@ k_threshold_peaks(const ThrArgs a) {
   }
 }
 
-__global__ void k_zero_i32(int32_t* p) { *p = 0; }
-
 }  // namespace
 
 int lpf_launch_sum_plane(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, cudaStream_t st) {
   const int blocks = c->n_sm * 8;
-  k_sum_plane<<<blocks, 256, 0, st>>>(d_cube, d_band_ok, c->p.B, c->N, L.sum_plane);
-  LPF_LAUNCH_CHECK(c);
+  LPF_KLAUNCH(c, KID_SUM_PLANE, st, k_sum_plane<<<blocks, 256, 0, st>>>(d_cube, d_band_ok, c->p.B, c->N, L.sum_plane));
   return LPF_OK;
 }
 
@@ -272,8 +269,7 @@ int lpf_launch_detect_general(lpf_ctx* c, LpfLane& L, const float* d_cube, const
                               lpf_det* d_dets, int32_t* d_ndets, cudaStream_t st) {
   const lpf_params& p = c->p;
   int rc;
-  k_zero_i32<<<1, 1, 0, st>>>(d_ndets);
-  LPF_LAUNCH_CHECK(c);
+  LPF_CUDA(cudaMemsetAsync(d_ndets, 0, sizeof(int32_t), st));
   if (p.detect_sum_plane) { rc = lpf_launch_sum_plane(c, L, d_cube, d_band_ok, st); if (rc) return rc; }
   if (p.n_iter > 1) LPF_CUDA(cudaMemsetAsync(L.Y, 0, (size_t)c->n_planes * c->N, st));
 
@@ -305,8 +301,7 @@ int lpf_launch_detect_general(lpf_ctx* c, LpfLane& L, const float* d_cube, const
     t.kappa2 = p.kappa * p.kappa; t.eps_rel = p.eps_rel;
     t.dets = d_dets; t.ndets = d_ndets; t.counters = c->counters;
     const dim3 grid((unsigned)((c->N + 255) / 256), 1, c->n_planes);
-    k_threshold_peaks<<<grid, 256, 0, st>>>(t);
-    LPF_LAUNCH_CHECK(c);
+    LPF_KLAUNCH(c, KID_THRESHOLD, st, k_threshold_peaks<<<grid, 256, 0, st>>>(t));
   }
   return LPF_OK;
 }

@@ -15,6 +15,24 @@ int lpf_cuda_fail(cudaError_t e, const char* what) {
   return LPF_E_CUDA;
 }
 
+static cudaEvent_t prof_event(lpf_ctx* c) {
+  if (c->prof_pool_used == c->prof_pool.size()) {
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    c->prof_pool.push_back(e);
+  }
+  return c->prof_pool[c->prof_pool_used++];
+}
+
+void lpf_prof_pre(lpf_ctx* c, int kid, cudaStream_t st) {
+  lpf_ctx::ProfRec r;
+  r.kid = kid; r.e0 = prof_event(c); r.e1 = prof_event(c);
+  cudaEventRecord(r.e0, st);
+  c->prof_recs.push_back(r);
+}
+
+void lpf_prof_post(lpf_ctx* c, cudaStream_t st) { cudaEventRecord(c->prof_recs.back().e1, st); }
+
 namespace {
 
 // eq. 2 taps, R1: g_i = exp(-i^2 / 2 s^2) / sum ; uniform: 1/(2k+1) ; s <= 0: identity.
@@ -188,6 +206,7 @@ int lpf_destroy(lpf_ctx* c) {
                   c->slotmap, c->free_list, c->ring, c->meta_t, c->meta_ok, c->counters};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (c->chain_ev) cudaEventDestroy(c->chain_ev);
+  for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
   delete c;
   return LPF_OK;
 }
@@ -310,6 +329,38 @@ int lpf_get_counters(lpf_ctx* c, int64_t* h_out) {
   h_out[0] = h[0]; h_out[1] = h[1]; h_out[2] = c->launches; h_out[3] = h[2];
   return LPF_OK;
 }
+
+static const char* const kKernelNames[KID_COUNT] = {
+    "qc_pass1", "qc_pass2", "qc_verdict", "sum_plane", "conv_mf", "conv_c", "conv_s", "conv_den", "threshold_peaks",
+    "fused_detect", "dedupe_scatter", "dedupe_select", "dedupe_sort", "assoc_match", "assoc_update", "measure_flux",
+    "append_dynspec", "misc"};
+
+int lpf_profile_begin(lpf_ctx* c) {
+  if (!c) return LPF_E_ARG;
+  LPF_CUDA(cudaDeviceSynchronize());
+  c->prof_recs.clear();
+  c->prof_pool_used = 0;
+  c->prof_on = true;
+  return LPF_OK;
+}
+
+int lpf_profile_end(lpf_ctx* c, int32_t* h_count, float* h_ms, int32_t n) {
+  if (!c || !h_count || !h_ms || n < KID_COUNT) return LPF_E_ARG;
+  c->prof_on = false;
+  LPF_CUDA(cudaDeviceSynchronize());
+  for (int i = 0; i < n; ++i) { h_count[i] = 0; h_ms[i] = 0.f; }
+  for (const auto& r : c->prof_recs) {
+    float ms = 0.f;
+    LPF_CUDA(cudaEventElapsedTime(&ms, r.e0, r.e1));
+    h_count[r.kid] += 1; h_ms[r.kid] += ms;
+  }
+  c->prof_recs.clear();
+  c->prof_pool_used = 0;
+  return LPF_OK;
+}
+
+int lpf_profile_kernel_count(void) { return KID_COUNT; }
+const char* lpf_profile_kernel_name(int kid) { return (kid >= 0 && kid < KID_COUNT) ? kKernelNames[kid] : ""; }
 
 int lpf_memcpy_d2h(void* h_dst, const void* d_src, int64_t bytes) {
   if (bytes < 0 || (bytes > 0 && (!h_dst || !d_src))) return LPF_E_ARG;

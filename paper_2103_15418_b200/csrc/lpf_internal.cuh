@@ -75,6 +75,12 @@ struct lpf_ctx {
   bool chain_valid = false;
   int64_t launches = 0;
   std::vector<LpfLane> lanes;
+  // per-kernel profile
+  bool prof_on = false;
+  struct ProfRec { int kid; cudaEvent_t e0, e1; };
+  std::vector<ProfRec> prof_recs;
+  std::vector<cudaEvent_t> prof_pool;
+  size_t prof_pool_used = 0;
 };
 
 extern thread_local char g_lpf_cuda_err[256];
@@ -86,11 +92,24 @@ int lpf_cuda_fail(cudaError_t e, const char* what);
     if (e__ != cudaSuccess) return lpf_cuda_fail(e__, #call); \
   } while (0)
 
-#define LPF_LAUNCH_CHECK(ctx)                                     \
+// Kernel ids for the optional per-kernel CUDA-event profile (lpf_profile_begin / lpf_profile_end).
+enum LpfKernelId {
+  KID_QC_PASS1 = 0, KID_QC_PASS2, KID_QC_VERDICT, KID_SUM_PLANE, KID_CONV_MF, KID_CONV_C, KID_CONV_S,
+  KID_CONV_DEN, KID_THRESHOLD, KID_FUSED_DETECT, KID_DEDUPE_SCATTER, KID_DEDUPE_SELECT, KID_DEDUPE_SORT,
+  KID_ASSOC_MATCH, KID_ASSOC_UPDATE, KID_MEASURE_FLUX, KID_APPEND, KID_MISC, KID_COUNT
+};
+void lpf_prof_pre(lpf_ctx* c, int kid, cudaStream_t st);
+void lpf_prof_post(lpf_ctx* c, cudaStream_t st);
+
+// Launch `...` (a kernel<<<>>>() expression) on stream st, count it, bracket it with events when profiling.
+#define LPF_KLAUNCH(ctx, kid, st, ...)                             \
   do {                                                            \
+    if ((ctx)->prof_on) lpf_prof_pre((ctx), (kid), (st));         \
+    __VA_ARGS__;                                                  \
+    if ((ctx)->prof_on) lpf_prof_post((ctx), (st));               \
     (ctx)->launches++;                                            \
     cudaError_t e__ = cudaPeekAtLastError();                      \
-    if (e__ != cudaSuccess) return lpf_cuda_fail(e__, "launch");  \
+    if (e__ != cudaSuccess) return lpf_cuda_fail(e__, #kid);      \
   } while (0)
 
 // ---- launchers implemented in the kernel translation units ---------------------------------

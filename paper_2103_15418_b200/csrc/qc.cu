@@ -189,11 +189,11 @@ k_qc_verdict(const float* __restrict__ cube, long long N, int first_valid, int B
 
 int lpf_launch_qc(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, cudaStream_t st) {
   const dim3 grid(c->qc_nblk, c->p.B);
-  k_qc_moments<false><<<grid, QC_THREADS, 0, st>>>(d_cube, c->W, c->N, c->first_valid, c->qc_nblk, nullptr, 0.f, L.qc_part1);
-  LPF_LAUNCH_CHECK(c);
-  k_qc_moments<true><<<grid, QC_THREADS, 0, st>>>(d_cube, c->W, c->N, c->first_valid, c->qc_nblk, L.qc_part1, c->p.qc_clip, L.qc_part2);
-  LPF_LAUNCH_CHECK(c);
-  k_qc_verdict<<<1, 64, 0, st>>>(d_cube, c->N, c->first_valid, c->p.B, c->qc_nblk, L.qc_part1, L.qc_part2, c->p.qc_tau, d_stats, d_band_ok);
-  LPF_LAUNCH_CHECK(c);
+  LPF_KLAUNCH(c, KID_QC_PASS1, st, k_qc_moments<false><<<grid, QC_THREADS, 0, st>>>(
+      d_cube, c->W, c->N, c->first_valid, c->qc_nblk, nullptr, 0.f, L.qc_part1));
+  LPF_KLAUNCH(c, KID_QC_PASS2, st, k_qc_moments<true><<<grid, QC_THREADS, 0, st>>>(
+      d_cube, c->W, c->N, c->first_valid, c->qc_nblk, L.qc_part1, c->p.qc_clip, L.qc_part2));
+  LPF_KLAUNCH(c, KID_QC_VERDICT, st, k_qc_verdict<<<1, 64, 0, st>>>(
+      d_cube, c->N, c->first_valid, c->p.B, c->qc_nblk, L.qc_part1, L.qc_part2, c->p.qc_tau, d_stats, d_band_ok));
   return LPF_OK;
 }
