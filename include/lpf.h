@@ -187,6 +187,13 @@ int lpf_process_frame_host(lpf_ctx* ctx, int lane, const float* h_cube, int64_t 
  * h_out[2] = kernels launched by this context so far, h_out[3] = active candidates.  Synchronises. */
 int lpf_get_counters(lpf_ctx* ctx, int64_t* h_out);
 
+/* Launch plan chosen at lpf_create: h_out[0] = 1 if the fused single-pass detection kernel is in use
+ * (box K = 12, k_mf = 3, n_iter = 1, Dx % 4 == 0; otherwise the general multi-kernel path),
+ * [1] strip width in columns, [2] threads per CTA, [3] CTAs per plane, [4] dynamic shared memory
+ * bytes per CTA, [5] planes, [6] SMs, [7] QC blocks per band.  Setting the environment variable
+ * LPF_FORCE_GENERAL=1 before lpf_create selects the general path (used by the parity tests). */
+int lpf_get_plan(lpf_ctx* ctx, int64_t* h_out);
+
 /* Optional per-kernel timing with CUDA events recorded on the launching stream, around every kernel
  * this context launches between lpf_profile_begin and lpf_profile_end (both synchronise).
  * h_count[k] / h_ms[k]: launches and summed milliseconds of kernel id k, n >= lpf_profile_kernel_count().

@@ -54,7 +54,7 @@ EXPORTS = [
     "lpf_create", "lpf_destroy", "lpf_cube_qc", "lpf_detect_sources", "lpf_associate", "lpf_add_candidates",
     "lpf_measure_flux", "lpf_append_dynspec", "lpf_get_dynspec", "lpf_process_frame", "lpf_get_frame_view",
     "lpf_process_frame_host", "lpf_get_counters", "lpf_memcpy_d2h", "lpf_strerror", "lpf_last_cuda_error",
-    "lpf_version", "lpf_profile_begin", "lpf_profile_end", "lpf_profile_kernel_count", "lpf_profile_kernel_name",
+    "lpf_version", "lpf_get_plan", "lpf_profile_begin", "lpf_profile_end", "lpf_profile_kernel_count", "lpf_profile_kernel_name",
 ]
 
 
@@ -90,6 +90,7 @@ def load_library(path: Optional[str] = None):
     lib.lpf_strerror.argtypes = [C.c_int]
     lib.lpf_strerror.restype = C.c_char_p
     lib.lpf_last_cuda_error.restype = C.c_char_p
+    lib.lpf_get_plan.argtypes = [vp, C.POINTER(i64)]
     lib.lpf_profile_begin.argtypes = [vp]
     lib.lpf_profile_end.argtypes = [vp, vp, vp, i32]
     lib.lpf_profile_kernel_name.argtypes = [C.c_int]
@@ -249,6 +250,12 @@ class LPF:
         _check(self.lib, self.lib.lpf_process_frame_host(self.h, lane, ptr, t, C.byref(res.c), _stream(stream)),
                "lpf_process_frame_host")
         return res
+
+    def plan(self) -> dict:
+        h = (C.c_int64 * 8)()
+        _check(self.lib, self.lib.lpf_get_plan(self.h, h), "lpf_get_plan")
+        return dict(fused=bool(h[0]), strip_cols=int(h[1]), threads=int(h[2]), ctas_per_plane=int(h[3]),
+                    smem_bytes=int(h[4]), planes=int(h[5]), sms=int(h[6]), qc_blocks_per_band=int(h[7]))
 
     def profile_begin(self):
         _check(self.lib, self.lib.lpf_profile_begin(self.h), "lpf_profile_begin")

@@ -120,6 +120,17 @@ void free_lane(LpfLane& L) {
   L = LpfLane();
 }
 
+}  // namespace
+
+// S3-S8 dispatch: the fused sweep kernel when the parameter set allows it, else the general path.
+int lpf_launch_detect(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, lpf_det* d_dets,
+                      int32_t* d_ndets, cudaStream_t st) {
+  if (c->fused) return lpf_launch_detect_fused(c, c->fused, L, d_cube, d_band_ok, d_dets, d_ndets, st);
+  return lpf_launch_detect_general(c, L, d_cube, d_band_ok, d_dets, d_ndets, st);
+}
+
+namespace {
+
 int lane_ok(lpf_ctx* c, int lane) { return (c && lane >= 0 && lane < (int)c->lanes.size()) ? LPF_OK : LPF_E_ARG; }
 
 }  // namespace
@@ -165,6 +176,7 @@ int lpf_create(lpf_ctx** out, const lpf_params* p, const uint8_t* d_valid_mask) 
     bool dirty = false;
     for (size_t i = 0; i < N; ++i) if (hW[i] > 1) { hW[i] = 1; dirty = true; }
     if (dirty) CUDAC(cudaMemcpy(c->W, hW.data(), N, cudaMemcpyHostToDevice));
+    TRYC(lpf_fused_plan(c, hW.data(), &c->fused));
   }
   TRYC(dalloc(&c->norm_mf, N));
   TRYC(dalloc(&c->norm_bg, N));
@@ -206,6 +218,7 @@ int lpf_destroy(lpf_ctx* c) {
                   c->slotmap, c->free_list, c->ring, c->meta_t, c->meta_ok, c->counters};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (c->chain_ev) cudaEventDestroy(c->chain_ev);
+  lpf_fused_plan_free(c->fused);
   for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
   delete c;
   return LPF_OK;
@@ -224,7 +237,7 @@ int lpf_detect_sources(lpf_ctx* c, int lane, const float* d_cube, const uint8_t*
   if (!d_cube || !d_band_ok || !d_dets || !d_ndets || !d_upos || !d_uplane || !d_usnr || !d_nu) return LPF_E_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   LpfLane& L = c->lanes[lane];
-  TRY(lpf_launch_detect_general(c, L, d_cube, d_band_ok, d_dets, d_ndets, st));
+  TRY(lpf_launch_detect(c, L, d_cube, d_band_ok, d_dets, d_ndets, st));
   return lpf_launch_dedupe(c, L, d_dets, d_ndets, d_upos, d_uplane, d_usnr, d_nu, st);
 }
 
@@ -266,7 +279,7 @@ int lpf_process_frame(lpf_ctx* c, int lane, const float* d_cube, int64_t t, void
   cudaStream_t st = (cudaStream_t)stream;
   LpfLane& L = c->lanes[lane];
   TRY(lpf_launch_qc(c, L, d_cube, L.stats, L.band_ok, st));
-  TRY(lpf_launch_detect_general(c, L, d_cube, L.band_ok, L.dets, L.ndets, st));
+  TRY(lpf_launch_detect(c, L, d_cube, L.band_ok, L.dets, L.ndets, st));
   TRY(lpf_launch_dedupe(c, L, L.dets, L.ndets, L.upos, L.uplane, L.usnr, L.nu, st));
   // the candidate table and the rings are shared by all lanes: order the chain across streams
   if (c->chain_valid) LPF_CUDA(cudaStreamWaitEvent(st, c->chain_ev, 0));
@@ -356,6 +369,14 @@ int lpf_profile_end(lpf_ctx* c, int32_t* h_count, float* h_ms, int32_t n) {
   }
   c->prof_recs.clear();
   c->prof_pool_used = 0;
+  return LPF_OK;
+}
+
+int lpf_get_plan(lpf_ctx* c, int64_t* h_out) {
+  if (!c || !h_out) return LPF_E_ARG;
+  int cw = 0, th = 0, ni = 0; long long sm = 0;
+  h_out[0] = lpf_fused_plan_info(c->fused, &cw, &th, &ni, &sm);
+  h_out[1] = cw; h_out[2] = th; h_out[3] = ni; h_out[4] = sm; h_out[5] = c->n_planes; h_out[6] = c->n_sm; h_out[7] = c->qc_nblk;
   return LPF_OK;
 }
 

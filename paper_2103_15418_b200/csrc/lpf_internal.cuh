@@ -47,7 +47,10 @@ struct LpfLane {
   int32_t* h_counts = nullptr; // pinned [4]
 };
 
+struct LpfFusedPlan;  // detect_fused.cu
+
 struct lpf_ctx {
+  LpfFusedPlan* fused = nullptr;  // non-null: the fused fast path serves lpf_detect_sources
   lpf_params p;
   int64_t N;        // Dy*Dx
   int n_planes;     // B + detect_sum_plane
@@ -118,6 +121,13 @@ int lpf_launch_qc(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, u
 int lpf_launch_sum_plane(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, cudaStream_t st);
 int lpf_launch_detect_general(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok,
                               lpf_det* d_dets, int32_t* d_ndets, cudaStream_t st);
+int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out);
+void lpf_fused_plan_free(LpfFusedPlan* pl);
+int lpf_fused_plan_info(const LpfFusedPlan* pl, int* cw, int* threads, int* n_items, long long* smem);
+int lpf_launch_detect_fused(lpf_ctx* c, LpfFusedPlan* pl, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok,
+                            lpf_det* d_dets, int32_t* d_ndets, cudaStream_t st);
+int lpf_launch_detect(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, lpf_det* d_dets,
+                      int32_t* d_ndets, cudaStream_t st);
 int lpf_launch_static_norm(lpf_ctx* c, const LpfTaps& g, float* d_norm, float* d_tmp, cudaStream_t st);
 
 int lpf_launch_dedupe(lpf_ctx* c, LpfLane& L, const lpf_det* d_dets, const int32_t* d_ndets, int32_t* d_upos,

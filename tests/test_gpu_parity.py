@@ -18,12 +18,22 @@ def torch_cuda():
 
 
 def _make(cfg, torch, **kw):
+    """Context for a config.  general=True forces the multi-kernel general path (LPF_FORCE_GENERAL);
+    otherwise box/K=12/n_iter=1 contexts take the fused single-pass kernel."""
+    import os
     from paper_2103_15418_b200.binding import LPF
     s = synth.CubeStream(cfg)
-    bg = kw.pop("bg", "box"); n_iter = kw.pop("n_iter", 1)
+    bg = kw.pop("bg", "box"); n_iter = kw.pop("n_iter", 1); general = kw.pop("general", False)
     p = synth.default_params(cfg, bg=bg, n_iter=n_iter)
     p.update(kw)
-    return s, p, LPF(p, s.mask)
+    os.environ["LPF_FORCE_GENERAL"] = "1" if general else "0"
+    try:
+        lpf = LPF(p, s.mask)
+    finally:
+        os.environ["LPF_FORCE_GENERAL"] = "0"
+    want_fused = (not general) and bg == "box" and n_iter == 1 and p["k_bg"] == 12 and p["k_mf"] == 3
+    assert lpf.plan()["fused"] == want_fused, lpf.plan()
+    return s, p, lpf
 
 
 def _run_chain(torch, s, p, lpf, frames, direct=False, via="calls", tag=""):
@@ -45,9 +55,10 @@ def _run_chain(torch, s, p, lpf, frames, direct=False, via="calls", tag=""):
 
 
 # ------------------------------------------------------------------ config 1
-@pytest.mark.parametrize("bg,n_iter", [("box", 1), ("gauss", 1), ("box", 3), ("gauss", 3)])
-def test_config1_all_frames(torch_cuda, bg, n_iter):
-    s, p, lpf = _make(1, torch_cuda, bg=bg, n_iter=n_iter)
+@pytest.mark.parametrize("bg,n_iter,general", [("box", 1, False), ("box", 1, True), ("gauss", 1, True), ("box", 3, True),
+                                               ("gauss", 3, True)])
+def test_config1_all_frames(torch_cuda, bg, n_iter, general):
+    s, p, lpf = _make(1, torch_cuda, bg=bg, n_iter=n_iter, general=general)
     pipe, wz, ties = _run_chain(torch_cuda, s, p, lpf, range(32), direct=True, via="calls", tag=f"cfg1 {bg} it{n_iter}")
     assert ties == 0
     # dynamic spectrum of the source's candidate: bit-exact, time ordered
@@ -79,9 +90,9 @@ def test_config2_chain_box(torch_cuda):
     lpf.close()
 
 
-@pytest.mark.parametrize("bg,n_iter", [("gauss", 1), ("box", 3), ("gauss", 3)])
+@pytest.mark.parametrize("bg,n_iter", [("box", 1), ("gauss", 1), ("box", 3), ("gauss", 3)])
 def test_config2_variants(torch_cuda, bg, n_iter):
-    s, p, lpf = _make(2, torch_cuda, bg=bg, n_iter=n_iter)
+    s, p, lpf = _make(2, torch_cuda, bg=bg, n_iter=n_iter, general=True)
     _run_chain(torch_cuda, s, p, lpf, range(4), via="calls", tag=f"cfg2 {bg} it{n_iter}")
     lpf.close()
 
@@ -113,9 +124,10 @@ def test_config3_frames_with_rfi(torch_cuda):
     lpf.close()
 
 
-def test_config3_gauss_one_frame(torch_cuda):
-    s, p, lpf = _make(3, torch_cuda, bg="gauss")
-    _run_chain(torch_cuda, s, p, lpf, [0], via="frame", tag="cfg3 gauss")
+@pytest.mark.parametrize("bg", ["gauss", "box"])
+def test_config3_general_path_one_frame(torch_cuda, bg):
+    s, p, lpf = _make(3, torch_cuda, bg=bg, general=True)
+    _run_chain(torch_cuda, s, p, lpf, [0], via="frame", tag=f"cfg3 general {bg}")
     lpf.close()
 
 
