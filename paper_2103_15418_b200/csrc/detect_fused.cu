@@ -19,6 +19,7 @@
 // F, C, d and S never leave the SM.  The dependent double stencil costs 27 warm-up rows per
 // segment and no redundant columns when the strip spans the valid width of the image.
 #include <algorithm>
+#include <cstdio>
 #include <cstdlib>
 
 #include "lpf_internal.cuh"
@@ -205,6 +206,11 @@ k_fused_box(const FusedArgs a) {
       const float dv[4] = {d4.x, d4.y, d4.z, d4.w};
       const float sv[4] = {bx[0] * ic.x, bx[1] * ic.y, bx[2] * ic.z, bx[3] * ic.w};
       unsigned pass = 0;
+#ifdef LPF_DEBUG_FUSED
+      if (p == 0 && sg == 20 && x == 36)
+        printf("dbg sg=%d x=%d d=%g %g %g %g  s=%g %g %g %g ic=%g bx=%g V2=%g f(sigma)=%g wF=%d wD=%d\n", sg, x, dv[0], dv[1], dv[2], dv[3],
+               sv[0], sv[1], sv[2], sv[3], ic.y, bx[1], V2[1], ringF[wrap_add(wrap_add(wF, j, DF), DF - 2 * KBG, DF) * CW + (x + 1 - it.xs)], wF, wD);
+#endif
 #pragma unroll
       for (int k = 0; k < 4; ++k)
         if (dv[k] > 0.f && dv[k] * dv[k] > a.kappa2 * sv[k] && (x + k) >= it.ux0 && (x + k) < it.ux1) pass |= (1u << k);
@@ -261,6 +267,7 @@ struct LpfFusedPlan {
   int CW = 0, threads = 0, n_items = 0;
   size_t smem = 0;
   FusedItem* d_items = nullptr;
+  float* d_inv_cnt = nullptr;
 };
 
 static size_t fused_smem_bytes(int CW) {
@@ -337,6 +344,15 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
   LpfFusedPlan* pl = new LpfFusedPlan();
   pl->CW = CW; pl->threads = CW / 4; pl->n_items = (int)items.size(); pl->smem = fused_smem_bytes(CW);
   if (pl->threads > 256) { delete pl; return LPF_OK; }
+  // 1 / (number of valid pixels in the 25x25 window), 0 at invalid pixels: box taps of 1 give exact counts
+  LPF_CUDA(cudaMalloc((void**)&pl->d_inv_cnt, (size_t)c->N * sizeof(float)));
+  {
+    LpfTaps ones;
+    ones.R = KBG;
+    for (int i = 0; i < LPF_NTAPS; ++i) ones.g[i] = i < WINB ? 1.f : 0.f;
+    int rc = lpf_launch_static_norm(c, ones, pl->d_inv_cnt, nullptr, 0);
+    if (rc) return rc;
+  }
   LPF_CUDA(cudaMalloc((void**)&pl->d_items, items.size() * sizeof(FusedItem)));
   LPF_CUDA(cudaMemcpy(pl->d_items, items.data(), items.size() * sizeof(FusedItem), cudaMemcpyHostToDevice));
   LPF_CUDA(cudaFuncSetAttribute(k_fused_box, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem));
@@ -348,6 +364,7 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
 void lpf_fused_plan_free(LpfFusedPlan* pl) {
   if (!pl) return;
   if (pl->d_items) cudaFree(pl->d_items);
+  if (pl->d_inv_cnt) cudaFree(pl->d_inv_cnt);
   delete pl;
 }
 
@@ -364,7 +381,7 @@ int lpf_launch_detect_fused(lpf_ctx* c, LpfFusedPlan* pl, LpfLane& L, const floa
   if (p.detect_sum_plane) { int rc = lpf_launch_sum_plane(c, L, d_cube, d_band_ok, st); if (rc) return rc; }
   FusedArgs a{};
   a.cube = d_cube; a.sum_plane = L.sum_plane; a.band_ok = d_band_ok; a.W = c->W;
-  a.norm_mf = c->norm_mf; a.inv_cnt = c->norm_bg; a.items = pl->d_items;
+  a.norm_mf = c->norm_mf; a.inv_cnt = pl->d_inv_cnt; a.items = pl->d_items;
   a.B = p.B; a.Dy = p.Dy; a.Dx = p.Dx; a.CW = pl->CW; a.k_max = p.k_max; a.max_det = p.max_det;
   a.g0 = c->g_mf.g[3]; a.g1 = c->g_mf.g[2]; a.g2 = c->g_mf.g[1]; a.g3 = c->g_mf.g[0];
   a.kappa2 = p.kappa * p.kappa; a.eps_rel = p.eps_rel;
