@@ -196,9 +196,13 @@ def run_ours(args):
     clocks = sampler.stop(ts0, max(ts1, ts1b))
 
     # per-kernel CUDA-event profile over the same step mix -> roofline of the dominant kernel
+    # (one lane, one stream: each kernel runs alone, so its events bracket only its own execution)
     kp = min(args.steps, 200)
+    torch.cuda.synchronize()
     lpf.profile_begin()
-    run_steps(t_next, kp); t_next += kp
+    for i in range(kp):
+        lpf.process_frame(pool_d[(t_next + i) % n_pool], t_next + i, lane=0, stream=streams[0])
+    t_next += kp
     prof = lpf.profile_end()
     kernels = {k: {"launches_per_step": c / kp, "us_per_launch": 1e3 * tm / c, "us_per_step": 1e3 * tm / kp}
                for k, (c, tm) in prof.items()}

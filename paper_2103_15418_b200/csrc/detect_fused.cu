@@ -3,10 +3,10 @@
 // (box background K = 12, Gaussian matched filter k_mf = 3, n_iter = 1).
 // (eqs. 2-7; O3-O6 and "Fused detection kernel".)
 //
-// Design (sm_100a): a CTA owns a column strip (as wide as shared memory allows: the two 26-row
-// ring buffers of a whole 922-column all-sky strip fit the 227 KB of one SM) and sweeps down a
-// segment of rows.  Each thread owns 4 adjacent columns and RB rows per iteration:
-//   A  128-bit global loads of X (masked by W)                                   [HBM/L2]
+// Design (sm_100a): a CTA owns a column strip (as wide as shared memory allows: the two ring
+// buffers of a whole 922-column all-sky strip fill the 227 KB of one SM) and sweeps down a
+// segment of rows.  Each thread owns 4 adjacent columns and RBF rows per iteration:
+//   A  128-bit global loads of X (masked by W), issued one iteration ahead            [HBM/L2]
 //   B  horizontal 7-tap matched filter (neighbour groups through shared memory)
 //   C  vertical 7-tap matched filter on a register window, x norm_mf  -> F
 //   D  vertical 25-row running sum of F (ring buffer of F rows in shared memory)
@@ -14,10 +14,10 @@
 //   F  d = F - C (F re-read from the ring at lag 12)
 //   G  vertical 25-row running sum of d^2 (ring buffer of d rows)
 //   H  horizontal 25-box, x 1/count                                             -> S   (eq. 4)
-//   I  eq. 5 on d at lag 12; only pixels that pass take the slow path: S_eff guard, eq. 6
-//      local-maximum test on the F ring, eq. 7 record with a warp-aggregated atomic.
-// F, C, d and S never leave the SM.  The dependent double stencil costs 27 warm-up rows per
-// segment and no redundant columns when the strip spans the valid width of the image.
+//   I  eq. 5 on d at lag 12; pixels that pass take the side path: S_eff guard, eq. 6
+//      local-maximum test on the F ring (early exit), eq. 7 record.
+// F, C, d and S never leave the SM.  Stages E-G / H-I are skipped while the pipeline warms up
+// (27 + 27 rows per segment); no redundant columns when the strip spans the valid width.
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
@@ -29,6 +29,7 @@ namespace {
 constexpr int RBF = 2;         // rows per iteration
 constexpr int KBG = 12;        // box half width
 constexpr int WINB = 2 * KBG + 1;
+constexpr int HALO = 2 * KBG + 3;   // rows of X above the first output row
 constexpr int DF = WINB + 1 + RBF;  // F ring depth: lag 25 (running sum) .. lag 26 (local max) + rows in flight
 constexpr int DD = WINB + 1;        // d ring depth
 
@@ -45,10 +46,10 @@ struct FusedArgs {
 __device__ __forceinline__ float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
 __device__ __forceinline__ void st4(float* p, const float4 v) { *reinterpret_cast<float4*>(p) = v; }
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
-
+__device__ __forceinline__ float4 zero4() { return make_float4(0.f, 0.f, 0.f, 0.f); }
 __device__ __forceinline__ int wrap_add(int a, int b, int m) { const int s = a + b; return s >= m ? s - m : s; }
 
-// horizontal 25-box of one row of per-column values held 4 per thread (own = v, group sum = t)
+// horizontal 25-box of one row of per-column values held 4 per thread (group sum of own = t)
 __device__ __forceinline__ void hbox25(const float* EVrow, const float* ETrow, int tid, float t, float out[4]) {
   const float tm2 = ETrow[tid], tm1 = ETrow[tid + 1], tp1 = ETrow[tid + 3], tp2 = ETrow[tid + 4];
   const float4 L = ld4(EVrow + 4 * tid);        // group q-3
@@ -59,6 +60,43 @@ __device__ __forceinline__ void hbox25(const float* EVrow, const float* ETrow, i
   out[1] = out[0] + (R.y - L.x);
   out[2] = out[1] + (R.z - L.y);
   out[3] = out[2] + (R.w - L.z);
+}
+
+// Side path for one pixel that passed eq. 5 without the guard: guard (R8), eq. 6 on the F ring, eq. 7.
+// Masked pixels hold F = 0 in the ring, so W is consulted only when such a zero would win.
+__device__ __noinline__ void fused_candidate(const FusedArgs& a, const FusedItem& it, const float* ringF, int CW,
+                                             int slot_sigma, int sg, int xx, float d, float s, int plane) {
+  const int cl = xx - it.xs;
+  const float fv = ringF[slot_sigma * CW + cl];
+  const float cc = fv - d;
+  const float gd = a.eps_rel * fabsf(cc);
+  const float se = fmaxf(s, gd * gd);
+  if (!(d * d > a.kappa2 * se)) return;
+  const int km = a.k_max;
+  for (int dy = -km; dy <= km; ++dy) {
+    const int yy = sg + dy;
+    if (yy < 0 || yy >= a.Dy) continue;
+    const int ns = (slot_sigma + DF + dy) % DF;
+    const float* row = ringF + ns * CW;
+    for (int dx = -km; dx <= km; ++dx) {
+      const int c2 = cl + dx;
+      if (c2 < 0 || c2 >= CW) continue;
+      const float fn = row[c2];
+      if (fn > fv) {
+        const int xn = xx + dx;
+        if (xn >= 0 && xn < a.Dx && a.W[(long long)yy * a.Dx + xn]) return;  // a valid neighbour is larger
+      }
+    }
+  }
+  const int idx = atomicAdd(a.ndets, 1);
+  if (idx < a.max_det) {
+    lpf_det r;
+    r.pix = sg * a.Dx + xx; r.plane = (int16_t)plane; r.iter = 1;
+    r.f = fv; r.c = cc; r.s = se; r.snr = d / sqrtf(se);
+    a.dets[idx] = r;
+  } else {
+    atomicAdd(&a.counters[0], 1);
+  }
 }
 
 __global__ void __launch_bounds__(256, 1)
@@ -78,8 +116,8 @@ k_fused_box(const FusedArgs a) {
   float* EV2 = EV + RBF * PEV;
   float* ET = EV2 + RBF * PEV;
   float* ET2 = ET + RBF * PET;
-  const int total = (DF + DD) * CW + RBF * (PEX + 2 * PEV + 2 * PET);
-  for (int i = tid; i < total; i += blockDim.x) sm[i] = 0.f;
+  const int total4 = ((DF + DD) * CW + RBF * (PEX + 2 * PEV + 2 * PET) + 3) >> 2;
+  for (int i = tid; i < total4; i += blockDim.x) sm4[i] = zero4();
   __syncthreads();
 
   const long long N = (long long)a.Dy * a.Dx;
@@ -95,33 +133,60 @@ k_fused_box(const FusedArgs a) {
     for (int k = 0; k < 4; ++k) hw[i][k] = 0.f;
   float V1[4] = {0.f, 0.f, 0.f, 0.f}, V2[4] = {0.f, 0.f, 0.f, 0.f};
 
-  const int y_start = it.ya - (2 * KBG + 3);
-  const int nb = (it.yb - it.ya + 2 * (2 * KBG + 3) + RBF - 1) / RBF;
+  const int y_start = it.ya - HALO;
+  const int nb = (it.yb - it.ya + 2 * HALO + RBF - 1) / RBF;
+  // first iteration whose rows reach rho >= ya - KBG (stages E-G) / sigma >= ya (stages H-I)
+  const int bE = (HALO + 3 - (RBF - 1)) / RBF;        // rho = y_start + b RBF + j - 15 >= ya - 12
+  const int bH = (2 * HALO - (RBF - 1)) / RBF;        // sigma = y_start + b RBF + j - 27 >= ya
   int wF = 0, wD = 0;  // ring slots of the next F row / next d row
+
+  // prefetch of the first rows
+  float4 xn[RBF]; unsigned wn[RBF];
+#pragma unroll
+  for (int j = 0; j < RBF; ++j) {
+    const int y = y_start + j;
+    xn[j] = zero4(); wn[j] = 0u;
+    if (col_in && y >= 0 && y < a.Dy) {
+      const long long q = (long long)y * a.Dx + x;
+      xn[j] = ldg4(X + q); wn[j] = __ldg(reinterpret_cast<const unsigned*>(a.W + q));
+    }
+  }
 
   for (int b = 0; b < nb; ++b) {
     const int yb0 = y_start + b * RBF;
-    // ---- A: load, mask; B: horizontal matched filter -----------------------------------
+    const bool doE = b >= bE, doH = b >= bH;
+    // ---- A: take the prefetched rows, mask, publish; issue this iteration's global loads -----
     float xm[RBF][4];
 #pragma unroll
     for (int j = 0; j < RBF; ++j) {
-      const int y = yb0 + j;
-      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (col_in && y >= 0 && y < a.Dy) {
-        const long long q = (long long)y * a.Dx + x;
-        v = ldg4(X + q);
-        const unsigned wm = __ldg(reinterpret_cast<const unsigned*>(a.W + q));
-        if (wm != 0x01010101u) {
-          if (!(wm & 0x000000ffu)) v.x = 0.f;
-          if (!(wm & 0x0000ff00u)) v.y = 0.f;
-          if (!(wm & 0x00ff0000u)) v.z = 0.f;
-          if (!(wm & 0xff000000u)) v.w = 0.f;
-        }
+      float4 v = xn[j];
+      const unsigned wm = wn[j];
+      if (wm != 0x01010101u) {
+        if (!(wm & 0x000000ffu)) v.x = 0.f;
+        if (!(wm & 0x0000ff00u)) v.y = 0.f;
+        if (!(wm & 0x00ff0000u)) v.z = 0.f;
+        if (!(wm & 0xff000000u)) v.w = 0.f;
       }
       xm[j][0] = v.x; xm[j][1] = v.y; xm[j][2] = v.z; xm[j][3] = v.w;
       st4(EX + j * PEX + 4 + 4 * tid, v);
     }
+    float4 nm[RBF], icr[RBF], ics[RBF];
+#pragma unroll
+    for (int j = 0; j < RBF; ++j) {
+      const int yn = yb0 + RBF + j, fr = yb0 + j - 3, rho = fr - KBG, sg = rho - KBG;
+      xn[j] = zero4(); wn[j] = 0u; nm[j] = zero4(); icr[j] = zero4(); ics[j] = zero4();
+      if (col_in) {
+        if (yn >= 0 && yn < a.Dy && b + 1 < nb) {
+          const long long q = (long long)yn * a.Dx + x;
+          xn[j] = ldg4(X + q); wn[j] = __ldg(reinterpret_cast<const unsigned*>(a.W + q));
+        }
+        if (fr >= 0 && fr < a.Dy) nm[j] = ldg4(a.norm_mf + (long long)fr * a.Dx + x);
+        if (doE && rho >= 0 && rho < a.Dy) icr[j] = ldg4(a.inv_cnt + (long long)rho * a.Dx + x);
+        if (doH && sg >= it.ya && sg < it.yb) ics[j] = ldg4(a.inv_cnt + (long long)sg * a.Dx + x);
+      }
+    }
     __syncthreads();  // (1)
+    // ---- B: horizontal matched filter ----------------------------------------------------
 #pragma unroll
     for (int j = 0; j < RBF; ++j) {
       const float4 L = ld4(EX + j * PEX + 4 * tid);
@@ -135,10 +200,7 @@ k_fused_box(const FusedArgs a) {
     float f[RBF][4];
 #pragma unroll
     for (int j = 0; j < RBF; ++j) {
-      const int fr = yb0 + j - 3;
-      float4 nm = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (col_in && fr >= 0 && fr < a.Dy) nm = ldg4(a.norm_mf + (long long)fr * a.Dx + x);
-      const float nmv[4] = {nm.x, nm.y, nm.z, nm.w};
+      const float nmv[4] = {nm[j].x, nm[j].y, nm[j].z, nm[j].w};
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
         const float acc = fmaf(g0, hw[j + 3][k], fmaf(g1, hw[j + 2][k] + hw[j + 4][k],
@@ -159,96 +221,62 @@ k_fused_box(const FusedArgs a) {
       const float4 fo = ld4(ringF + os * CW + 4 * tid);
       V1[0] += f[j][0] - fo.x; V1[1] += f[j][1] - fo.y; V1[2] += f[j][2] - fo.z; V1[3] += f[j][3] - fo.w;
       st4(ringF + ws * CW + 4 * tid, make_float4(f[j][0], f[j][1], f[j][2], f[j][3]));
-      st4(EV + j * PEV + 12 + 4 * tid, make_float4(V1[0], V1[1], V1[2], V1[3]));
-      t1[j] = (V1[0] + V1[1]) + (V1[2] + V1[3]);
-      ET[j * PET + 2 + tid] = t1[j];
+      if (doE) {
+        st4(EV + j * PEV + 12 + 4 * tid, make_float4(V1[0], V1[1], V1[2], V1[3]));
+        t1[j] = (V1[0] + V1[1]) + (V1[2] + V1[3]);
+        ET[j * PET + 2 + tid] = t1[j];
+      }
     }
-    __syncthreads();  // (2)
-    // ---- E: C = box / count ; F: d = F - C ; G: running sum of d^2 --------------------------
-    float t2[RBF];
+    if (doE) {
+      __syncthreads();  // (2)
+      // ---- E: C = box / count ; F: d = F - C ; G: running sum of d^2 --------------------------
+      float t2[RBF];
 #pragma unroll
-    for (int j = 0; j < RBF; ++j) {
-      const int rho = yb0 + j - 3 - KBG;
-      float bx[4];
-      hbox25(EV + j * PEV, ET + j * PET, tid, t1[j], bx);
-      float4 ic = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (col_in && rho >= 0 && rho < a.Dy) ic = ldg4(a.inv_cnt + (long long)rho * a.Dx + x);
-      const int ws = wrap_add(wF, j, DF);
-      const int rs = wrap_add(ws, DF - KBG, DF);
-      const float4 fr4 = ld4(ringF + rs * CW + 4 * tid);
-      const float d0 = fr4.x - bx[0] * ic.x, d1 = fr4.y - bx[1] * ic.y, d2 = fr4.z - bx[2] * ic.z, d3 = fr4.w - bx[3] * ic.w;
-      const int wd = wrap_add(wD, j, DD);
-      const int od = wrap_add(wd, DD - WINB, DD);
-      const float4 dold = ld4(ringD + od * CW + 4 * tid);
-      V2[0] = fmaf(-dold.x, dold.x, fmaf(d0, d0, V2[0]));
-      V2[1] = fmaf(-dold.y, dold.y, fmaf(d1, d1, V2[1]));
-      V2[2] = fmaf(-dold.z, dold.z, fmaf(d2, d2, V2[2]));
-      V2[3] = fmaf(-dold.w, dold.w, fmaf(d3, d3, V2[3]));
-      st4(ringD + wd * CW + 4 * tid, make_float4(d0, d1, d2, d3));
-      st4(EV2 + j * PEV + 12 + 4 * tid, make_float4(V2[0], V2[1], V2[2], V2[3]));
-      t2[j] = (V2[0] + V2[1]) + (V2[2] + V2[3]);
-      ET2[j * PET + 2 + tid] = t2[j];
-    }
-    __syncthreads();  // (3)
-    // ---- H: S = box / count ; I: eq. 5 at sigma = rho - 12 -----------------------------------
-#pragma unroll
-    for (int j = 0; j < RBF; ++j) {
-      const int sg = yb0 + j - 3 - 2 * KBG;
-      float bx[4];
-      hbox25(EV2 + j * PEV, ET2 + j * PET, tid, t2[j], bx);
-      const bool row_emit = (sg >= it.ya && sg < it.yb);   // uniform
-      if (!row_emit) continue;
-      float4 ic = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (col_in) ic = ldg4(a.inv_cnt + (long long)sg * a.Dx + x);
-      const int wd = wrap_add(wD, j, DD);
-      const int sd = wrap_add(wd, DD - KBG, DD);
-      const float4 d4 = ld4(ringD + sd * CW + 4 * tid);
-      const float dv[4] = {d4.x, d4.y, d4.z, d4.w};
-      const float sv[4] = {bx[0] * ic.x, bx[1] * ic.y, bx[2] * ic.z, bx[3] * ic.w};
-      unsigned pass = 0;
-#ifdef LPF_DEBUG_FUSED
-      if (p == 0 && sg == 20 && x == 36)
-        printf("dbg sg=%d x=%d d=%g %g %g %g  s=%g %g %g %g ic=%g bx=%g V2=%g f(sigma)=%g wF=%d wD=%d\n", sg, x, dv[0], dv[1], dv[2], dv[3],
-               sv[0], sv[1], sv[2], sv[3], ic.y, bx[1], V2[1], ringF[wrap_add(wrap_add(wF, j, DF), DF - 2 * KBG, DF) * CW + (x + 1 - it.xs)], wF, wD);
-#endif
-#pragma unroll
-      for (int k = 0; k < 4; ++k)
-        if (dv[k] > 0.f && dv[k] * dv[k] > a.kappa2 * sv[k] && (x + k) >= it.ux0 && (x + k) < it.ux1) pass |= (1u << k);
-      if (pass) {   // rare: guard, local maximum, record
+      for (int j = 0; j < RBF; ++j) {
+        float bx[4];
+        hbox25(EV + j * PEV, ET + j * PET, tid, t1[j], bx);
         const int ws = wrap_add(wF, j, DF);
-        for (int k = 0; k < 4; ++k) {
-          if (!(pass & (1u << k))) continue;
-          const int xx = x + k;
-          const float d = dv[k];
-          const int fs = wrap_add(ws, DF - 2 * KBG, DF);
-          const float fv = ringF[fs * CW + (xx - it.xs)];
-          const float cc = fv - d;
-          const float gd = a.eps_rel * fabsf(cc);
-          const float se = fmaxf(sv[k], gd * gd);
-          if (!(d * d > a.kappa2 * se)) continue;
-          if (!a.W[(long long)sg * a.Dx + xx]) continue;
-          bool peak = true;
-          for (int dy = -a.k_max; dy <= a.k_max && peak; ++dy) {
-            const int yy = sg + dy;
-            if (yy < 0 || yy >= a.Dy) continue;
-            const int ns = (ws + 2 * DF - 2 * KBG + dy) % DF;
-            for (int dx = -a.k_max; dx <= a.k_max; ++dx) {
-              const int xn = xx + dx;
-              if (xn < 0 || xn >= a.Dx || !a.W[(long long)yy * a.Dx + xn]) continue;
-              const int cl = xn - it.xs;
-              if (cl < 0 || cl >= CW) continue;
-              if (ringF[ns * CW + cl] > fv) { peak = false; break; }
-            }
-          }
-          if (!peak) continue;
-          const int idx = atomicAdd(a.ndets, 1);
-          if (idx < a.max_det) {
-            lpf_det r;
-            r.pix = sg * a.Dx + xx; r.plane = (int16_t)p; r.iter = 1;
-            r.f = fv; r.c = cc; r.s = se; r.snr = d / sqrtf(se);
-            a.dets[idx] = r;
-          } else {
-            atomicAdd(&a.counters[0], 1);
+        const int rs = wrap_add(ws, DF - KBG, DF);
+        const float4 fr4 = ld4(ringF + rs * CW + 4 * tid);
+        const float d0 = fr4.x - bx[0] * icr[j].x, d1 = fr4.y - bx[1] * icr[j].y;
+        const float d2 = fr4.z - bx[2] * icr[j].z, d3 = fr4.w - bx[3] * icr[j].w;
+        const int wd = wrap_add(wD, j, DD);
+        const int od = wrap_add(wd, DD - WINB, DD);
+        const float4 dold = ld4(ringD + od * CW + 4 * tid);
+        V2[0] = fmaf(-dold.x, dold.x, fmaf(d0, d0, V2[0]));
+        V2[1] = fmaf(-dold.y, dold.y, fmaf(d1, d1, V2[1]));
+        V2[2] = fmaf(-dold.z, dold.z, fmaf(d2, d2, V2[2]));
+        V2[3] = fmaf(-dold.w, dold.w, fmaf(d3, d3, V2[3]));
+        st4(ringD + wd * CW + 4 * tid, make_float4(d0, d1, d2, d3));
+        if (doH) {
+          st4(EV2 + j * PEV + 12 + 4 * tid, make_float4(V2[0], V2[1], V2[2], V2[3]));
+          t2[j] = (V2[0] + V2[1]) + (V2[2] + V2[3]);
+          ET2[j * PET + 2 + tid] = t2[j];
+        }
+      }
+      if (doH) {
+        __syncthreads();  // (3)
+        // ---- H: S = box / count ; I: eq. 5 at sigma = rho - 12 ---------------------------------
+#pragma unroll
+        for (int j = 0; j < RBF; ++j) {
+          const int sg = yb0 + j - 3 - 2 * KBG;
+          if (sg < it.ya || sg >= it.yb) continue;   // uniform
+          float bx[4];
+          hbox25(EV2 + j * PEV, ET2 + j * PET, tid, t2[j], bx);
+          const int wd = wrap_add(wD, j, DD);
+          const int sd = wrap_add(wd, DD - KBG, DD);
+          const float4 d4 = ld4(ringD + sd * CW + 4 * tid);
+          const float s0 = bx[0] * ics[j].x, s1 = bx[1] * ics[j].y, s2 = bx[2] * ics[j].z, s3 = bx[3] * ics[j].w;
+          const bool p0 = d4.x > 0.f && d4.x * d4.x > a.kappa2 * s0 && x >= it.ux0 && x < it.ux1;
+          const bool p1 = d4.y > 0.f && d4.y * d4.y > a.kappa2 * s1 && x + 1 >= it.ux0 && x + 1 < it.ux1;
+          const bool p2 = d4.z > 0.f && d4.z * d4.z > a.kappa2 * s2 && x + 2 >= it.ux0 && x + 2 < it.ux1;
+          const bool p3 = d4.w > 0.f && d4.w * d4.w > a.kappa2 * s3 && x + 3 >= it.ux0 && x + 3 < it.ux1;
+          if (p0 | p1 | p2 | p3) {
+            const int slot_sigma = wrap_add(wrap_add(wF, j, DF), DF - 2 * KBG, DF);
+            if (p0) fused_candidate(a, it, ringF, CW, slot_sigma, sg, x, d4.x, s0, p);
+            if (p1) fused_candidate(a, it, ringF, CW, slot_sigma, sg, x + 1, d4.y, s1, p);
+            if (p2) fused_candidate(a, it, ringF, CW, slot_sigma, sg, x + 2, d4.z, s2, p);
+            if (p3) fused_candidate(a, it, ringF, CW, slot_sigma, sg, x + 3, d4.w, s3, p);
           }
         }
       }
