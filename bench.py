@@ -36,6 +36,31 @@ def env_rank():
     return int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
 
 
+def reduce_over_ranks(ms: float, launches: int, device, world: int):
+    """Multi-rank aggregation of one timed region: the step time is the MAX over ranks (every rank ran the
+    same number of steps on its own stream), the launch count the SUM.  `device` is where the scratch
+    tensors live (the rank's GPU under NCCL, "cpu" under gloo)."""
+    if world <= 1:
+        return float(ms), int(launches)
+    import torch
+    import torch.distributed as dist
+    tms = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+    tl = torch.tensor([launches], device=device, dtype=torch.int64)
+    dist.all_reduce(tl, op=dist.ReduceOp.SUM)
+    return float(tms.item()), int(tl.item())
+
+
+def whole_job_value(world: int, steps: int, ms: float) -> float:
+    """frames/s of the whole job: every rank processed `steps` frames of its own stream in `ms` (max over ranks)."""
+    return world * steps / (ms / 1e3)
+
+
+def rank_seed(rank: int) -> int:
+    """Each rank streams its own seeded sky (weak scaling, no data-path collective)."""
+    return int(rank)
+
+
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -128,7 +153,7 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     cfg = args.config
-    s = synth.CubeStream(cfg, seed=rank)           # every rank: its own independent stream (weak scaling)
+    s = synth.CubeStream(cfg, seed=rank_seed(rank))   # every rank: its own independent stream (weak scaling)
     p = synth.default_params(cfg, bg=args.bg, n_iter=args.n_iter)
     p["n_lanes"] = args.lanes
     B, D = p["B"], p["Dy"]
@@ -178,13 +203,7 @@ def run_ours(args):
     ts1 = sampler.mark()
     ms = ev0.elapsed_time(ev1)
     launches = lpf.counters()["launches"] - l0
-    if world > 1:
-        tms = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-        ms = float(tms.item())
-        tl = torch.tensor([launches], device=dev, dtype=torch.int64)
-        dist.all_reduce(tl, op=dist.ReduceOp.SUM)
-        launches = int(tl.item())
+    ms, launches = reduce_over_ranks(ms, launches, dev, world)
     t_next = args.warmup + args.steps
 
     # keep the GPU under the same load until nvidia-smi has had time to sample it
@@ -222,7 +241,7 @@ def run_ours(args):
                  "algorithmic_bytes": abytes, "algorithmic_flops": aflops, "hbm_gbs": gbs, "hbm_frac": gbs / hbm_peak,
                  "peak_source": peak_src, "alu_peak_source": "148 SM x 128 fp32 lanes x 2 x 1.965 GHz", "traffic": args.traffic})
 
-    frames_s = world * args.steps / (ms / 1e3)
+    frames_s = whole_job_value(world, args.steps, ms)
     step_gbs = cube_bytes * frames_s / 1e9 / world
 
     # end to end through the host entry point: pinned host cube -> H2D -> path -> D2H of the results
