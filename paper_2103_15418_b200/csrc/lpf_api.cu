@@ -176,12 +176,12 @@ int lpf_create(lpf_ctx** out, const lpf_params* p, const uint8_t* d_valid_mask) 
     bool dirty = false;
     for (size_t i = 0; i < N; ++i) if (hW[i] > 1) { hW[i] = 1; dirty = true; }
     if (dirty) CUDAC(cudaMemcpy(c->W, hW.data(), N, cudaMemcpyHostToDevice));
-    TRYC(lpf_fused_plan(c, hW.data(), &c->fused));
+    TRYC(dalloc(&c->norm_mf, N));
+    TRYC(dalloc(&c->norm_bg, N));
+    TRYC(lpf_launch_static_norm(c, c->g_mf, c->norm_mf, nullptr, 0));
+    TRYC(lpf_launch_static_norm(c, c->g_bg, c->norm_bg, nullptr, 0));
+    TRYC(lpf_fused_plan(c, hW.data(), &c->fused));   // reads norm_mf back for its interior constant
   }
-  TRYC(dalloc(&c->norm_mf, N));
-  TRYC(dalloc(&c->norm_bg, N));
-  TRYC(lpf_launch_static_norm(c, c->g_mf, c->norm_mf, nullptr, 0));
-  TRYC(lpf_launch_static_norm(c, c->g_bg, c->norm_bg, nullptr, 0));
 
   const size_t nc = (size_t)p->n_cand_max;
   TRYC(dalloc(&c->active, nc)); TRYC(dalloc(&c->forced, nc)); TRYC(dalloc(&c->cpix, nc)); TRYC(dalloc(&c->miss, nc));
