@@ -19,14 +19,17 @@
 // The 26-row histories of F and d that the running sums and the lagged reads need are private to
 // a thread, so they live in TENSOR MEMORY (tcgen05.st/ld 32x32b.x4: 208 of a thread's 256/512
 // columns) rather than in shared memory: shared memory carries only what threads exchange.
-// Rows x warps that are fully inside the valid region use constant normalisers and load no mask
-// or normaliser plane (a per-item class table built by the host plan); F, C, d, S never leave
-// the SM.
+// Everything a warp has to decide in an iteration (are its input rows all valid / partly masked /
+// empty, which normalisers are the interior constants, which stages run) is one 32-bit word of a
+// per-item table built by the host plan, so the steady-state iteration is branch-poor and loads
+// no mask or normaliser plane inside the valid region.  F, C, d, S never leave the SM.
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
 
 #include "lpf_internal.cuh"
+
+extern __shared__ float4 g_sm4[];
 
 namespace {
 
@@ -39,26 +42,34 @@ constexpr int LAG_C = LAG_B + KBG + RB;      // sig = y - 31
 constexpr int DFS = 32;             // shared-memory ring of F rows (local maxima): power of two
 constexpr int DT = WINB + 1;        // tensor-memory ring depth (rows) of F and of d
 constexpr int TM_D = 4 * DT;        // first tensor-memory column of the d ring (F ring starts at 0)
-constexpr int CLS_PAD = 64;         // class table covers rows ya-64 .. yb+64
+constexpr int PADR = 64;            // zero rows above and below the padded normaliser planes
 
-// class bits of a (row, warp) cell
-constexpr int CL_ANYW = 1;   // some valid pixel among the warp's columns +-4
-constexpr int CL_ALLW = 2;   // every pixel among the warp's columns +-4 is valid (and in the strip)
-constexpr int CL_NM1 = 4;    // norm_mf is the interior constant on all the warp's columns
-constexpr int CL_IC1 = 8;    // 1/count is 1/625 on all the warp's columns
+// per-(iteration, warp) control word
+constexpr unsigned FL_XMODE = 3u;          // bits 0-1: input rows consumed now: 0 empty, 1 all valid, 2 masked
+constexpr int FL_PMODE_SH = 2;             // bits 2-3: the same for the rows loaded now (two iterations ahead)
+constexpr unsigned FL_NM_LD = 1u << 4;     // F rows of this iteration use the loaded norm_mf (else the constant)
+constexpr unsigned FL_ICR_LD = 1u << 5;    // rho rows use the loaded 1/count
+constexpr unsigned FL_ICS_LD = 1u << 6;    // sigma rows use the loaded 1/count
+constexpr unsigned FL_NM_PF = 1u << 7;     // load the planes of the next iteration
+constexpr unsigned FL_ICR_PF = 1u << 8;
+constexpr unsigned FL_ICS_PF = 1u << 9;
+constexpr unsigned FL_GATE_A = 1u << 10;   // some F row precedes the segment's first needed one
+constexpr unsigned FL_GATE_B = 1u << 11;   // some rho row precedes the segment's first needed one
+constexpr unsigned FL_DO_B = 1u << 12;
+constexpr unsigned FL_C0 = 1u << 13;       // sigma row j is an output row of this item
+constexpr unsigned FL_C1 = 1u << 14;
 
-struct FusedItem { int xs, ux0, ux1, ya, yb, cls_off, pad0, pad1; };
+struct FusedItem { int xs, ux0, ux1, ya, yb, y_start, nb, fl_off; };
 
 struct FusedArgs {
   const float* cube; const float* sum_plane; const uint8_t* band_ok; const uint8_t* W;
-  const float* norm_mf; const float* inv_cnt; const FusedItem* items; const uint8_t* cls;
+  const float* nm_pad; const float* ic_pad;      // [(Dy + 2 PADR)][Dx], zero rows around the image
+  const FusedItem* items; const uint32_t* flags;
   int B, Dy, Dx, CW, k_max, max_det;
   float g0, g1, g2, g3, kappa2, eps_rel, nm_const, ic_const;
   lpf_det* dets; int32_t* ndets; int32_t* counters;
 };
 
-__device__ __forceinline__ float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
-__device__ __forceinline__ void st4(float* p, const float4 v) { *reinterpret_cast<float4*>(p) = v; }
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 __device__ __forceinline__ float4 zero4() { return make_float4(0.f, 0.f, 0.f, 0.f); }
 
@@ -68,6 +79,7 @@ __device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a
 __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
 __device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __ffma2_rn(b, make_float2(-1.f, -1.f), a); }
 __device__ __forceinline__ float2 splat(float s) { return make_float2(s, s); }
+__device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
 
 // ---- tensor memory as a thread-private scratch ring ---------------------------------------------
 __device__ __forceinline__ void tm_st4(uint32_t taddr, float2 lo, float2 hi) {
@@ -95,242 +107,278 @@ __device__ __forceinline__ float4 mask4(float4 v, unsigned wm) {
   return v;
 }
 
+// shared memory through the kernel's one dynamic array: float index -> value
+__device__ __forceinline__ float4 lds4(int i) { return *reinterpret_cast<const float4*>(reinterpret_cast<const float*>(g_sm4) + i); }
+__device__ __forceinline__ float lds1(int i) { return reinterpret_cast<const float*>(g_sm4)[i]; }
+__device__ __forceinline__ void sts4(int i, float4 v) { *reinterpret_cast<float4*>(reinterpret_cast<float*>(g_sm4) + i) = v; }
+__device__ __forceinline__ void sts1(int i, float v) { reinterpret_cast<float*>(g_sm4)[i] = v; }
+
 // horizontal 25-box of a row of per-column values, 4 per thread: the six group sums q-3..q+2 give the
 // window of the thread's first column up to one pixel, the other three windows slide.
-__device__ __forceinline__ void hbox25(const float* EVrow, const float* ETrow, int tid, float out[4]) {
-  const float4 L = ld4(EVrow + 4 * tid);        // group q-3
-  const float4 R = ld4(EVrow + 4 * tid + 24);   // group q+3
-  const float t0 = ETrow[tid], t1 = ETrow[tid + 1], t2 = ETrow[tid + 2], t3 = ETrow[tid + 3], t4 = ETrow[tid + 4],
-              t5 = ETrow[tid + 5];
+// ev: float index of the thread's group q-3 in the value row; et: index of group sum q-3.
+__device__ __forceinline__ void hbox25(int ev, int et, float out[4]) {
+  const float4 L = lds4(ev);        // group q-3
+  const float4 R = lds4(ev + 24);   // group q+3
+  const float t0 = lds1(et), t1 = lds1(et + 1), t2 = lds1(et + 2), t3 = lds1(et + 3), t4 = lds1(et + 4), t5 = lds1(et + 5);
   out[0] = (((t0 + t1) + (t2 + t3)) + (t4 + t5)) + R.x;
   out[1] = out[0] + (R.y - L.x);
   out[2] = out[1] + (R.z - L.y);
   out[3] = out[2] + (R.w - L.z);
 }
 
+// eq. 5 guard + eq. 6 + eq. 7 for one pixel that passed the unguarded eq. 5, by the whole warp:
+// lane k < (2 k_max + 1)^2 looks at one neighbour in the shared-memory ring of F (float index ringF,
+// row pitch CWP).  d, s: the pixel's residual and spread (already broadcast); cl: its column in the strip.
+__device__ __noinline__ void fused_candidate(const FusedArgs* ap, int ringF, int CWP, int xs, int plane, int lane,
+                                             float d, float s, int cl, int sg) {
+  const FusedArgs& a = *ap;
+  const float fv = lds1(ringF + (sg & (DFS - 1)) * CWP + cl);
+  const float cc = fv - d;
+  const float gd = a.eps_rel * fabsf(cc);
+  const float se = fmaxf(s, gd * gd);
+  if (!(d > 0.f && d * d > a.kappa2 * se)) return;   // warp-uniform
+  const int km = a.k_max, side = 2 * km + 1;
+  bool bigger = false;
+  if (lane < side * side) {
+    const int dy = lane / side - km, dx = lane - (lane / side) * side - km;
+    const int yy = sg + dy, c2 = cl + dx, xn = xs + c2;
+    if (yy >= 0 && yy < a.Dy && c2 >= 0 && c2 < CWP && xn < a.Dx) {
+      const float fn = lds1(ringF + (yy & (DFS - 1)) * CWP + c2);
+      // masked pixels hold F = 0 in the ring: W is consulted only when such a zero would win
+      if (fn > fv) bigger = (fn != 0.f) || (a.W[(long long)yy * a.Dx + xn] != 0);
+    }
+  }
+  if (__any_sync(0xffffffffu, bigger)) return;
+  if (lane == 0) {
+    const int idx = atomicAdd(a.ndets, 1);
+    if (idx < a.max_det) {
+      lpf_det r;
+      r.pix = sg * a.Dx + xs + cl; r.plane = (int16_t)plane; r.iter = 1;
+      r.f = fv; r.c = cc; r.s = se; r.snr = d / sqrtf(se);
+      a.dets[idx] = r;
+    } else {
+      atomicAdd(&a.counters[0], 1);
+    }
+  }
+}
+
 struct Prefetch {          // one iteration's worth of input rows, loaded two iterations ahead
   float4 x[RB], xe[RB];    // own 4 pixels; the neighbouring warp's 4 pixels (lanes 0 and 31 only)
-  unsigned w[RB], we[RB];  // their mask bytes
+  unsigned w[RB], we[RB];  // their mask bytes (masked rows only)
 };
 
-struct Planes {            // normaliser values of a non-interior cell, loaded one iteration ahead
+struct Planes {            // normaliser values of non-interior cells, loaded one iteration ahead
   float4 nm[RB], icr[RB], ics[RB];
 };
 
 template <int NW>
 struct Sweep {
+  static constexpr int CWP = NW * 128;             // shared-memory row pitch: the CTA's full width
+  static constexpr int PEV = CWP + 2 * KBG, PET = NW * 32 + 8;
+  static constexpr int O_RING = 0;
+  static constexpr int O_EV1 = DFS * CWP;
+  static constexpr int O_EV2 = O_EV1 + 2 * RB * PEV;
+  static constexpr int O_ET1 = O_EV2 + 2 * RB * PEV;
+  static constexpr int O_ET2 = O_ET1 + 2 * RB * PET;
+  static constexpr int O_FL = O_ET2 + 2 * RB * PET;   // control words, [nb][NW]
   // ---- constants of the thread -----------------------------------------------------------------
   const FusedArgs& a;
-  FusedItem it;
-  const float* X;
-  float* ringF; float* EV1; float* EV2; float* ET1; float* ET2; const uint8_t* cls;
-  int tid, lane, warp, x, CW, PEV, PET, plane;
-  bool col_in, ld_left, ld_right;
+  const FusedArgs* a_sh;   // the same arguments in shared memory (for the out-of-line candidate path)
+  int xs, plane, tid, lane, warp;
+  int sx, eoff;            // row stride (0 for lanes outside the strip); offset of the edge lanes' extra load
+  bool ld_edge;
   unsigned umask;
   uint32_t tm;             // tensor-memory address of the thread's column 0
-  int y_start;
+  int f_lim, r_lim;        // first needed F row (ya - 24), first needed rho row (ya - 12)
   // ---- running state -----------------------------------------------------------------------------
-  float2 hw[8][2];         // horizontally filtered rows y-7 .. y (rotating, static indices per phase)
+  const float* xp;         // X at the first row of the next prefetch
+  const uint8_t* wp;       // W at the same place
+  const float* nmp;        // padded norm_mf at the next iteration's first F row
+  const float* icrp;       // padded 1/count at the next iteration's first rho row
+  const float* icsp;       // padded 1/count at the next iteration's first sigma row
+  int y0;                  // first input row of the current iteration
+  int w26;                 // tensor-memory ring slot of this iteration's first row
+  float2 hw[8][2];         // horizontally filtered rows (rotating; static indices per phase)
   float2 V1[2], V2[2];     // vertical running sums
   Prefetch pf[2];
-  Planes pl;
-  int w26;                 // tensor-memory ring slot of this iteration's first row
+  Planes pl[2];
 
   __device__ __forceinline__ Sweep(const FusedArgs& a_) : a(a_) {}
 
-  __device__ __forceinline__ int cls_at(int row) const { return cls[(row - (it.ya - CLS_PAD)) * NW + warp]; }
+  __device__ __forceinline__ unsigned ctl(int b) const {
+    return reinterpret_cast<const uint32_t*>(g_sm4)[O_FL + b * NW + warp];
+  }
 
-  // global loads of the rows y0+j into pf[slot]; rows past y_stop are not needed by any output
-  __device__ __forceinline__ void prefetch(int slot, int y0, int y_stop) {
-#pragma unroll
-    for (int j = 0; j < RB; ++j) {
-      const int y = y0 + j;
+  // global loads of two input rows into pf[slot]; mode 1: all valid, 2: masked (W loaded too)
+  __device__ __forceinline__ void load_rows(int slot, unsigned mode) {
+    if (mode) {
       Prefetch& p = pf[slot];
-      p.x[j] = zero4(); p.xe[j] = zero4(); p.w[j] = 0u; p.we[j] = 0u;
-      if (y < 0 || y >= a.Dy || y > y_stop) continue;
-      const int c = cls_at(y);
-      if (!(c & CL_ANYW)) continue;
-      const long long q = (long long)y * a.Dx + x;
-      if (c & CL_ALLW) {
-        p.w[j] = 0x01010101u; p.we[j] = 0x01010101u;
-        if (col_in) p.x[j] = ldg4(X + q);
-        if (ld_left) p.xe[j] = ldg4(X + q - 4);
-        if (ld_right) p.xe[j] = ldg4(X + q + 4);
-      } else {
-        if (col_in) { p.x[j] = ldg4(X + q); p.w[j] = __ldg(reinterpret_cast<const unsigned*>(a.W + q)); }
-        if (ld_left) { p.xe[j] = ldg4(X + q - 4); p.we[j] = __ldg(reinterpret_cast<const unsigned*>(a.W + q - 4)); }
-        if (ld_right) { p.xe[j] = ldg4(X + q + 4); p.we[j] = __ldg(reinterpret_cast<const unsigned*>(a.W + q + 4)); }
+      p.x[0] = ldg4(xp); p.x[1] = ldg4(xp + sx);
+      if (ld_edge) { p.xe[0] = ldg4(xp + eoff); p.xe[1] = ldg4(xp + sx + eoff); }
+      if (mode == 2u) {
+        p.w[0] = __ldg(reinterpret_cast<const unsigned*>(wp));
+        p.w[1] = __ldg(reinterpret_cast<const unsigned*>(wp + sx));
+        if (ld_edge) {
+          p.we[0] = __ldg(reinterpret_cast<const unsigned*>(wp + eoff));
+          p.we[1] = __ldg(reinterpret_cast<const unsigned*>(wp + sx + eoff));
+        }
       }
     }
+    xp += RB * sx; wp += RB * sx;
   }
 
-  // normaliser planes for the rows the NEXT iteration's stages touch (only where the cell is not interior)
-  __device__ __forceinline__ void prefetch_planes(int y0n) {
-#pragma unroll
-    for (int j = 0; j < RB; ++j) {
-      const int fr = y0n + j - 3, rho = y0n + j - LAG_B, sg = y0n + j - LAG_C;
-      pl.nm[j] = zero4(); pl.icr[j] = zero4(); pl.ics[j] = zero4();
-      if (!col_in) continue;
-      if (fr >= 0 && fr < a.Dy && !(cls_at(fr) & CL_NM1)) pl.nm[j] = ldg4(a.norm_mf + (long long)fr * a.Dx + x);
-      if (rho >= 0 && rho < a.Dy && !(cls_at(rho) & CL_IC1)) pl.icr[j] = ldg4(a.inv_cnt + (long long)rho * a.Dx + x);
-      if (sg >= it.ya && sg < it.yb && !(cls_at(sg) & CL_IC1)) pl.ics[j] = ldg4(a.inv_cnt + (long long)sg * a.Dx + x);
-    }
-  }
-
-  // eq. 5 guard + eq. 6 + eq. 7 for one pixel that passed the unguarded eq. 5, by the whole warp:
-  // lane k < (2 k_max + 1)^2 looks at one neighbour in the shared-memory ring of F.
-  __device__ __forceinline__ void candidate(int src, float dsrc, float ssrc, int kcol, int sg) {
-    const float d = __shfl_sync(0xffffffffu, dsrc, src);
-    const float s = __shfl_sync(0xffffffffu, ssrc, src);
-    const int cl = 4 * (warp * 32 + src) + kcol;       // column within the strip
-    const float fv = ringF[(sg & (DFS - 1)) * CW + cl];
-    const float cc = fv - d;
-    const float gd = a.eps_rel * fabsf(cc);
-    const float se = fmaxf(s, gd * gd);
-    if (!(d > 0.f && d * d > a.kappa2 * se)) return;   // warp-uniform
-    const int km = a.k_max, side = 2 * km + 1;
-    bool bigger = false;
-    if (lane < side * side) {
-      const int dy = lane / side - km, dx = lane - (lane / side) * side - km;
-      const int yy = sg + dy, c2 = cl + dx, xn = it.xs + c2;
-      if (yy >= 0 && yy < a.Dy && c2 >= 0 && c2 < CW && xn < a.Dx) {
-        const float fn = ringF[(yy & (DFS - 1)) * CW + c2];
-        // masked pixels hold F = 0 in the ring: W is consulted only when such a zero would win
-        if (fn > fv) bigger = (fn != 0.f) || (a.W[(long long)yy * a.Dx + xn] != 0);
-      }
-    }
-    if (__any_sync(0xffffffffu, bigger)) return;
-    if (lane == 0) {
-      const int idx = atomicAdd(a.ndets, 1);
-      if (idx < a.max_det) {
-        lpf_det r;
-        r.pix = sg * a.Dx + it.xs + cl; r.plane = (int16_t)plane; r.iter = 1;
-        r.f = fv; r.c = cc; r.s = se; r.snr = d / sqrtf(se);
-        a.dets[idx] = r;
-      } else {
-        atomicAdd(&a.counters[0], 1);
-      }
-    }
+  __device__ __forceinline__ void load_planes(int slot, unsigned fl_nm, unsigned fl_icr, unsigned fl_ics) {
+    Planes& q = pl[slot];
+    if (fl_nm) { q.nm[0] = ldg4(nmp); q.nm[1] = ldg4(nmp + sx); }
+    if (fl_icr) { q.icr[0] = ldg4(icrp); q.icr[1] = ldg4(icrp + sx); }
+    if (fl_ics) { q.ics[0] = ldg4(icsp); q.ics[1] = ldg4(icsp + sx); }
+    nmp += RB * sx; icrp += RB * sx; icsp += RB * sx;
   }
 
   // One iteration: rows y0, y0+1 enter stage A; PH = iteration index mod 4 fixes the register rotation.
   template <int PH>
-  __device__ __forceinline__ void iteration(int b, int nb, int y_stop) {
-    const int y0 = y_start + RB * b;
-    const int buf = PH & 1, pbuf = buf ^ 1;
-    const bool doB = (y0 + 1 - LAG_B) >= it.ya - KBG;     // some rho of this iteration is inside the d range
-    const bool doC = (y0 + 1 - LAG_C) >= it.ya;           // some sigma of this iteration is an output row
+  __device__ __forceinline__ void iteration(int b) {
+    constexpr int buf = PH & 1, pbuf = buf ^ 1;
+    const unsigned fl = ctl(b);
     const float2 g0 = splat(a.g0), g1 = splat(a.g1), g2 = splat(a.g2), g3 = splat(a.g3);
 
-    // ---- tensor-memory reads of the whole iteration: F(fr-25), F(rho), d(rho-25), d(sig) ------------
-    float2 fold[RB][2], flag[RB][2], dold[RB][2], dlag[RB][2];
+    // ---- tensor-memory reads, first batch: F(fr - 25) ------------------------------------------------
+    float2 fold[RB][2];
+#pragma unroll
+    for (int j = 0; j < RB; ++j) tm_ld4(tm + 4 * wrap26(w26 + j + 1), fold[j][0], fold[j][1]);
+
+    // ---- stage A, part 1: take the prefetched rows, mask, horizontal matched filter -----------------
+    {
+      float4 v[RB], e[RB];
+      const unsigned mode = fl & FL_XMODE;
+      if (mode == 0u) {
+#pragma unroll
+        for (int j = 0; j < RB; ++j) { v[j] = zero4(); e[j] = zero4(); }
+      } else {
+#pragma unroll
+        for (int j = 0; j < RB; ++j) { v[j] = pf[buf].x[j]; e[j] = pf[buf].xe[j]; }
+        if (mode == 2u) {
+#pragma unroll
+          for (int j = 0; j < RB; ++j) { v[j] = mask4(v[j], pf[buf].w[j]); e[j] = mask4(e[j], pf[buf].we[j]); }
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < RB; ++j) {
+        float l1 = __shfl_up_sync(0xffffffffu, v[j].y, 1), l2 = __shfl_up_sync(0xffffffffu, v[j].z, 1),
+              l3 = __shfl_up_sync(0xffffffffu, v[j].w, 1);
+        float r0 = __shfl_down_sync(0xffffffffu, v[j].x, 1), r1 = __shfl_down_sync(0xffffffffu, v[j].y, 1),
+              r2 = __shfl_down_sync(0xffffffffu, v[j].z, 1);
+        if (lane == 0) { l1 = e[j].y; l2 = e[j].z; l3 = e[j].w; }
+        if (lane == 31) { r0 = e[j].x; r1 = e[j].y; r2 = e[j].z; }
+        const float wv[10] = {l1, l2, l3, v[j].x, v[j].y, v[j].z, v[j].w, r0, r1, r2};
+        float h[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+          h[k] = fmaf(a.g0, wv[k + 3], fmaf(a.g1, wv[k + 2] + wv[k + 4], fmaf(a.g2, wv[k + 1] + wv[k + 5], a.g3 * (wv[k] + wv[k + 6]))));
+        hw[(2 * PH + 6 + j) & 7][0] = make_float2(h[0], h[1]);
+        hw[(2 * PH + 6 + j) & 7][1] = make_float2(h[2], h[3]);
+      }
+    }
+    // ---- issue the global loads of iteration b+2 (inputs) and b+1 (normaliser planes) --------------
+    load_rows(buf, (fl >> FL_PMODE_SH) & 3u);
+    load_planes(pbuf, fl & FL_NM_PF, fl & FL_ICR_PF, fl & FL_ICS_PF);
+
+    tm_wait_ld();
+#pragma unroll
+    for (int j = 0; j < RB; ++j) tm_use(fold[j][0], fold[j][1]);
+    // ---- second batch: F(rho), d(rho - 25), d(sigma) -------------------------------------------------
+    float2 flag[RB][2], dold[RB][2], dlag[RB][2];
 #pragma unroll
     for (int j = 0; j < RB; ++j) {
       const int so = wrap26(w26 + j + 1), sl = wrap26(w26 + j + KBG);
-      tm_ld4(tm + 4 * so, fold[j][0], fold[j][1]);
       tm_ld4(tm + 4 * sl, flag[j][0], flag[j][1]);
       tm_ld4(tm + TM_D + 4 * so, dold[j][0], dold[j][1]);
       tm_ld4(tm + TM_D + 4 * sl, dlag[j][0], dlag[j][1]);
     }
 
-    // ---- stage A, part 1: take the prefetched rows, mask, horizontal matched filter -----------------
-    Planes cur = pl;
+    // ---- stage A, part 2: vertical matched filter -> F(fr), running sum V1, exchange ----------------
+    {
+      float2 f[RB][2];
 #pragma unroll
-    for (int j = 0; j < RB; ++j) {
-      float4 v = pf[buf].x[j], e = pf[buf].xe[j];
-      const unsigned wm = pf[buf].w[j], wme = pf[buf].we[j];
-      if (wm != 0x01010101u) v = mask4(v, wm);
-      if (wme != 0x01010101u) e = mask4(e, wme);
-      float l1 = __shfl_up_sync(0xffffffffu, v.y, 1), l2 = __shfl_up_sync(0xffffffffu, v.z, 1),
-            l3 = __shfl_up_sync(0xffffffffu, v.w, 1);
-      float r0 = __shfl_down_sync(0xffffffffu, v.x, 1), r1 = __shfl_down_sync(0xffffffffu, v.y, 1),
-            r2 = __shfl_down_sync(0xffffffffu, v.z, 1);
-      if (lane == 0) { l1 = e.y; l2 = e.z; l3 = e.w; }
-      if (lane == 31) { r0 = e.x; r1 = e.y; r2 = e.z; }
-      const float wv[10] = {l1, l2, l3, v.x, v.y, v.z, v.w, r0, r1, r2};
-      float h[4];
+      for (int j = 0; j < RB; ++j)
 #pragma unroll
-      for (int k = 0; k < 4; ++k)
-        h[k] = fmaf(a.g0, wv[k + 3], fmaf(a.g1, wv[k + 2] + wv[k + 4], fmaf(a.g2, wv[k + 1] + wv[k + 5], a.g3 * (wv[k] + wv[k + 6]))));
-      hw[(2 * PH + 6 + j) & 7][0] = make_float2(h[0], h[1]);
-      hw[(2 * PH + 6 + j) & 7][1] = make_float2(h[2], h[3]);
+        for (int p = 0; p < 2; ++p) {
+          const float2 h0 = hw[(2 * PH + j + 0) & 7][p], h1 = hw[(2 * PH + j + 1) & 7][p], h2 = hw[(2 * PH + j + 2) & 7][p],
+                       h3 = hw[(2 * PH + j + 3) & 7][p], h4 = hw[(2 * PH + j + 4) & 7][p], h5 = hw[(2 * PH + j + 5) & 7][p],
+                       h6 = hw[(2 * PH + j + 6) & 7][p];
+          f[j][p] = fma2(g0, h3, fma2(g1, add2(h2, h4), fma2(g2, add2(h1, h5), mul2(g3, add2(h0, h6)))));
+        }
+      if (fl & FL_NM_LD) {
+#pragma unroll
+        for (int j = 0; j < RB; ++j) {
+          f[j][0] = mul2(f[j][0], make_float2(pl[buf].nm[j].x, pl[buf].nm[j].y));
+          f[j][1] = mul2(f[j][1], make_float2(pl[buf].nm[j].z, pl[buf].nm[j].w));
+        }
+      } else {
+        const float2 c = splat(a.nm_const);
+#pragma unroll
+        for (int j = 0; j < RB; ++j) { f[j][0] = mul2(f[j][0], c); f[j][1] = mul2(f[j][1], c); }
+      }
+      if (fl & FL_GATE_A) {                          // rows before the segment's first needed F row
+#pragma unroll
+        for (int j = 0; j < RB; ++j)
+          if (y0 + j - 3 < f_lim) { f[j][0] = splat(0.f); f[j][1] = splat(0.f); }
+      }
+#pragma unroll
+      for (int j = 0; j < RB; ++j) {
+        V1[0] = add2(V1[0], sub2(f[j][0], fold[j][0]));
+        V1[1] = add2(V1[1], sub2(f[j][1], fold[j][1]));
+        tm_st4(tm + 4 * wrap26(w26 + j), f[j][0], f[j][1]);
+        sts4(O_RING + ((y0 + j - 3) & (DFS - 1)) * CWP + 4 * tid, make_float4(f[j][0].x, f[j][0].y, f[j][1].x, f[j][1].y));
+        sts4(O_EV1 + (buf * RB + j) * PEV + KBG + 4 * tid, make_float4(V1[0].x, V1[0].y, V1[1].x, V1[1].y));
+        const float2 ts = add2(V1[0], V1[1]);
+        sts1(O_ET1 + (buf * RB + j) * PET + 3 + tid, ts.x + ts.y);
+      }
     }
-    // ---- issue the global loads of iteration b+2 (inputs) and b+1 (normaliser planes) --------------
-    prefetch(buf, y0 + 2 * RB, y_stop);
-    prefetch_planes(y0 + RB);
 
     tm_wait_ld();
 #pragma unroll
-    for (int j = 0; j < RB; ++j) {
-      tm_use(fold[j][0], fold[j][1]); tm_use(flag[j][0], flag[j][1]);
-      tm_use(dold[j][0], dold[j][1]); tm_use(dlag[j][0], dlag[j][1]);
-    }
-
-    // ---- stage A, part 2: vertical matched filter -> F(fr), running sum V1, exchange ----------------
-#pragma unroll
-    for (int j = 0; j < RB; ++j) {
-      const int fr = y0 + j - 3;
-      const int cf = (fr >= 0 && fr < a.Dy) ? cls_at(fr) : 0;
-      float2 f[2];
-#pragma unroll
-      for (int p = 0; p < 2; ++p) {
-        const float2 h0 = hw[(2 * PH + j + 0) & 7][p], h1 = hw[(2 * PH + j + 1) & 7][p], h2 = hw[(2 * PH + j + 2) & 7][p],
-                     h3 = hw[(2 * PH + j + 3) & 7][p], h4 = hw[(2 * PH + j + 4) & 7][p], h5 = hw[(2 * PH + j + 5) & 7][p],
-                     h6 = hw[(2 * PH + j + 6) & 7][p];
-        f[p] = fma2(g0, h3, fma2(g1, add2(h2, h4), fma2(g2, add2(h1, h5), mul2(g3, add2(h0, h6)))));
-      }
-      if (fr < it.ya - 2 * KBG) {                      // rows before the segment's first needed F row
-        f[0] = splat(0.f); f[1] = splat(0.f);
-      } else if (cf & CL_NM1) {
-        f[0] = mul2(f[0], splat(a.nm_const)); f[1] = mul2(f[1], splat(a.nm_const));
-      } else {
-        f[0] = mul2(f[0], make_float2(cur.nm[j].x, cur.nm[j].y)); f[1] = mul2(f[1], make_float2(cur.nm[j].z, cur.nm[j].w));
-      }
-      V1[0] = add2(V1[0], sub2(f[0], fold[j][0]));
-      V1[1] = add2(V1[1], sub2(f[1], fold[j][1]));
-      tm_st4(tm + 4 * wrap26(w26 + j), f[0], f[1]);
-      st4(ringF + (fr & (DFS - 1)) * CW + 4 * tid, make_float4(f[0].x, f[0].y, f[1].x, f[1].y));
-      st4(EV1 + (buf * RB + j) * PEV + KBG + 4 * tid, make_float4(V1[0].x, V1[0].y, V1[1].x, V1[1].y));
-      const float2 ts = add2(V1[0], V1[1]);
-      ET1[(buf * RB + j) * PET + 3 + tid] = ts.x + ts.y;
-    }
+    for (int j = 0; j < RB; ++j) { tm_use(flag[j][0], flag[j][1]); tm_use(dold[j][0], dold[j][1]); tm_use(dlag[j][0], dlag[j][1]); }
 
     // ---- stage B: C = box(V1) / count at rho ; d = F - C ; running sum V2 of d^2 ---------------------
-    if (doB) {
+    if (fl & FL_DO_B) {
+      float2 dd[RB][2];
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
-        const int rho = y0 + j - LAG_B;
         float bx[4];
-        hbox25(EV1 + (pbuf * RB + j) * PEV, ET1 + (pbuf * RB + j) * PET, tid, bx);
-        const int cr = (rho >= 0 && rho < a.Dy) ? cls_at(rho) : 0;
+        hbox25(O_EV1 + (pbuf * RB + j) * PEV + 4 * tid, O_ET1 + (pbuf * RB + j) * PET + tid, bx);
         float2 ic0, ic1;
-        if (rho < it.ya - KBG) { ic0 = splat(0.f); ic1 = splat(0.f); flag[j][0] = splat(0.f); flag[j][1] = splat(0.f); }
-        else if (cr & CL_IC1) { ic0 = splat(a.ic_const); ic1 = ic0; }
-        else { ic0 = make_float2(cur.icr[j].x, cur.icr[j].y); ic1 = make_float2(cur.icr[j].z, cur.icr[j].w); }
-        // d = F - box * (1/count)
-        const float2 d0 = fma2(make_float2(-bx[0], -bx[1]), ic0, flag[j][0]);
-        const float2 d1 = fma2(make_float2(-bx[2], -bx[3]), ic1, flag[j][1]);
-        V2[0] = fma2(make_float2(-dold[j][0].x, -dold[j][0].y), dold[j][0], fma2(d0, d0, V2[0]));
-        V2[1] = fma2(make_float2(-dold[j][1].x, -dold[j][1].y), dold[j][1], fma2(d1, d1, V2[1]));
-        tm_st4(tm + TM_D + 4 * wrap26(w26 + j), d0, d1);
-        st4(EV2 + (buf * RB + j) * PEV + KBG + 4 * tid, make_float4(V2[0].x, V2[0].y, V2[1].x, V2[1].y));
+        if (fl & FL_ICR_LD) { ic0 = make_float2(pl[buf].icr[j].x, pl[buf].icr[j].y); ic1 = make_float2(pl[buf].icr[j].z, pl[buf].icr[j].w); }
+        else { ic0 = splat(a.ic_const); ic1 = ic0; }
+        dd[j][0] = fma2(make_float2(-bx[0], -bx[1]), ic0, flag[j][0]);     // d = F - box * (1/count)
+        dd[j][1] = fma2(make_float2(-bx[2], -bx[3]), ic1, flag[j][1]);
+      }
+      if (fl & FL_GATE_B) {                          // rows before the segment's first needed rho row
+#pragma unroll
+        for (int j = 0; j < RB; ++j)
+          if (y0 + j - LAG_B < r_lim) { dd[j][0] = splat(0.f); dd[j][1] = splat(0.f); }
+      }
+#pragma unroll
+      for (int j = 0; j < RB; ++j) {
+        V2[0] = fma2(neg2(dold[j][0]), dold[j][0], fma2(dd[j][0], dd[j][0], V2[0]));
+        V2[1] = fma2(neg2(dold[j][1]), dold[j][1], fma2(dd[j][1], dd[j][1], V2[1]));
+        tm_st4(tm + TM_D + 4 * wrap26(w26 + j), dd[j][0], dd[j][1]);
+        sts4(O_EV2 + (buf * RB + j) * PEV + KBG + 4 * tid, make_float4(V2[0].x, V2[0].y, V2[1].x, V2[1].y));
         const float2 ts = add2(V2[0], V2[1]);
-        ET2[(buf * RB + j) * PET + 3 + tid] = ts.x + ts.y;
+        sts1(O_ET2 + (buf * RB + j) * PET + 3 + tid, ts.x + ts.y);
       }
     }
 
     // ---- stage C: S = box(V2) / count at sigma ; eq. 5 ; candidates -----------------------------------
-    if (doC) {
+    if (fl & (FL_C0 | FL_C1)) {
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
-        const int sg = y0 + j - LAG_C;
-        if (sg < it.ya || sg >= it.yb) continue;       // uniform
+        if (!(fl & (FL_C0 << j))) continue;          // uniform
         float bx[4];
-        hbox25(EV2 + (pbuf * RB + j) * PEV, ET2 + (pbuf * RB + j) * PET, tid, bx);
-        const int cs = cls_at(sg);
+        hbox25(O_EV2 + (pbuf * RB + j) * PEV + 4 * tid, O_ET2 + (pbuf * RB + j) * PET + tid, bx);
         float2 ic0, ic1;
-        if (cs & CL_IC1) { ic0 = splat(a.ic_const); ic1 = ic0; }
-        else { ic0 = make_float2(cur.ics[j].x, cur.ics[j].y); ic1 = make_float2(cur.ics[j].z, cur.ics[j].w); }
+        if (fl & FL_ICS_LD) { ic0 = make_float2(pl[buf].ics[j].x, pl[buf].ics[j].y); ic1 = make_float2(pl[buf].ics[j].z, pl[buf].ics[j].w); }
+        else { ic0 = splat(a.ic_const); ic1 = ic0; }
         const float2 s0 = mul2(make_float2(bx[0], bx[1]), ic0), s1 = mul2(make_float2(bx[2], bx[3]), ic1);
         const float2 k0 = mul2(s0, splat(a.kappa2)), k1 = mul2(s1, splat(a.kappa2));
         const float2 q0 = mul2(dlag[j][0], dlag[j][0]), q1 = mul2(dlag[j][1], dlag[j][1]);
@@ -339,36 +387,41 @@ struct Sweep {
         if (__any_sync(0xffffffffu, bits != 0u)) {
           const float dv[4] = {dlag[j][0].x, dlag[j][0].y, dlag[j][1].x, dlag[j][1].y};
           const float sv[4] = {s0.x, s0.y, s1.x, s1.y};
+          const int sg = y0 + j - LAG_C;
 #pragma unroll
           for (int k = 0; k < 4; ++k) {
             unsigned m = __ballot_sync(0xffffffffu, (bits >> k) & 1u);
             while (m) {
               const int src = __ffs(m) - 1;
               m &= m - 1;
-              candidate(src, dv[k], sv[k], k, sg);
+              const float d = __shfl_sync(0xffffffffu, dv[k], src);
+              const float s = __shfl_sync(0xffffffffu, sv[k], src);
+              fused_candidate(a_sh, O_RING, CWP, xs, plane, lane, d, s, 4 * (warp * 32 + src) + k, sg);
             }
           }
         }
       }
     }
     w26 = wrap26(w26 + RB);
-    (void)nb;
+    y0 += RB;
     tm_wait_st();
     __syncthreads();
   }
 
-  __device__ __forceinline__ void run() {
-    const int nb = (it.yb - it.ya + HALO + LAG_C + RB - 1) / RB;   // last sigma = yb-1 enters stage C at y = yb-1+LAG_C
-    const int y_stop = it.yb - 1 + HALO;                            // last input row any output needs
-    prefetch(0, y_start, y_stop);
-    prefetch(1, y_start + RB, y_stop);
-    prefetch_planes(y_start);
+  __device__ __forceinline__ void run(int nb) {
+    // prologue: the input rows of iterations 0 and 1, the planes of iteration 0
+    load_rows(0, ctl(0) & FL_XMODE);
+    load_rows(1, nb > 1 ? (ctl(1) & FL_XMODE) : 0u);
+    {
+      const unsigned f0 = ctl(0);
+      load_planes(0, f0 & FL_NM_LD, f0 & FL_ICR_LD, f0 & FL_ICS_LD);
+    }
     int b = 0;
     while (true) {
-      iteration<0>(b, nb, y_stop); if (++b >= nb) break;
-      iteration<1>(b, nb, y_stop); if (++b >= nb) break;
-      iteration<2>(b, nb, y_stop); if (++b >= nb) break;
-      iteration<3>(b, nb, y_stop); if (++b >= nb) break;
+      iteration<0>(b); if (++b >= nb) break;
+      iteration<1>(b); if (++b >= nb) break;
+      iteration<2>(b); if (++b >= nb) break;
+      iteration<3>(b); if (++b >= nb) break;
     }
   }
 };
@@ -376,32 +429,24 @@ struct Sweep {
 template <int NW>
 __global__ void __launch_bounds__(NW * 32, 1)
 k_fused_box(const FusedArgs a) {
-  extern __shared__ float4 sm4[];
   __shared__ uint32_t s_tmem;
+  __shared__ FusedArgs s_args;
   constexpr int TM_COLS = NW > 4 ? 512 : 256;
-  float* sm = reinterpret_cast<float*>(sm4);
+  using SW = Sweep<NW>;
   const int p = blockIdx.y;
   if (!a.band_ok[a.B]) return;
   if (p < a.B && !a.band_ok[p]) return;
 
-  Sweep<NW> s(a);
-  s.it = a.items[blockIdx.x];
-  // shared-memory rows are as wide as the CTA (lanes past the strip's CW columns carry zeros)
-  s.CW = NW * 128; s.tid = threadIdx.x; s.lane = threadIdx.x & 31; s.warp = threadIdx.x >> 5; s.plane = p;
-  s.PEV = s.CW + 2 * KBG; s.PET = NW * 32 + 8;
-  s.ringF = sm;
-  s.EV1 = s.ringF + DFS * s.CW;
-  s.EV2 = s.EV1 + 2 * RB * s.PEV;
-  s.ET1 = s.EV2 + 2 * RB * s.PEV;
-  s.ET2 = s.ET1 + 2 * RB * s.PET;
-  const int nfl = DFS * s.CW + 4 * RB * s.PEV + 4 * RB * s.PET;   // floats, multiple of 4
-  uint8_t* cls_s = reinterpret_cast<uint8_t*>(sm + nfl);
-  s.cls = cls_s;
-  for (int i = s.tid; i < (nfl >> 2); i += NW * 32) sm4[i] = zero4();
+  SW s(a);
+  const FusedItem it = a.items[blockIdx.x];
+  s.a_sh = &s_args;
+  s.tid = threadIdx.x; s.lane = threadIdx.x & 31; s.warp = threadIdx.x >> 5; s.plane = p; s.xs = it.xs;
+  if (s.tid == 0) s_args = a;
+  for (int i = s.tid; i < (SW::O_FL >> 2); i += NW * 32) g_sm4[i] = zero4();
   {
-    const int nrows = s.it.yb - s.it.ya + 2 * CLS_PAD;
-    const uint8_t* src = a.cls + s.it.cls_off;
-    for (int i = s.tid; i < nrows * NW; i += NW * 32) cls_s[i] = src[i];
+    uint32_t* fl_s = reinterpret_cast<uint32_t*>(g_sm4) + SW::O_FL;
+    const uint32_t* src = a.flags + it.fl_off;
+    for (int i = s.tid; i < it.nb * NW; i += NW * 32) fl_s[i] = src[i];
   }
   if (s.warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n"
@@ -418,23 +463,45 @@ k_fused_box(const FusedArgs a) {
   tm_wait_st();
 
   const long long N = (long long)a.Dy * a.Dx;
-  s.X = (p < a.B) ? a.cube + (long long)p * N : a.sum_plane;
-  s.x = s.it.xs + 4 * s.tid;
-  s.col_in = 4 * s.tid < a.CW && s.x < a.Dx;
-  s.ld_left = s.col_in && s.lane == 0 && s.tid > 0;
-  s.ld_right = s.col_in && s.lane == 31 && 4 * (s.tid + 1) < a.CW && s.x + 4 < a.Dx;
+  const float* X = (p < a.B) ? a.cube + (long long)p * N : a.sum_plane;
+  const int x = it.xs + 4 * s.tid;
+  const bool col_in = 4 * s.tid < a.CW && x < a.Dx;
+  const bool ld_left = col_in && s.lane == 0 && s.tid > 0;
+  const bool ld_right = col_in && s.lane == 31 && 4 * (s.tid + 1) < a.CW && x + 4 < a.Dx;
+  s.ld_edge = ld_left || ld_right;
+  s.eoff = ld_left ? -4 : 4;
   s.umask = 0u;
 #pragma unroll
   for (int k = 0; k < 4; ++k)
-    if (s.col_in && s.x + k >= s.it.ux0 && s.x + k < s.it.ux1) s.umask |= 1u << k;
-  s.y_start = s.it.ya - HALO;
+    if (col_in && x + k >= it.ux0 && x + k < it.ux1) s.umask |= 1u << k;
+  s.f_lim = it.ya - 2 * KBG; s.r_lim = it.ya - KBG;
+  s.y0 = it.y_start;
+  if (col_in) {
+    s.sx = a.Dx;
+    s.xp = X + (long long)it.y_start * a.Dx + x;
+    s.wp = a.W + (long long)it.y_start * a.Dx + x;
+    s.nmp = a.nm_pad + (long long)(it.y_start - 3 + PADR) * a.Dx + x;
+    s.icrp = a.ic_pad + (long long)(it.y_start - LAG_B + PADR) * a.Dx + x;
+    s.icsp = a.ic_pad + (long long)(it.y_start - LAG_C + PADR) * a.Dx + x;
+  } else {              // lanes outside the strip read the zero row of a padded plane, over and over
+    s.sx = 0;
+    s.xp = a.nm_pad; s.wp = reinterpret_cast<const uint8_t*>(a.nm_pad);
+    s.nmp = a.nm_pad; s.icrp = a.nm_pad; s.icsp = a.nm_pad;
+  }
 #pragma unroll
   for (int i = 0; i < 8; ++i) { s.hw[i][0] = splat(0.f); s.hw[i][1] = splat(0.f); }
   s.V1[0] = s.V1[1] = s.V2[0] = s.V2[1] = splat(0.f);
+#pragma unroll
+  for (int q = 0; q < 2; ++q)
+#pragma unroll
+    for (int j = 0; j < RB; ++j) {
+      s.pf[q].x[j] = zero4(); s.pf[q].xe[j] = zero4(); s.pf[q].w[j] = 0u; s.pf[q].we[j] = 0u;
+      s.pl[q].nm[j] = zero4(); s.pl[q].icr[j] = zero4(); s.pl[q].ics[j] = zero4();
+    }
   s.w26 = 0;
   __syncthreads();
 
-  s.run();
+  s.run(it.nb);
 
   tm_wait_st();
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
@@ -447,21 +514,22 @@ k_fused_box(const FusedArgs a) {
 
 // ------------------------------------------------------------------------------------------------
 // Work plan (host, once per context): column strips over the valid bounding box, row segments,
-// and the (row, warp) class table of every strip.
+// the per-(iteration, warp) control words of every item, zero-padded normaliser planes.
 struct LpfFusedPlan {
   bool ok = false;
   int CW = 0, NW = 0, threads = 0, n_items = 0;
   size_t smem = 0;
   float nm_const = 1.f, ic_const = 1.f / 625.f;
   FusedItem* d_items = nullptr;
-  uint8_t* d_cls = nullptr;
-  float* d_inv_cnt = nullptr;
+  uint32_t* d_flags = nullptr;
+  float* d_nm_pad = nullptr;
+  float* d_ic_pad = nullptr;
 };
 
-static size_t fused_smem_bytes(int NW, int max_rows) {
+static size_t fused_smem_bytes(int NW, int max_nb) {
   const int CWP = NW * 128, PEV = CWP + 2 * KBG, PET = NW * 32 + 8;
   const size_t nfl = (size_t)DFS * CWP + 4 * RB * PEV + 4 * RB * PET;
-  return nfl * sizeof(float) + (((size_t)(max_rows + 2 * CLS_PAD) * NW + 15) & ~(size_t)15);
+  return (nfl + (size_t)max_nb * NW) * sizeof(float) + 16;
 }
 
 template <int NW>
@@ -480,21 +548,28 @@ static cudaError_t fused_dispatch(int NW, const FusedArgs& a, dim3 grid, size_t 
   }
 }
 
+// class bits of a (row, warp) cell of a strip
+enum { CL_ANYW = 1,    // some valid pixel among the warp's columns +-4
+       CL_ALLW = 2,    // every pixel among the warp's columns +-4 is valid (and the warp is full)
+       CL_NM1 = 4,     // norm_mf is the interior constant on all the warp's columns
+       CL_IC1 = 8 };   // 1/count is 1/625 on all the warp's columns
+
 int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
   *out = nullptr;
   const lpf_params& p = c->p;
   const char* force = getenv("LPF_FORCE_GENERAL");
   if (force && force[0] == '1') return LPF_OK;
-  if (!(p.bg_kernel == 1 && p.k_bg == KBG && p.k_mf == 3 && p.sigma_mf > 0 && p.n_iter == 1 && (p.Dx % 4) == 0 && p.k_max <= 2))
+  if (!(p.bg_kernel == 1 && p.k_bg == KBG && p.k_mf == 3 && p.sigma_mf > 0 && p.n_iter == 1 && (p.Dx % 4) == 0 &&
+        (p.Dy % 2) == 0 && p.k_max <= 2))
     return LPF_OK;
   const int Dy = p.Dy, Dx = p.Dx;
   // valid bounding box, per-column row ranges
-  int vx0 = Dx, vx1 = 0, vy0 = Dy, vy1 = 0;
+  int vx0 = Dx, vx1 = 0;
   std::vector<int> col_y0(Dx, Dy), col_y1(Dx, 0);
   for (int y = 0; y < Dy; ++y)
     for (int x = 0; x < Dx; ++x)
       if (hW[(size_t)y * Dx + x]) {
-        vx0 = std::min(vx0, x); vx1 = std::max(vx1, x + 1); vy0 = std::min(vy0, y); vy1 = std::max(vy1, y + 1);
+        vx0 = std::min(vx0, x); vx1 = std::max(vx1, x + 1);
         col_y0[x] = std::min(col_y0[x], y); col_y1[x] = std::max(col_y1[x], y + 1);
       }
   if (vx1 <= vx0) return LPF_OK;  // nothing valid: the general path handles it
@@ -560,8 +635,8 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
     const double cost = waves * (rows + warm);
     if (cost < best_cost - 1e-9) { best_cost = cost; best_seg = nseg; }
   }
-  std::vector<FusedItem> items;
-  int max_rows = 0;
+  struct ItemEx { FusedItem it; int strip; };
+  std::vector<ItemEx> items;
   for (size_t si = 0; si < strips.size(); ++si) {
     const FusedItem& s = strips[si];
     const int rows = s.yb - s.ya;
@@ -571,28 +646,24 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
     for (int k = 0; k < nseg; ++k) {
       FusedItem it = s;
       it.ya = s.ya + k * th; it.yb = std::min(s.yb, it.ya + th);
-      it.pad0 = (int)si;
-      if (it.ya < it.yb) { items.push_back(it); max_rows = std::max(max_rows, it.yb - it.ya); }
+      if (it.ya < it.yb) items.push_back({it, (int)si});
     }
   }
   if (items.empty()) return LPF_OK;
-  // class table per item: rows ya-64 .. yb+64, NW cells per row
-  std::vector<uint8_t> cls;
-  float nm_interior_pix = -1.f;
+  // (row, warp) classes of every strip, rows -CPAD .. Dy+CPAD
+  const int CPAD = 128;
+  std::vector<std::vector<uint8_t>> cls(strips.size());
   long long interior_pix = -1;
-  for (auto& it : items) {
-    it.cls_off = (int)cls.size();
-    const int nrows = it.yb - it.ya + 2 * CLS_PAD;
-    cls.resize(cls.size() + (size_t)nrows * NW, 0);
-    for (int r = 0; r < nrows; ++r) {
-      const int y = it.ya - CLS_PAD + r;
-      if (y < 0 || y >= Dy) continue;
+  for (size_t si = 0; si < strips.size(); ++si) {
+    const int xs = strips[si].xs;
+    cls[si].assign((size_t)(Dy + 2 * CPAD) * NW, 0);
+    for (int y = 0; y < Dy; ++y)
       for (int w = 0; w < NW; ++w) {
-        const int c0 = it.xs + 128 * w, c1 = std::min(c0 + 128, it.xs + CW);   // own columns [c0, c1)
-        if (c0 >= it.xs + CW) continue;
+        const int c0 = xs + 128 * w, c1 = std::min(c0 + 128, xs + CW);   // own columns [c0, c1)
+        if (c0 >= xs + CW) continue;
         int any = 0, all = 1, nm1 = 1, ic1 = 1;
         for (int x = c0 - 4; x < c0 + 132; ++x) {
-          const bool in = x >= 0 && x < Dx && x >= it.xs - 4 && x < it.xs + CW + 4;
+          const bool in = x >= 0 && x < Dx && x >= xs - 4 && x < xs + CW + 4;
           const bool v = in && hW[(size_t)y * Dx + x];
           any |= v ? 1 : 0;
           if (!v) all = 0;
@@ -605,50 +676,101 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
           if (!nm1 && !ic1) break;
         }
         if (nm1 && interior_pix < 0) interior_pix = (long long)y * Dx + c0;
-        cls[(size_t)it.cls_off + (size_t)r * NW + w] =
+        cls[si][(size_t)(y + CPAD) * NW + w] =
             (uint8_t)((any ? CL_ANYW : 0) | (all ? CL_ALLW : 0) | (nm1 ? CL_NM1 : 0) | (ic1 ? CL_IC1 : 0));
       }
-    }
   }
-  (void)nm_interior_pix;
+  // control words
+  std::vector<uint32_t> flags;
+  std::vector<FusedItem> ditems;
+  int max_nb = 0;
+  for (auto& ie : items) {
+    FusedItem it = ie.it;
+    const std::vector<uint8_t>& cl = cls[ie.strip];
+    auto cell = [&](int y, int w) -> int { return (y < -CPAD || y >= Dy + CPAD) ? 0 : cl[(size_t)(y + CPAD) * NW + w]; };
+    int ys = it.ya - HALO;
+    if (ys & 1) ys -= 1;               // even first row: a row pair never straddles the image edge (Dy is even)
+    it.y_start = ys;
+    it.nb = (it.yb - 1 + LAG_C - ys) / RB + 1;
+    it.fl_off = (int)flags.size();
+    max_nb = std::max(max_nb, it.nb);
+    auto xmode = [&](int y, int w) -> unsigned {
+      const int a0 = cell(y, w), a1 = cell(y + 1, w);
+      if (!((a0 | a1) & CL_ANYW)) return 0u;
+      return (a0 & a1 & CL_ALLW) ? 1u : 2u;
+    };
+    auto both = [&](int y, int w, int bit) -> bool { return (cell(y, w) & cell(y + 1, w) & bit) != 0; };
+    for (int b = 0; b < it.nb; ++b)
+      for (int w = 0; w < NW; ++w) {
+        const int y0 = ys + RB * b;
+        auto ld_bits = [&](int yy) -> unsigned {
+          unsigned f = 0;
+          if (!both(yy - 3, w, CL_NM1)) f |= FL_NM_LD;
+          if (!both(yy - LAG_B, w, CL_IC1)) f |= FL_ICR_LD;
+          const bool c0 = yy - LAG_C >= it.ya && yy - LAG_C < it.yb, c1 = yy + 1 - LAG_C >= it.ya && yy + 1 - LAG_C < it.yb;
+          if ((c0 || c1) && !both(yy - LAG_C, w, CL_IC1)) f |= FL_ICS_LD;
+          return f;
+        };
+        unsigned f = xmode(y0, w);
+        if (b + 2 < it.nb) f |= xmode(y0 + 2 * RB, w) << FL_PMODE_SH;
+        f |= ld_bits(y0);
+        if (b + 1 < it.nb) f |= ld_bits(y0 + RB) << 3;     // FL_*_LD -> FL_*_PF
+        if (y0 - 3 < it.ya - 2 * KBG) f |= FL_GATE_A;
+        if (y0 - LAG_B < it.ya - KBG) f |= FL_GATE_B;
+        if (y0 + 1 - LAG_B >= it.ya - KBG) f |= FL_DO_B;
+        if (y0 - LAG_C >= it.ya && y0 - LAG_C < it.yb) f |= FL_C0;
+        if (y0 + 1 - LAG_C >= it.ya && y0 + 1 - LAG_C < it.yb) f |= FL_C1;
+        flags.push_back(f);
+      }
+    ditems.push_back(it);
+  }
+  static_assert((FL_NM_LD << 3) == FL_NM_PF && (FL_ICR_LD << 3) == FL_ICR_PF && (FL_ICS_LD << 3) == FL_ICS_PF, "flag layout");
+
   LpfFusedPlan* pl = new LpfFusedPlan();
-  pl->CW = CW; pl->NW = NW; pl->threads = NW * 32; pl->n_items = (int)items.size();
-  pl->smem = fused_smem_bytes(NW, max_rows);
+  pl->CW = CW; pl->NW = NW; pl->threads = NW * 32; pl->n_items = (int)ditems.size();
+  pl->smem = fused_smem_bytes(NW, max_nb);
   int dev = 0; cudaGetDevice(&dev);
   int max_smem = 0;
   cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   if (pl->smem > (size_t)max_smem) { delete pl; return LPF_OK; }
+  *out = pl;   // owned by the context from here on (freed by lpf_destroy on any later failure)
   if (interior_pix >= 0) LPF_CUDA(cudaMemcpy(&pl->nm_const, c->norm_mf + interior_pix, sizeof(float), cudaMemcpyDeviceToHost));
-  // 1 / (number of valid pixels in the 25x25 window), 0 at invalid pixels: box taps of 1 give exact counts
-  LPF_CUDA(cudaMalloc((void**)&pl->d_inv_cnt, (size_t)c->N * sizeof(float)));
+  // zero-padded copies of norm_mf and of 1 / (number of valid pixels in the 25x25 window; 0 at invalid
+  // pixels: box taps of 1 give exact counts)
+  const size_t npad = (size_t)(Dy + 2 * PADR) * Dx;
+  LPF_CUDA(cudaMalloc((void**)&pl->d_nm_pad, npad * sizeof(float)));
+  LPF_CUDA(cudaMalloc((void**)&pl->d_ic_pad, npad * sizeof(float)));
+  LPF_CUDA(cudaMemset(pl->d_nm_pad, 0, npad * sizeof(float)));
+  LPF_CUDA(cudaMemset(pl->d_ic_pad, 0, npad * sizeof(float)));
+  LPF_CUDA(cudaMemcpy(pl->d_nm_pad + (size_t)PADR * Dx, c->norm_mf, (size_t)c->N * sizeof(float), cudaMemcpyDeviceToDevice));
   {
     LpfTaps ones;
     ones.R = KBG;
     for (int i = 0; i < LPF_NTAPS; ++i) ones.g[i] = i < WINB ? 1.f : 0.f;
-    int rc = lpf_launch_static_norm(c, ones, pl->d_inv_cnt, nullptr, 0);
+    int rc = lpf_launch_static_norm(c, ones, pl->d_ic_pad + (size_t)PADR * Dx, nullptr, 0);
     if (rc) return rc;
   }
-  LPF_CUDA(cudaMalloc((void**)&pl->d_items, items.size() * sizeof(FusedItem)));
-  LPF_CUDA(cudaMemcpy(pl->d_items, items.data(), items.size() * sizeof(FusedItem), cudaMemcpyHostToDevice));
-  LPF_CUDA(cudaMalloc((void**)&pl->d_cls, cls.size()));
-  LPF_CUDA(cudaMemcpy(pl->d_cls, cls.data(), cls.size(), cudaMemcpyHostToDevice));
+  LPF_CUDA(cudaMalloc((void**)&pl->d_items, ditems.size() * sizeof(FusedItem)));
+  LPF_CUDA(cudaMemcpy(pl->d_items, ditems.data(), ditems.size() * sizeof(FusedItem), cudaMemcpyHostToDevice));
+  LPF_CUDA(cudaMalloc((void**)&pl->d_flags, flags.size() * sizeof(uint32_t)));
+  LPF_CUDA(cudaMemcpy(pl->d_flags, flags.data(), flags.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
   FusedArgs dummy{};
   LPF_CUDA(fused_dispatch(NW, dummy, dim3(1), pl->smem, 0, true));
   pl->ok = true;
-  *out = pl;
   return LPF_OK;
 }
 
 void lpf_fused_plan_free(LpfFusedPlan* pl) {
   if (!pl) return;
   if (pl->d_items) cudaFree(pl->d_items);
-  if (pl->d_cls) cudaFree(pl->d_cls);
-  if (pl->d_inv_cnt) cudaFree(pl->d_inv_cnt);
+  if (pl->d_flags) cudaFree(pl->d_flags);
+  if (pl->d_nm_pad) cudaFree(pl->d_nm_pad);
+  if (pl->d_ic_pad) cudaFree(pl->d_ic_pad);
   delete pl;
 }
 
 int lpf_fused_plan_info(const LpfFusedPlan* pl, int* cw, int* threads, int* n_items, long long* smem) {
-  if (!pl) return 0;
+  if (!pl || !pl->ok) return 0;
   *cw = pl->CW; *threads = pl->threads; *n_items = pl->n_items; *smem = (long long)pl->smem;
   return 1;
 }
@@ -660,7 +782,7 @@ int lpf_launch_detect_fused(lpf_ctx* c, LpfFusedPlan* pl, LpfLane& L, const floa
   if (p.detect_sum_plane) { int rc = lpf_launch_sum_plane(c, L, d_cube, d_band_ok, st); if (rc) return rc; }
   FusedArgs a{};
   a.cube = d_cube; a.sum_plane = L.sum_plane; a.band_ok = d_band_ok; a.W = c->W;
-  a.norm_mf = c->norm_mf; a.inv_cnt = pl->d_inv_cnt; a.items = pl->d_items; a.cls = pl->d_cls;
+  a.nm_pad = pl->d_nm_pad; a.ic_pad = pl->d_ic_pad; a.items = pl->d_items; a.flags = pl->d_flags;
   a.B = p.B; a.Dy = p.Dy; a.Dx = p.Dx; a.CW = pl->CW; a.k_max = p.k_max; a.max_det = p.max_det;
   a.g0 = c->g_mf.g[3]; a.g1 = c->g_mf.g[2]; a.g2 = c->g_mf.g[1]; a.g3 = c->g_mf.g[0];
   a.kappa2 = p.kappa * p.kappa; a.eps_rel = p.eps_rel; a.nm_const = pl->nm_const; a.ic_const = pl->ic_const;
