@@ -39,7 +39,9 @@ constexpr int RB = 2;               // rows per iteration
 constexpr int HALO = 2 * KBG + 3;   // rows of X above the first output row (27)
 constexpr int LAG_B = 3 + KBG + RB;          // rho = y - 17
 constexpr int LAG_C = LAG_B + KBG + RB;      // sig = y - 31
-constexpr int DFS = 32;             // shared-memory ring of F rows (local maxima): power of two
+constexpr int DFS = 36;             // shared-memory ring of F rows (local maxima are tested one iteration late)
+constexpr int QCAP = 32;            // queued candidates per warp and iteration (more are tested in place)
+constexpr int RCAP = 32;            // staged records per warp between flushes
 constexpr int DT = WINB + 1;        // tensor-memory ring depth (rows) of F and of d
 constexpr int TM_D = 4 * DT;        // first tensor-memory column of the d ring (F ring starts at 0)
 constexpr int PADR = 64;            // zero rows above and below the padded normaliser planes
@@ -127,39 +129,40 @@ __device__ __forceinline__ void hbox25(int ev, int et, float out[4]) {
 }
 
 // eq. 5 guard + eq. 6 + eq. 7 for one pixel that passed the unguarded eq. 5, by the whole warp:
-// lane k < (2 k_max + 1)^2 looks at one neighbour in the shared-memory ring of F (float index ringF,
-// row pitch CWP).  d, s: the pixel's residual and spread (already broadcast); cl: its column in the strip.
-__device__ __noinline__ void fused_candidate(const FusedArgs* ap, int ringF, int CWP, int xs, int plane, int lane,
-                                             float d, float s, int cl, int sg) {
+// lane k < (2 k_max + 1)^2 looks at one neighbour in the shared-memory ring of F (float index 0, row
+// pitch CWP, DFS rows, row r in slot (r - ring_y0) mod DFS).  d, s: the pixel's residual and spread;
+// cl: its column in the strip.  An accepted record is written to shared memory at float index
+// rec_at (6 words) and true is returned (warp-uniform).
+__device__ __noinline__ bool fused_candidate(const FusedArgs* ap, int CWP, int xs, int plane, int lane, int ring_y0,
+                                             float d, float s, int cl, int sg, int rec_at) {
   const FusedArgs& a = *ap;
-  const float fv = lds1(ringF + (sg & (DFS - 1)) * CWP + cl);
+  const float fv = lds1((unsigned)(sg - ring_y0) % DFS * CWP + cl);
   const float cc = fv - d;
   const float gd = a.eps_rel * fabsf(cc);
   const float se = fmaxf(s, gd * gd);
-  if (!(d > 0.f && d * d > a.kappa2 * se)) return;   // warp-uniform
+  if (!(d > 0.f && d * d > a.kappa2 * se)) return false;   // warp-uniform
   const int km = a.k_max, side = 2 * km + 1;
   bool bigger = false;
   if (lane < side * side) {
-    const int dy = lane / side - km, dx = lane - (lane / side) * side - km;
+    const int q = (lane * 13) >> 6;                        // lane / 5 for lane < 25 (side <= 5: k_max <= 2)
+    const int row = side == 5 ? q : (side == 3 ? (lane * 11) >> 5 : 0);
+    const int dy = row - km, dx = lane - row * side - km;
     const int yy = sg + dy, c2 = cl + dx, xn = xs + c2;
     if (yy >= 0 && yy < a.Dy && c2 >= 0 && c2 < CWP && xn < a.Dx) {
-      const float fn = lds1(ringF + (yy & (DFS - 1)) * CWP + c2);
+      const float fn = lds1((unsigned)(yy - ring_y0) % DFS * CWP + c2);
       // masked pixels hold F = 0 in the ring: W is consulted only when such a zero would win
       if (fn > fv) bigger = (fn != 0.f) || (a.W[(long long)yy * a.Dx + xn] != 0);
     }
   }
-  if (__any_sync(0xffffffffu, bigger)) return;
+  if (__any_sync(0xffffffffu, bigger)) return false;
   if (lane == 0) {
-    const int idx = atomicAdd(a.ndets, 1);
-    if (idx < a.max_det) {
-      lpf_det r;
-      r.pix = sg * a.Dx + xs + cl; r.plane = (int16_t)plane; r.iter = 1;
-      r.f = fv; r.c = cc; r.s = se; r.snr = d / sqrtf(se);
-      a.dets[idx] = r;
-    } else {
-      atomicAdd(&a.counters[0], 1);
-    }
+    uint32_t* r = reinterpret_cast<uint32_t*>(g_sm4) + rec_at;
+    r[0] = (uint32_t)(sg * a.Dx + xs + cl);
+    r[1] = (uint32_t)(plane & 0xffff) | (1u << 16);        // int16 plane, int16 iter = 1
+    r[2] = __float_as_uint(fv); r[3] = __float_as_uint(cc); r[4] = __float_as_uint(se);
+    r[5] = __float_as_uint(d / sqrtf(se));
   }
+  return true;
 }
 
 struct Prefetch {          // one iteration's worth of input rows, loaded two iterations ahead
@@ -180,7 +183,10 @@ struct Sweep {
   static constexpr int O_EV2 = O_EV1 + 2 * RB * PEV;
   static constexpr int O_ET1 = O_EV2 + 2 * RB * PEV;
   static constexpr int O_ET2 = O_ET1 + 2 * RB * PET;
-  static constexpr int O_FL = O_ET2 + 2 * RB * PET;   // control words, [nb][NW]
+  static constexpr int O_Q = O_ET2 + 2 * RB * PET;    // candidate queues, [2][NW][QCAP] x {col, row, d, s}
+  static constexpr int O_QN = O_Q + 2 * NW * QCAP * 4;  // their lengths, [2][NW] (padded to 16 words)
+  static constexpr int O_ST = O_QN + 16;                // staged records, [NW][RCAP] x 8 words
+  static constexpr int O_FL = O_ST + NW * RCAP * 8;     // control words, [nb][NW]
   // ---- constants of the thread -----------------------------------------------------------------
   const FusedArgs& a;
   const FusedArgs* a_sh;   // the same arguments in shared memory (for the out-of-line candidate path)
@@ -198,6 +204,9 @@ struct Sweep {
   const float* icsp;       // padded 1/count at the next iteration's first sigma row
   int y0;                  // first input row of the current iteration
   int w26;                 // tensor-memory ring slot of this iteration's first row
+  int wF;                  // shared-memory ring slot of this iteration's first F row
+  int ring_y0;             // the row that sits in slot 0 of the shared-memory ring (mod DFS)
+  int qcount, nrec;        // candidates queued in this iteration; records staged by this warp
   float2 hw[8][2];         // horizontally filtered rows (rotating; static indices per phase)
   float2 V1[2], V2[2];     // vertical running sums
   Prefetch pf[2];
@@ -207,6 +216,52 @@ struct Sweep {
 
   __device__ __forceinline__ unsigned ctl(int b) const {
     return reinterpret_cast<const uint32_t*>(g_sm4)[O_FL + b * NW + warp];
+  }
+
+  // staged records of the warp -> global list: one atomic for the lot
+  __device__ __forceinline__ void flush_records() {
+    if (nrec > 0) {
+      int base = 0;
+      if (lane == 0) base = atomicAdd(a.ndets, nrec);
+      base = __shfl_sync(0xffffffffu, base, 0);
+      __syncwarp();
+      if (lane < nrec) {
+        const uint2* r = reinterpret_cast<const uint2*>(reinterpret_cast<const uint32_t*>(g_sm4) + O_ST + (warp * RCAP + lane) * 8);
+        const int idx = base + lane;
+        if (idx < a.max_det) {
+          uint2* dst = reinterpret_cast<uint2*>(a.dets + idx);
+          dst[0] = r[0]; dst[1] = r[1]; dst[2] = r[2];
+        } else {
+          atomicAdd(&a.counters[0], 1);
+        }
+      }
+      __syncwarp();
+      nrec = 0;
+    }
+  }
+
+  __device__ __forceinline__ void test_candidate(float d, float sp, int cl, int sg) {
+    if (fused_candidate(a_sh, CWP, xs, plane, lane, ring_y0, d, sp, cl, sg, O_ST + (warp * RCAP + nrec) * 8)) {
+      if (++nrec == RCAP) flush_records();
+    }
+  }
+
+  // eq. 6 / eq. 7 for the pixels all warps queued in the previous iteration, dealt round-robin to the warps
+  __device__ __forceinline__ void process_queue(int qb) {
+    const int n_mine = lane < NW ? reinterpret_cast<const int*>(g_sm4)[O_QN + qb * NW + lane] : 0;
+    int pre = n_mine;
+#pragma unroll
+    for (int o = 1; o < NW; o <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, pre, o);
+      if (lane >= o) pre += t;
+    }
+    const int total = __shfl_sync(0xffffffffu, pre, NW - 1);
+    for (int e = warp; e < total; e += NW) {
+      const int owner = __popc(__ballot_sync(0xffffffffu, lane < NW && pre <= e));
+      const int start = __shfl_sync(0xffffffffu, pre - n_mine, owner);
+      const float4 q = lds4(O_Q + ((qb * NW + owner) * QCAP + (e - start)) * 4);
+      test_candidate(q.z, q.w, __float_as_int(q.x), __float_as_int(q.y));
+    }
   }
 
   // global loads of two input rows into pf[slot]; mode 1: all valid, 2: masked (W loaded too)
@@ -284,6 +339,7 @@ struct Sweep {
     load_planes(pbuf, fl & FL_NM_PF, fl & FL_ICR_PF, fl & FL_ICS_PF);
 
     tm_wait_ld();
+    process_queue(pbuf);
 #pragma unroll
     for (int j = 0; j < RB; ++j) tm_use(fold[j][0], fold[j][1]);
     // ---- second batch: F(rho), d(rho - 25), d(sigma) -------------------------------------------------
@@ -329,7 +385,7 @@ struct Sweep {
         V1[0] = add2(V1[0], sub2(f[j][0], fold[j][0]));
         V1[1] = add2(V1[1], sub2(f[j][1], fold[j][1]));
         tm_st4(tm + 4 * wrap26(w26 + j), f[j][0], f[j][1]);
-        sts4(O_RING + ((y0 + j - 3) & (DFS - 1)) * CWP + 4 * tid, make_float4(f[j][0].x, f[j][0].y, f[j][1].x, f[j][1].y));
+        sts4(O_RING + (wF + j >= DFS ? wF + j - DFS : wF + j) * CWP + 4 * tid, make_float4(f[j][0].x, f[j][0].y, f[j][1].x, f[j][1].y));
         sts4(O_EV1 + (buf * RB + j) * PEV + KBG + 4 * tid, make_float4(V1[0].x, V1[0].y, V1[1].x, V1[1].y));
         const float2 ts = add2(V1[0], V1[1]);
         sts1(O_ET1 + (buf * RB + j) * PET + 3 + tid, ts.x + ts.y);
@@ -388,20 +444,32 @@ struct Sweep {
           const float dv[4] = {dlag[j][0].x, dlag[j][0].y, dlag[j][1].x, dlag[j][1].y};
           const float sv[4] = {s0.x, s0.y, s1.x, s1.y};
           const int sg = y0 + j - LAG_C;
+          const unsigned lt = (1u << lane) - 1u;
 #pragma unroll
           for (int k = 0; k < 4; ++k) {
-            unsigned m = __ballot_sync(0xffffffffu, (bits >> k) & 1u);
-            while (m) {
-              const int src = __ffs(m) - 1;
-              m &= m - 1;
-              const float d = __shfl_sync(0xffffffffu, dv[k], src);
-              const float s = __shfl_sync(0xffffffffu, sv[k], src);
-              fused_candidate(a_sh, O_RING, CWP, xs, plane, lane, d, s, 4 * (warp * 32 + src) + k, sg);
+            const bool on = (bits >> k) & 1u;
+            const unsigned m = __ballot_sync(0xffffffffu, on);
+            const int pos = qcount + __popc(m & lt);
+            if (on && pos < QCAP)
+              sts4(O_Q + ((buf * NW + warp) * QCAP + pos) * 4,
+                   make_float4(__int_as_float(4 * tid + k), __int_as_float(sg), dv[k], sv[k]));
+            qcount += __popc(m);
+            if (qcount > QCAP) {                     // queue full (rare): test the rest in place
+              unsigned ovf = __ballot_sync(0xffffffffu, on && pos >= QCAP);
+              while (ovf) {
+                const int src = __ffs(ovf) - 1;
+                ovf &= ovf - 1;
+                test_candidate(__shfl_sync(0xffffffffu, dv[k], src), __shfl_sync(0xffffffffu, sv[k], src),
+                               4 * (warp * 32 + src) + k, sg);
+              }
             }
           }
         }
       }
     }
+    if (lane == 0) reinterpret_cast<int*>(g_sm4)[O_QN + buf * NW + warp] = qcount < QCAP ? qcount : QCAP;
+    qcount = 0;
+    wF = wF + RB >= DFS ? wF + RB - DFS : wF + RB;
     w26 = wrap26(w26 + RB);
     y0 += RB;
     tm_wait_st();
@@ -423,6 +491,8 @@ struct Sweep {
       iteration<2>(b); if (++b >= nb) break;
       iteration<3>(b); if (++b >= nb) break;
     }
+    process_queue((nb - 1) & 1);     // what the last iteration queued
+    flush_records();
   }
 };
 
@@ -498,7 +568,7 @@ k_fused_box(const FusedArgs a) {
       s.pf[q].x[j] = zero4(); s.pf[q].xe[j] = zero4(); s.pf[q].w[j] = 0u; s.pf[q].we[j] = 0u;
       s.pl[q].nm[j] = zero4(); s.pl[q].icr[j] = zero4(); s.pl[q].ics[j] = zero4();
     }
-  s.w26 = 0;
+  s.w26 = 0; s.wF = 0; s.ring_y0 = it.y_start - 3; s.qcount = 0; s.nrec = 0;
   __syncthreads();
 
   s.run(it.nb);
@@ -528,7 +598,7 @@ struct LpfFusedPlan {
 
 static size_t fused_smem_bytes(int NW, int max_nb) {
   const int CWP = NW * 128, PEV = CWP + 2 * KBG, PET = NW * 32 + 8;
-  const size_t nfl = (size_t)DFS * CWP + 4 * RB * PEV + 4 * RB * PET;
+  const size_t nfl = (size_t)DFS * CWP + 4 * RB * PEV + 4 * RB * PET + 2 * NW * QCAP * 4 + 16 + NW * RCAP * 8;
   return (nfl + (size_t)max_nb * NW) * sizeof(float) + 16;
 }
 
@@ -630,6 +700,7 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
   for (int nseg = 1; nseg <= 64; ++nseg) {
     const double rows = (double)max_rows_strip / nseg;
     if (nseg > 1 && rows < 24) break;
+    if (rows > 900 && nseg < 64) continue;      // keeps an item's control words within shared memory
     const long long ctas = (long long)nseg * n_strips * n_planes;
     const double waves = (double)((ctas + c->n_sm - 1) / c->n_sm);
     const double cost = waves * (rows + warm);
