@@ -86,13 +86,13 @@ __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y
 // ---- tensor memory as a thread-private scratch ring ---------------------------------------------
 __device__ __forceinline__ void tm_st4(uint32_t taddr, float2 lo, float2 hi) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};\n"
-               ::"r"(taddr), "f"(lo.x), "f"(lo.y), "f"(hi.x), "f"(hi.y) : "memory");
+               ::"r"(taddr), "f"(lo.x), "f"(lo.y), "f"(hi.x), "f"(hi.y));
 }
 __device__ __forceinline__ void tm_ld4(uint32_t taddr, float2& lo, float2& hi) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];\n"
-               : "=f"(lo.x), "=f"(lo.y), "=f"(hi.x), "=f"(hi.y) : "r"(taddr) : "memory");
+               : "=f"(lo.x), "=f"(lo.y), "=f"(hi.x), "=f"(hi.y) : "r"(taddr));
 }
-__device__ __forceinline__ void tm_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory"); }
+__device__ __forceinline__ void tm_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;\n"); }
 __device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;\n" ::: "memory"); }
 // pins a value loaded by tm_ld4 behind the tm_wait_ld that precedes this statement
 __device__ __forceinline__ void tm_use(float2& lo, float2& hi) {
@@ -128,41 +128,99 @@ __device__ __forceinline__ void hbox25(int ev, int et, float out[4]) {
   out[3] = out[2] + (R.w - L.z);
 }
 
+// ---- candidate path (out of line: it is the rare part, and it keeps the sweep's code small) -------
+struct CandCtx {           // what the out-of-line functions need, by value
+  const FusedArgs* ap;     // kernel arguments (shared-memory copy)
+  int CWP, xs, plane, lane, ring_y0;
+  int o_st;                // float index of the warp's record staging area (RCAP x 8 words)
+};
+
+// staged records of a warp -> global list: one atomic for the lot.  Returns the new count (0).
+__device__ __noinline__ int cand_flush(const FusedArgs* ap, int o_st, int lane, int nrec) {
+  if (nrec <= 0) return 0;
+  int base = 0;
+  if (lane == 0) base = atomicAdd(ap->ndets, nrec);
+  base = __shfl_sync(0xffffffffu, base, 0);
+  __syncwarp();
+  if (lane < nrec) {
+    const uint2* r = reinterpret_cast<const uint2*>(reinterpret_cast<const uint32_t*>(g_sm4) + o_st + lane * 8);
+    const int idx = base + lane;
+    if (idx < ap->max_det) {
+      uint2* dst = reinterpret_cast<uint2*>(ap->dets + idx);
+      dst[0] = r[0]; dst[1] = r[1]; dst[2] = r[2];
+    } else {
+      atomicAdd(&ap->counters[0], 1);
+    }
+  }
+  __syncwarp();
+  return 0;
+}
+
 // eq. 5 guard + eq. 6 + eq. 7 for one pixel that passed the unguarded eq. 5, by the whole warp:
 // lane k < (2 k_max + 1)^2 looks at one neighbour in the shared-memory ring of F (float index 0, row
 // pitch CWP, DFS rows, row r in slot (r - ring_y0) mod DFS).  d, s: the pixel's residual and spread;
-// cl: its column in the strip.  An accepted record is written to shared memory at float index
-// rec_at (6 words) and true is returned (warp-uniform).
-__device__ __noinline__ bool fused_candidate(const FusedArgs* ap, int CWP, int xs, int plane, int lane, int ring_y0,
-                                             float d, float s, int cl, int sg, int rec_at) {
-  const FusedArgs& a = *ap;
-  const float fv = lds1((unsigned)(sg - ring_y0) % DFS * CWP + cl);
+// cl: its column in the strip; sg: its row.  An accepted record is staged in shared memory; returns the
+// warp's new staged count (flushing when the stage is full).
+__device__ __forceinline__ int cand_test_body(const CandCtx& c, int nrec, float d, float s, int cl, int sg) {
+  const FusedArgs& a = *c.ap;
+  const int CWP = c.CWP, lane = c.lane;
+  const float fv = lds1((unsigned)(sg - c.ring_y0) % DFS * CWP + cl);
   const float cc = fv - d;
   const float gd = a.eps_rel * fabsf(cc);
   const float se = fmaxf(s, gd * gd);
-  if (!(d > 0.f && d * d > a.kappa2 * se)) return false;   // warp-uniform
+  if (!(d > 0.f && d * d > a.kappa2 * se)) return nrec;   // warp-uniform
   const int km = a.k_max, side = 2 * km + 1;
   bool bigger = false;
   if (lane < side * side) {
-    const int q = (lane * 13) >> 6;                        // lane / 5 for lane < 25 (side <= 5: k_max <= 2)
-    const int row = side == 5 ? q : (side == 3 ? (lane * 11) >> 5 : 0);
+    const int row = side == 5 ? (lane * 13) >> 6 : (side == 3 ? (lane * 11) >> 5 : 0);   // lane / side (k_max <= 2)
     const int dy = row - km, dx = lane - row * side - km;
-    const int yy = sg + dy, c2 = cl + dx, xn = xs + c2;
+    const int yy = sg + dy, c2 = cl + dx, xn = c.xs + c2;
     if (yy >= 0 && yy < a.Dy && c2 >= 0 && c2 < CWP && xn < a.Dx) {
-      const float fn = lds1((unsigned)(yy - ring_y0) % DFS * CWP + c2);
+      const float fn = lds1((unsigned)(yy - c.ring_y0) % DFS * CWP + c2);
       // masked pixels hold F = 0 in the ring: W is consulted only when such a zero would win
       if (fn > fv) bigger = (fn != 0.f) || (a.W[(long long)yy * a.Dx + xn] != 0);
     }
   }
-  if (__any_sync(0xffffffffu, bigger)) return false;
+  if (__any_sync(0xffffffffu, bigger)) return nrec;
   if (lane == 0) {
-    uint32_t* r = reinterpret_cast<uint32_t*>(g_sm4) + rec_at;
-    r[0] = (uint32_t)(sg * a.Dx + xs + cl);
-    r[1] = (uint32_t)(plane & 0xffff) | (1u << 16);        // int16 plane, int16 iter = 1
+    uint32_t* r = reinterpret_cast<uint32_t*>(g_sm4) + c.o_st + nrec * 8;
+    r[0] = (uint32_t)(sg * a.Dx + c.xs + cl);
+    r[1] = (uint32_t)(c.plane & 0xffff) | (1u << 16);        // int16 plane, int16 iter = 1
     r[2] = __float_as_uint(fv); r[3] = __float_as_uint(cc); r[4] = __float_as_uint(se);
     r[5] = __float_as_uint(d / sqrtf(se));
   }
-  return true;
+  ++nrec;
+  if (nrec == RCAP) nrec = cand_flush(c.ap, c.o_st, lane, nrec);
+  return nrec;
+}
+
+// entries e = first, first + step, ... < total of the CTA's queue qb (per-warp lists of lengths n_mine
+// held by lanes < nw, inclusive prefix pre): the calling warp's share of last iteration's candidates
+__device__ __noinline__ int cand_drain(CandCtx c, int nrec, int o_q, int nw, int first, int n_mine, int pre) {
+  const int total = __shfl_sync(0xffffffffu, pre, nw - 1);
+  for (int e = first; e < total; e += nw) {
+    const int owner = __popc(__ballot_sync(0xffffffffu, c.lane < nw && pre <= e));
+    const int start = __shfl_sync(0xffffffffu, pre - n_mine, owner);
+    const float4 q = lds4(o_q + (owner * QCAP + (e - start)) * 4);
+    nrec = cand_test_body(c, nrec, q.z, q.w, __float_as_int(q.x), __float_as_int(q.y));
+  }
+  return nrec;
+}
+
+// a row whose candidates do not fit the queue any more (rare): tested in place
+__device__ __noinline__ int cand_row_in_place(CandCtx c, int nrec, unsigned bits, float4 dv, float4 sv, int cl0, int sg) {
+  for (int k = 0; k < 4; ++k) {
+    unsigned m = __ballot_sync(0xffffffffu, (bits >> k) & 1u);
+    const float dk = k == 0 ? dv.x : (k == 1 ? dv.y : (k == 2 ? dv.z : dv.w));
+    const float sk = k == 0 ? sv.x : (k == 1 ? sv.y : (k == 2 ? sv.z : sv.w));
+    while (m) {
+      const int src = __ffs(m) - 1;
+      m &= m - 1;
+      nrec = cand_test_body(c, nrec, __shfl_sync(0xffffffffu, dk, src), __shfl_sync(0xffffffffu, sk, src),
+                            __shfl_sync(0xffffffffu, cl0, src) + k, sg);
+    }
+  }
+  return nrec;
 }
 
 struct Prefetch {          // one iteration's worth of input rows, loaded two iterations ahead
@@ -218,32 +276,11 @@ struct Sweep {
     return reinterpret_cast<const uint32_t*>(g_sm4)[O_FL + b * NW + warp];
   }
 
-  // staged records of the warp -> global list: one atomic for the lot
-  __device__ __forceinline__ void flush_records() {
-    if (nrec > 0) {
-      int base = 0;
-      if (lane == 0) base = atomicAdd(a.ndets, nrec);
-      base = __shfl_sync(0xffffffffu, base, 0);
-      __syncwarp();
-      if (lane < nrec) {
-        const uint2* r = reinterpret_cast<const uint2*>(reinterpret_cast<const uint32_t*>(g_sm4) + O_ST + (warp * RCAP + lane) * 8);
-        const int idx = base + lane;
-        if (idx < a.max_det) {
-          uint2* dst = reinterpret_cast<uint2*>(a.dets + idx);
-          dst[0] = r[0]; dst[1] = r[1]; dst[2] = r[2];
-        } else {
-          atomicAdd(&a.counters[0], 1);
-        }
-      }
-      __syncwarp();
-      nrec = 0;
-    }
-  }
-
-  __device__ __forceinline__ void test_candidate(float d, float sp, int cl, int sg) {
-    if (fused_candidate(a_sh, CWP, xs, plane, lane, ring_y0, d, sp, cl, sg, O_ST + (warp * RCAP + nrec) * 8)) {
-      if (++nrec == RCAP) flush_records();
-    }
+  __device__ __forceinline__ CandCtx cand_ctx() const {
+    CandCtx c;
+    c.ap = a_sh; c.CWP = CWP; c.xs = xs; c.plane = plane; c.lane = lane; c.ring_y0 = ring_y0;
+    c.o_st = O_ST + warp * RCAP * 8;
+    return c;
   }
 
   // eq. 6 / eq. 7 for the pixels all warps queued in the previous iteration, dealt round-robin to the warps
@@ -255,13 +292,8 @@ struct Sweep {
       const int t = __shfl_up_sync(0xffffffffu, pre, o);
       if (lane >= o) pre += t;
     }
-    const int total = __shfl_sync(0xffffffffu, pre, NW - 1);
-    for (int e = warp; e < total; e += NW) {
-      const int owner = __popc(__ballot_sync(0xffffffffu, lane < NW && pre <= e));
-      const int start = __shfl_sync(0xffffffffu, pre - n_mine, owner);
-      const float4 q = lds4(O_Q + ((qb * NW + owner) * QCAP + (e - start)) * 4);
-      test_candidate(q.z, q.w, __float_as_int(q.x), __float_as_int(q.y));
-    }
+    if (__shfl_sync(0xffffffffu, pre, NW - 1) > warp)      // something for this warp
+      nrec = cand_drain(cand_ctx(), nrec, O_Q + qb * NW * QCAP * 4, NW, warp, n_mine, pre);
   }
 
   // global loads of two input rows into pf[slot]; mode 1: all valid, 2: masked (W loaded too)
@@ -296,6 +328,7 @@ struct Sweep {
     constexpr int buf = PH & 1, pbuf = buf ^ 1;
     const unsigned fl = ctl(b);
     const float2 g0 = splat(a.g0), g1 = splat(a.g1), g2 = splat(a.g2), g3 = splat(a.g3);
+    process_queue(pbuf);
 
     // ---- tensor-memory reads, first batch: F(fr - 25) ------------------------------------------------
     float2 fold[RB][2];
@@ -339,7 +372,6 @@ struct Sweep {
     load_planes(pbuf, fl & FL_NM_PF, fl & FL_ICR_PF, fl & FL_ICS_PF);
 
     tm_wait_ld();
-    process_queue(pbuf);
 #pragma unroll
     for (int j = 0; j < RB; ++j) tm_use(fold[j][0], fold[j][1]);
     // ---- second batch: F(rho), d(rho - 25), d(sigma) -------------------------------------------------
@@ -445,29 +477,26 @@ struct Sweep {
           const float sv[4] = {s0.x, s0.y, s1.x, s1.y};
           const int sg = y0 + j - LAG_C;
           const unsigned lt = (1u << lane) - 1u;
+          const int nrow = __popc(__ballot_sync(0xffffffffu, bits & 1u)) + __popc(__ballot_sync(0xffffffffu, bits & 2u)) +
+                           __popc(__ballot_sync(0xffffffffu, bits & 4u)) + __popc(__ballot_sync(0xffffffffu, bits & 8u));
+          if (qcount + nrow > QCAP) {                // queue full (rare): test the row in place
+            nrec = cand_row_in_place(cand_ctx(), nrec, bits, make_float4(dv[0], dv[1], dv[2], dv[3]),
+                                     make_float4(sv[0], sv[1], sv[2], sv[3]), 4 * tid, sg);
+          } else {
 #pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            const bool on = (bits >> k) & 1u;
-            const unsigned m = __ballot_sync(0xffffffffu, on);
-            const int pos = qcount + __popc(m & lt);
-            if (on && pos < QCAP)
-              sts4(O_Q + ((buf * NW + warp) * QCAP + pos) * 4,
-                   make_float4(__int_as_float(4 * tid + k), __int_as_float(sg), dv[k], sv[k]));
-            qcount += __popc(m);
-            if (qcount > QCAP) {                     // queue full (rare): test the rest in place
-              unsigned ovf = __ballot_sync(0xffffffffu, on && pos >= QCAP);
-              while (ovf) {
-                const int src = __ffs(ovf) - 1;
-                ovf &= ovf - 1;
-                test_candidate(__shfl_sync(0xffffffffu, dv[k], src), __shfl_sync(0xffffffffu, sv[k], src),
-                               4 * (warp * 32 + src) + k, sg);
-              }
+            for (int k = 0; k < 4; ++k) {
+              const bool on = (bits >> k) & 1u;
+              const unsigned m = __ballot_sync(0xffffffffu, on);
+              if (on)
+                sts4(O_Q + ((buf * NW + warp) * QCAP + qcount + __popc(m & lt)) * 4,
+                     make_float4(__int_as_float(4 * tid + k), __int_as_float(sg), dv[k], sv[k]));
+              qcount += __popc(m);
             }
           }
         }
       }
     }
-    if (lane == 0) reinterpret_cast<int*>(g_sm4)[O_QN + buf * NW + warp] = qcount < QCAP ? qcount : QCAP;
+    if (lane == 0) reinterpret_cast<int*>(g_sm4)[O_QN + buf * NW + warp] = qcount;
     qcount = 0;
     wF = wF + RB >= DFS ? wF + RB - DFS : wF + RB;
     w26 = wrap26(w26 + RB);
@@ -492,7 +521,7 @@ struct Sweep {
       iteration<3>(b); if (++b >= nb) break;
     }
     process_queue((nb - 1) & 1);     // what the last iteration queued
-    flush_records();
+    nrec = cand_flush(a_sh, O_ST + warp * RCAP * 8, lane, nrec);
   }
 };
 
