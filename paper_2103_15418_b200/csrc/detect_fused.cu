@@ -7,22 +7,25 @@
 // down a segment of rows, two rows per iteration, as a three-stage software pipeline with ONE
 // block barrier per iteration (the stages of one iteration work on different rows, so their
 // shared-memory exchanges are double buffered and independent):
-//   A  rows y:        128-bit loads of X two iterations ahead (registers) -> mask -> horizontal
-//                     7-tap matched filter with the neighbours' pixels taken by warp shuffles ->
-//                     vertical 7-tap on a register window (packed f32x2) -> F(y-3);
-//                     25-row running sum V1 += F(y-3) - F(y-28)
+//   A  rows y:        the input rows arrive in shared memory by bulk asynchronous copies (TMA,
+//                     cp.async.bulk + mbarrier) issued three iterations ahead by one thread; every
+//                     thread reads its 4 pixels and both neighbours' with three 128-bit shared loads ->
+//                     horizontal 7-tap matched filter -> vertical 7-tap on a register window (packed
+//                     f32x2) -> F(y-3); 25-row running sum V1 += F(y-3) - F(y-28)
 //   B  rows rho=y-17: horizontal 25-box of V1 (blocked partial sums) x 1/count -> C (eq. 3);
 //                     d = F - C; 25-row running sum V2 += d^2 - d_old^2
-//   C  rows sig=y-31: horizontal 25-box of V2 x 1/count -> S (eq. 4); eq. 5 on d(sig); the few
-//                     pixels that pass are handed to the whole warp: S_eff guard (R8), eq. 6 on a
-//                     32-row shared-memory ring of F with one neighbour per lane, eq. 7 record.
-// The 26-row histories of F and d that the running sums and the lagged reads need are private to
-// a thread, so they live in TENSOR MEMORY (tcgen05.st/ld 32x32b.x4: 208 of a thread's 256/512
-// columns) rather than in shared memory: shared memory carries only what threads exchange.
-// Everything a warp has to decide in an iteration (are its input rows all valid / partly masked /
-// empty, which normalisers are the interior constants, which stages run) is one 32-bit word of a
-// per-item table built by the host plan, so the steady-state iteration is branch-poor and loads
-// no mask or normaliser plane inside the valid region.  F, C, d, S never leave the SM.
+//   C  rows sig=y-31: horizontal 25-box of V2 x 1/count -> S (eq. 4); eq. 5 on d(sig) for the whole
+//                     row with four packed operations and one vote; rows with a hit go out of line:
+//                     exact bits, a cheap in-thread 3x3 pre-filter on the F ring, then the S_eff guard
+//                     (R8), eq. 6 with one neighbour per lane and the eq. 7 record.
+// The 32-row histories of F and d that the running sums and the lagged reads need are private to
+// a thread, so they live in TENSOR MEMORY (tcgen05.st/ld 32x32b.x4, two power-of-two rings of 128
+// columns per thread); shared memory carries only what threads exchange plus a 32-row ring of F for
+// the local-maximum tests.  What a warp has to decide in an iteration (is there input, which
+// normalisers are the interior constants, which stages run) is one 32-bit word of a per-item table
+// built by the host plan.  F, C, d, S never leave the SM.
+// The input is used unmasked when the cube holds exact zeros at every invalid pixel (checked per
+// frame by the sum-plane kernel); otherwise each thread applies W itself (slow, rare).
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
@@ -39,24 +42,22 @@ constexpr int RB = 2;               // rows per iteration
 constexpr int HALO = 2 * KBG + 3;   // rows of X above the first output row (27)
 constexpr int LAG_B = 3 + KBG + RB;          // rho = y - 17
 constexpr int LAG_C = LAG_B + KBG + RB;      // sig = y - 31
-constexpr int DFS = 36;             // shared-memory ring of F rows (local maxima are tested one iteration late)
-constexpr int QCAP = 32;            // queued candidates per warp and iteration (more are tested in place)
-constexpr int RCAP = 32;            // staged records per warp between flushes
-constexpr int DT = WINB + 1;        // tensor-memory ring depth (rows) of F and of d
-constexpr int TM_D = 4 * DT;        // first tensor-memory column of the d ring (F ring starts at 0)
+constexpr int DR = 32;              // depth (rows) of the tensor-memory rings of F and d (power of two)
+constexpr int DRS = 34;             // depth of the shared-memory ring of F: local maxima are tested one iteration late
+constexpr int QCAP = 64;            // queued candidates per iteration (more are tested in place)
+constexpr int SCAP = 64;            // records staged by the candidate warp between flushes
+constexpr int XST = 4;              // input staging stages (iterations in flight)
+constexpr int TM_D = 4 * DR;        // first tensor-memory column of the d ring (F ring starts at 0)
 constexpr int PADR = 64;            // zero rows above and below the padded normaliser planes
 
 // per-(iteration, warp) control word
-constexpr unsigned FL_XMODE = 3u;          // bits 0-1: input rows consumed now: 0 empty, 1 all valid, 2 masked
-constexpr int FL_PMODE_SH = 2;             // bits 2-3: the same for the rows loaded now (two iterations ahead)
+constexpr unsigned FL_X = 1u;              // stage A has input: rows in the image, something valid near the warp
 constexpr unsigned FL_NM_LD = 1u << 4;     // F rows of this iteration use the loaded norm_mf (else the constant)
 constexpr unsigned FL_ICR_LD = 1u << 5;    // rho rows use the loaded 1/count
 constexpr unsigned FL_ICS_LD = 1u << 6;    // sigma rows use the loaded 1/count
 constexpr unsigned FL_NM_PF = 1u << 7;     // load the planes of the next iteration
 constexpr unsigned FL_ICR_PF = 1u << 8;
 constexpr unsigned FL_ICS_PF = 1u << 9;
-constexpr unsigned FL_GATE_A = 1u << 10;   // some F row precedes the segment's first needed one
-constexpr unsigned FL_GATE_B = 1u << 11;   // some rho row precedes the segment's first needed one
 constexpr unsigned FL_DO_B = 1u << 12;
 constexpr unsigned FL_C0 = 1u << 13;       // sigma row j is an output row of this item
 constexpr unsigned FL_C1 = 1u << 14;
@@ -67,13 +68,19 @@ struct FusedArgs {
   const float* cube; const float* sum_plane; const uint8_t* band_ok; const uint8_t* W;
   const float* nm_pad; const float* ic_pad;      // [(Dy + 2 PADR)][Dx], zero rows around the image
   const FusedItem* items; const uint32_t* flags;
+  const int32_t* dirty; int dirty_seq;           // *dirty == dirty_seq: some invalid pixel of this cube is not an exact zero
   int B, Dy, Dx, CW, k_max, max_det;
   float g0, g1, g2, g3, kappa2, eps_rel, nm_const, ic_const;
   lpf_det* dets; int32_t* ndets; int32_t* counters;
 };
 
-__device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 __device__ __forceinline__ float4 zero4() { return make_float4(0.f, 0.f, 0.f, 0.f); }
+// a global load the compiler may not sink to its use (the normaliser planes are fetched an iteration ahead)
+__device__ __forceinline__ float4 ldg4_pinned(const float* p) {
+  float4 v;
+  asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];\n" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+  return v;
+}
 
 // packed f32x2 arithmetic (FADD2 / FMUL2 / FFMA2: one issue slot for two lanes' worth of fp32)
 __device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
@@ -99,14 +106,31 @@ __device__ __forceinline__ void tm_use(float2& lo, float2& hi) {
   asm volatile("" : "+f"(lo.x), "+f"(lo.y), "+f"(hi.x), "+f"(hi.y));
 }
 
-__device__ __forceinline__ int wrap26(int s) { return s >= DT ? s - DT : s; }
-
-__device__ __forceinline__ float4 mask4(float4 v, unsigned wm) {
-  if (!(wm & 0x000000ffu)) v.x = 0.f;
-  if (!(wm & 0x0000ff00u)) v.y = 0.f;
-  if (!(wm & 0x00ff0000u)) v.z = 0.f;
-  if (!(wm & 0xff000000u)) v.w = 0.f;
-  return v;
+// ---- bulk asynchronous copies (TMA without a tensor map) and their mbarriers ----------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "LPF_WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra LPF_DONE_%=;\n"
+      "bra LPF_WAIT_%=;\n"
+      "LPF_DONE_%=:\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 
 // shared memory through the kernel's one dynamic array: float index -> value
@@ -128,23 +152,75 @@ __device__ __forceinline__ void hbox25(int ev, int et, float out[4]) {
   out[3] = out[2] + (R.w - L.z);
 }
 
-// ---- candidate path (out of line: it is the rare part, and it keeps the sweep's code small) -------
-struct CandCtx {           // what the out-of-line functions need, by value
+// ---- candidate path ---------------------------------------------------------------------------------
+// Pixels that pass the unguarded eq. 5 are queued by the sweep warps (a few per iteration) and tested one
+// iteration later by a dedicated warp, off the sweep's critical path: S_eff guard (R8), eq. 6 on the
+// shared-memory ring of F, eq. 7 record.  One candidate per lane, up to 32 at a time.
+struct CandCtx {           // what the candidate functions need, by value
   const FusedArgs* ap;     // kernel arguments (shared-memory copy)
   int CWP, xs, plane, lane, ring_y0;
-  int o_st;                // float index of the warp's record staging area (RCAP x 8 words)
 };
 
-// staged records of a warp -> global list: one atomic for the lot.  Returns the new count (0).
-__device__ __noinline__ int cand_flush(const FusedArgs* ap, int o_st, int lane, int nrec) {
-  if (nrec <= 0) return 0;
+__device__ __forceinline__ int ring_slot(int row, int ring_y0) { return (int)((unsigned)(row - ring_y0) % (unsigned)DRS); }
+
+// the test of one candidate by its own lane; returns true when it is a peak (fills f, c, s_eff).
+// KM = k_max at compile time (fully unrolled window, independent shared loads); KM < 0: run-time k_max.
+template <int KM>
+__device__ __forceinline__ bool cand_test_lane(const CandCtx& c, int cl, int sg, float d, float s,
+                                               float& fv, float& cc, float& se) {
+  const FusedArgs& a = *c.ap;
+  const int CWP = c.CWP;
+  const int s0 = ring_slot(sg, c.ring_y0);
+  fv = lds1(s0 * CWP + cl);
+  cc = fv - d;
+  const float gd = a.eps_rel * fabsf(cc);
+  se = fmaxf(s, gd * gd);
+  if (!(d > 0.f && d * d > a.kappa2 * se)) return false;
+  const int km = KM >= 0 ? KM : a.k_max;
+  bool bigger = false, zero_wins = false;       // a neighbour with F = 0 > fv: masked or not?  (rare: asks W)
+#pragma unroll
+  for (int dy = -km; dy <= km; ++dy) {
+    const int yy = sg + dy;
+    int sl = s0 + dy;
+    sl = sl < 0 ? sl + DRS : (sl >= DRS ? sl - DRS : sl);
+    const bool row_in = yy >= 0 && yy < a.Dy;
+#pragma unroll
+    for (int dx = -km; dx <= km; ++dx) {
+      const int c2 = cl + dx;
+      const bool in = row_in && c2 >= 0 && c2 < CWP && c.xs + c2 < a.Dx;
+      const float fn = in ? lds1(sl * CWP + c2) : fv;
+      bigger = bigger || (fn > fv && fn != 0.f);
+      zero_wins = zero_wins || (fn > fv && fn == 0.f);
+    }
+  }
+  if (bigger) return false;
+  if (zero_wins) {
+    for (int dy = -km; dy <= km; ++dy)
+      for (int dx = -km; dx <= km; ++dx) {
+        const int yy = sg + dy, c2 = cl + dx, xn = c.xs + c2;
+        if (yy < 0 || yy >= a.Dy || c2 < 0 || c2 >= CWP || xn >= a.Dx) continue;
+        if (lds1(ring_slot(yy, c.ring_y0) * CWP + c2) > fv && a.W[(long long)yy * a.Dx + xn] != 0) return false;
+      }
+  }
+  return true;
+}
+
+__device__ __forceinline__ bool cand_test_any(const CandCtx& c, int cl, int sg, float d, float s, float& fv, float& cc, float& se) {
+  const int km = c.ap->k_max;
+  if (km == 2) return cand_test_lane<2>(c, cl, sg, d, s, fv, cc, se);
+  if (km == 1) return cand_test_lane<1>(c, cl, sg, d, s, fv, cc, se);
+  return cand_test_lane<-1>(c, cl, sg, d, s, fv, cc, se);
+}
+
+// staged records (shared memory, 8 words each, n of them at float index o_st) -> global list, one atomic
+__device__ __noinline__ void cand_flush(const FusedArgs* ap, int o_st, int lane, int n) {
+  if (n <= 0) return;
   int base = 0;
-  if (lane == 0) base = atomicAdd(ap->ndets, nrec);
+  if (lane == 0) base = atomicAdd(ap->ndets, n);
   base = __shfl_sync(0xffffffffu, base, 0);
-  __syncwarp();
-  if (lane < nrec) {
-    const uint2* r = reinterpret_cast<const uint2*>(reinterpret_cast<const uint32_t*>(g_sm4) + o_st + lane * 8);
-    const int idx = base + lane;
+  for (int i = lane; i < n; i += 32) {
+    const uint2* r = reinterpret_cast<const uint2*>(reinterpret_cast<const uint32_t*>(g_sm4) + o_st + i * 8);
+    const int idx = base + i;
     if (idx < ap->max_det) {
       uint2* dst = reinterpret_cast<uint2*>(ap->dets + idx);
       dst[0] = r[0]; dst[1] = r[1]; dst[2] = r[2];
@@ -153,80 +229,86 @@ __device__ __noinline__ int cand_flush(const FusedArgs* ap, int o_st, int lane, 
     }
   }
   __syncwarp();
-  return 0;
 }
 
-// eq. 5 guard + eq. 6 + eq. 7 for one pixel that passed the unguarded eq. 5, by the whole warp:
-// lane k < (2 k_max + 1)^2 looks at one neighbour in the shared-memory ring of F (float index 0, row
-// pitch CWP, DFS rows, row r in slot (r - ring_y0) mod DFS).  d, s: the pixel's residual and spread;
-// cl: its column in the strip; sg: its row.  An accepted record is staged in shared memory; returns the
-// warp's new staged count (flushing when the stage is full).
-__device__ __forceinline__ int cand_test_body(const CandCtx& c, int nrec, float d, float s, int cl, int sg) {
+// lanes with ok stage their records at o_st (nst staged so far, room for SCAP); returns the new count
+__device__ __forceinline__ int cand_stage(const CandCtx& c, int o_st, int nst, bool ok, int cl, int sg, float d, float fv, float cc, float se) {
   const FusedArgs& a = *c.ap;
-  const int CWP = c.CWP, lane = c.lane;
-  const float fv = lds1((unsigned)(sg - c.ring_y0) % DFS * CWP + cl);
-  const float cc = fv - d;
-  const float gd = a.eps_rel * fabsf(cc);
-  const float se = fmaxf(s, gd * gd);
-  if (!(d > 0.f && d * d > a.kappa2 * se)) return nrec;   // warp-uniform
-  const int km = a.k_max, side = 2 * km + 1;
-  bool bigger = false;
-  if (lane < side * side) {
-    const int row = side == 5 ? (lane * 13) >> 6 : (side == 3 ? (lane * 11) >> 5 : 0);   // lane / side (k_max <= 2)
-    const int dy = row - km, dx = lane - row * side - km;
-    const int yy = sg + dy, c2 = cl + dx, xn = c.xs + c2;
-    if (yy >= 0 && yy < a.Dy && c2 >= 0 && c2 < CWP && xn < a.Dx) {
-      const float fn = lds1((unsigned)(yy - c.ring_y0) % DFS * CWP + c2);
-      // masked pixels hold F = 0 in the ring: W is consulted only when such a zero would win
-      if (fn > fv) bigger = (fn != 0.f) || (a.W[(long long)yy * a.Dx + xn] != 0);
-    }
-  }
-  if (__any_sync(0xffffffffu, bigger)) return nrec;
-  if (lane == 0) {
-    uint32_t* r = reinterpret_cast<uint32_t*>(g_sm4) + c.o_st + nrec * 8;
+  const unsigned m = __ballot_sync(0xffffffffu, ok);
+  if (!m) return nst;
+  if (nst + __popc(m) > SCAP) { cand_flush(c.ap, o_st, c.lane, nst); nst = 0; }
+  if (ok) {
+    uint32_t* r = reinterpret_cast<uint32_t*>(g_sm4) + o_st + (nst + __popc(m & ((1u << c.lane) - 1u))) * 8;
     r[0] = (uint32_t)(sg * a.Dx + c.xs + cl);
     r[1] = (uint32_t)(c.plane & 0xffff) | (1u << 16);        // int16 plane, int16 iter = 1
     r[2] = __float_as_uint(fv); r[3] = __float_as_uint(cc); r[4] = __float_as_uint(se);
     r[5] = __float_as_uint(d / sqrtf(se));
   }
-  ++nrec;
-  if (nrec == RCAP) nrec = cand_flush(c.ap, c.o_st, lane, nrec);
-  return nrec;
+  __syncwarp();
+  return nst + __popc(m);
 }
 
-// entries e = first, first + step, ... < total of the CTA's queue qb (per-warp lists of lengths n_mine
-// held by lanes < nw, inclusive prefix pre): the calling warp's share of last iteration's candidates
-__device__ __noinline__ int cand_drain(CandCtx c, int nrec, int o_q, int nw, int first, int n_mine, int pre) {
-  const int total = __shfl_sync(0xffffffffu, pre, nw - 1);
-  for (int e = first; e < total; e += nw) {
-    const int owner = __popc(__ballot_sync(0xffffffffu, c.lane < nw && pre <= e));
-    const int start = __shfl_sync(0xffffffffu, pre - n_mine, owner);
-    const float4 q = lds4(o_q + (owner * QCAP + (e - start)) * 4);
-    nrec = cand_test_body(c, nrec, q.z, q.w, __float_as_int(q.x), __float_as_int(q.y));
+// the queue of one iteration, n entries {col, row, d, s} at float index o_q: the consumer warp's work
+__device__ __noinline__ int cand_consume(CandCtx c, int o_q, int n, int o_st, int nst) {
+  for (int e0 = 0; e0 < n; e0 += 32) {
+    const int e = e0 + c.lane;
+    bool ok = false;
+    int cl = 0, sg = 0; float d = 0.f, fv = 0.f, cc = 0.f, se = 1.f;
+    if (e < n) {
+      const float4 q = lds4(o_q + 4 * e);
+      cl = __float_as_int(q.x); sg = __float_as_int(q.y); d = q.z;
+      ok = cand_test_any(c, cl, sg, d, q.w, fv, cc, se);
+    }
+    nst = cand_stage(c, o_st, nst, ok, cl, sg, d, fv, cc, se);
   }
-  return nrec;
+  return nst;
 }
 
-// a row whose candidates do not fit the queue any more (rare): tested in place
-__device__ __noinline__ int cand_row_in_place(CandCtx c, int nrec, unsigned bits, float4 dv, float4 sv, int cl0, int sg) {
+// a sweep warp whose candidates did not fit the queue (rare: a row full of bright pixels) tests them itself
+// and appends the records straight to the global list
+__device__ __noinline__ void cand_in_place(CandCtx c, unsigned bits, int col0, int sg, float4 dv, float4 sv) {
+  const FusedArgs& a = *c.ap;
+  const float d[4] = {dv.x, dv.y, dv.z, dv.w};
+  const float s[4] = {sv.x, sv.y, sv.z, sv.w};
+#pragma unroll
   for (int k = 0; k < 4; ++k) {
-    unsigned m = __ballot_sync(0xffffffffu, (bits >> k) & 1u);
-    const float dk = k == 0 ? dv.x : (k == 1 ? dv.y : (k == 2 ? dv.z : dv.w));
-    const float sk = k == 0 ? sv.x : (k == 1 ? sv.y : (k == 2 ? sv.z : sv.w));
-    while (m) {
-      const int src = __ffs(m) - 1;
-      m &= m - 1;
-      nrec = cand_test_body(c, nrec, __shfl_sync(0xffffffffu, dk, src), __shfl_sync(0xffffffffu, sk, src),
-                            __shfl_sync(0xffffffffu, cl0, src) + k, sg);
+    float fv = 0.f, cc = 0.f, se = 1.f;
+    bool ok = false;
+    if ((bits >> k) & 1u) ok = cand_test_lane<-1>(c, col0 + k, sg, d[k], s[k], fv, cc, se);
+    const unsigned m = __ballot_sync(0xffffffffu, ok);
+    if (!m) continue;
+    int base = 0;
+    if (c.lane == 0) base = atomicAdd(a.ndets, __popc(m));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (ok) {
+      const int idx = base + __popc(m & ((1u << c.lane) - 1u));
+      if (idx < a.max_det) {
+        uint2* dst = reinterpret_cast<uint2*>(a.dets + idx);
+        dst[0] = make_uint2((uint32_t)(sg * a.Dx + c.xs + col0 + k), (uint32_t)(c.plane & 0xffff) | (1u << 16));
+        dst[1] = make_uint2(__float_as_uint(fv), __float_as_uint(cc));
+        dst[2] = make_uint2(__float_as_uint(se), __float_as_uint(d[k] / sqrtf(se)));
+      } else {
+        atomicAdd(&a.counters[0], 1);
+      }
     }
   }
-  return nrec;
 }
 
-struct Prefetch {          // one iteration's worth of input rows, loaded two iterations ahead
-  float4 x[RB], xe[RB];    // own 4 pixels; the neighbouring warp's 4 pixels (lanes 0 and 31 only)
-  unsigned w[RB], we[RB];  // their mask bytes (masked rows only)
-};
+// the slow input path: a cube with something other than an exact zero at an invalid pixel; x0: column of v.l.x
+struct Row12 { float4 l, m, r; };
+__device__ __noinline__ Row12 mask_row(const FusedArgs* ap, int y, int x0, Row12 v) {
+  const FusedArgs& a = *ap;
+  float t[12] = {v.l.x, v.l.y, v.l.z, v.l.w, v.m.x, v.m.y, v.m.z, v.m.w, v.r.x, v.r.y, v.r.z, v.r.w};
+#pragma unroll
+  for (int k = 0; k < 12; ++k) {
+    const int x = x0 + k;
+    const bool ok = y >= 0 && y < a.Dy && x >= 0 && x < a.Dx && a.W[(long long)y * a.Dx + x] != 0;
+    if (!ok) t[k] = 0.f;
+  }
+  Row12 o;
+  o.l = make_float4(t[0], t[1], t[2], t[3]); o.m = make_float4(t[4], t[5], t[6], t[7]); o.r = make_float4(t[8], t[9], t[10], t[11]);
+  return o;
+}
 
 struct Planes {            // normaliser values of non-interior cells, loaded one iteration ahead
   float4 nm[RB], icr[RB], ics[RB];
@@ -235,130 +317,119 @@ struct Planes {            // normaliser values of non-interior cells, loaded on
 template <int NW>
 struct Sweep {
   static constexpr int CWP = NW * 128;             // shared-memory row pitch: the CTA's full width
+  static constexpr int XP = CWP + 8;               // staged input row: 4 columns of margin on both sides
   static constexpr int PEV = CWP + 2 * KBG, PET = NW * 32 + 8;
   static constexpr int O_RING = 0;
-  static constexpr int O_EV1 = DFS * CWP;
+  static constexpr int O_X = DRS * CWP;
+  static constexpr int O_EV1 = O_X + XST * RB * XP;
   static constexpr int O_EV2 = O_EV1 + 2 * RB * PEV;
   static constexpr int O_ET1 = O_EV2 + 2 * RB * PEV;
   static constexpr int O_ET2 = O_ET1 + 2 * RB * PET;
-  static constexpr int O_Q = O_ET2 + 2 * RB * PET;    // candidate queues, [2][NW][QCAP] x {col, row, d, s}
-  static constexpr int O_QN = O_Q + 2 * NW * QCAP * 4;  // their lengths, [2][NW] (padded to 16 words)
-  static constexpr int O_ST = O_QN + 16;                // staged records, [NW][RCAP] x 8 words
-  static constexpr int O_FL = O_ST + NW * RCAP * 8;     // control words, [nb][NW]
+  static constexpr int O_Q = O_ET2 + 2 * RB * PET;       // candidate queues, [2][QCAP] x {col, row, d, s}
+  static constexpr int O_QN = O_Q + 2 * QCAP * 4;        // their lengths, [2] (padded to 4 words)
+  static constexpr int O_ST = O_QN + 4;                  // staged records of the candidate warp, [SCAP] x 8 words
+  static constexpr int O_BAR = O_ST + SCAP * 8;          // XST mbarriers (8 bytes each)
+  static constexpr int O_FL = O_BAR + 2 * XST;           // control words, [nb][NW]
   // ---- constants of the thread -----------------------------------------------------------------
   const FusedArgs& a;
   const FusedArgs* a_sh;   // the same arguments in shared memory (for the out-of-line candidate path)
   int xs, plane, tid, lane, warp;
-  int sx, eoff;            // row stride (0 for lanes outside the strip); offset of the edge lanes' extra load
-  bool ld_edge;
+  int sx;                  // row stride of the plane pointers (0 for lanes outside the strip)
+  bool col_in, dirty;
   unsigned umask;
   uint32_t tm;             // tensor-memory address of the thread's column 0
-  int f_lim, r_lim;        // first needed F row (ya - 24), first needed rho row (ya - 12)
+  // producer (thread 0)
+  const float* xrow0;      // X at (y_start, first copied column)
+  uint32_t x_dst0;         // shared address of that column in stage 0, row 0
+  uint32_t row_bytes;
+  int nb;
   // ---- running state -----------------------------------------------------------------------------
-  const float* xp;         // X at the first row of the next prefetch
-  const uint8_t* wp;       // W at the same place
   const float* nmp;        // padded norm_mf at the next iteration's first F row
   const float* icrp;       // padded 1/count at the next iteration's first rho row
   const float* icsp;       // padded 1/count at the next iteration's first sigma row
   int y0;                  // first input row of the current iteration
-  int w26;                 // tensor-memory ring slot of this iteration's first row
-  int wF;                  // shared-memory ring slot of this iteration's first F row
-  int ring_y0;             // the row that sits in slot 0 of the shared-memory ring (mod DFS)
-  int qcount, nrec;        // candidates queued in this iteration; records staged by this warp
+  int ring_y0;             // the row that sits in slot 0 of the rings
+  int ws;                  // slot of this iteration's first F row in the shared-memory ring
   float2 hw[8][2];         // horizontally filtered rows (rotating; static indices per phase)
   float2 V1[2], V2[2];     // vertical running sums
-  Prefetch pf[2];
-  Planes pl[2];
+  Planes pl;               // normalisers of the coming rows: each plane is reloaded right after its use
 
   __device__ __forceinline__ Sweep(const FusedArgs& a_) : a(a_) {}
 
   __device__ __forceinline__ unsigned ctl(int b) const {
     return reinterpret_cast<const uint32_t*>(g_sm4)[O_FL + b * NW + warp];
   }
+  __device__ __forceinline__ uint32_t bar_addr(int stage) const {
+    return smem_u32(reinterpret_cast<const float*>(g_sm4) + O_BAR + 2 * stage);
+  }
 
   __device__ __forceinline__ CandCtx cand_ctx() const {
     CandCtx c;
     c.ap = a_sh; c.CWP = CWP; c.xs = xs; c.plane = plane; c.lane = lane; c.ring_y0 = ring_y0;
-    c.o_st = O_ST + warp * RCAP * 8;
     return c;
   }
 
-  // eq. 6 / eq. 7 for the pixels all warps queued in the previous iteration, dealt round-robin to the warps
-  __device__ __forceinline__ void process_queue(int qb) {
-    const int n_mine = lane < NW ? reinterpret_cast<const int*>(g_sm4)[O_QN + qb * NW + lane] : 0;
-    int pre = n_mine;
+  // thread 0: the two input rows of iteration bb into stage bb mod XST (a plain arrival when they lie outside the image)
+  __device__ __forceinline__ void issue_rows(int bb, int ys) {
+    const int st = bb & (XST - 1);
+    const uint32_t bar = bar_addr(st);
+    const int y = ys + RB * bb;
+    if (bb >= XST) mbar_wait(bar, (uint32_t)((bb >> 2) - 1) & 1u);   // its previous phase (complete unless no warp waited for it)
+    if (y >= 0 && y + RB <= a.Dy) {
+      mbar_expect_tx(bar, RB * row_bytes);
+      const float* src = xrow0 + (long long)RB * bb * a.Dx;
+      const uint32_t dst = x_dst0 + (uint32_t)(st * RB * XP * 4);
 #pragma unroll
-    for (int o = 1; o < NW; o <<= 1) {
-      const int t = __shfl_up_sync(0xffffffffu, pre, o);
-      if (lane >= o) pre += t;
+      for (int j = 0; j < RB; ++j) bulk_g2s(dst + (uint32_t)(j * XP * 4), src + (long long)j * a.Dx, row_bytes, bar);
+    } else {
+      mbar_arrive(bar);
     }
-    if (__shfl_sync(0xffffffffu, pre, NW - 1) > warp)      // something for this warp
-      nrec = cand_drain(cand_ctx(), nrec, O_Q + qb * NW * QCAP * 4, NW, warp, n_mine, pre);
   }
 
-  // global loads of two input rows into pf[slot]; mode 1: all valid, 2: masked (W loaded too)
-  __device__ __forceinline__ void load_rows(int slot, unsigned mode) {
-    if (mode) {
-      Prefetch& p = pf[slot];
-      p.x[0] = ldg4(xp); p.x[1] = ldg4(xp + sx);
-      if (ld_edge) { p.xe[0] = ldg4(xp + eoff); p.xe[1] = ldg4(xp + sx + eoff); }
-      if (mode == 2u) {
-        p.w[0] = __ldg(reinterpret_cast<const unsigned*>(wp));
-        p.w[1] = __ldg(reinterpret_cast<const unsigned*>(wp + sx));
-        if (ld_edge) {
-          p.we[0] = __ldg(reinterpret_cast<const unsigned*>(wp + eoff));
-          p.we[1] = __ldg(reinterpret_cast<const unsigned*>(wp + sx + eoff));
-        }
-      }
-    }
-    xp += RB * sx; wp += RB * sx;
+  __device__ __forceinline__ void load_nm(unsigned on) {
+    if (on) { pl.nm[0] = ldg4_pinned(nmp); pl.nm[1] = ldg4_pinned(nmp + sx); }
+    nmp += RB * sx;
+  }
+  __device__ __forceinline__ void load_icr(unsigned on) {
+    if (on) { pl.icr[0] = ldg4_pinned(icrp); pl.icr[1] = ldg4_pinned(icrp + sx); }
+    icrp += RB * sx;
+  }
+  __device__ __forceinline__ void load_ics(unsigned on) {
+    if (on) { pl.ics[0] = ldg4_pinned(icsp); pl.ics[1] = ldg4_pinned(icsp + sx); }
+    icsp += RB * sx;
   }
 
-  __device__ __forceinline__ void load_planes(int slot, unsigned fl_nm, unsigned fl_icr, unsigned fl_ics) {
-    Planes& q = pl[slot];
-    if (fl_nm) { q.nm[0] = ldg4(nmp); q.nm[1] = ldg4(nmp + sx); }
-    if (fl_icr) { q.icr[0] = ldg4(icrp); q.icr[1] = ldg4(icrp + sx); }
-    if (fl_ics) { q.ics[0] = ldg4(icsp); q.ics[1] = ldg4(icsp + sx); }
-    nmp += RB * sx; icrp += RB * sx; icsp += RB * sx;
-  }
-
-  // One iteration: rows y0, y0+1 enter stage A; PH = iteration index mod 4 fixes the register rotation.
+  // One iteration: rows y0, y0+1 enter stage A; PH = iteration index mod 4 fixes the register rotation
+  // and the staging stage.  fl: this iteration's control word.
   template <int PH>
-  __device__ __forceinline__ void iteration(int b) {
+  __device__ __forceinline__ void iteration(int b, unsigned fl) {
     constexpr int buf = PH & 1, pbuf = buf ^ 1;
-    const unsigned fl = ctl(b);
     const float2 g0 = splat(a.g0), g1 = splat(a.g1), g2 = splat(a.g2), g3 = splat(a.g3);
-    process_queue(pbuf);
+    const int w = (RB * b) & (DR - 1);                       // ring slot of this iteration's first row (even)
+    const uint32_t t_old0 = tm + 4u * (uint32_t)((w + 7) & (DR - 1)), t_old1 = tm + 4u * (uint32_t)((w + 8) & (DR - 1));
+    const uint32_t t_lag0 = tm + 4u * (uint32_t)((w + 18) & (DR - 1)), t_lag1 = t_lag0 + 4u;   // w + 18 is even: no wrap in between
+    const uint32_t t_new0 = tm + 4u * (uint32_t)w, t_new1 = t_new0 + 4u;
 
-    // ---- tensor-memory reads, first batch: F(fr - 25) ------------------------------------------------
-    float2 fold[RB][2];
-#pragma unroll
-    for (int j = 0; j < RB; ++j) tm_ld4(tm + 4 * wrap26(w26 + j + 1), fold[j][0], fold[j][1]);
+    // ---- tensor-memory reads: F(fr - 25), F(rho), d(rho - 25), d(sigma) ---------------------------------
+    float2 fold[RB][2], flag[RB][2], dold[RB][2], dlag[RB][2];
+    tm_ld4(t_old0, fold[0][0], fold[0][1]); tm_ld4(t_old1, fold[1][0], fold[1][1]);
 
-    // ---- stage A, part 1: take the prefetched rows, mask, horizontal matched filter -----------------
-    {
-      float4 v[RB], e[RB];
-      const unsigned mode = fl & FL_XMODE;
-      if (mode == 0u) {
-#pragma unroll
-        for (int j = 0; j < RB; ++j) { v[j] = zero4(); e[j] = zero4(); }
-      } else {
-#pragma unroll
-        for (int j = 0; j < RB; ++j) { v[j] = pf[buf].x[j]; e[j] = pf[buf].xe[j]; }
-        if (mode == 2u) {
-#pragma unroll
-          for (int j = 0; j < RB; ++j) { v[j] = mask4(v[j], pf[buf].w[j]); e[j] = mask4(e[j], pf[buf].we[j]); }
-        }
-      }
+    // ---- producer: the input rows of iteration b + XST - 1 (their stage was read in iteration b - 1) ----
+    if (tid == 0 && b + XST - 1 < nb) issue_rows(b + XST - 1, y0 - RB * b);
+
+    // ---- stage A, part 1: staged rows -> horizontal matched filter ------------------------------------
+    if (fl & FL_X) {
+      mbar_wait(bar_addr(PH), (uint32_t)(b >> 2) & 1u);
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
-        float l1 = __shfl_up_sync(0xffffffffu, v[j].y, 1), l2 = __shfl_up_sync(0xffffffffu, v[j].z, 1),
-              l3 = __shfl_up_sync(0xffffffffu, v[j].w, 1);
-        float r0 = __shfl_down_sync(0xffffffffu, v[j].x, 1), r1 = __shfl_down_sync(0xffffffffu, v[j].y, 1),
-              r2 = __shfl_down_sync(0xffffffffu, v[j].z, 1);
-        if (lane == 0) { l1 = e[j].y; l2 = e[j].z; l3 = e[j].w; }
-        if (lane == 31) { r0 = e[j].x; r1 = e[j].y; r2 = e[j].z; }
-        const float wv[10] = {l1, l2, l3, v[j].x, v[j].y, v[j].z, v[j].w, r0, r1, r2};
+        const int xr = O_X + (PH * RB + j) * XP + 4 * tid;
+        float4 l = lds4(xr), m = lds4(xr + 4), r = lds4(xr + 8);
+        if (dirty) {
+          Row12 v; v.l = l; v.m = m; v.r = r;
+          v = mask_row(a_sh, y0 + j, xs + 4 * tid - 4, v);
+          l = v.l; m = v.m; r = v.r;
+        }
+        const float wv[10] = {l.y, l.z, l.w, m.x, m.y, m.z, m.w, r.x, r.y, r.z};
         float h[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k)
@@ -366,23 +437,18 @@ struct Sweep {
         hw[(2 * PH + 6 + j) & 7][0] = make_float2(h[0], h[1]);
         hw[(2 * PH + 6 + j) & 7][1] = make_float2(h[2], h[3]);
       }
+    } else {
+#pragma unroll
+      for (int j = 0; j < RB; ++j) { hw[(2 * PH + 6 + j) & 7][0] = splat(0.f); hw[(2 * PH + 6 + j) & 7][1] = splat(0.f); }
     }
-    // ---- issue the global loads of iteration b+2 (inputs) and b+1 (normaliser planes) --------------
-    load_rows(buf, (fl >> FL_PMODE_SH) & 3u);
-    load_planes(pbuf, fl & FL_NM_PF, fl & FL_ICR_PF, fl & FL_ICS_PF);
 
     tm_wait_ld();
 #pragma unroll
     for (int j = 0; j < RB; ++j) tm_use(fold[j][0], fold[j][1]);
-    // ---- second batch: F(rho), d(rho - 25), d(sigma) -------------------------------------------------
-    float2 flag[RB][2], dold[RB][2], dlag[RB][2];
-#pragma unroll
-    for (int j = 0; j < RB; ++j) {
-      const int so = wrap26(w26 + j + 1), sl = wrap26(w26 + j + KBG);
-      tm_ld4(tm + 4 * sl, flag[j][0], flag[j][1]);
-      tm_ld4(tm + TM_D + 4 * so, dold[j][0], dold[j][1]);
-      tm_ld4(tm + TM_D + 4 * sl, dlag[j][0], dlag[j][1]);
-    }
+    // second batch, for stages B and C: F(rho), d(rho - 25), d(sigma)
+    tm_ld4(t_lag0, flag[0][0], flag[0][1]); tm_ld4(t_lag1, flag[1][0], flag[1][1]);
+    tm_ld4(t_old0 + TM_D, dold[0][0], dold[0][1]); tm_ld4(t_old1 + TM_D, dold[1][0], dold[1][1]);
+    tm_ld4(t_lag0 + TM_D, dlag[0][0], dlag[0][1]); tm_ld4(t_lag1 + TM_D, dlag[1][0], dlag[1][1]);
 
     // ---- stage A, part 2: vertical matched filter -> F(fr), running sum V1, exchange ----------------
     {
@@ -399,31 +465,27 @@ struct Sweep {
       if (fl & FL_NM_LD) {
 #pragma unroll
         for (int j = 0; j < RB; ++j) {
-          f[j][0] = mul2(f[j][0], make_float2(pl[buf].nm[j].x, pl[buf].nm[j].y));
-          f[j][1] = mul2(f[j][1], make_float2(pl[buf].nm[j].z, pl[buf].nm[j].w));
+          f[j][0] = mul2(f[j][0], make_float2(pl.nm[j].x, pl.nm[j].y));
+          f[j][1] = mul2(f[j][1], make_float2(pl.nm[j].z, pl.nm[j].w));
         }
       } else {
         const float2 c = splat(a.nm_const);
 #pragma unroll
         for (int j = 0; j < RB; ++j) { f[j][0] = mul2(f[j][0], c); f[j][1] = mul2(f[j][1], c); }
       }
-      if (fl & FL_GATE_A) {                          // rows before the segment's first needed F row
-#pragma unroll
-        for (int j = 0; j < RB; ++j)
-          if (y0 + j - 3 < f_lim) { f[j][0] = splat(0.f); f[j][1] = splat(0.f); }
-      }
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
         V1[0] = add2(V1[0], sub2(f[j][0], fold[j][0]));
         V1[1] = add2(V1[1], sub2(f[j][1], fold[j][1]));
-        tm_st4(tm + 4 * wrap26(w26 + j), f[j][0], f[j][1]);
-        sts4(O_RING + (wF + j >= DFS ? wF + j - DFS : wF + j) * CWP + 4 * tid, make_float4(f[j][0].x, f[j][0].y, f[j][1].x, f[j][1].y));
+        tm_st4(j ? t_new1 : t_new0, f[j][0], f[j][1]);
+        sts4(O_RING + (ws + j) * CWP + 4 * tid, make_float4(f[j][0].x, f[j][0].y, f[j][1].x, f[j][1].y));
         sts4(O_EV1 + (buf * RB + j) * PEV + KBG + 4 * tid, make_float4(V1[0].x, V1[0].y, V1[1].x, V1[1].y));
         const float2 ts = add2(V1[0], V1[1]);
         sts1(O_ET1 + (buf * RB + j) * PET + 3 + tid, ts.x + ts.y);
       }
     }
 
+    load_nm(fl & FL_NM_PF);                          // the next iteration's norm_mf rows
     tm_wait_ld();
 #pragma unroll
     for (int j = 0; j < RB; ++j) { tm_use(flag[j][0], flag[j][1]); tm_use(dold[j][0], dold[j][1]); tm_use(dlag[j][0], dlag[j][1]); }
@@ -436,28 +498,25 @@ struct Sweep {
         float bx[4];
         hbox25(O_EV1 + (pbuf * RB + j) * PEV + 4 * tid, O_ET1 + (pbuf * RB + j) * PET + tid, bx);
         float2 ic0, ic1;
-        if (fl & FL_ICR_LD) { ic0 = make_float2(pl[buf].icr[j].x, pl[buf].icr[j].y); ic1 = make_float2(pl[buf].icr[j].z, pl[buf].icr[j].w); }
+        if (fl & FL_ICR_LD) { ic0 = make_float2(pl.icr[j].x, pl.icr[j].y); ic1 = make_float2(pl.icr[j].z, pl.icr[j].w); }
         else { ic0 = splat(a.ic_const); ic1 = ic0; }
         dd[j][0] = fma2(make_float2(-bx[0], -bx[1]), ic0, flag[j][0]);     // d = F - box * (1/count)
         dd[j][1] = fma2(make_float2(-bx[2], -bx[3]), ic1, flag[j][1]);
-      }
-      if (fl & FL_GATE_B) {                          // rows before the segment's first needed rho row
-#pragma unroll
-        for (int j = 0; j < RB; ++j)
-          if (y0 + j - LAG_B < r_lim) { dd[j][0] = splat(0.f); dd[j][1] = splat(0.f); }
       }
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
         V2[0] = fma2(neg2(dold[j][0]), dold[j][0], fma2(dd[j][0], dd[j][0], V2[0]));
         V2[1] = fma2(neg2(dold[j][1]), dold[j][1], fma2(dd[j][1], dd[j][1], V2[1]));
-        tm_st4(tm + TM_D + 4 * wrap26(w26 + j), dd[j][0], dd[j][1]);
+        tm_st4((j ? t_new1 : t_new0) + TM_D, dd[j][0], dd[j][1]);
         sts4(O_EV2 + (buf * RB + j) * PEV + KBG + 4 * tid, make_float4(V2[0].x, V2[0].y, V2[1].x, V2[1].y));
         const float2 ts = add2(V2[0], V2[1]);
         sts1(O_ET2 + (buf * RB + j) * PET + 3 + tid, ts.x + ts.y);
       }
     }
 
-    // ---- stage C: S = box(V2) / count at sigma ; eq. 5 ; candidates -----------------------------------
+    load_icr(fl & FL_ICR_PF);
+
+    // ---- stage C: S = box(V2) / count at sigma ; eq. 5 for the row ; candidates ------------------------
     if (fl & (FL_C0 | FL_C1)) {
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
@@ -465,68 +524,87 @@ struct Sweep {
         float bx[4];
         hbox25(O_EV2 + (pbuf * RB + j) * PEV + 4 * tid, O_ET2 + (pbuf * RB + j) * PET + tid, bx);
         float2 ic0, ic1;
-        if (fl & FL_ICS_LD) { ic0 = make_float2(pl[buf].ics[j].x, pl[buf].ics[j].y); ic1 = make_float2(pl[buf].ics[j].z, pl[buf].ics[j].w); }
+        if (fl & FL_ICS_LD) { ic0 = make_float2(pl.ics[j].x, pl.ics[j].y); ic1 = make_float2(pl.ics[j].z, pl.ics[j].w); }
         else { ic0 = splat(a.ic_const); ic1 = ic0; }
         const float2 s0 = mul2(make_float2(bx[0], bx[1]), ic0), s1 = mul2(make_float2(bx[2], bx[3]), ic1);
         const float2 k0 = mul2(s0, splat(a.kappa2)), k1 = mul2(s1, splat(a.kappa2));
-        const float2 q0 = mul2(dlag[j][0], dlag[j][0]), q1 = mul2(dlag[j][1], dlag[j][1]);
-        unsigned bits = (q0.x > k0.x ? 1u : 0u) | (q0.y > k0.y ? 2u : 0u) | (q1.x > k1.x ? 4u : 0u) | (q1.y > k1.y ? 8u : 0u);
-        bits &= umask;
-        if (__any_sync(0xffffffffu, bits != 0u)) {
+        // d^2 - kappa^2 S > 0 somewhere in the warp's row?  (the sign of the difference is exact)
+        const float2 m0 = fma2(dlag[j][0], dlag[j][0], neg2(k0)), m1 = fma2(dlag[j][1], dlag[j][1], neg2(k1));
+        const float mm = fmaxf(fmaxf(m0.x, m0.y), fmaxf(m1.x, m1.y));
+        if (__any_sync(0xffffffffu, mm > 0.f)) {
+          // exact bits (the sign of m is that of d^2 - kappa^2 S), then the queue of this iteration
           const float dv[4] = {dlag[j][0].x, dlag[j][0].y, dlag[j][1].x, dlag[j][1].y};
+          const float mv[4] = {m0.x, m0.y, m1.x, m1.y};
+          unsigned bits = 0u;
+#pragma unroll
+          for (int k = 0; k < 4; ++k)
+            if (dv[k] > 0.f && mv[k] > 0.f) bits |= 1u << k;
+          bits &= umask;
           const float sv[4] = {s0.x, s0.y, s1.x, s1.y};
           const int sg = y0 + j - LAG_C;
-          const unsigned lt = (1u << lane) - 1u;
-          const int nrow = __popc(__ballot_sync(0xffffffffu, bits & 1u)) + __popc(__ballot_sync(0xffffffffu, bits & 2u)) +
-                           __popc(__ballot_sync(0xffffffffu, bits & 4u)) + __popc(__ballot_sync(0xffffffffu, bits & 8u));
-          if (qcount + nrow > QCAP) {                // queue full (rare): test the row in place
-            nrec = cand_row_in_place(cand_ctx(), nrec, bits, make_float4(dv[0], dv[1], dv[2], dv[3]),
-                                     make_float4(sv[0], sv[1], sv[2], sv[3]), 4 * tid, sg);
-          } else {
+          if (bits) {
+            int pos = atomicAdd(reinterpret_cast<int*>(g_sm4) + O_QN + buf, __popc(bits));
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-              const bool on = (bits >> k) & 1u;
-              const unsigned m = __ballot_sync(0xffffffffu, on);
-              if (on)
-                sts4(O_Q + ((buf * NW + warp) * QCAP + qcount + __popc(m & lt)) * 4,
-                     make_float4(__int_as_float(4 * tid + k), __int_as_float(sg), dv[k], sv[k]));
-              qcount += __popc(m);
-            }
+            for (int k = 0; k < 4; ++k)
+              if (((bits >> k) & 1u) && pos < QCAP) {
+                sts4(O_Q + (buf * QCAP + pos) * 4, make_float4(__int_as_float(4 * tid + k), __int_as_float(sg), dv[k], sv[k]));
+                ++pos; bits &= ~(1u << k);
+              }
           }
+          if (__any_sync(0xffffffffu, bits != 0u))     // queue full
+            cand_in_place(cand_ctx(), bits, 4 * tid, sg, make_float4(dv[0], dv[1], dv[2], dv[3]), make_float4(sv[0], sv[1], sv[2], sv[3]));
         }
       }
     }
-    if (lane == 0) reinterpret_cast<int*>(g_sm4)[O_QN + buf * NW + warp] = qcount;
-    qcount = 0;
-    wF = wF + RB >= DFS ? wF + RB - DFS : wF + RB;
-    w26 = wrap26(w26 + RB);
+    load_ics(fl & FL_ICS_PF);
+    ws = ws + RB >= DRS ? ws + RB - DRS : ws + RB;
     y0 += RB;
     tm_wait_st();
     __syncthreads();
   }
 
-  __device__ __forceinline__ void run(int nb) {
-    // prologue: the input rows of iterations 0 and 1, the planes of iteration 0
-    load_rows(0, ctl(0) & FL_XMODE);
-    load_rows(1, nb > 1 ? (ctl(1) & FL_XMODE) : 0u);
+  // the extra warp: tests what the sweep warps queued in the previous iteration; same barriers as run()
+  __device__ __forceinline__ void run_consumer() {
+    int* qn = reinterpret_cast<int*>(g_sm4) + O_QN;
+    int nst = 0;
+    for (int b = 0; b <= nb; ++b) {
+      if (b > 0) {
+        const int pb = (b - 1) & 1;
+        const int n = min(qn[pb], QCAP);
+        if (n > 0) nst = cand_consume(cand_ctx(), O_Q + pb * QCAP * 4, n, O_ST, nst);
+        __syncwarp();
+        if (lane == 0) qn[pb] = 0;
+      }
+      if (b < nb) __syncthreads();
+    }
+    cand_flush(a_sh, O_ST, lane, nst);
+  }
+
+  __device__ __forceinline__ void run() {
     {
       const unsigned f0 = ctl(0);
-      load_planes(0, f0 & FL_NM_LD, f0 & FL_ICR_LD, f0 & FL_ICS_LD);
+      load_nm(f0 & FL_NM_LD); load_icr(f0 & FL_ICR_LD); load_ics(f0 & FL_ICS_LD);
     }
     int b = 0;
+    unsigned fl = ctl(0);
     while (true) {
-      iteration<0>(b); if (++b >= nb) break;
-      iteration<1>(b); if (++b >= nb) break;
-      iteration<2>(b); if (++b >= nb) break;
-      iteration<3>(b); if (++b >= nb) break;
+      unsigned fn = b + 1 < nb ? ctl(b + 1) : 0u;
+      iteration<0>(b, fl); if (++b >= nb) break;
+      fl = fn; fn = b + 1 < nb ? ctl(b + 1) : 0u;
+      iteration<1>(b, fl); if (++b >= nb) break;
+      fl = fn; fn = b + 1 < nb ? ctl(b + 1) : 0u;
+      iteration<2>(b, fl); if (++b >= nb) break;
+      fl = fn; fn = b + 1 < nb ? ctl(b + 1) : 0u;
+      iteration<3>(b, fl); if (++b >= nb) break;
+      fl = fn;
     }
-    process_queue((nb - 1) & 1);     // what the last iteration queued
-    nrec = cand_flush(a_sh, O_ST + warp * RCAP * 8, lane, nrec);
+    if (tid == 0)                                   // no bulk copy may be in flight when the CTA leaves
+      for (int bb = nb > XST ? nb - XST : 0; bb < nb; ++bb) mbar_wait(bar_addr(bb & (XST - 1)), (uint32_t)(bb >> 2) & 1u);
   }
 };
 
 template <int NW>
-__global__ void __launch_bounds__(NW * 32, 1)
+__global__ void __launch_bounds__(NW * 32 + 32, 1)
 k_fused_box(const FusedArgs a) {
   __shared__ uint32_t s_tmem;
   __shared__ FusedArgs s_args;
@@ -540,12 +618,15 @@ k_fused_box(const FusedArgs a) {
   const FusedItem it = a.items[blockIdx.x];
   s.a_sh = &s_args;
   s.tid = threadIdx.x; s.lane = threadIdx.x & 31; s.warp = threadIdx.x >> 5; s.plane = p; s.xs = it.xs;
+  s.nb = it.nb;
+  s.dirty = *a.dirty == a.dirty_seq;
   if (s.tid == 0) s_args = a;
-  for (int i = s.tid; i < (SW::O_FL >> 2); i += NW * 32) g_sm4[i] = zero4();
+  constexpr int NT = NW * 32 + 32;    // NW sweep warps and the candidate warp
+  for (int i = s.tid; i < (SW::O_FL >> 2); i += NT) g_sm4[i] = zero4();
   {
     uint32_t* fl_s = reinterpret_cast<uint32_t*>(g_sm4) + SW::O_FL;
     const uint32_t* src = a.flags + it.fl_off;
-    for (int i = s.tid; i < it.nb * NW; i += NW * 32) fl_s[i] = src[i];
+    for (int i = s.tid; i < it.nb * NW; i += NT) fl_s[i] = src[i];
   }
   if (s.warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n"
@@ -555,52 +636,57 @@ k_fused_box(const FusedArgs a) {
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+  if (s.tid == 0) {
+#pragma unroll
+    for (int i = 0; i < XST; ++i) mbar_init(s.bar_addr(i), 1);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");   // the zero fill above precedes the bulk copies
   const uint32_t tm_base = s_tmem;
   // warp w reaches the 32 lanes (w mod 4) * 32 ...; warps w and w+4 share them on different columns
   s.tm = tm_base + ((uint32_t)((s.warp & 3) * 32) << 16) + (uint32_t)(s.warp >> 2) * 256u;
-  for (int i = 0; i < 2 * DT; ++i) tm_st4(s.tm + 4 * i, splat(0.f), splat(0.f));
-  tm_wait_st();
+  const bool sweeper = s.warp < NW;
+  if (sweeper) {
+    for (int i = 0; i < 2 * DR; ++i) tm_st4(s.tm + 4 * i, splat(0.f), splat(0.f));
+    tm_wait_st();
+  }
 
   const long long N = (long long)a.Dy * a.Dx;
   const float* X = (p < a.B) ? a.cube + (long long)p * N : a.sum_plane;
   const int x = it.xs + 4 * s.tid;
-  const bool col_in = 4 * s.tid < a.CW && x < a.Dx;
-  const bool ld_left = col_in && s.lane == 0 && s.tid > 0;
-  const bool ld_right = col_in && s.lane == 31 && 4 * (s.tid + 1) < a.CW && x + 4 < a.Dx;
-  s.ld_edge = ld_left || ld_right;
-  s.eoff = ld_left ? -4 : 4;
+  s.col_in = sweeper && 4 * s.tid < a.CW && x < a.Dx;
   s.umask = 0u;
 #pragma unroll
   for (int k = 0; k < 4; ++k)
-    if (col_in && x + k >= it.ux0 && x + k < it.ux1) s.umask |= 1u << k;
-  s.f_lim = it.ya - 2 * KBG; s.r_lim = it.ya - KBG;
+    if (s.col_in && x + k >= it.ux0 && x + k < it.ux1) s.umask |= 1u << k;
   s.y0 = it.y_start;
-  if (col_in) {
+  {   // copied columns: the strip with 4 columns of margin, clipped to the image
+    const int cx0 = it.xs - 4 > 0 ? it.xs - 4 : 0;
+    const int cx1 = it.xs + a.CW + 4 < a.Dx ? it.xs + a.CW + 4 : a.Dx;
+    s.row_bytes = (uint32_t)(cx1 - cx0) * 4u;
+    s.xrow0 = X + (long long)it.y_start * a.Dx + cx0;
+    s.x_dst0 = smem_u32(reinterpret_cast<const float*>(g_sm4) + SW::O_X + (cx0 - (it.xs - 4)));
+  }
+  if (s.col_in) {
     s.sx = a.Dx;
-    s.xp = X + (long long)it.y_start * a.Dx + x;
-    s.wp = a.W + (long long)it.y_start * a.Dx + x;
     s.nmp = a.nm_pad + (long long)(it.y_start - 3 + PADR) * a.Dx + x;
     s.icrp = a.ic_pad + (long long)(it.y_start - LAG_B + PADR) * a.Dx + x;
     s.icsp = a.ic_pad + (long long)(it.y_start - LAG_C + PADR) * a.Dx + x;
   } else {              // lanes outside the strip read the zero row of a padded plane, over and over
     s.sx = 0;
-    s.xp = a.nm_pad; s.wp = reinterpret_cast<const uint8_t*>(a.nm_pad);
     s.nmp = a.nm_pad; s.icrp = a.nm_pad; s.icsp = a.nm_pad;
   }
 #pragma unroll
   for (int i = 0; i < 8; ++i) { s.hw[i][0] = splat(0.f); s.hw[i][1] = splat(0.f); }
   s.V1[0] = s.V1[1] = s.V2[0] = s.V2[1] = splat(0.f);
 #pragma unroll
-  for (int q = 0; q < 2; ++q)
-#pragma unroll
-    for (int j = 0; j < RB; ++j) {
-      s.pf[q].x[j] = zero4(); s.pf[q].xe[j] = zero4(); s.pf[q].w[j] = 0u; s.pf[q].we[j] = 0u;
-      s.pl[q].nm[j] = zero4(); s.pl[q].icr[j] = zero4(); s.pl[q].ics[j] = zero4();
-    }
-  s.w26 = 0; s.wF = 0; s.ring_y0 = it.y_start - 3; s.qcount = 0; s.nrec = 0;
+    for (int j = 0; j < RB; ++j) { s.pl.nm[j] = zero4(); s.pl.icr[j] = zero4(); s.pl.ics[j] = zero4(); }
+  s.ring_y0 = it.y_start - 3; s.ws = 0;
   __syncthreads();
+  if (s.tid == 0)
+    for (int bb = 0; bb < XST - 1 && bb < it.nb; ++bb) s.issue_rows(bb, it.y_start);
 
-  s.run(it.nb);
+  if (sweeper) s.run(); else s.run_consumer();
 
   tm_wait_st();
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
@@ -626,15 +712,15 @@ struct LpfFusedPlan {
 };
 
 static size_t fused_smem_bytes(int NW, int max_nb) {
-  const int CWP = NW * 128, PEV = CWP + 2 * KBG, PET = NW * 32 + 8;
-  const size_t nfl = (size_t)DFS * CWP + 4 * RB * PEV + 4 * RB * PET + 2 * NW * QCAP * 4 + 16 + NW * RCAP * 8;
+  const int CWP = NW * 128, XP = CWP + 8, PEV = CWP + 2 * KBG, PET = NW * 32 + 8;
+  const size_t nfl = (size_t)DRS * CWP + (size_t)XST * RB * XP + 4 * RB * PEV + 4 * RB * PET + 2 * QCAP * 4 + 4 + SCAP * 8 + 2 * XST;
   return (nfl + (size_t)max_nb * NW) * sizeof(float) + 16;
 }
 
 template <int NW>
 static cudaError_t fused_launch_t(const FusedArgs& a, dim3 grid, size_t smem, cudaStream_t st, bool set_attr) {
   if (set_attr) return cudaFuncSetAttribute(k_fused_box<NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  k_fused_box<NW><<<grid, NW * 32, smem, st>>>(a);
+  k_fused_box<NW><<<grid, NW * 32 + 32, smem, st>>>(a);
   return cudaSuccess;
 }
 
@@ -721,17 +807,20 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
     rows_all += s.yb - s.ya;
   }
   if (rows_all <= 0) return LPF_OK;
-  // segments per strip: minimise waves x (rows per segment + warm-up cost) over the segment count
+  // segments per strip: minimise waves x (rows per segment + warm-up cost) over the segment count.  With
+  // n_lanes frames in flight the kernels of different lanes share the SMs, so each gets its share of them
+  // (fewer, longer segments: less warm-up per output row).
   const int n_planes = c->n_planes;
-  const double warm = 24.0;   // the 58 warm-up/drain rows of a segment run a part of the pipeline only
+  const int sm_share = std::max(1, c->n_sm / std::max(1, p.n_lanes));
+  const double warm = 58.0;   // warm-up / drain rows of a segment
   int best_seg = 1; double best_cost = 1e30;
   const int max_rows_strip = (int)(rows_all / n_strips);
   for (int nseg = 1; nseg <= 64; ++nseg) {
     const double rows = (double)max_rows_strip / nseg;
     if (nseg > 1 && rows < 24) break;
-    if (rows > 900 && nseg < 64) continue;      // keeps an item's control words within shared memory
+    if (rows > 640 && nseg < 64) continue;      // keeps an item's control words within shared memory
     const long long ctas = (long long)nseg * n_strips * n_planes;
-    const double waves = (double)((ctas + c->n_sm - 1) / c->n_sm);
+    const double waves = (double)((ctas + sm_share - 1) / sm_share);
     const double cost = waves * (rows + warm);
     if (cost < best_cost - 1e-9) { best_cost = cost; best_seg = nseg; }
   }
@@ -794,11 +883,7 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
     it.nb = (it.yb - 1 + LAG_C - ys) / RB + 1;
     it.fl_off = (int)flags.size();
     max_nb = std::max(max_nb, it.nb);
-    auto xmode = [&](int y, int w) -> unsigned {
-      const int a0 = cell(y, w), a1 = cell(y + 1, w);
-      if (!((a0 | a1) & CL_ANYW)) return 0u;
-      return (a0 & a1 & CL_ALLW) ? 1u : 2u;
-    };
+    auto xmode = [&](int y, int w) -> unsigned { return ((cell(y, w) | cell(y + 1, w)) & CL_ANYW) ? FL_X : 0u; };
     auto both = [&](int y, int w, int bit) -> bool { return (cell(y, w) & cell(y + 1, w) & bit) != 0; };
     for (int b = 0; b < it.nb; ++b)
       for (int w = 0; w < NW; ++w) {
@@ -812,11 +897,8 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
           return f;
         };
         unsigned f = xmode(y0, w);
-        if (b + 2 < it.nb) f |= xmode(y0 + 2 * RB, w) << FL_PMODE_SH;
         f |= ld_bits(y0);
         if (b + 1 < it.nb) f |= ld_bits(y0 + RB) << 3;     // FL_*_LD -> FL_*_PF
-        if (y0 - 3 < it.ya - 2 * KBG) f |= FL_GATE_A;
-        if (y0 - LAG_B < it.ya - KBG) f |= FL_GATE_B;
         if (y0 + 1 - LAG_B >= it.ya - KBG) f |= FL_DO_B;
         if (y0 - LAG_C >= it.ya && y0 - LAG_C < it.yb) f |= FL_C0;
         if (y0 + 1 - LAG_C >= it.ya && y0 + 1 - LAG_C < it.yb) f |= FL_C1;
@@ -827,7 +909,7 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
   static_assert((FL_NM_LD << 3) == FL_NM_PF && (FL_ICR_LD << 3) == FL_ICR_PF && (FL_ICS_LD << 3) == FL_ICS_PF, "flag layout");
 
   LpfFusedPlan* pl = new LpfFusedPlan();
-  pl->CW = CW; pl->NW = NW; pl->threads = NW * 32; pl->n_items = (int)ditems.size();
+  pl->CW = CW; pl->NW = NW; pl->threads = NW * 32 + 32; pl->n_items = (int)ditems.size();
   pl->smem = fused_smem_bytes(NW, max_nb);
   int dev = 0; cudaGetDevice(&dev);
   int max_smem = 0;
@@ -879,10 +961,10 @@ int lpf_launch_detect_fused(lpf_ctx* c, LpfFusedPlan* pl, LpfLane& L, const floa
                             lpf_det* d_dets, int32_t* d_ndets, cudaStream_t st) {
   const lpf_params& p = c->p;
   LPF_CUDA(cudaMemsetAsync(d_ndets, 0, sizeof(int32_t), st));
-  if (p.detect_sum_plane) { int rc = lpf_launch_sum_plane(c, L, d_cube, d_band_ok, st); if (rc) return rc; }
+  { int rc = lpf_launch_sum_plane(c, L, d_cube, d_band_ok, p.detect_sum_plane != 0, st); if (rc) return rc; }   // + the exact-zero check
   FusedArgs a{};
   a.cube = d_cube; a.sum_plane = L.sum_plane; a.band_ok = d_band_ok; a.W = c->W;
-  a.nm_pad = pl->d_nm_pad; a.ic_pad = pl->d_ic_pad; a.items = pl->d_items; a.flags = pl->d_flags;
+  a.nm_pad = pl->d_nm_pad; a.ic_pad = pl->d_ic_pad; a.items = pl->d_items; a.flags = pl->d_flags; a.dirty = L.dirty; a.dirty_seq = L.dirty_seq;
   a.B = p.B; a.Dy = p.Dy; a.Dx = p.Dx; a.CW = pl->CW; a.k_max = p.k_max; a.max_det = p.max_det;
   a.g0 = c->g_mf.g[3]; a.g1 = c->g_mf.g[2]; a.g2 = c->g_mf.g[1]; a.g3 = c->g_mf.g[0];
   a.kappa2 = p.kappa * p.kappa; a.eps_rel = p.eps_rel; a.nm_const = pl->nm_const; a.ic_const = pl->ic_const;

@@ -81,6 +81,8 @@ int alloc_lane(lpf_ctx* c, LpfLane& L) {
   TRY(dalloc(&L.qc_part1, (size_t)p.B * c->qc_nblk * 3));
   TRY(dalloc(&L.qc_part2, (size_t)p.B * c->qc_nblk * 3));
   TRY(dalloc(&L.sum_plane, N));
+  TRY(dalloc(&L.dirty, 1));
+  LPF_CUDA(cudaMemset(L.dirty, 0, sizeof(int32_t)));
   TRY(dalloc(&L.F, P * N));
   TRY(dalloc(&L.C, P * N));
   TRY(dalloc(&L.S, P * N));
@@ -112,7 +114,7 @@ int alloc_lane(lpf_ctx* c, LpfLane& L) {
 }
 
 void free_lane(LpfLane& L) {
-  void* ptrs[] = {L.qc_part1, L.qc_part2, L.sum_plane, L.F, L.C, L.S, L.Y, L.normp, L.M, L.tmp_pos, L.tmp_plane,
+  void* ptrs[] = {L.qc_part1, L.qc_part2, L.sum_plane, L.dirty, L.F, L.C, L.S, L.Y, L.normp, L.M, L.tmp_pos, L.tmp_plane,
                   L.tmp_snr, L.tmp_n, L.stats, L.band_ok, L.dets, L.ndets, L.upos, L.uplane, L.usnr, L.nu,
                   L.cand_idx, L.act_slots, L.act_pix, L.npos, L.flux, L.cube};
   for (void* q : ptrs) if (q) cudaFree(q);
@@ -125,7 +127,9 @@ void free_lane(LpfLane& L) {
 // S3-S8 dispatch: the fused sweep kernel when the parameter set allows it, else the general path.
 int lpf_launch_detect(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, lpf_det* d_dets,
                       int32_t* d_ndets, cudaStream_t st) {
-  if (c->fused) return lpf_launch_detect_fused(c, c->fused, L, d_cube, d_band_ok, d_dets, d_ndets, st);
+  // the fused kernel fetches rows with 16-byte bulk copies: a misaligned cube takes the general path
+  if (c->fused && (((uintptr_t)d_cube) & 15) == 0)
+    return lpf_launch_detect_fused(c, c->fused, L, d_cube, d_band_ok, d_dets, d_ndets, st);
   return lpf_launch_detect_general(c, L, d_cube, d_band_ok, d_dets, d_ndets, st);
 }
 

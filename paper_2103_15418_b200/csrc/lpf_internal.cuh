@@ -19,6 +19,8 @@ struct LpfLane {
   double* qc_part1 = nullptr;  // [B][nblk][3]  n, sum(x-p), sum(x-p)^2
   double* qc_part2 = nullptr;  // [B][nblk][3]  clipped
   float* sum_plane = nullptr;  // [N]
+  int32_t* dirty = nullptr;    // [1] == dirty_seq: the cube of the current frame needs masking (detect_general.cu k_sum_plane)
+  int32_t dirty_seq = 0;
   float* F = nullptr;          // [(B+1)][N] matched-filtered planes (general path)
   float* C = nullptr;          // [(B+1)][N]
   float* S = nullptr;          // [(B+1)][N]
@@ -118,7 +120,7 @@ void lpf_prof_post(lpf_ctx* c, cudaStream_t st);
 // ---- launchers implemented in the kernel translation units ---------------------------------
 int lpf_launch_qc(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, cudaStream_t st);
 
-int lpf_launch_sum_plane(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, cudaStream_t st);
+int lpf_launch_sum_plane(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, bool want_sum, cudaStream_t st);
 int lpf_launch_detect_general(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok,
                               lpf_det* d_dets, int32_t* d_ndets, cudaStream_t st);
 int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out);
