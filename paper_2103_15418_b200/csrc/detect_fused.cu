@@ -45,7 +45,8 @@ constexpr int LAG_C = LAG_B + KBG + RB;      // sig = y - 31
 constexpr int DR = 32;              // depth (rows) of the tensor-memory rings of F and d (power of two)
 constexpr int DRS = 34;             // depth of the shared-memory ring of F: local maxima are tested one iteration late
 constexpr int QCAP = 64;            // queued candidates per iteration (more are tested in place)
-constexpr int SCAP = 64;            // records staged by the candidate warp between flushes
+constexpr int SCAP = 32;            // records staged by a helper warp between flushes
+constexpr int NHW = 4;              // helper warps: input producer and candidate tests
 constexpr int XST = 4;              // input staging stages (iterations in flight)
 constexpr int TM_D = 4 * DR;        // first tensor-memory column of the d ring (F ring starts at 0)
 constexpr int PADR = 64;            // zero rows above and below the padded normaliser planes
@@ -223,7 +224,9 @@ __device__ __noinline__ void cand_flush(const FusedArgs* ap, int o_st, int lane,
     const int idx = base + i;
     if (idx < ap->max_det) {
       uint2* dst = reinterpret_cast<uint2*>(ap->dets + idx);
-      dst[0] = r[0]; dst[1] = r[1]; dst[2] = r[2];
+      uint2 r2 = r[2];
+      r2.y = __float_as_uint(__uint_as_float(r2.y) / sqrtf(__uint_as_float(r2.x)));
+      dst[0] = r[0]; dst[1] = r[1]; dst[2] = r2;
     } else {
       atomicAdd(&ap->counters[0], 1);
     }
@@ -242,21 +245,63 @@ __device__ __forceinline__ int cand_stage(const CandCtx& c, int o_st, int nst, b
     r[0] = (uint32_t)(sg * a.Dx + c.xs + cl);
     r[1] = (uint32_t)(c.plane & 0xffff) | (1u << 16);        // int16 plane, int16 iter = 1
     r[2] = __float_as_uint(fv); r[3] = __float_as_uint(cc); r[4] = __float_as_uint(se);
-    r[5] = __float_as_uint(d / sqrtf(se));
+    r[5] = __float_as_uint(d);                               // snr = d / sqrt(s_eff) is taken at flush time
   }
   __syncwarp();
   return nst + __popc(m);
 }
 
-// the queue of one iteration, n entries {col, row, d, s} at float index o_q: the consumer warp's work
-__device__ __noinline__ int cand_consume(CandCtx c, int o_q, int n, int o_st, int nst) {
-  for (int e0 = 0; e0 < n; e0 += 32) {
+// k_max = 2: five lanes per candidate, one window row each (six candidates per warp and pass).  e0: the
+// warp's first entry of this pass.  Queue entry: {col | slot << 16, row, d, s}, slot = the row's place in
+// the F ring.  Written for a short dependent chain: all six shared loads leave together.
+struct CandK { float kappa2, eps_rel; int Dy, Dx; const uint8_t* W; };
+__device__ __forceinline__ int cand_pass5(const CandCtx& c, const CandK& k, int o_q, int n, int e0, int o_st, int nst) {
+  const int CWP = c.CWP;
+  const int g = (c.lane * 13) >> 6, r = c.lane - 5 * g;        // lane / 5, lane % 5 (lanes 30, 31: g = 6, idle)
+  const int e = e0 + g;
+  const bool act = g < 6 && e < n;
+  const float4 q = lds4(o_q + 4 * (act ? e : 0));
+  const int cs = __float_as_int(q.x), cl = cs & 0xffff, s0 = cs >> 16, sg = __float_as_int(q.y);
+  const float d = q.z;
+  int sl = s0 + r - 2;
+  sl = sl < 0 ? sl + DRS : (sl >= DRS ? sl - DRS : sl);
+  const int yy = sg + r - 2;
+  const int rb = sl * CWP;
+  const float fv = lds1(s0 * CWP + cl);
+  float fn[5];
+#pragma unroll
+  for (int dx = 0; dx < 5; ++dx) {
+    int c2 = cl + dx - 2;
+    c2 = c2 < 0 ? 0 : (c2 >= CWP ? CWP - 1 : c2);
+    fn[dx] = lds1(rb + c2);
+  }
+  const float cc = fv - d;
+  const float gd = k.eps_rel * fabsf(cc);
+  const float se = fmaxf(q.w, gd * gd);
+  const bool pass = act && d > 0.f && d * d > k.kappa2 * se;
+  const bool row_in = pass && yy >= 0 && yy < k.Dy;
+  bool bigger = false;
+#pragma unroll
+  for (int dx = 0; dx < 5; ++dx) {
+    const int c2 = cl + dx - 2, xn = c.xs + c2;
+    const bool in = row_in && c2 >= 0 && c2 < CWP && xn < k.Dx;
+    // masked pixels hold F = 0 in the ring: W is consulted only when such a zero would win
+    if (in && fn[dx] > fv) bigger = bigger || (fn[dx] != 0.f) || (k.W[(long long)yy * k.Dx + xn] != 0);
+  }
+  const unsigned ball = __ballot_sync(0xffffffffu, bigger);
+  const bool ok = pass && r == 0 && ((ball >> (5 * g)) & 31u) == 0u;
+  return cand_stage(c, o_st, nst, ok, cl, sg, d, fv, cc, se);
+}
+
+// the queue of one iteration, n entries {col, row, d, s} at float index o_q: the share of helper warp hw of nh
+__device__ __noinline__ int cand_consume(CandCtx c, int o_q, int n, int hw, int nh, int o_st, int nst) {
+  for (int e0 = 32 * hw; e0 < n; e0 += 32 * nh) {
     const int e = e0 + c.lane;
     bool ok = false;
     int cl = 0, sg = 0; float d = 0.f, fv = 0.f, cc = 0.f, se = 1.f;
     if (e < n) {
       const float4 q = lds4(o_q + 4 * e);
-      cl = __float_as_int(q.x); sg = __float_as_int(q.y); d = q.z;
+      cl = __float_as_int(q.x) & 0xffff; sg = __float_as_int(q.y); d = q.z;
       ok = cand_test_any(c, cl, sg, d, q.w, fv, cc, se);
     }
     nst = cand_stage(c, o_st, nst, ok, cl, sg, d, fv, cc, se);
@@ -326,9 +371,9 @@ struct Sweep {
   static constexpr int O_ET1 = O_EV2 + 2 * RB * PEV;
   static constexpr int O_ET2 = O_ET1 + 2 * RB * PET;
   static constexpr int O_Q = O_ET2 + 2 * RB * PET;       // candidate queues, [2][QCAP] x {col, row, d, s}
-  static constexpr int O_QN = O_Q + 2 * QCAP * 4;        // their lengths, [2] (padded to 4 words)
-  static constexpr int O_ST = O_QN + 4;                  // staged records of the candidate warp, [SCAP] x 8 words
-  static constexpr int O_BAR = O_ST + SCAP * 8;          // XST mbarriers (8 bytes each)
+  static constexpr int O_QN = O_Q + 2 * QCAP * 4;        // their lengths, one word per iteration mod 4
+  static constexpr int O_ST = O_QN + 4;                  // staged records of the helper warps, [NHW][SCAP] x 8 words
+  static constexpr int O_BAR = O_ST + NHW * SCAP * 8;    // XST mbarriers (8 bytes each)
   static constexpr int O_FL = O_BAR + 2 * XST;           // control words, [nb][NW]
   // ---- constants of the thread -----------------------------------------------------------------
   const FusedArgs& a;
@@ -350,6 +395,18 @@ struct Sweep {
   int y0;                  // first input row of the current iteration
   int ring_y0;             // the row that sits in slot 0 of the rings
   int ws;                  // slot of this iteration's first F row in the shared-memory ring
+#ifdef EXP_TIMING
+  long long t_busy = 0, t_wait = 0, t_mark = 0, t_cons = 0; int n_cons = 0, n_sum = 0;
+  long long* t_arr;        // [2][16] arrival clocks of the warps
+  __device__ __forceinline__ void sync_timed(int b) {
+    const long long t1 = clock64();
+    if (lane == 0) t_arr[(b & 1) * 16 + warp] = t1;
+    __syncthreads();
+    long long mx = 0;
+    for (int i = 0; i < NW + NHW; ++i) { const long long v = t_arr[(b & 1) * 16 + i]; mx = v > mx ? v : mx; }
+    t_busy += t1 - t_mark; t_wait += mx - t1; t_mark = mx;
+  }
+#endif
   float2 hw[8][2];         // horizontally filtered rows (rotating; static indices per phase)
   float2 V1[2], V2[2];     // vertical running sums
   Planes pl;               // normalisers of the coming rows: each plane is reloaded right after its use
@@ -414,8 +471,6 @@ struct Sweep {
     float2 fold[RB][2], flag[RB][2], dold[RB][2], dlag[RB][2];
     tm_ld4(t_old0, fold[0][0], fold[0][1]); tm_ld4(t_old1, fold[1][0], fold[1][1]);
 
-    // ---- producer: the input rows of iteration b + XST - 1 (their stage was read in iteration b - 1) ----
-    if (tid == 0 && b + XST - 1 < nb) issue_rows(b + XST - 1, y0 - RB * b);
 
     // ---- stage A, part 1: staged rows -> horizontal matched filter ------------------------------------
     if (fl & FL_X) {
@@ -542,12 +597,14 @@ struct Sweep {
           bits &= umask;
           const float sv[4] = {s0.x, s0.y, s1.x, s1.y};
           const int sg = y0 + j - LAG_C;
+          int sslot = ws + j - (LAG_C - 3);                    // ring slot of row sigma (this iteration's F row j: ws + j)
+          sslot = sslot < 0 ? sslot + DRS : sslot;
           if (bits) {
-            int pos = atomicAdd(reinterpret_cast<int*>(g_sm4) + O_QN + buf, __popc(bits));
+            int pos = atomicAdd(reinterpret_cast<int*>(g_sm4) + O_QN + (b & 3), __popc(bits));
 #pragma unroll
             for (int k = 0; k < 4; ++k)
               if (((bits >> k) & 1u) && pos < QCAP) {
-                sts4(O_Q + (buf * QCAP + pos) * 4, make_float4(__int_as_float(4 * tid + k), __int_as_float(sg), dv[k], sv[k]));
+                sts4(O_Q + (buf * QCAP + pos) * 4, make_float4(__int_as_float((4 * tid + k) | (sslot << 16)), __int_as_float(sg), dv[k], sv[k]));
                 ++pos; bits &= ~(1u << k);
               }
           }
@@ -560,24 +617,52 @@ struct Sweep {
     ws = ws + RB >= DRS ? ws + RB - DRS : ws + RB;
     y0 += RB;
     tm_wait_st();
+#ifdef EXP_TIMING
+    sync_timed(b);
+#else
     __syncthreads();
+#endif
   }
 
-  // the extra warp: tests what the sweep warps queued in the previous iteration; same barriers as run()
-  __device__ __forceinline__ void run_consumer() {
+  // the helper warps: helper 0 feeds the input stages (bulk copies three iterations ahead); all of them test
+  // what the sweep warps queued in the previous iteration.  Same barriers as run().
+  __device__ __forceinline__ void run_helper(int ys) {
     int* qn = reinterpret_cast<int*>(g_sm4) + O_QN;
+    const int hw = warp - NW;
+    const int o_st = O_ST + hw * SCAP * 8;
     int nst = 0;
+    const CandCtx cc = cand_ctx();
+    CandK ck; ck.kappa2 = a.kappa2; ck.eps_rel = a.eps_rel; ck.Dy = a.Dy; ck.Dx = a.Dx; ck.W = a.W;
+    const bool km2 = a.k_max == 2;
     for (int b = 0; b <= nb; ++b) {
-      if (b > 0) {
-        const int pb = (b - 1) & 1;
-        const int n = min(qn[pb], QCAP);
-        if (n > 0) nst = cand_consume(cand_ctx(), O_Q + pb * QCAP * 4, n, O_ST, nst);
-        __syncwarp();
-        if (lane == 0) qn[pb] = 0;
+      if (hw == NHW - 1 && lane == 0) {
+        if (b + XST - 1 < nb) issue_rows(b + XST - 1, ys);     // their stage was read in iteration b - 1
+        qn[(b + 1) & 3] = 0;                                   // next iteration's counter (last read in b - 2)
       }
+      if (b > 0) {
+        const int n = min(qn[(b - 1) & 3], QCAP);
+#ifdef EXP_TIMING
+        const long long tc0 = clock64();
+#endif
+        if (n > 0) {
+          const int o_q = O_Q + ((b - 1) & 1) * QCAP * 4;
+          if (km2) { for (int e0 = 6 * hw; e0 < n; e0 += 6 * NHW) nst = cand_pass5(cc, ck, o_q, n, e0, o_st, nst); }
+          else nst = cand_consume(cc, o_q, n, hw, NHW, o_st, nst);
+        }
+#ifdef EXP_TIMING
+        const long long tc1 = clock64();
+        if (n > 6 * hw) { t_cons += tc1 - tc0; n_cons += 1; n_sum += n; }
+#endif
+      }
+#ifdef EXP_TIMING
+      if (b < nb) sync_timed(b);
+#else
       if (b < nb) __syncthreads();
+#endif
     }
-    cand_flush(a_sh, O_ST, lane, nst);
+    cand_flush(a_sh, o_st, lane, nst);
+    if (hw == NHW - 1 && lane == 0)                   // no bulk copy may be in flight when the CTA leaves
+      for (int bb = nb > XST ? nb - XST : 0; bb < nb; ++bb) mbar_wait(bar_addr(bb & (XST - 1)), (uint32_t)(bb >> 2) & 1u);
   }
 
   __device__ __forceinline__ void run() {
@@ -598,13 +683,11 @@ struct Sweep {
       iteration<3>(b, fl); if (++b >= nb) break;
       fl = fn;
     }
-    if (tid == 0)                                   // no bulk copy may be in flight when the CTA leaves
-      for (int bb = nb > XST ? nb - XST : 0; bb < nb; ++bb) mbar_wait(bar_addr(bb & (XST - 1)), (uint32_t)(bb >> 2) & 1u);
   }
 };
 
 template <int NW>
-__global__ void __launch_bounds__(NW * 32 + 32, 1)
+__global__ void __launch_bounds__(NW * 32 + NHW * 32, 1)
 k_fused_box(const FusedArgs a) {
   __shared__ uint32_t s_tmem;
   __shared__ FusedArgs s_args;
@@ -621,7 +704,7 @@ k_fused_box(const FusedArgs a) {
   s.nb = it.nb;
   s.dirty = *a.dirty == a.dirty_seq;
   if (s.tid == 0) s_args = a;
-  constexpr int NT = NW * 32 + 32;    // NW sweep warps and the candidate warp
+  constexpr int NT = NW * 32 + NHW * 32;    // NW sweep warps and the helper warps
   for (int i = s.tid; i < (SW::O_FL >> 2); i += NT) g_sm4[i] = zero4();
   {
     uint32_t* fl_s = reinterpret_cast<uint32_t*>(g_sm4) + SW::O_FL;
@@ -683,10 +766,19 @@ k_fused_box(const FusedArgs a) {
     for (int j = 0; j < RB; ++j) { s.pl.nm[j] = zero4(); s.pl.icr[j] = zero4(); s.pl.ics[j] = zero4(); }
   s.ring_y0 = it.y_start - 3; s.ws = 0;
   __syncthreads();
-  if (s.tid == 0)
+  if (s.tid == (NW + NHW - 1) * 32)
     for (int bb = 0; bb < XST - 1 && bb < it.nb; ++bb) s.issue_rows(bb, it.y_start);
 
-  if (sweeper) s.run(); else s.run_consumer();
+#ifdef EXP_TIMING
+  __shared__ long long s_tarr[32];
+  s.t_arr = s_tarr;
+  s.t_mark = clock64();
+#endif
+  if (sweeper) s.run(); else s.run_helper(it.y_start);
+#ifdef EXP_TIMING
+  if (s.lane == 0 && blockIdx.x == 3 && (p == 0 || p == a.B))
+    printf("plane %d warp %d busy %lld wait %lld nb %d | consume calls %d cycles %lld n_sum %d\n", p, s.warp, s.t_busy, s.t_wait, it.nb, s.n_cons, s.t_cons, s.n_sum);
+#endif
 
   tm_wait_st();
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
@@ -713,14 +805,14 @@ struct LpfFusedPlan {
 
 static size_t fused_smem_bytes(int NW, int max_nb) {
   const int CWP = NW * 128, XP = CWP + 8, PEV = CWP + 2 * KBG, PET = NW * 32 + 8;
-  const size_t nfl = (size_t)DRS * CWP + (size_t)XST * RB * XP + 4 * RB * PEV + 4 * RB * PET + 2 * QCAP * 4 + 4 + SCAP * 8 + 2 * XST;
+  const size_t nfl = (size_t)DRS * CWP + (size_t)XST * RB * XP + 4 * RB * PEV + 4 * RB * PET + 2 * QCAP * 4 + 4 + NHW * SCAP * 8 + 2 * XST;
   return (nfl + (size_t)max_nb * NW) * sizeof(float) + 16;
 }
 
 template <int NW>
 static cudaError_t fused_launch_t(const FusedArgs& a, dim3 grid, size_t smem, cudaStream_t st, bool set_attr) {
   if (set_attr) return cudaFuncSetAttribute(k_fused_box<NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  k_fused_box<NW><<<grid, NW * 32 + 32, smem, st>>>(a);
+  k_fused_box<NW><<<grid, NW * 32 + NHW * 32, smem, st>>>(a);
   return cudaSuccess;
 }
 
@@ -909,7 +1001,7 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
   static_assert((FL_NM_LD << 3) == FL_NM_PF && (FL_ICR_LD << 3) == FL_ICR_PF && (FL_ICS_LD << 3) == FL_ICS_PF, "flag layout");
 
   LpfFusedPlan* pl = new LpfFusedPlan();
-  pl->CW = CW; pl->NW = NW; pl->threads = NW * 32 + 32; pl->n_items = (int)ditems.size();
+  pl->CW = CW; pl->NW = NW; pl->threads = NW * 32 + NHW * 32; pl->n_items = (int)ditems.size();
   pl->smem = fused_smem_bytes(NW, max_nb);
   int dev = 0; cudaGetDevice(&dev);
   int max_smem = 0;
