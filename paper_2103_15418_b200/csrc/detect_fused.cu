@@ -1050,10 +1050,13 @@ int lpf_fused_plan_info(const LpfFusedPlan* pl, int* cw, int* threads, int* n_it
 }
 
 int lpf_launch_detect_fused(lpf_ctx* c, LpfFusedPlan* pl, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok,
-                            lpf_det* d_dets, int32_t* d_ndets, cudaStream_t st) {
+                            lpf_det* d_dets, int32_t* d_ndets, bool sum_done, cudaStream_t st) {
   const lpf_params& p = c->p;
-  LPF_CUDA(cudaMemsetAsync(d_ndets, 0, sizeof(int32_t), st));
-  { int rc = lpf_launch_sum_plane(c, L, d_cube, d_band_ok, p.detect_sum_plane != 0, st); if (rc) return rc; }   // + the exact-zero check
+  if (!sum_done) {     // the chained frame call has done both in its second QC pass
+    LPF_CUDA(cudaMemsetAsync(d_ndets, 0, sizeof(int32_t), st));
+    int rc = lpf_launch_sum_plane(c, L, d_cube, d_band_ok, p.detect_sum_plane != 0, st);   // + the exact-zero check
+    if (rc) return rc;
+  }
   FusedArgs a{};
   a.cube = d_cube; a.sum_plane = L.sum_plane; a.band_ok = d_band_ok; a.W = c->W;
   a.nm_pad = pl->d_nm_pad; a.ic_pad = pl->d_ic_pad; a.items = pl->d_items; a.flags = pl->d_flags; a.dirty = L.dirty; a.dirty_seq = L.dirty_seq;

@@ -162,42 +162,6 @@ int launch_sepconv(lpf_ctx* c, const ConvArgs& a, cudaStream_t st) {
   return LPF_OK;
 }
 
-// X_sum = sum over accepted bands (plane B).  Plain streaming add, 128-bit loads.  The same pass checks
-// that every invalid pixel of the accepted bands holds an exact zero (then W X = X and the fused kernel
-// reads the cube unmasked); if not it writes seq to *dirty.  out == nullptr: the check only.
-__global__ void __launch_bounds__(256)
-k_sum_plane(const float* __restrict__ cube, const uint8_t* __restrict__ band_ok, const uint8_t* __restrict__ W,
-            int B, long long N, float* __restrict__ out, int32_t* __restrict__ dirty, int seq) {
-  if (!band_ok[B]) return;
-  const bool vec = ((N & 3) == 0) && ((((uintptr_t)cube) & 15) == 0);
-  const long long stride = (long long)gridDim.x * blockDim.x;
-  bool bad = false;
-  if (vec) {
-    const long long n4 = N >> 2;
-    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n4; q += stride) {
-      float4 s = make_float4(0.f, 0.f, 0.f, 0.f);
-      const unsigned wm = __ldg(reinterpret_cast<const unsigned*>(W) + q);
-      const bool m0 = !(wm & 0x000000ffu), m1 = !(wm & 0x0000ff00u), m2 = !(wm & 0x00ff0000u), m3 = !(wm & 0xff000000u);
-      for (int b = 0; b < B; ++b) {
-        if (!band_ok[b]) continue;
-        const float4 x = __ldg(reinterpret_cast<const float4*>(cube + (long long)b * N) + q);
-        s.x += x.x; s.y += x.y; s.z += x.z; s.w += x.w;
-        bad = bad || (m0 && x.x != 0.f) || (m1 && x.y != 0.f) || (m2 && x.z != 0.f) || (m3 && x.w != 0.f);
-      }
-      if (out) reinterpret_cast<float4*>(out)[q] = s;
-    }
-  } else {
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
-      float s = 0.f;
-      const bool inv = W[i] == 0;
-      for (int b = 0; b < B; ++b)
-        if (band_ok[b]) { const float x = cube[(long long)b * N + i]; s += x; bad = bad || (inv && x != 0.f); }
-      if (out) out[i] = s;
-    }
-  }
-  if (bad) *dirty = seq;
-}
-
 struct ThrArgs {
   const float* F; const float* C; const float* S;
   const uint8_t* W; uint8_t* Y; const uint8_t* band_ok;
@@ -260,14 +224,6 @@ k_threshold_peaks(const ThrArgs a) {
 
 }  // namespace
 
-int lpf_launch_sum_plane(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, bool want_sum, cudaStream_t st) {
-  const int blocks = c->n_sm * 8;
-  L.dirty_seq = L.dirty_seq >= 0x7ffffff0 ? 1 : L.dirty_seq + 1;
-  LPF_KLAUNCH(c, KID_SUM_PLANE, st, k_sum_plane<<<blocks, 256, 0, st>>>(d_cube, d_band_ok, c->W, c->p.B, c->N,
-                                                                       want_sum ? L.sum_plane : nullptr, L.dirty, L.dirty_seq));
-  return LPF_OK;
-}
-
 // norm = W / (g (*) W) for the static mask (R7).  d_tmp unused (kept for symmetry).
 int lpf_launch_static_norm(lpf_ctx* c, const LpfTaps& g, float* d_norm, float* /*d_tmp*/, cudaStream_t st) {
   ConvArgs a{};
@@ -277,11 +233,13 @@ int lpf_launch_static_norm(lpf_ctx* c, const LpfTaps& g, float* d_norm, float* /
 }
 
 int lpf_launch_detect_general(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok,
-                              lpf_det* d_dets, int32_t* d_ndets, cudaStream_t st) {
+                              lpf_det* d_dets, int32_t* d_ndets, bool sum_done, cudaStream_t st) {
   const lpf_params& p = c->p;
   int rc;
-  LPF_CUDA(cudaMemsetAsync(d_ndets, 0, sizeof(int32_t), st));
-  if (p.detect_sum_plane) { rc = lpf_launch_sum_plane(c, L, d_cube, d_band_ok, true, st); if (rc) return rc; }
+  if (!sum_done) {
+    LPF_CUDA(cudaMemsetAsync(d_ndets, 0, sizeof(int32_t), st));
+    if (p.detect_sum_plane) { rc = lpf_launch_sum_plane(c, L, d_cube, d_band_ok, true, st); if (rc) return rc; }
+  }
   if (p.n_iter > 1) LPF_CUDA(cudaMemsetAsync(L.Y, 0, (size_t)c->n_planes * c->N, st));
 
   ConvArgs a{};

@@ -79,7 +79,10 @@ int alloc_lane(lpf_ctx* c, LpfLane& L) {
   const lpf_params& p = c->p;
   const size_t N = (size_t)c->N, P = (size_t)p.B + 1;
   TRY(dalloc(&L.qc_part1, (size_t)p.B * c->qc_nblk * 3));
-  TRY(dalloc(&L.qc_part2, (size_t)p.B * c->qc_nblk * 3));
+  TRY(dalloc(&L.qc_part2, (size_t)lpf_qc2_blocks(c) * p.B * 3));
+  TRY(dalloc(&L.qc_band_clip, (size_t)p.B * 2));
+  TRY(dalloc(&L.qc_counter, 2));
+  LPF_CUDA(cudaMemset(L.qc_counter, 0, 2 * sizeof(int32_t)));
   TRY(dalloc(&L.sum_plane, N));
   TRY(dalloc(&L.dirty, 1));
   LPF_CUDA(cudaMemset(L.dirty, 0, sizeof(int32_t)));
@@ -114,7 +117,7 @@ int alloc_lane(lpf_ctx* c, LpfLane& L) {
 }
 
 void free_lane(LpfLane& L) {
-  void* ptrs[] = {L.qc_part1, L.qc_part2, L.sum_plane, L.dirty, L.F, L.C, L.S, L.Y, L.normp, L.M, L.tmp_pos, L.tmp_plane,
+  void* ptrs[] = {L.qc_part1, L.qc_part2, L.qc_band_clip, L.qc_counter, L.sum_plane, L.dirty, L.F, L.C, L.S, L.Y, L.normp, L.M, L.tmp_pos, L.tmp_plane,
                   L.tmp_snr, L.tmp_n, L.stats, L.band_ok, L.dets, L.ndets, L.upos, L.uplane, L.usnr, L.nu,
                   L.cand_idx, L.act_slots, L.act_pix, L.npos, L.flux, L.cube};
   for (void* q : ptrs) if (q) cudaFree(q);
@@ -126,11 +129,11 @@ void free_lane(LpfLane& L) {
 
 // S3-S8 dispatch: the fused sweep kernel when the parameter set allows it, else the general path.
 int lpf_launch_detect(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, lpf_det* d_dets,
-                      int32_t* d_ndets, cudaStream_t st) {
+                      int32_t* d_ndets, bool sum_done, cudaStream_t st) {
   // the fused kernel fetches rows with 16-byte bulk copies: a misaligned cube takes the general path
   if (c->fused && (((uintptr_t)d_cube) & 15) == 0)
-    return lpf_launch_detect_fused(c, c->fused, L, d_cube, d_band_ok, d_dets, d_ndets, st);
-  return lpf_launch_detect_general(c, L, d_cube, d_band_ok, d_dets, d_ndets, st);
+    return lpf_launch_detect_fused(c, c->fused, L, d_cube, d_band_ok, d_dets, d_ndets, sum_done, st);
+  return lpf_launch_detect_general(c, L, d_cube, d_band_ok, d_dets, d_ndets, sum_done, st);
 }
 
 namespace {
@@ -241,7 +244,7 @@ int lpf_detect_sources(lpf_ctx* c, int lane, const float* d_cube, const uint8_t*
   if (!d_cube || !d_band_ok || !d_dets || !d_ndets || !d_upos || !d_uplane || !d_usnr || !d_nu) return LPF_E_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   LpfLane& L = c->lanes[lane];
-  TRY(lpf_launch_detect(c, L, d_cube, d_band_ok, d_dets, d_ndets, st));
+  TRY(lpf_launch_detect(c, L, d_cube, d_band_ok, d_dets, d_ndets, false, st));
   return lpf_launch_dedupe(c, L, d_dets, d_ndets, d_upos, d_uplane, d_usnr, d_nu, st);
 }
 
@@ -282,8 +285,8 @@ int lpf_process_frame(lpf_ctx* c, int lane, const float* d_cube, int64_t t, void
   if (!d_cube || t < 0) return LPF_E_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   LpfLane& L = c->lanes[lane];
-  TRY(lpf_launch_qc(c, L, d_cube, L.stats, L.band_ok, st));
-  TRY(lpf_launch_detect(c, L, d_cube, L.band_ok, L.dets, L.ndets, st));
+  TRY(lpf_launch_qc_sum(c, L, d_cube, L.stats, L.band_ok, L.ndets, st));      // S1-S3, one kernel per pass over the cube
+  TRY(lpf_launch_detect(c, L, d_cube, L.band_ok, L.dets, L.ndets, true, st));
   TRY(lpf_launch_dedupe(c, L, L.dets, L.ndets, L.upos, L.uplane, L.usnr, L.nu, st));
   // the candidate table and the rings are shared by all lanes: order the chain across streams
   if (c->chain_valid) LPF_CUDA(cudaStreamWaitEvent(st, c->chain_ev, 0));

@@ -17,7 +17,9 @@ struct LpfTaps {
 // Scratch and owned outputs of one frame in flight.
 struct LpfLane {
   double* qc_part1 = nullptr;  // [B][nblk][3]  n, sum(x-p), sum(x-p)^2
-  double* qc_part2 = nullptr;  // [B][nblk][3]  clipped
+  double* qc_part2 = nullptr;  // [blocks of pass 2][B][3]  clipped
+  float* qc_band_clip = nullptr;   // [B][2] centre, half width of the clip round
+  int32_t* qc_counter = nullptr;   // [2] last-block counters of the two passes
   float* sum_plane = nullptr;  // [N]
   int32_t* dirty = nullptr;    // [1] == dirty_seq: the cube of the current frame needs masking (detect_general.cu k_sum_plane)
   int32_t dirty_seq = 0;
@@ -119,17 +121,20 @@ void lpf_prof_post(lpf_ctx* c, cudaStream_t st);
 
 // ---- launchers implemented in the kernel translation units ---------------------------------
 int lpf_launch_qc(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, cudaStream_t st);
+int lpf_launch_qc_sum(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, int32_t* zero_me,
+                      cudaStream_t st);
+int lpf_qc2_blocks(const lpf_ctx* c);
 
 int lpf_launch_sum_plane(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, bool want_sum, cudaStream_t st);
 int lpf_launch_detect_general(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok,
-                              lpf_det* d_dets, int32_t* d_ndets, cudaStream_t st);
+                              lpf_det* d_dets, int32_t* d_ndets, bool sum_done, cudaStream_t st);
 int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out);
 void lpf_fused_plan_free(LpfFusedPlan* pl);
 int lpf_fused_plan_info(const LpfFusedPlan* pl, int* cw, int* threads, int* n_items, long long* smem);
 int lpf_launch_detect_fused(lpf_ctx* c, LpfFusedPlan* pl, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok,
-                            lpf_det* d_dets, int32_t* d_ndets, cudaStream_t st);
+                            lpf_det* d_dets, int32_t* d_ndets, bool sum_done, cudaStream_t st);
 int lpf_launch_detect(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, lpf_det* d_dets,
-                      int32_t* d_ndets, cudaStream_t st);
+                      int32_t* d_ndets, bool sum_done, cudaStream_t st);
 int lpf_launch_static_norm(lpf_ctx* c, const LpfTaps& g, float* d_norm, float* d_tmp, cudaStream_t st);
 
 int lpf_launch_dedupe(lpf_ctx* c, LpfLane& L, const lpf_det* d_dets, const int32_t* d_ndets, int32_t* d_upos,

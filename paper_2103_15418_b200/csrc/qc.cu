@@ -1,17 +1,24 @@
-// S1 + S2: quality control (App. A, eq. A.1; O1, O2).
+// S1 + S2 (+ S3): quality control (App. A, eq. A.1; O1, O2) and the sum plane.
 //
-// Pass 1 streams the cube once with 128-bit loads and accumulates, per band over valid
-// pixels, n, sum(x - p) and sum(x - p)^2 about a per-band pivot p (the band's first valid
-// pixel): fp32 over runs of <= 16 values, float64 across runs, warp-shuffle + shared-memory
-// block reduction, one partial per block.  Pass 2 (the cube is L2-resident by then) does the
-// same for the pixels inside the one qc_clip-sigma clip round, about the band mean.  The
-// verdict kernel finishes the moments and evaluates eq. A.1 across bands (median, MAD, SE
-// floor) for the mean vector and the rms vector.
+// Pass 1 streams the cube once with 128-bit loads and accumulates, per band over valid pixels, n,
+// sum(x - p) and sum(x - p)^2 about a per-band pivot p (the band's first valid pixel): fp32 over
+// runs of <= 16 values, float64 across runs, warp-shuffle + shared-memory block reduction, one
+// partial per block.  The LAST block to finish (a device-wide counter) finishes the moments and
+// evaluates eq. A.1 across bands (median, MAD, SE floor) for the mean vector and the rms vector:
+// band_ok, frame_ok, and the centre / half width of the clip round.
+// Pass 2 reads the cube a second time, all bands of a pixel group together, and does up to three
+// things with that one read: the moments of the pixels inside the one qc_clip-sigma clip round
+// (O1), the sum plane X_B = sum of the accepted bands (O4, S3) and the check that every invalid
+// pixel of the accepted bands holds an exact zero (then W X = X and the fused detection kernel
+// reads the cube unmasked).  Its last block finishes the clipped moments.
 #include "lpf_internal.cuh"
 
 namespace {
 
 constexpr int QC_THREADS = 256;
+constexpr int QC_WARPS = QC_THREADS / 32;
+constexpr int QC2_THREADS = 128;   // pass 2: 4 pixel groups per thread and band in flight
+constexpr int QC2_WARPS = QC2_THREADS / 32;
 
 __device__ __forceinline__ void block_reduce3(double& a, double& b, double& c, double* sm /*[3][8]*/) {
   a = lpf_warp_sum(a); b = lpf_warp_sum(b); c = lpf_warp_sum(c);
@@ -20,124 +27,71 @@ __device__ __forceinline__ void block_reduce3(double& a, double& b, double& c, d
   if (l == 0) { sm[w] = a; sm[8 + w] = b; sm[16 + w] = c; }
   __syncthreads();
   if (w == 0) {
-    a = l < (QC_THREADS / 32) ? sm[l] : 0.0;
-    b = l < (QC_THREADS / 32) ? sm[8 + l] : 0.0;
-    c = l < (QC_THREADS / 32) ? sm[16 + l] : 0.0;
+    a = l < QC_WARPS ? sm[l] : 0.0;
+    b = l < QC_WARPS ? sm[8 + l] : 0.0;
+    c = l < QC_WARPS ? sm[16 + l] : 0.0;
     a = lpf_warp_sum(a); b = lpf_warp_sum(b); c = lpf_warp_sum(c);
   }
 }
 
-// CLIP = false: all valid pixels, about pivot.  CLIP = true: |x - mean| <= thr, about mean.
-template <bool CLIP>
-__global__ void __launch_bounds__(QC_THREADS)
-k_qc_moments(const float* __restrict__ cube, const uint8_t* __restrict__ W, long long N, int first_valid,
-             int nblk, const double* __restrict__ part1, float qc_clip, double* __restrict__ part_out) {
-  __shared__ double sm[24];
-  __shared__ float s_piv, s_thr;
-  const int b = blockIdx.y;
-  const float* X = cube + (long long)b * N;
-  if (!CLIP) {
-    if (threadIdx.x == 0) { s_piv = X[first_valid]; s_thr = 0.f; }
-  } else {
-    // finish pass 1 for this band: mean and rms (every block redoes this tiny reduction)
-    double n = 0, s1 = 0, s2 = 0;
-    for (int i = threadIdx.x; i < nblk; i += QC_THREADS) {
-      const double* q = part1 + ((long long)b * nblk + i) * 3;
-      n += q[0]; s1 += q[1]; s2 += q[2];
-    }
-    block_reduce3(n, s1, s2, sm);
-    if (threadIdx.x == 0) {
-      const double piv = (double)X[first_valid];
-      double mean = 0, rms = 0;
-      if (n > 0) { const double m1 = s1 / n; mean = piv + m1; double var = s2 / n - m1 * m1; rms = sqrt(var > 0 ? var : 0.0); }
-      s_piv = (float)mean;
-      s_thr = (float)((double)qc_clip * rms);
-    }
+// true in exactly one block of the grid: the last one to get here.  The counter is left at zero.
+__device__ __forceinline__ bool last_block_done(int32_t* counter, int total) {
+  __shared__ int s_last;
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const int prev = atomicAdd(counter, 1);
+    s_last = (prev == total - 1) ? 1 : 0;
+    if (s_last) *counter = 0;
   }
   __syncthreads();
-  const float piv = s_piv, thr = s_thr;
-
-  // contiguous chunk of this band for this block, in units of 4 pixels
-  const long long n4 = (N + 3) >> 2;
-  const long long per = (n4 + nblk - 1) / nblk;
-  const long long q0 = (long long)blockIdx.x * per;
-  const long long q1 = (q0 + per < n4) ? q0 + per : n4;
-  const bool vec = ((N & 3) == 0) && ((((uintptr_t)cube) & 15) == 0);
-
-  double dn = 0, d1 = 0, d2 = 0;
-  float fn = 0, f1 = 0, f2 = 0;
-  int run = 0;
-  for (long long q = q0 + threadIdx.x; q < q1; q += QC_THREADS) {
-    float v[4]; unsigned wm;
-    const long long i0 = q << 2;
-    if (vec) {
-      const float4 x = __ldg(reinterpret_cast<const float4*>(X) + q);
-      v[0] = x.x; v[1] = x.y; v[2] = x.z; v[3] = x.w;
-      wm = __ldg(reinterpret_cast<const unsigned*>(W) + q);
-    } else {
-      wm = 0;
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const bool in = (i0 + j) < N;
-        v[j] = in ? X[i0 + j] : 0.f;
-        if (in && W[i0 + j]) wm |= (1u << (8 * j));
-      }
-    }
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const float d = v[j] - piv;
-      bool take = ((wm >> (8 * j)) & 0xffu) != 0;
-      if (CLIP) take = take && (fabsf(d) <= thr);
-      if (take) { fn += 1.f; f1 += d; f2 = fmaf(d, d, f2); }
-    }
-    if (++run == 4) { dn += fn; d1 += f1; d2 += f2; fn = f1 = f2 = 0.f; run = 0; }
-  }
-  dn += fn; d1 += f1; d2 += f2;
-  block_reduce3(dn, d1, d2, sm);
-  if (threadIdx.x == 0) {
-    double* o = part_out + ((long long)b * nblk + blockIdx.x) * 3;
-    o[0] = dn; o[1] = d1; o[2] = d2;
-  }
+  if (s_last) __threadfence();
+  return s_last != 0;
 }
 
-// One block of 64 threads: thread b owns band b.
-__global__ void __launch_bounds__(64)
-k_qc_verdict(const float* __restrict__ cube, long long N, int first_valid, int B, int nblk,
-             const double* __restrict__ part1, const double* __restrict__ part2, float tau,
-             float* __restrict__ stats, uint8_t* __restrict__ band_ok) {
-  __shared__ double s_mean[64], s_rms[64], s_sorted[64], s_dev[64];
-  __shared__ int s_fin[64];
+struct QcArgs {
+  const float* cube; const uint8_t* W; long long N; int first_valid, B, nblk;
+  double* part1;          // [B][nblk][3]
+  float qc_clip, tau;
+  float* stats;           // [B][8]
+  uint8_t* band_ok;       // [B + 1]
+  float* band_clip;       // [B][2] centre and half width of the clip round
+  int32_t* counter;
+};
+
+// eq. A.1 for all bands, by one block of QC_THREADS threads.
+__device__ void qc_verdict(const QcArgs& a) {
+  __shared__ double s_mean[LPF_MAX_BANDS], s_rms[LPF_MAX_BANDS], s_n[LPF_MAX_BANDS], s_sorted[LPF_MAX_BANDS], s_dev[LPF_MAX_BANDS];
+  __shared__ int s_fin[LPF_MAX_BANDS];
   __shared__ int s_nfin, s_nok;
-  const int b = threadIdx.x;
-  double n = 0, mean = 0, rms = 0, nc = 0, cmean = 0, crms = 0;
-  int fin = 0;
-  if (b < B) {
-    double s1 = 0, s2 = 0, c1 = 0, c2 = 0;
-    for (int i = 0; i < nblk; ++i) {
-      const double* q = part1 + ((long long)b * nblk + i) * 3;
-      n += q[0]; s1 += q[1]; s2 += q[2];
-      const double* r = part2 + ((long long)b * nblk + i) * 3;
-      nc += r[0]; c1 += r[1]; c2 += r[2];
+  const int B = a.B, nblk = a.nblk;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  // finish pass 1: warp w takes bands w, w + 8, ...; lanes share the partials of a band
+  for (int b = warp; b < B; b += QC_WARPS) {
+    double n = 0, s1 = 0, s2 = 0;
+    for (int i = lane; i < nblk; i += 32) {
+      const double* q = a.part1 + ((long long)b * nblk + i) * 3;
+      n += __ldcg(q); s1 += __ldcg(q + 1); s2 += __ldcg(q + 2);
     }
-    if (n > 0) {
-      const double piv = (double)cube[(long long)b * N + first_valid];
-      const double m1 = s1 / n;
-      mean = piv + m1;
-      const double var = s2 / n - m1 * m1;
-      rms = sqrt(var > 0 ? var : 0.0);
-      if (nc > 0) {
-        const double meanf = (double)(float)mean;  // pass 2 centred on the fp32 mean
-        const double k1 = c1 / nc;
-        cmean = meanf + k1;
-        const double cv = c2 / nc - k1 * k1;
-        crms = sqrt(cv > 0 ? cv : 0.0);
+    n = lpf_warp_sum(n); s1 = lpf_warp_sum(s1); s2 = lpf_warp_sum(s2);
+    if (lane == 0) {
+      double mean = 0, rms = 0;
+      if (n > 0) {
+        const double piv = (double)a.cube[(long long)b * a.N + a.first_valid];
+        const double m1 = s1 / n;
+        mean = piv + m1;
+        const double var = s2 / n - m1 * m1;
+        rms = sqrt(var > 0 ? var : 0.0);
       }
+      s_mean[b] = mean; s_rms[b] = rms; s_n[b] = n;
+      s_fin[b] = (n > 0 && isfinite(mean) && isfinite(rms)) ? 1 : 0;
     }
-    fin = (n > 0 && isfinite(mean) && isfinite(rms)) ? 1 : 0;
-    s_mean[b] = mean; s_rms[b] = rms; s_fin[b] = fin;
   }
   if (threadIdx.x == 0) { s_nfin = 0; s_nok = 0; }
   __syncthreads();
+  const int b = threadIdx.x;
+  const double n = b < B ? s_n[b] : 0.0, mean = b < B ? s_mean[b] : 0.0, rms = b < B ? s_rms[b] : 0.0;
+  const int fin = b < B ? s_fin[b] : 0;
   if (b < B && fin) atomicAdd(&s_nfin, 1);
   __syncthreads();
   const int m = s_nfin;
@@ -158,6 +112,7 @@ k_qc_verdict(const float* __restrict__ cube, long long N, int first_valid, int B
   };
   const double med_m = median_of(s_mean, mean);
   const double med_r = median_of(s_rms, rms);
+  __syncthreads();
   if (b < B) s_dev[b] = fabs(mean - med_m);
   const double mad_m = median_of(s_dev, fabs(mean - med_m));
   __syncthreads();
@@ -172,28 +127,286 @@ k_qc_verdict(const float* __restrict__ cube, long long N, int first_valid, int B
     const double num_m = mean - med_m, num_r = rms - med_r;
     zm = den_m > 0 ? num_m / den_m : (num_m == 0 ? 0.0 : (num_m > 0 ? INFINITY : -INFINITY));
     zr = den_r > 0 ? num_r / den_r : (num_r == 0 ? 0.0 : (num_r > 0 ? INFINITY : -INFINITY));
-    ok = (fabs(zm) <= (double)tau && fabs(zr) <= (double)tau) ? 1 : 0;
+    ok = (fabs(zm) <= (double)a.tau && fabs(zr) <= (double)a.tau) ? 1 : 0;
     if (ok) atomicAdd(&s_nok, 1);
   }
   __syncthreads();
   if (b < B) {
-    float* o = stats + LPF_STATS_PER_BAND * b;
-    o[0] = (float)n; o[1] = (float)mean; o[2] = (float)rms; o[3] = (float)nc; o[4] = (float)cmean; o[5] = (float)crms;
+    float* o = a.stats + LPF_STATS_PER_BAND * b;
+    o[0] = (float)n; o[1] = (float)mean; o[2] = (float)rms; o[3] = 0.f; o[4] = 0.f; o[5] = 0.f;
     o[6] = (float)zm; o[7] = (float)zr;
-    band_ok[b] = (uint8_t)ok;
+    a.band_ok[b] = (uint8_t)ok;
+    a.band_clip[2 * b] = (float)mean;                          // the clip round is decided in float32 (R25)
+    a.band_clip[2 * b + 1] = (float)((double)a.qc_clip * rms);
   }
-  if (threadIdx.x == 0) band_ok[B] = (s_nok >= (B + 1) / 2) ? 1 : 0;
+  if (threadIdx.x == 0) a.band_ok[B] = (s_nok >= (B + 1) / 2) ? 1 : 0;
+}
+
+__global__ void __launch_bounds__(QC_THREADS)
+k_qc_pass1(const QcArgs a) {
+  __shared__ double sm[24];
+  const int b = blockIdx.y, nblk = a.nblk;
+  const long long N = a.N;
+  const float* X = a.cube + (long long)b * N;
+  const float piv = X[a.first_valid];
+
+  // contiguous chunk of this band for this block, in units of 4 pixels
+  const long long n4 = (N + 3) >> 2;
+  const long long per = (n4 + nblk - 1) / nblk;
+  const long long q0 = (long long)blockIdx.x * per;
+  const long long q1 = (q0 + per < n4) ? q0 + per : n4;
+  const bool vec = ((N & 3) == 0) && ((((uintptr_t)a.cube) & 15) == 0);
+
+  double dn = 0, d1 = 0, d2 = 0;
+  if (vec) {
+    // four 128-bit loads (and their mask words) in flight per thread; fp32 over those 16 values, float64 across
+    for (long long q = q0 + threadIdx.x; q < q1; q += 4 * QC_THREADS) {
+      float4 x[4]; unsigned wm[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const long long qq = q + k * QC_THREADS;
+        const bool in = qq < q1;
+        x[k] = in ? __ldg(reinterpret_cast<const float4*>(X) + qq) : make_float4(0.f, 0.f, 0.f, 0.f);
+        wm[k] = in ? __ldg(reinterpret_cast<const unsigned*>(a.W) + qq) : 0u;
+      }
+      float fn = 0.f, f1 = 0.f, f2 = 0.f;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const float v[4] = {x[k].x, x[k].y, x[k].z, x[k].w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const float d = v[j] - piv;
+          if (((wm[k] >> (8 * j)) & 0xffu) != 0) { fn += 1.f; f1 += d; f2 = fmaf(d, d, f2); }
+        }
+      }
+      dn += fn; d1 += f1; d2 += f2;
+    }
+  } else {
+    float fn = 0.f, f1 = 0.f, f2 = 0.f;
+    int run = 0;
+    for (long long q = q0 + threadIdx.x; q < q1; q += QC_THREADS) {
+      const long long i0 = q << 2;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        if ((i0 + j) < N && a.W[i0 + j]) { const float d = X[i0 + j] - piv; fn += 1.f; f1 += d; f2 = fmaf(d, d, f2); }
+      }
+      if (++run == 4) { dn += fn; d1 += f1; d2 += f2; fn = f1 = f2 = 0.f; run = 0; }
+    }
+    dn += fn; d1 += f1; d2 += f2;
+  }
+  block_reduce3(dn, d1, d2, sm);
+  if (threadIdx.x == 0) {
+    double* o = a.part1 + ((long long)b * nblk + blockIdx.x) * 3;
+    o[0] = dn; o[1] = d1; o[2] = d2;
+  }
+  if (last_block_done(a.counter, gridDim.x * gridDim.y)) qc_verdict(a);
+}
+
+struct Qc2Args {
+  const float* cube; const uint8_t* W; const uint8_t* band_ok; long long N; int B;
+  const float* band_clip;  // [B][2]
+  double* part2;           // [gridDim.x][B][3]
+  float* stats;            // [B][8]: columns 3..5 are written here
+  float* sum_out;          // [N] or null
+  int32_t* dirty; int seq;
+  int32_t* zero_me;        // a counter this kernel resets (the record count of the frame), or null
+  int32_t* counter;
+};
+
+// CLIP: the clipped moments of every band; SUM: the sum plane of the accepted bands + the exact-zero check.
+template <bool CLIP, bool SUM>
+__global__ void __launch_bounds__(QC2_THREADS)
+k_qc_pass2(const Qc2Args a) {
+  __shared__ double s_acc[QC2_WARPS][LPF_MAX_BANDS][3];
+  __shared__ float s_clip[LPF_MAX_BANDS][2];
+  __shared__ uint8_t s_ok[LPF_MAX_BANDS + 1];
+  const int B = a.B, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long N = a.N;
+  for (int i = threadIdx.x; i < B; i += QC2_THREADS) {
+    if (CLIP) { s_clip[i][0] = a.band_clip[2 * i]; s_clip[i][1] = a.band_clip[2 * i + 1]; }
+    s_ok[i] = a.band_ok[i];
+  }
+  if (threadIdx.x == 0) s_ok[B] = a.band_ok[B];
+  if (CLIP)
+    for (int i = threadIdx.x; i < QC2_WARPS * LPF_MAX_BANDS * 3; i += QC2_THREADS) (&s_acc[0][0][0])[i] = 0.0;
+  if (a.zero_me && blockIdx.x == 0 && threadIdx.x == 0) *a.zero_me = 0;
+  __syncthreads();
+  const bool do_sum = SUM && s_ok[B] != 0;      // a rejected frame has no sum plane (and no detections)
+  const bool vec = ((N & 3) == 0) && ((((uintptr_t)a.cube) & 15) == 0);
+  bool bad = false;
+  if (vec) {
+    // a thread owns 4 pixel groups (16 pixels), QC2_THREADS groups apart, for all bands
+    const long long n4 = N >> 2;
+    const long long chunk = 4LL * QC2_THREADS;
+    for (long long c0 = (long long)blockIdx.x * chunk; c0 < n4; c0 += (long long)gridDim.x * chunk) {
+      long long q[4]; unsigned wm[4]; bool in[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        q[k] = c0 + k * QC2_THREADS + threadIdx.x;
+        in[k] = q[k] < n4;
+        wm[k] = in[k] ? __ldg(reinterpret_cast<const unsigned*>(a.W) + q[k]) : 0u;
+      }
+      float4 s[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) s[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+      // the loads of the next needed band are issued before the current band is consumed
+      auto needed = [&](int b) { return CLIP || (do_sum && s_ok[b] != 0); };
+      auto fetch = [&](int b, float4 (&x)[4]) {
+        const float4* Xb = reinterpret_cast<const float4*>(a.cube + (long long)b * N);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) x[k] = in[k] ? __ldg(Xb + q[k]) : make_float4(0.f, 0.f, 0.f, 0.f);
+      };
+      int bn = 0;
+      while (bn < B && !needed(bn)) ++bn;
+      float4 xn[4];
+      if (bn < B) fetch(bn, xn);
+      while (bn < B) {
+        const int b = bn;
+        const bool okb = s_ok[b] != 0;
+        float4 x[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) x[k] = xn[k];
+        ++bn;
+        while (bn < B && !needed(bn)) ++bn;
+        if (bn < B) fetch(bn, xn);
+        if (SUM && do_sum && okb) {
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            s[k].x += x[k].x; s[k].y += x[k].y; s[k].z += x[k].z; s[k].w += x[k].w;
+            bad = bad || (!(wm[k] & 0x000000ffu) && x[k].x != 0.f) || (!(wm[k] & 0x0000ff00u) && x[k].y != 0.f) ||
+                  (!(wm[k] & 0x00ff0000u) && x[k].z != 0.f) || (!(wm[k] & 0xff000000u) && x[k].w != 0.f);
+          }
+        }
+        if (CLIP) {
+          const float mean = s_clip[b][0], thr = s_clip[b][1];
+          float fn = 0.f, f1 = 0.f, f2 = 0.f;
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const float v[4] = {x[k].x, x[k].y, x[k].z, x[k].w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const float d = v[j] - mean;
+              if (((wm[k] >> (8 * j)) & 0xffu) != 0 && fabsf(d) <= thr) { fn += 1.f; f1 += d; f2 = fmaf(d, d, f2); }
+            }
+          }
+          fn = lpf_warp_sum(fn); f1 = lpf_warp_sum(f1); f2 = lpf_warp_sum(f2);   // 512 values in fp32, float64 from here on
+          if (lane == 0) { s_acc[warp][b][0] += (double)fn; s_acc[warp][b][1] += (double)f1; s_acc[warp][b][2] += (double)f2; }
+        }
+      }
+      if (SUM && do_sum && a.sum_out) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+          if (in[k]) reinterpret_cast<float4*>(a.sum_out)[q[k]] = s[k];
+      }
+    }
+  } else {
+    for (long long i0 = (long long)blockIdx.x * QC2_THREADS; i0 < N; i0 += (long long)gridDim.x * QC2_THREADS) {
+      const long long i = i0 + threadIdx.x;
+      const bool in = i < N;
+      const bool valid = in && a.W[i] != 0;
+      float s = 0.f;
+      for (int b = 0; b < B; ++b) {
+        const bool okb = s_ok[b] != 0;
+        if (!CLIP && !(do_sum && okb)) continue;
+        const float x = in ? a.cube[(long long)b * N + i] : 0.f;
+        if (SUM && do_sum && okb) { s += x; bad = bad || (in && !valid && x != 0.f); }
+        if (CLIP) {
+          const float d = x - s_clip[b][0];
+          const bool take = valid && fabsf(d) <= s_clip[b][1];
+          float fn = take ? 1.f : 0.f, f1 = take ? d : 0.f, f2 = take ? d * d : 0.f;
+          fn = lpf_warp_sum(fn); f1 = lpf_warp_sum(f1); f2 = lpf_warp_sum(f2);
+          if (lane == 0) { s_acc[warp][b][0] += (double)fn; s_acc[warp][b][1] += (double)f1; s_acc[warp][b][2] += (double)f2; }
+        }
+      }
+      if (SUM && do_sum && a.sum_out && in) a.sum_out[i] = s;
+    }
+  }
+  if (SUM && bad) *a.dirty = a.seq;
+  if (!CLIP) return;
+  __syncthreads();
+  for (int i = threadIdx.x; i < B * 3; i += QC2_THREADS) {
+    const int b = i / 3, k = i - 3 * b;
+    double t = 0;
+#pragma unroll
+    for (int w = 0; w < QC2_WARPS; ++w) t += s_acc[w][b][k];
+    a.part2[((long long)blockIdx.x * B + b) * 3 + k] = t;
+  }
+  if (!last_block_done(a.counter, gridDim.x)) return;
+  // the clipped moments: warp w takes bands w, w + 8, ...
+  for (int b = warp; b < B; b += QC2_WARPS) {
+    double nc = 0, c1 = 0, c2 = 0;
+    for (int i = lane; i < (int)gridDim.x; i += 32) {
+      const double* r = a.part2 + ((long long)i * B + b) * 3;
+      nc += __ldcg(r); c1 += __ldcg(r + 1); c2 += __ldcg(r + 2);
+    }
+    nc = lpf_warp_sum(nc); c1 = lpf_warp_sum(c1); c2 = lpf_warp_sum(c2);
+    if (lane == 0) {
+      double cmean = 0, crms = 0;
+      if (nc > 0) {
+        const double k1 = c1 / nc;
+        cmean = (double)s_clip[b][0] + k1;             // pass 2 is centred on the fp32 mean
+        const double cv = c2 / nc - k1 * k1;
+        crms = sqrt(cv > 0 ? cv : 0.0);
+      }
+      float* o = a.stats + LPF_STATS_PER_BAND * b;
+      o[3] = (float)nc; o[4] = (float)cmean; o[5] = (float)crms;
+    }
+  }
 }
 
 }  // namespace
 
-int lpf_launch_qc(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, cudaStream_t st) {
+static Qc2Args make_qc2(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, float* d_stats, bool want_sum,
+                        int32_t* zero_me) {
+  Qc2Args a{};
+  a.cube = d_cube; a.W = c->W; a.band_ok = d_band_ok; a.N = c->N; a.B = c->p.B;
+  a.band_clip = L.qc_band_clip; a.part2 = L.qc_part2; a.stats = d_stats;
+  a.sum_out = want_sum ? L.sum_plane : nullptr;
+  a.dirty = L.dirty; a.seq = L.dirty_seq; a.zero_me = zero_me; a.counter = L.qc_counter + 1;
+  return a;
+}
+
+static int qc_launch_pass1(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, cudaStream_t st) {
+  QcArgs a{};
+  a.cube = d_cube; a.W = c->W; a.N = c->N; a.first_valid = c->first_valid; a.B = c->p.B; a.nblk = c->qc_nblk;
+  a.part1 = L.qc_part1; a.qc_clip = c->p.qc_clip; a.tau = c->p.qc_tau; a.stats = d_stats; a.band_ok = d_band_ok;
+  a.band_clip = L.qc_band_clip; a.counter = L.qc_counter;
   const dim3 grid(c->qc_nblk, c->p.B);
-  LPF_KLAUNCH(c, KID_QC_PASS1, st, k_qc_moments<false><<<grid, QC_THREADS, 0, st>>>(
-      d_cube, c->W, c->N, c->first_valid, c->qc_nblk, nullptr, 0.f, L.qc_part1));
-  LPF_KLAUNCH(c, KID_QC_PASS2, st, k_qc_moments<true><<<grid, QC_THREADS, 0, st>>>(
-      d_cube, c->W, c->N, c->first_valid, c->qc_nblk, L.qc_part1, c->p.qc_clip, L.qc_part2));
-  LPF_KLAUNCH(c, KID_QC_VERDICT, st, k_qc_verdict<<<1, 64, 0, st>>>(
-      d_cube, c->N, c->first_valid, c->p.B, c->qc_nblk, L.qc_part1, L.qc_part2, c->p.qc_tau, d_stats, d_band_ok));
+  LPF_KLAUNCH(c, KID_QC_PASS1, st, k_qc_pass1<<<grid, QC_THREADS, 0, st>>>(a));
+  return LPF_OK;
+}
+
+int lpf_qc2_blocks(const lpf_ctx* c) {
+  const long long chunks = ((c->N + 3) / 4 + 4 * QC2_THREADS - 1) / (4 * QC2_THREADS);
+  const long long cap = (long long)c->n_sm * 8;
+  return (int)(chunks < 1 ? 1 : (chunks < cap ? chunks : cap));
+}
+
+// S1 + S2 as the C-ABI's lpf_cube_qc: statistics and verdict only.
+int lpf_launch_qc(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, cudaStream_t st) {
+  int rc = qc_launch_pass1(c, L, d_cube, d_stats, d_band_ok, st);
+  if (rc) return rc;
+  const Qc2Args a = make_qc2(c, L, d_cube, d_band_ok, d_stats, false, nullptr);
+  LPF_KLAUNCH(c, KID_QC_PASS2, st, k_qc_pass2<true, false><<<lpf_qc2_blocks(c), QC2_THREADS, 0, st>>>(a));
+  return LPF_OK;
+}
+
+// S1 + S2 + S3 for the chained frame call: the clip round, the sum plane and the exact-zero check share one
+// read of the cube; *zero_me (the frame's record counter) is reset on the way.
+int lpf_launch_qc_sum(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, int32_t* zero_me,
+                      cudaStream_t st) {
+  int rc = qc_launch_pass1(c, L, d_cube, d_stats, d_band_ok, st);
+  if (rc) return rc;
+  L.dirty_seq = L.dirty_seq >= 0x7ffffff0 ? 1 : L.dirty_seq + 1;
+  const Qc2Args a = make_qc2(c, L, d_cube, d_band_ok, d_stats, c->p.detect_sum_plane != 0, zero_me);
+  LPF_KLAUNCH(c, KID_QC_PASS2, st, k_qc_pass2<true, true><<<lpf_qc2_blocks(c), QC2_THREADS, 0, st>>>(a));
+  return LPF_OK;
+}
+
+// S3 alone (lpf_detect_sources): the sum plane of the accepted bands (want_sum) and the exact-zero check.
+int lpf_launch_sum_plane(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, bool want_sum, cudaStream_t st) {
+  L.dirty_seq = L.dirty_seq >= 0x7ffffff0 ? 1 : L.dirty_seq + 1;
+  const Qc2Args a = make_qc2(c, L, d_cube, d_band_ok, nullptr, want_sum, nullptr);
+  LPF_KLAUNCH(c, KID_SUM_PLANE, st, k_qc_pass2<false, true><<<lpf_qc2_blocks(c), QC2_THREADS, 0, st>>>(a));
   return LPF_OK;
 }

@@ -284,3 +284,67 @@ def test_host_entry_point(torch_cuda):
         assert np.array_equal(res.act_slots[:res.npos].numpy(), o["act_slots"])
         assert np.array_equal(res.flux[:res.npos].numpy(), o["flux"])
     lpf.close()
+
+
+def test_fused_kernel_special_paths(torch_cuda):
+    """The fused sweep's rare paths: (a) a cube that is not an exact zero at invalid pixels (the kernel then
+    applies W itself), (b) more eq.-5 hits in a row pair than the candidate queue holds (tested in place),
+    (c) a cube that is not 16-byte aligned (bulk copies impossible: the general path serves the call)."""
+    torch = torch_cuda
+    from paper_2103_15418_b200.binding import LPF
+    rng = np.random.default_rng(5)
+    B, D = 4, 256
+    p = synth.default_params(2); p.update(B=B, Dy=D, Dx=D)
+    yy, xx = np.mgrid[0:D, 0:D]
+    c = (D - 1) / 2
+    W = (((yy - c) ** 2 + (xx - c) ** 2) <= (0.45 * D) ** 2).astype(np.uint8)
+    W[100:104, 60:90] = 0                       # a hole as well
+    base = rng.standard_normal((B, D, D)).astype(np.float32)
+    for (y, x, a) in [(80, 70, 12.0), (128, 128, 30.0), (150, 200, 9.0), (101, 58, 15.0), (30, 128, 10.0)]:
+        g = np.exp(-0.5 * ((yy - y) ** 2 + (xx - x) ** 2) / 0.85 ** 2).astype(np.float32)
+        base += a * g
+    lpf = LPF(p, W)
+    assert lpf.plan()["fused"]
+    pipe = O.OraclePipeline(p, W, direct=False)
+    # (a) garbage (also non-finite) at the invalid pixels of some frames; clean frames in between
+    for t in range(4):
+        cube = base + 0.1 * rng.standard_normal(base.shape).astype(np.float32)
+        if t in (1, 3):
+            junk = (50.0 * rng.standard_normal(base.shape)).astype(np.float32)
+            cube = np.where(W[None] != 0, cube, junk)
+            cube[0, 0, 0] = np.nan; cube[2, 101, 70] = np.inf
+        else:
+            cube = cube * W
+        o = pipe.step(cube, t)
+        lpf.process_frame(torch.from_numpy(cube).cuda(), t)
+        gv = lpf.frame_view(0)
+        r = parity.check_frame(gv, o, pipe, cube, f"dirty t={t}")
+        assert r["in_sync"] and gv["band_ok"].all() and gv["upos"].size >= 4
+    lpf.close()
+    # (b) kappa = 1: about 80 noise pixels pass eq. 5 in every row pair of a strip (the queue holds 64), plus rows of
+    # bright sources
+    p2 = dict(p); p2["max_det"] = 65536; p2["kappa"] = 1.0
+    W1 = np.ones((D, D), np.uint8)
+    cube = rng.standard_normal((B, D, D)).astype(np.float32)
+    for y in (60, 61, 130, 200):
+        for x in range(8, D - 8, 5):
+            g = np.exp(-0.5 * ((yy - y) ** 2 + (xx - x) ** 2) / 0.85 ** 2).astype(np.float32)
+            cube += (40.0 + (x % 7)) * g
+    lpf = LPF(p2, W1)
+    pipe = O.OraclePipeline(p2, W1, direct=False)
+    o = pipe.step(cube, 0)
+    lpf.process_frame(torch.from_numpy(cube).cuda(), 0)
+    gv = lpf.frame_view(0)
+    assert parity.check_frame(gv, o, pipe, cube, "queue overflow")["in_sync"]
+    assert gv["ndets"] > 2000 and lpf.counters()["dropped_records"] == 0
+    # (c) the same frame from a pointer that is only 4-byte aligned
+    big = torch.empty(cube.size + 1, dtype=torch.float32, device="cuda")
+    mis = big[1:].view(B, D, D)
+    mis.copy_(torch.from_numpy(cube))
+    assert mis.data_ptr() % 16 != 0
+    pipe2 = O.OraclePipeline(p2, W1, direct=False)
+    o2 = pipe2.step(cube, 0)
+    lpf2 = LPF(p2, W1)
+    lpf2.process_frame(mis, 0)
+    assert parity.check_frame(lpf2.frame_view(0), o2, pipe2, cube, "misaligned cube")["in_sync"]
+    lpf.close(); lpf2.close()
