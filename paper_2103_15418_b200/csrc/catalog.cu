@@ -7,6 +7,7 @@
 namespace {
 
 constexpr int CAT_BLOCKS = 64, CAT_THREADS = 256;
+constexpr int SORT_CAP = 8192;      // unique positions ranked from shared memory (more: from global memory)
 
 // key: larger snr wins, equal snr -> lower plane wins.  snr > 0 so its bit pattern is monotone.
 __device__ __forceinline__ unsigned long long dd_key(float snr, int plane) {
@@ -34,17 +35,38 @@ k_dedupe_select(const lpf_det* __restrict__ dets, const int32_t* __restrict__ nd
     if (M[d.pix] != key) continue;  // not the best plane at this pixel
     const int y = d.pix / Dx, x = d.pix - y * Dx;
     bool keep = true;
-    for (int j = -r; j <= r && keep; ++j) {
-      const int yy = y + j;
-      if (yy < 0 || yy >= Dy) continue;
-      for (int k = -r; k <= r; ++k) {
-        const int xx = x + k;
-        if (xx < 0 || xx >= Dx || (j == 0 && k == 0) || j * j + k * k > r * r) continue;
-        const int q = yy * Dx + xx;
-        const unsigned long long kq = M[q];
-        if (!kq) continue;
-        const unsigned sq = (unsigned)(kq >> 32), si = (unsigned)(key >> 32);
-        if (sq > si || (sq == si && q < d.pix)) { keep = false; break; }
+    const unsigned si = (unsigned)(key >> 32);
+    if (r <= 2) {                       // the usual radius: the 5x5 loads are independent and leave together
+      unsigned long long kq[25];
+#pragma unroll
+      for (int j = -2; j <= 2; ++j)
+#pragma unroll
+        for (int k = -2; k <= 2; ++k) {
+          const int yy = y + j, xx = x + k;
+          const bool in = yy >= 0 && yy < Dy && xx >= 0 && xx < Dx && !(j == 0 && k == 0) && j * j + k * k <= r * r;
+          kq[(j + 2) * 5 + k + 2] = in ? M[yy * Dx + xx] : 0ull;
+        }
+#pragma unroll
+      for (int j = -2; j <= 2; ++j)
+#pragma unroll
+        for (int k = -2; k <= 2; ++k) {
+          const unsigned long long v = kq[(j + 2) * 5 + k + 2];
+          const unsigned sq = (unsigned)(v >> 32);
+          if (v && (sq > si || (sq == si && (y + j) * Dx + x + k < d.pix))) keep = false;
+        }
+    } else {
+      for (int j = -r; j <= r && keep; ++j) {
+        const int yy = y + j;
+        if (yy < 0 || yy >= Dy) continue;
+        for (int k = -r; k <= r; ++k) {
+          const int xx = x + k;
+          if (xx < 0 || xx >= Dx || (j == 0 && k == 0) || j * j + k * k > r * r) continue;
+          const int q = yy * Dx + xx;
+          const unsigned long long kq = M[q];
+          if (!kq) continue;
+          const unsigned sq = (unsigned)(kq >> 32);
+          if (sq > si || (sq == si && q < d.pix)) { keep = false; break; }
+        }
       }
     }
     if (keep) {
@@ -61,12 +83,27 @@ k_dedupe_sort(const lpf_det* __restrict__ dets, const int32_t* __restrict__ ndet
               const int16_t* __restrict__ tmp_plane, const float* __restrict__ tmp_snr,
               const int32_t* __restrict__ tmp_n, int32_t* __restrict__ upos, int16_t* __restrict__ uplane,
               float* __restrict__ usnr, int32_t* __restrict__ nu) {
+  __shared__ int s_pos[SORT_CAP];
   const int n = min(*ndets, max_det);
   const int m = *tmp_n;
+  const bool staged = m <= SORT_CAP;
+  if (staged) {
+    for (int j = threadIdx.x; j < m; j += blockDim.x) s_pos[j] = tmp_pos[j];
+    for (int j = m + threadIdx.x; j < ((m + 3) & ~3); j += blockDim.x) s_pos[j] = 0x7fffffff;
+    __syncthreads();
+  }
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < m; i += gridDim.x * blockDim.x) {
     const int mine = tmp_pos[i];
     int rank = 0;
-    for (int j = 0; j < m; ++j) rank += (tmp_pos[j] < mine);
+    if (staged) {
+      const int4* p4 = reinterpret_cast<const int4*>(s_pos);
+      for (int j = 0; j < (m + 3) / 4; ++j) {
+        const int4 v = p4[j];
+        rank += (v.x < mine) + (v.y < mine) + (v.z < mine) + (v.w < mine);
+      }
+    } else {
+      for (int j = 0; j < m; ++j) rank += (tmp_pos[j] < mine);
+    }
     upos[rank] = mine; uplane[rank] = tmp_plane[i]; usnr[rank] = tmp_snr[i];
   }
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) M[dets[i].pix] = 0ull;
@@ -86,6 +123,24 @@ k_assoc_match(const int32_t* __restrict__ upos, const int32_t* __restrict__ nu, 
       const int pix = upos[i];
       const int y = pix / Dx, x = pix - y * Dx;
       int best_d = 0x7fffffff;
+      if (r <= 3) {
+        int sl[49];
+#pragma unroll
+        for (int j = -3; j <= 3; ++j)
+#pragma unroll
+          for (int k = -3; k <= 3; ++k) {
+            const int yy = y + j, xx = x + k;
+            const bool in = yy >= 0 && yy < Dy && xx >= 0 && xx < Dx && j * j + k * k <= r * r;
+            sl[(j + 3) * 7 + k + 3] = in ? slotmap[yy * Dx + xx] : -1;
+          }
+#pragma unroll
+        for (int j = -3; j <= 3; ++j)
+#pragma unroll
+          for (int k = -3; k <= 3; ++k) {
+            const int s = sl[(j + 3) * 7 + k + 3], d2 = j * j + k * k;
+            if (s >= 0 && (d2 < best_d || (d2 == best_d && s < best))) { best_d = d2; best = s; }
+          }
+      } else
       for (int j = -r; j <= r; ++j) {
         const int yy = y + j;
         if (yy < 0 || yy >= Dy) continue;
@@ -134,7 +189,9 @@ struct AssocArgs {
 };
 
 // Single block: age / retire, rebuild the slot map around retired pixels, hand the lowest free
-// slots to the unmatched detections in ascending pix, compact the active list.
+// slots to the unmatched detections in ascending pix, compact the active list.  A thread owns a run of
+// consecutive slots and keeps their "active" bits in a register, so each phase issues its global loads
+// together instead of one dependent chain per slot.
 __global__ void __launch_bounds__(1024)
 k_assoc_update(const AssocArgs a) {
   __shared__ int s_warp[33];
@@ -143,23 +200,45 @@ k_assoc_update(const AssocArgs a) {
   const bool frame_ok = a.band_ok[a.B] != 0;
   const int per = (a.n_cand_max + T - 1) / T;
   const int s0 = tid * per, s1 = min(s0 + per, a.n_cand_max);
-  if (frame_ok) {
-    // 1. age and retire
-    for (int s = s0; s < s1; ++s) {
-      if (!a.active[s]) continue;
-      if (a.matched_t[s] == a.t) a.miss[s] = 0;
-      else {
-        const int m = a.miss[s] + 1;
-        a.miss[s] = m;
-        if (!a.forced[s] && m >= a.n_forget) { a.active[s] = 0; a.slotmap[a.cpix[s]] = -1; }
+  // the active bits of this thread's slots, 32 at a time (per <= 32 for every configuration in use)
+  for (int c0 = s0; c0 < s1; c0 += 32) {
+    const int c1 = min(c0 + 32, s1);
+    unsigned act = 0u;
+#pragma unroll 8
+    for (int s = c0; s < c1; ++s) act |= (a.active[s] ? 1u : 0u) << (s - c0);
+    if (frame_ok) {
+      // 1. age and retire
+      unsigned hit = 0u;
+#pragma unroll 8
+      for (int s = c0; s < c1; ++s) hit |= (a.matched_t[s] == a.t ? 1u : 0u) << (s - c0);
+      unsigned retire = 0u;
+#pragma unroll 8
+      for (int s = c0; s < c1; ++s) {
+        const unsigned bit = 1u << (s - c0);
+        if (!(act & bit)) continue;
+        if (hit & bit) a.miss[s] = 0;
+        else {
+          const int m = a.miss[s] + 1;
+          a.miss[s] = m;
+          if (!a.forced[s] && m >= a.n_forget) retire |= bit;
+        }
       }
+      for (unsigned r = retire; r; r &= r - 1) {
+        const int s = c0 + __ffs(r) - 1;
+        a.active[s] = 0; a.slotmap[a.cpix[s]] = -1;
+      }
+      act &= ~retire;
     }
-    __syncthreads();
+  }
+  __syncthreads();
+  if (frame_ok) {
     // 2. another (forced) candidate may share a retired pixel: restore the lowest active slot there
+#pragma unroll 4
     for (int s = s0; s < s1; ++s)
       if (a.active[s]) atomicMin(reinterpret_cast<unsigned*>(&a.slotmap[a.cpix[s]]), (unsigned)s);
     // 3. free list (ascending)
     int nfree_mine = 0;
+#pragma unroll 8
     for (int s = s0; s < s1; ++s) nfree_mine += a.active[s] ? 0 : 1;
     int n_free;
     int off = block_excl_scan(nfree_mine, s_warp, n_free);
@@ -190,9 +269,11 @@ k_assoc_update(const AssocArgs a) {
   }
   // 5. active list, ascending slot
   int na_mine = 0;
+#pragma unroll 8
   for (int s = s0; s < s1; ++s) na_mine += a.active[s] ? 1 : 0;
   int n_act;
   int ao = block_excl_scan(na_mine, s_warp, n_act);
+#pragma unroll 4
   for (int s = s0; s < s1; ++s)
     if (a.active[s]) { a.act_slots[ao] = s; a.act_pix[ao] = a.cpix[s]; ++ao; }
   if (tid == 0) { *a.npos = n_act; a.counters[2] = n_act; }

@@ -46,7 +46,7 @@ constexpr int DR = 32;              // depth (rows) of the tensor-memory rings o
 constexpr int DRS = 34;             // depth of the shared-memory ring of F: local maxima are tested one iteration late
 constexpr int QCAP = 64;            // queued candidates per iteration (more are tested in place)
 constexpr int SCAP = 32;            // records staged by a helper warp between flushes
-constexpr int NHW = 4;              // helper warps: input producer and candidate tests
+constexpr int NHW = 2;              // helper warps: input producer and candidate tests
 constexpr int XST = 4;              // input staging stages (iterations in flight)
 constexpr int TM_D = 4 * DR;        // first tensor-memory column of the d ring (F ring starts at 0)
 constexpr int PADR = 64;            // zero rows above and below the padded normaliser planes
