@@ -182,6 +182,14 @@ int lpf_get_frame_view(lpf_ctx* ctx, int lane, lpf_frame_view* out);
  * buffer, runs the chain, copies the results back into `res`.  Synchronises `stream`. */
 int lpf_process_frame_host(lpf_ctx* ctx, int lane, const float* h_cube, int64_t t, lpf_host_result* res,
                            void* stream);
+/* The same call in two halves, so that several lanes can be in flight from the host: _begin enqueues the
+ * copy in, the chain and the copy out of the counts / statistics on `stream` and returns at once
+ * (h_cube and res must stay untouched until _end); _end waits for the stream, copies the variable-length
+ * lists (nu, npos known by then) and returns with `res` filled.  One _begin per lane at a time; issue
+ * the _begin calls in increasing t. */
+int lpf_process_frame_host_begin(lpf_ctx* ctx, int lane, const float* h_cube, int64_t t, lpf_host_result* res,
+                                 void* stream);
+int lpf_process_frame_host_end(lpf_ctx* ctx, int lane, lpf_host_result* res, void* stream);
 
 /* h_out[0] = records dropped (max_det), h_out[1] = detections dropped (n_cand_max full),
  * h_out[2] = kernels launched by this context so far, h_out[3] = active candidates.  Synchronises. */

@@ -53,7 +53,7 @@ DET_DTYPE = np.dtype([("pix", "<i4"), ("plane", "<i2"), ("iter", "<i2"), ("f", "
 EXPORTS = [
     "lpf_create", "lpf_destroy", "lpf_cube_qc", "lpf_detect_sources", "lpf_associate", "lpf_add_candidates",
     "lpf_measure_flux", "lpf_append_dynspec", "lpf_get_dynspec", "lpf_process_frame", "lpf_get_frame_view",
-    "lpf_process_frame_host", "lpf_get_counters", "lpf_memcpy_d2h", "lpf_strerror", "lpf_last_cuda_error",
+    "lpf_process_frame_host", "lpf_process_frame_host_begin", "lpf_process_frame_host_end", "lpf_get_counters", "lpf_memcpy_d2h", "lpf_strerror", "lpf_last_cuda_error",
     "lpf_version", "lpf_get_plan", "lpf_profile_begin", "lpf_profile_end", "lpf_profile_kernel_count", "lpf_profile_kernel_name",
 ]
 
@@ -85,6 +85,8 @@ def load_library(path: Optional[str] = None):
     lib.lpf_process_frame.argtypes = [vp, C.c_int, vp, i64, vp]
     lib.lpf_get_frame_view.argtypes = [vp, C.c_int, C.POINTER(LpfFrameView)]
     lib.lpf_process_frame_host.argtypes = [vp, C.c_int, vp, i64, C.POINTER(LpfHostResult), vp]
+    lib.lpf_process_frame_host_begin.argtypes = [vp, C.c_int, vp, i64, C.POINTER(LpfHostResult), vp]
+    lib.lpf_process_frame_host_end.argtypes = [vp, C.c_int, C.POINTER(LpfHostResult), vp]
     lib.lpf_get_counters.argtypes = [vp, C.POINTER(i64)]
     lib.lpf_memcpy_d2h.argtypes = [vp, vp, i64]
     lib.lpf_strerror.argtypes = [C.c_int]
@@ -249,6 +251,16 @@ class LPF:
         ptr = h_cube.data_ptr() if hasattr(h_cube, "data_ptr") else h_cube.ctypes.data
         _check(self.lib, self.lib.lpf_process_frame_host(self.h, lane, ptr, t, C.byref(res.c), _stream(stream)),
                "lpf_process_frame_host")
+        return res
+
+    def process_frame_host_begin(self, h_cube, t: int, res: "HostResult", lane: int = 0, stream=None):
+        ptr = h_cube.data_ptr() if hasattr(h_cube, "data_ptr") else h_cube.ctypes.data
+        _check(self.lib, self.lib.lpf_process_frame_host_begin(self.h, lane, ptr, t, C.byref(res.c), _stream(stream)),
+               "lpf_process_frame_host_begin")
+
+    def process_frame_host_end(self, res: "HostResult", lane: int = 0, stream=None):
+        _check(self.lib, self.lib.lpf_process_frame_host_end(self.h, lane, C.byref(res.c), _stream(stream)),
+               "lpf_process_frame_host_end")
         return res
 
     def plan(self) -> dict:

@@ -308,7 +308,7 @@ int lpf_get_frame_view(lpf_ctx* c, int lane, lpf_frame_view* v) {
   return LPF_OK;
 }
 
-int lpf_process_frame_host(lpf_ctx* c, int lane, const float* h_cube, int64_t t, lpf_host_result* res, void* stream) {
+int lpf_process_frame_host_begin(lpf_ctx* c, int lane, const float* h_cube, int64_t t, lpf_host_result* res, void* stream) {
   TRY(lane_ok(c, lane));
   if (!h_cube || !res) return LPF_E_ARG;
   cudaStream_t st = (cudaStream_t)stream;
@@ -323,6 +323,15 @@ int lpf_process_frame_host(lpf_ctx* c, int lane, const float* h_cube, int64_t t,
   LPF_CUDA(cudaMemcpyAsync(&L.h_counts[2], L.ndets, 4, cudaMemcpyDeviceToHost, st));
   if (res->h_stats) LPF_CUDA(cudaMemcpyAsync(res->h_stats, L.stats, (size_t)p.B * LPF_STATS_PER_BAND * 4, cudaMemcpyDeviceToHost, st));
   if (res->h_band_ok) LPF_CUDA(cudaMemcpyAsync(res->h_band_ok, L.band_ok, (size_t)p.B + 1, cudaMemcpyDeviceToHost, st));
+  return LPF_OK;
+}
+
+int lpf_process_frame_host_end(lpf_ctx* c, int lane, lpf_host_result* res, void* stream) {
+  TRY(lane_ok(c, lane));
+  if (!res) return LPF_E_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  LpfLane& L = c->lanes[lane];
+  const lpf_params& p = c->p;
   LPF_CUDA(cudaStreamSynchronize(st));
   res->nu = L.h_counts[0]; res->npos = L.h_counts[1]; res->ndets = L.h_counts[2];
   const size_t nu = (size_t)(res->nu < res->cap_u ? res->nu : res->cap_u);
@@ -339,6 +348,11 @@ int lpf_process_frame_host(lpf_ctx* c, int lane, const float* h_cube, int64_t t,
   }
   LPF_CUDA(cudaStreamSynchronize(st));
   return LPF_OK;
+}
+
+int lpf_process_frame_host(lpf_ctx* c, int lane, const float* h_cube, int64_t t, lpf_host_result* res, void* stream) {
+  TRY(lpf_process_frame_host_begin(c, lane, h_cube, t, res, stream));
+  return lpf_process_frame_host_end(c, lane, res, stream);
 }
 
 int lpf_get_counters(lpf_ctx* c, int64_t* h_out) {

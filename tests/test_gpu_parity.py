@@ -348,3 +348,34 @@ def test_fused_kernel_special_paths(torch_cuda):
     lpf2.process_frame(mis, 0)
     assert parity.check_frame(lpf2.frame_view(0), o2, pipe2, cube, "misaligned cube")["in_sync"]
     lpf.close(); lpf2.close()
+
+
+def test_host_entry_point_pipelined(torch_cuda):
+    """lpf_process_frame_host_begin/_end with three lanes in flight gives what the synchronous call gives."""
+    torch = torch_cuda
+    from paper_2103_15418_b200.binding import HostResult
+    s, p, lpf = _make(2, torch, n_lanes=3)
+    pipe = O.OraclePipeline(p, s.mask, direct=False)
+    L = 3
+    res = [HostResult(p) for _ in range(L)]
+    streams = [torch.cuda.Stream() for _ in range(L)]
+    cubes = [s.frame(t) for t in range(7)]
+    pinned = [torch.from_numpy(c).pin_memory() for c in cubes]
+    outs = []
+    for t in range(7):
+        ln = t % L
+        if t >= L:
+            lpf.process_frame_host_end(res[ln], lane=ln, stream=streams[ln])
+            outs.append({k: getattr(res[ln], k)[: (res[ln].nu if k in ("upos", "cand_idx") else res[ln].npos)].numpy().copy()
+                         for k in ("upos", "cand_idx", "act_slots", "flux")} | {"band_ok": res[ln].band_ok.numpy().copy()})
+        lpf.process_frame_host_begin(pinned[t], t, res[ln], lane=ln, stream=streams[ln])
+    for t in range(7 - L, 7):
+        ln = t % L
+        lpf.process_frame_host_end(res[ln], lane=ln, stream=streams[ln])
+        outs.append({k: getattr(res[ln], k)[: (res[ln].nu if k in ("upos", "cand_idx") else res[ln].npos)].numpy().copy()
+                     for k in ("upos", "cand_idx", "act_slots", "flux")} | {"band_ok": res[ln].band_ok.numpy().copy()})
+    for t in range(7):
+        o = pipe.step(cubes[t], t)
+        for k in ("band_ok", "upos", "cand_idx", "act_slots", "flux"):
+            assert np.array_equal(outs[t][k], o[k]), (t, k)
+    lpf.close()
