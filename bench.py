@@ -243,6 +243,19 @@ def run_ours(args):
 
     frames_s = whole_job_value(world, args.steps, ms)
     step_gbs = cube_bytes * frames_s / 1e9 / world
+    # With several lanes in flight the plan gives one launch of the fused kernel only a share of the SMs
+    # (n_sm / n_lanes: fewer, longer row segments), so a launch timed ALONE leaves most of the GPU idle.  The plain
+    # per-launch figures above stand as measured; "occupancy" says how much of the GPU that launch could use, and
+    # "in_timed_region" is the same kernel's work rate over the timed multi-lane region (all launches / wall time).
+    if dom == "fused_detect":
+        pl = lpf.plan()
+        ctas = pl["ctas_per_plane"] * pl["planes"]
+        smf = min(1.0, ctas / float(pl["sms"]))
+        per_s = frames_s / world
+        roof["occupancy"] = {"ctas_per_launch": ctas, "sms": pl["sms"], "sm_fraction": smf,
+                             "frac_of_occupied_sms": roof["frac"] / smf}
+        roof["in_timed_region"] = {"tflops": aflops * per_s / 1e12, "alu_frac": aflops * per_s / 1e12 / ALU_PEAK_TFLOPS,
+                                   "hbm_gbs": abytes * per_s / 1e9, "hbm_frac": abytes * per_s / 1e9 / hbm_peak}
 
     # end to end through the host entry point: pinned host cube -> H2D -> path -> D2H of the results
     e2e = None

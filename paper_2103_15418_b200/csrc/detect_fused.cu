@@ -379,6 +379,7 @@ struct Sweep {
   const FusedArgs& a;
   const FusedArgs* a_sh;   // the same arguments in shared memory (for the out-of-line candidate path)
   int xs, plane, tid, lane, warp;
+  const uint32_t* flp;     // this warp's control words, [nb] with stride NW
   int sx;                  // row stride of the plane pointers (0 for lanes outside the strip)
   bool col_in, dirty;
   unsigned umask;
@@ -413,8 +414,11 @@ struct Sweep {
 
   __device__ __forceinline__ Sweep(const FusedArgs& a_) : a(a_) {}
 
+  // the control word of iteration b, from global memory (fetched three iterations ahead; 0 past the end)
   __device__ __forceinline__ unsigned ctl(int b) const {
-    return reinterpret_cast<const uint32_t*>(g_sm4)[O_FL + b * NW + warp];
+    unsigned v = 0u;
+    if (b < nb) asm volatile("ld.global.nc.u32 %0, [%1];\n" : "=r"(v) : "l"(flp + b * NW));
+    return v;
   }
   __device__ __forceinline__ uint32_t bar_addr(int stage) const {
     return smem_u32(reinterpret_cast<const float*>(g_sm4) + O_BAR + 2 * stage);
@@ -671,17 +675,16 @@ struct Sweep {
       load_nm(f0 & FL_NM_LD); load_icr(f0 & FL_ICR_LD); load_ics(f0 & FL_ICS_LD);
     }
     int b = 0;
-    unsigned fl = ctl(0);
+    unsigned f0 = ctl(0), f1 = ctl(1), f2 = ctl(2);
     while (true) {
-      unsigned fn = b + 1 < nb ? ctl(b + 1) : 0u;
-      iteration<0>(b, fl); if (++b >= nb) break;
-      fl = fn; fn = b + 1 < nb ? ctl(b + 1) : 0u;
-      iteration<1>(b, fl); if (++b >= nb) break;
-      fl = fn; fn = b + 1 < nb ? ctl(b + 1) : 0u;
-      iteration<2>(b, fl); if (++b >= nb) break;
-      fl = fn; fn = b + 1 < nb ? ctl(b + 1) : 0u;
-      iteration<3>(b, fl); if (++b >= nb) break;
-      fl = fn;
+      unsigned f3 = ctl(b + 3);
+      iteration<0>(b, f0); if (++b >= nb) break;
+      f0 = ctl(b + 3);
+      iteration<1>(b, f1); if (++b >= nb) break;
+      f1 = ctl(b + 3);
+      iteration<2>(b, f2); if (++b >= nb) break;
+      f2 = ctl(b + 3);
+      iteration<3>(b, f3); if (++b >= nb) break;
     }
   }
 };
@@ -706,11 +709,7 @@ k_fused_box(const FusedArgs a) {
   if (s.tid == 0) s_args = a;
   constexpr int NT = NW * 32 + NHW * 32;    // NW sweep warps and the helper warps
   for (int i = s.tid; i < (SW::O_FL >> 2); i += NT) g_sm4[i] = zero4();
-  {
-    uint32_t* fl_s = reinterpret_cast<uint32_t*>(g_sm4) + SW::O_FL;
-    const uint32_t* src = a.flags + it.fl_off;
-    for (int i = s.tid; i < it.nb * NW; i += NT) fl_s[i] = src[i];
-  }
+  s.flp = a.flags + it.fl_off + (s.warp < NW ? s.warp : 0);
   if (s.warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n"
                  ::"l"((uint64_t)__cvta_generic_to_shared(&s_tmem)), "n"(TM_COLS));
@@ -806,7 +805,8 @@ struct LpfFusedPlan {
 static size_t fused_smem_bytes(int NW, int max_nb) {
   const int CWP = NW * 128, XP = CWP + 8, PEV = CWP + 2 * KBG, PET = NW * 32 + 8;
   const size_t nfl = (size_t)DRS * CWP + (size_t)XST * RB * XP + 4 * RB * PEV + 4 * RB * PET + 2 * QCAP * 4 + 4 + NHW * SCAP * 8 + 2 * XST;
-  return (nfl + (size_t)max_nb * NW) * sizeof(float) + 16;
+  (void)max_nb;                 // the control words stay in global memory
+  return nfl * sizeof(float) + 16;
 }
 
 template <int NW>
@@ -903,14 +903,13 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
   // n_lanes frames in flight the kernels of different lanes share the SMs, so each gets its share of them
   // (fewer, longer segments: less warm-up per output row).
   const int n_planes = c->n_planes;
-  const int sm_share = std::max(1, c->n_sm / std::max(1, p.n_lanes));
+  const int sm_share = std::max(1, c->n_sm / std::max(1, std::min(p.n_lanes, 4)));   // (more lanes in flight only deepen the queue)
   const double warm = 58.0;   // warm-up / drain rows of a segment
   int best_seg = 1; double best_cost = 1e30;
   const int max_rows_strip = (int)(rows_all / n_strips);
   for (int nseg = 1; nseg <= 64; ++nseg) {
     const double rows = (double)max_rows_strip / nseg;
     if (nseg > 1 && rows < 24) break;
-    if (rows > 640 && nseg < 64) continue;      // keeps an item's control words within shared memory
     const long long ctas = (long long)nseg * n_strips * n_planes;
     const double waves = (double)((ctas + sm_share - 1) / sm_share);
     const double cost = waves * (rows + warm);
