@@ -46,7 +46,7 @@ constexpr int DR = 32;              // depth (rows) of the tensor-memory rings o
 constexpr int DRS = 34;             // depth of the shared-memory ring of F: local maxima are tested one iteration late
 constexpr int QCAP = 64;            // queued candidates per iteration (more are tested in place)
 constexpr int SCAP = 32;            // records staged by a helper warp between flushes
-constexpr int NHW = 2;              // helper warps: input producer and candidate tests
+constexpr int NHW = 3;              // helper warps: input producer and candidate tests
 constexpr int XST = 4;              // input staging stages (iterations in flight)
 constexpr int TM_D = 4 * DR;        // first tensor-memory column of the d ring (F ring starts at 0)
 constexpr int PADR = 64;            // zero rows above and below the padded normaliser planes
@@ -478,7 +478,11 @@ struct Sweep {
 
     // ---- stage A, part 1: staged rows -> horizontal matched filter ------------------------------------
     if (fl & FL_X) {
+#ifdef EXP_TIMING
+      { const long long tw0 = clock64(); mbar_wait(bar_addr(PH), (uint32_t)(b >> 2) & 1u); t_cons += clock64() - tw0; n_cons += 1; }
+#else
       mbar_wait(bar_addr(PH), (uint32_t)(b >> 2) & 1u);
+#endif
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
         const int xr = O_X + (PH * RB + j) * XP + 4 * tid;
@@ -775,7 +779,7 @@ k_fused_box(const FusedArgs a) {
 #endif
   if (sweeper) s.run(); else s.run_helper(it.y_start);
 #ifdef EXP_TIMING
-  if (s.lane == 0 && blockIdx.x == 3 && (p == 0 || p == a.B))
+  if (s.lane == 0 && blockIdx.x == 0 && (p == 0 || p == a.B))
     printf("plane %d warp %d busy %lld wait %lld nb %d | consume calls %d cycles %lld n_sum %d\n", p, s.warp, s.t_busy, s.t_wait, it.nb, s.n_cons, s.t_cons, s.n_sum);
 #endif
 
