@@ -401,7 +401,8 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--cpu-crop", type=int, default=256)
-    ap.add_argument("--traffic", type=float, default=None, help="dram bytes/launch of the dominant kernel from ncu (profiles/)")
+    ap.add_argument("--traffic", type=float, default=68.68e6,
+                    help="dram read+write bytes per launch of the dominant kernel from ncu --set full (profiles/r1_c_fused_v6.md)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
