@@ -189,60 +189,64 @@ struct AssocArgs {
 };
 
 // Single block: age / retire, rebuild the slot map around retired pixels, hand the lowest free
-// slots to the unmatched detections in ascending pix, compact the active list.  A thread owns a run of
-// consecutive slots and keeps their "active" bits in a register, so each phase issues its global loads
-// together instead of one dependent chain per slot.
+// slots to the unmatched detections in ascending pix, compact the active list.  A warp owns a run of
+// consecutive slots and walks it 32 at a time (lane = slot: every table access is coalesced); ordered
+// compaction by ballot + popc within a step, a running offset across steps, a scan of the warp totals across
+// warps.
+__device__ __forceinline__ int warp_totals_excl(int my_total, int* s_tot /*[33]*/, int& grand) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  __syncthreads();
+  if (lane == 0) s_tot[w] = my_total;
+  __syncthreads();
+  int pre = 0, all = 0;
+  for (int i = 0; i < nw; ++i) { const int v = s_tot[i]; all += v; if (i < w) pre += v; }
+  grand = all;
+  return pre;
+}
+
 __global__ void __launch_bounds__(1024)
 k_assoc_update(const AssocArgs a) {
   __shared__ int s_warp[33];
   const int T = blockDim.x;
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, nw = T >> 5;
+  const unsigned lt = (1u << lane) - 1u;
   const bool frame_ok = a.band_ok[a.B] != 0;
-  const int per = (a.n_cand_max + T - 1) / T;
-  const int s0 = tid * per, s1 = min(s0 + per, a.n_cand_max);
-  // the active bits of this thread's slots, 32 at a time (per <= 32 for every configuration in use)
-  for (int c0 = s0; c0 < s1; c0 += 32) {
-    const int c1 = min(c0 + 32, s1);
-    unsigned act = 0u;
-#pragma unroll 8
-    for (int s = c0; s < c1; ++s) act |= (a.active[s] ? 1u : 0u) << (s - c0);
-    if (frame_ok) {
-      // 1. age and retire
-      unsigned hit = 0u;
-#pragma unroll 8
-      for (int s = c0; s < c1; ++s) hit |= (a.matched_t[s] == a.t ? 1u : 0u) << (s - c0);
-      unsigned retire = 0u;
-#pragma unroll 8
-      for (int s = c0; s < c1; ++s) {
-        const unsigned bit = 1u << (s - c0);
-        if (!(act & bit)) continue;
-        if (hit & bit) a.miss[s] = 0;
-        else {
-          const int m = a.miss[s] + 1;
-          a.miss[s] = m;
-          if (!a.forced[s] && m >= a.n_forget) retire |= bit;
-        }
-      }
-      for (unsigned r = retire; r; r &= r - 1) {
-        const int s = c0 + __ffs(r) - 1;
-        a.active[s] = 0; a.slotmap[a.cpix[s]] = -1;
-      }
-      act &= ~retire;
-    }
-  }
-  __syncthreads();
+  const int spw = ((a.n_cand_max + nw - 1) / nw + 31) & ~31;          // slots per warp, a multiple of 32
+  const int w0 = min(w * spw, a.n_cand_max), w1 = min(w0 + spw, a.n_cand_max);
   if (frame_ok) {
-    // 2. another (forced) candidate may share a retired pixel: restore the lowest active slot there
+    // 1. age and retire
+    int any_retired = 0;
 #pragma unroll 4
-    for (int s = s0; s < s1; ++s)
-      if (a.active[s]) atomicMin(reinterpret_cast<unsigned*>(&a.slotmap[a.cpix[s]]), (unsigned)s);
+    for (int s = w0 + lane; s < w1; s += 32) {
+      const uint8_t act = a.active[s], frc = a.forced[s];      // independent loads: they leave together
+      const long long mt = a.matched_t[s];
+      const int m0 = a.miss[s], px = a.cpix[s];
+      if (!act) continue;
+      const bool hit = mt == a.t;
+      const int m = hit ? 0 : m0 + 1;
+      if (m != m0) a.miss[s] = m;
+      if (!hit && !frc && m >= a.n_forget) { a.active[s] = 0; a.slotmap[px] = -1; any_retired = 1; }
+    }
+    // 2. another (forced) candidate may share a retired pixel: restore the lowest active slot there
+    if (__syncthreads_or(any_retired)) {
+      for (int s = w0 + lane; s < w1; s += 32)
+        if (a.active[s]) atomicMin(reinterpret_cast<unsigned*>(&a.slotmap[a.cpix[s]]), (unsigned)s);
+    }
     // 3. free list (ascending)
-    int nfree_mine = 0;
-#pragma unroll 8
-    for (int s = s0; s < s1; ++s) nfree_mine += a.active[s] ? 0 : 1;
+    int nfree_w = 0;
+    for (int s0 = w0; s0 < w1; s0 += 32) {
+      const int s = s0 + lane;
+      nfree_w += __popc(__ballot_sync(0xffffffffu, s < w1 && !a.active[s]));
+    }
     int n_free;
-    int off = block_excl_scan(nfree_mine, s_warp, n_free);
-    for (int s = s0; s < s1; ++s) if (!a.active[s]) a.free_list[off++] = s;
+    int off = warp_totals_excl(nfree_w, s_warp, n_free);
+    for (int s0 = w0; s0 < w1; s0 += 32) {
+      const int s = s0 + lane;
+      const bool fr = s < w1 && !a.active[s];
+      const unsigned m = __ballot_sync(0xffffffffu, fr);
+      if (fr) a.free_list[off + __popc(m & lt)] = s;
+      off += __popc(m);
+    }
     __syncthreads();
     // 4. unmatched detections, ascending pix (upos is sorted)
     const int nu = *a.nu;
@@ -268,14 +272,21 @@ k_assoc_update(const AssocArgs a) {
     __syncthreads();
   }
   // 5. active list, ascending slot
-  int na_mine = 0;
-#pragma unroll 8
-  for (int s = s0; s < s1; ++s) na_mine += a.active[s] ? 1 : 0;
+  int nact_w = 0;
+  for (int s0 = w0; s0 < w1; s0 += 32) {
+    const int s = s0 + lane;
+    nact_w += __popc(__ballot_sync(0xffffffffu, s < w1 && a.active[s]));
+  }
   int n_act;
-  int ao = block_excl_scan(na_mine, s_warp, n_act);
-#pragma unroll 4
-  for (int s = s0; s < s1; ++s)
-    if (a.active[s]) { a.act_slots[ao] = s; a.act_pix[ao] = a.cpix[s]; ++ao; }
+  int ao = warp_totals_excl(nact_w, s_warp, n_act);
+  for (int s0 = w0; s0 < w1; s0 += 32) {
+    const int s = s0 + lane;
+    const bool ac = s < w1 && a.active[s];
+    const int px = s < w1 ? a.cpix[s] : 0;
+    const unsigned m = __ballot_sync(0xffffffffu, ac);
+    if (ac) { const int o = ao + __popc(m & lt); a.act_slots[o] = s; a.act_pix[o] = px; }
+    ao += __popc(m);
+  }
   if (tid == 0) { *a.npos = n_act; a.counters[2] = n_act; }
 }
 
