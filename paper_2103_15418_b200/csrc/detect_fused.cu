@@ -374,7 +374,7 @@ struct Sweep {
   static constexpr int O_QN = O_Q + 2 * QCAP * 4;        // their lengths, one word per iteration mod 4
   static constexpr int O_ST = O_QN + 4;                  // staged records of the helper warps, [NHW][SCAP] x 8 words
   static constexpr int O_BAR = O_ST + NHW * SCAP * 8;    // XST mbarriers (8 bytes each)
-  static constexpr int O_FL = O_BAR + 2 * XST;           // control words, [nb][NW]
+  static constexpr int O_FL = O_BAR + 2 * XST + 2;       // end of the layout (XST input barriers + the iteration barrier)
   // ---- constants of the thread -----------------------------------------------------------------
   const FusedArgs& a;
   const FusedArgs* a_sh;   // the same arguments in shared memory (for the out-of-line candidate path)
@@ -396,18 +396,6 @@ struct Sweep {
   int y0;                  // first input row of the current iteration
   int ring_y0;             // the row that sits in slot 0 of the rings
   int ws;                  // slot of this iteration's first F row in the shared-memory ring
-#ifdef EXP_TIMING
-  long long t_busy = 0, t_wait = 0, t_mark = 0, t_cons = 0; int n_cons = 0, n_sum = 0;
-  long long* t_arr;        // [2][16] arrival clocks of the warps
-  __device__ __forceinline__ void sync_timed(int b) {
-    const long long t1 = clock64();
-    if (lane == 0) t_arr[(b & 1) * 16 + warp] = t1;
-    __syncthreads();
-    long long mx = 0;
-    for (int i = 0; i < NW + NHW; ++i) { const long long v = t_arr[(b & 1) * 16 + i]; mx = v > mx ? v : mx; }
-    t_busy += t1 - t_mark; t_wait += mx - t1; t_mark = mx;
-  }
-#endif
   float2 hw[8][2];         // horizontally filtered rows (rotating; static indices per phase)
   float2 V1[2], V2[2];     // vertical running sums
   Planes pl;               // normalisers of the coming rows: each plane is reloaded right after its use
@@ -423,6 +411,10 @@ struct Sweep {
   __device__ __forceinline__ uint32_t bar_addr(int stage) const {
     return smem_u32(reinterpret_cast<const float*>(g_sm4) + O_BAR + 2 * stage);
   }
+
+  // the per-iteration barrier of all warps, in two halves (an mbarrier with one arrival per thread)
+  __device__ __forceinline__ void sync_arrive() const { mbar_arrive(bar_addr(XST)); }
+  __device__ __forceinline__ void sync_wait(int b) const { mbar_wait(bar_addr(XST), (uint32_t)b & 1u); }
 
   __device__ __forceinline__ CandCtx cand_ctx() const {
     CandCtx c;
@@ -460,36 +452,20 @@ struct Sweep {
     icsp += RB * sx;
   }
 
-  // One iteration: rows y0, y0+1 enter stage A; PH = iteration index mod 4 fixes the register rotation
-  // and the staging stage.  fl: this iteration's control word.
+  // Stage A, part 1 for iteration bn (PH = bn mod 4): staged input rows -> horizontal matched filter -> hw.
+  // It touches only the input stages and registers, so it runs in the shadow of the previous iteration's
+  // barrier (between the arrival and the wait).  yn: first input row of iteration bn.
   template <int PH>
-  __device__ __forceinline__ void iteration(int b, unsigned fl) {
-    constexpr int buf = PH & 1, pbuf = buf ^ 1;
-    const float2 g0 = splat(a.g0), g1 = splat(a.g1), g2 = splat(a.g2), g3 = splat(a.g3);
-    const int w = (RB * b) & (DR - 1);                       // ring slot of this iteration's first row (even)
-    const uint32_t t_old0 = tm + 4u * (uint32_t)((w + 7) & (DR - 1)), t_old1 = tm + 4u * (uint32_t)((w + 8) & (DR - 1));
-    const uint32_t t_lag0 = tm + 4u * (uint32_t)((w + 18) & (DR - 1)), t_lag1 = t_lag0 + 4u;   // w + 18 is even: no wrap in between
-    const uint32_t t_new0 = tm + 4u * (uint32_t)w, t_new1 = t_new0 + 4u;
-
-    // ---- tensor-memory reads: F(fr - 25), F(rho), d(rho - 25), d(sigma) ---------------------------------
-    float2 fold[RB][2], flag[RB][2], dold[RB][2], dlag[RB][2];
-    tm_ld4(t_old0, fold[0][0], fold[0][1]); tm_ld4(t_old1, fold[1][0], fold[1][1]);
-
-
-    // ---- stage A, part 1: staged rows -> horizontal matched filter ------------------------------------
+  __device__ __forceinline__ void stage_a1(int bn, unsigned fl, int yn) {
     if (fl & FL_X) {
-#ifdef EXP_TIMING
-      { const long long tw0 = clock64(); mbar_wait(bar_addr(PH), (uint32_t)(b >> 2) & 1u); t_cons += clock64() - tw0; n_cons += 1; }
-#else
-      mbar_wait(bar_addr(PH), (uint32_t)(b >> 2) & 1u);
-#endif
+      mbar_wait(bar_addr(PH), (uint32_t)(bn >> 2) & 1u);
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
         const int xr = O_X + (PH * RB + j) * XP + 4 * tid;
         float4 l = lds4(xr), m = lds4(xr + 4), r = lds4(xr + 8);
         if (dirty) {
           Row12 v; v.l = l; v.m = m; v.r = r;
-          v = mask_row(a_sh, y0 + j, xs + 4 * tid - 4, v);
+          v = mask_row(a_sh, yn + j, xs + 4 * tid - 4, v);
           l = v.l; m = v.m; r = v.r;
         }
         const float wv[10] = {l.y, l.z, l.w, m.x, m.y, m.z, m.w, r.x, r.y, r.z};
@@ -504,6 +480,24 @@ struct Sweep {
 #pragma unroll
       for (int j = 0; j < RB; ++j) { hw[(2 * PH + 6 + j) & 7][0] = splat(0.f); hw[(2 * PH + 6 + j) & 7][1] = splat(0.f); }
     }
+
+  }
+
+  // One iteration: rows y0, y0+1 enter stage A; PH = iteration index mod 4 fixes the register rotation
+  // and the staging stage.  fl: this iteration's control word.
+  template <int PH>
+  __device__ __forceinline__ void iteration(int b, unsigned fl, unsigned fl_next) {
+    constexpr int buf = PH & 1, pbuf = buf ^ 1;
+    const float2 g0 = splat(a.g0), g1 = splat(a.g1), g2 = splat(a.g2), g3 = splat(a.g3);
+    const int w = (RB * b) & (DR - 1);                       // ring slot of this iteration's first row (even)
+    const uint32_t t_old0 = tm + 4u * (uint32_t)((w + 7) & (DR - 1)), t_old1 = tm + 4u * (uint32_t)((w + 8) & (DR - 1));
+    const uint32_t t_lag0 = tm + 4u * (uint32_t)((w + 18) & (DR - 1)), t_lag1 = t_lag0 + 4u;   // w + 18 is even: no wrap in between
+    const uint32_t t_new0 = tm + 4u * (uint32_t)w, t_new1 = t_new0 + 4u;
+
+    // ---- tensor-memory reads: F(fr - 25), F(rho), d(rho - 25), d(sigma) ---------------------------------
+    float2 fold[RB][2], flag[RB][2], dold[RB][2], dlag[RB][2];
+    tm_ld4(t_old0, fold[0][0], fold[0][1]); tm_ld4(t_old1, fold[1][0], fold[1][1]);
+
 
     tm_wait_ld();
 #pragma unroll
@@ -625,11 +619,10 @@ struct Sweep {
     ws = ws + RB >= DRS ? ws + RB - DRS : ws + RB;
     y0 += RB;
     tm_wait_st();
-#ifdef EXP_TIMING
-    sync_timed(b);
-#else
-    __syncthreads();
-#endif
+    // split barrier: arrive, filter the next iteration's input rows while the slower warps finish, wait
+    sync_arrive();
+    stage_a1<(PH + 1) & 3>(b + 1, fl_next, y0);
+    sync_wait(b);
   }
 
   // the helper warps: helper 0 feeds the input stages (bulk copies three iterations ahead); all of them test
@@ -649,24 +642,13 @@ struct Sweep {
       }
       if (b > 0) {
         const int n = min(qn[(b - 1) & 3], QCAP);
-#ifdef EXP_TIMING
-        const long long tc0 = clock64();
-#endif
         if (n > 0) {
           const int o_q = O_Q + ((b - 1) & 1) * QCAP * 4;
           if (km2) { for (int e0 = 6 * hw; e0 < n; e0 += 6 * NHW) nst = cand_pass5(cc, ck, o_q, n, e0, o_st, nst); }
           else nst = cand_consume(cc, o_q, n, hw, NHW, o_st, nst);
         }
-#ifdef EXP_TIMING
-        const long long tc1 = clock64();
-        if (n > 6 * hw) { t_cons += tc1 - tc0; n_cons += 1; n_sum += n; }
-#endif
       }
-#ifdef EXP_TIMING
-      if (b < nb) sync_timed(b);
-#else
-      if (b < nb) __syncthreads();
-#endif
+      if (b < nb) { sync_arrive(); sync_wait(b); }
     }
     cand_flush(a_sh, o_st, lane, nst);
     if (hw == NHW - 1 && lane == 0)                   // no bulk copy may be in flight when the CTA leaves
@@ -680,15 +662,16 @@ struct Sweep {
     }
     int b = 0;
     unsigned f0 = ctl(0), f1 = ctl(1), f2 = ctl(2);
+    stage_a1<0>(0, f0, y0);
     while (true) {
       unsigned f3 = ctl(b + 3);
-      iteration<0>(b, f0); if (++b >= nb) break;
+      iteration<0>(b, f0, f1); if (++b >= nb) break;
       f0 = ctl(b + 3);
-      iteration<1>(b, f1); if (++b >= nb) break;
+      iteration<1>(b, f1, f2); if (++b >= nb) break;
       f1 = ctl(b + 3);
-      iteration<2>(b, f2); if (++b >= nb) break;
+      iteration<2>(b, f2, f3); if (++b >= nb) break;
       f2 = ctl(b + 3);
-      iteration<3>(b, f3); if (++b >= nb) break;
+      iteration<3>(b, f3, f0); if (++b >= nb) break;
     }
   }
 };
@@ -725,6 +708,7 @@ k_fused_box(const FusedArgs a) {
   if (s.tid == 0) {
 #pragma unroll
     for (int i = 0; i < XST; ++i) mbar_init(s.bar_addr(i), 1);
+    mbar_init(s.bar_addr(XST), NT);
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
   asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");   // the zero fill above precedes the bulk copies
@@ -772,16 +756,7 @@ k_fused_box(const FusedArgs a) {
   if (s.tid == (NW + NHW - 1) * 32)
     for (int bb = 0; bb < XST - 1 && bb < it.nb; ++bb) s.issue_rows(bb, it.y_start);
 
-#ifdef EXP_TIMING
-  __shared__ long long s_tarr[32];
-  s.t_arr = s_tarr;
-  s.t_mark = clock64();
-#endif
   if (sweeper) s.run(); else s.run_helper(it.y_start);
-#ifdef EXP_TIMING
-  if (s.lane == 0 && blockIdx.x == 0 && (p == 0 || p == a.B))
-    printf("plane %d warp %d busy %lld wait %lld nb %d | consume calls %d cycles %lld n_sum %d\n", p, s.warp, s.t_busy, s.t_wait, it.nb, s.n_cons, s.t_cons, s.n_sum);
-#endif
 
   tm_wait_st();
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
@@ -808,7 +783,7 @@ struct LpfFusedPlan {
 
 static size_t fused_smem_bytes(int NW, int max_nb) {
   const int CWP = NW * 128, XP = CWP + 8, PEV = CWP + 2 * KBG, PET = NW * 32 + 8;
-  const size_t nfl = (size_t)DRS * CWP + (size_t)XST * RB * XP + 4 * RB * PEV + 4 * RB * PET + 2 * QCAP * 4 + 4 + NHW * SCAP * 8 + 2 * XST;
+  const size_t nfl = (size_t)DRS * CWP + (size_t)XST * RB * XP + 4 * RB * PEV + 4 * RB * PET + 2 * QCAP * 4 + 4 + NHW * SCAP * 8 + 2 * XST + 2;
   (void)max_nb;                 // the control words stay in global memory
   return nfl * sizeof(float) + 16;
 }
