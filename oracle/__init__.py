@@ -217,6 +217,8 @@ class OraclePipeline:
         self.direct = direct
         p = self.p
         self.table = CandidateTable(p["n_cand_max"], p["T_ring"], p["B"], p["Dx"], p["r_assoc"], p["n_forget"])
+        self.n_back = int(p.get("n_back", 0))
+        self.history = []   # O11: the last n_back frames as (t, cube, band_ok)
 
     # -- steps ---------------------------------------------------------------
     def cube_qc(self, cube):
@@ -252,6 +254,26 @@ class OraclePipeline:
             out["planes"] = per_plane
         return out
 
+    def backfill(self, cube, ok, t: int):
+        """O11, backward fill ("we backward fill the catalog ... add a pre-specified number of
+        timesteps to the catalog and measure from cached images"): every slot born at t gets, for each cached
+        frame tau in [t - n_back, t - 1] whose ring column still belongs to tau, the O9 flux of that frame at
+        the slot's pixel.  Then frame t joins the cache."""
+        if self.n_back <= 0:
+            return
+        tb = self.table
+        new = np.flatnonzero((tb.active != 0) & (tb.born == t))
+        if new.size:
+            pix = tb.cpix[new]
+            for (tau, c_tau, ok_tau) in self.history:
+                if tau < t - self.n_back or tau >= t or tb.meta_t[tau % tb.T] != tau:
+                    continue
+                f = measure_flux(c_tau, ok_tau, self.W, pix, self.p["r_flux"])
+                tb.ring[new, tau % tb.T, :] = f
+        self.history.append((t, np.array(cube, dtype=np.float32, copy=True), np.array(ok, dtype=np.uint8, copy=True)))
+        if len(self.history) > self.n_back:
+            self.history.pop(0)
+
     def step(self, cube, t: int, keep_planes: bool = False) -> dict:
         """One frame through the whole path."""
         p = self.p
@@ -260,5 +282,6 @@ class OraclePipeline:
         cand, act_s, act_p = self.table.associate(det["upos"], t, int(ok[p["B"]]))
         flux = measure_flux(cube, ok, self.W, act_p, p["r_flux"])
         self.table.append(act_s, flux, ok, t)
+        self.backfill(cube, ok, t)
         det.update(stats=stats, band_ok=ok, cand_idx=cand, act_slots=act_s, act_pix=act_p, flux=flux)
         return det

@@ -639,3 +639,88 @@ def test_injected_sources_recovered_config2():
         fl = r["flux"][k]                                           # forced flux ~ amplitude (+ max-of-9 noise bias)
         assert abs(np.median(fl) - st["amp"][i]) < 1.5
     assert r["upos"].size < 1.5 * st["y"].size                      # and not swamped by false positives
+
+
+# ------------------------------------------------------------------ O11 backward fill
+def _ramp_stream(n_frames=14, D=64, B=4, seed=3):
+    rng = np.random.default_rng(seed)
+    yy, xx = np.mgrid[0:D, 0:D]
+    g = np.exp(-0.5 * ((yy - 30) ** 2 + (xx - 41) ** 2) / 0.85 ** 2).astype(np.float32)
+    amp = [0, 0, 0, 0, 0, 1.5, 2.5, 3.5, 4.5, 6.0, 9.0, 14.0, 20.0, 20.0]
+    return [(rng.standard_normal((B, D, D)).astype(np.float32) + amp[t] * g) for t in range(n_frames)]
+
+
+def test_backward_fill_shows_the_build_up():
+    """A source that brightens slowly is first detected at t_d; with n_back = 4 its dynamic spectrum must then
+    hold, for t_d-4 .. t_d-1, the box maximum of those EARLIER cubes at its pixel (computed here with plain
+    NumPy slicing), NaN before that, and the ordinary monitored fluxes from t_d on.  n_back = 0: NaN before t_d."""
+    import oracle as O
+    from paper_2103_15418_b200 import synth
+    cubes = _ramp_stream()
+    B, D, _ = cubes[0].shape
+    p = synth.default_params(1); p.update(B=B, Dy=D, Dx=D, T_ring=16)
+    res = {}
+    for nb in (0, 4):
+        q = dict(p); q["n_back"] = nb
+        pipe = O.OraclePipeline(q, None, direct=False)
+        for t, c in enumerate(cubes):
+            pipe.step(c, t)
+        tb = pipe.table
+        slots = [s for s in np.flatnonzero(tb.active) if abs(tb.cpix[s] // D - 30) <= 1 and abs(tb.cpix[s] % D - 41) <= 1]
+        assert len(slots) == 1
+        s = slots[0]
+        res[nb] = (int(tb.born[s]), int(tb.cpix[s]), pipe.table.dynspec(int(s), len(cubes) - 1))
+    t_d, pix, ds0 = res[0]
+    assert res[4][0] == t_d and res[4][1] == pix and 5 < t_d < 12
+    y, x = divmod(pix, D)
+    T = 16
+    col = lambda t: T - 1 - (len(cubes) - 1 - t)          # dynspec is time ordered, newest last
+    ds4 = res[4][2]
+    for t in range(len(cubes)):
+        want = np.array([cubes[t][b, y - 1:y + 2, x - 1:x + 2].max() for b in range(B)], np.float32)
+        if t >= t_d:                                        # monitored from birth on, with or without backfill
+            assert np.array_equal(ds0[:, col(t)], want) and np.array_equal(ds4[:, col(t)], want)
+        else:
+            assert np.isnan(ds0[:, col(t)]).all()
+            if t >= t_d - 4:
+                assert np.array_equal(ds4[:, col(t)], want), t
+            else:
+                assert np.isnan(ds4[:, col(t)]).all()
+
+
+def test_backward_fill_respects_rejected_bands_and_ring_age():
+    import oracle as O
+    from paper_2103_15418_b200 import synth
+    cubes = _ramp_stream()
+    B, D, _ = cubes[0].shape
+
+    def run(T_ring, n_back, nan_at=None):
+        p = synth.default_params(1); p.update(B=B, Dy=D, Dx=D, T_ring=T_ring, n_back=n_back)
+        pipe = O.OraclePipeline(p, None, direct=False)
+        for t, c in enumerate(cubes):
+            c = c.copy()
+            if nan_at is not None and t == nan_at:
+                c[2, 0, 0] = np.nan              # band 2 is rejected in that frame (non-finite statistics)
+            pipe.step(c, t)
+            tb = pipe.table
+            hit = [s for s in np.flatnonzero(tb.active) if abs(tb.cpix[s] // D - 30) <= 1 and abs(tb.cpix[s] % D - 41) <= 1]
+            if hit:
+                return t, int(tb.cpix[hit[0]]), tb.ring[int(hit[0])].copy(), tb.meta_t.copy()
+        raise AssertionError("never detected")
+
+    t_d, pix, _, _ = run(16, 4)
+    y, x = divmod(pix, D)
+    # a band rejected in a cached frame: its back-filled flux is 0, the other bands are the box maxima
+    t2, pix2, ring, meta = run(16, 4, nan_at=t_d - 2)
+    assert (t2, pix2) == (t_d, pix)
+    colv = ring[(t_d - 2) % 16]
+    assert colv[2] == 0.0
+    for b in (0, 1, 3):
+        assert colv[b] == cubes[t_d - 2][b, y - 1:y + 2, x - 1:x + 2].max()
+    # a ring shorter than the cache: only columns that still belong to their frame are filled
+    t3, pix3, ring, meta = run(3, 6)
+    assert (t3, pix3) == (t_d, pix)
+    assert sorted(meta.tolist()) == [t_d - 2, t_d - 1, t_d]
+    for tau in (t_d - 2, t_d - 1, t_d):
+        want = np.array([cubes[tau][b, y - 1:y + 2, x - 1:x + 2].max() for b in range(B)], np.float32)
+        assert np.array_equal(ring[tau % 3], want)
