@@ -76,6 +76,8 @@ typedef struct {
   int32_t n_cand_max;       /* candidate-table capacity */
   int32_t max_det;          /* capacity of the per-plane record list, per frame */
   int32_t n_lanes;          /* frames in flight */
+  int32_t n_back;           /* backward fill: a slot created at t also gets the fluxes of the last n_back
+                             * cubes, which lpf_process_frame then keeps in a device cache; 0 = off, <= 64 */
 } lpf_params;
 
 /* One peak (eq. 7: p = q and y) of one plane.  24 bytes. */

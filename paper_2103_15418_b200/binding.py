@@ -29,6 +29,7 @@ class LpfParams(C.Structure):
         ("qc_tau", C.c_float), ("qc_clip", C.c_float),
         ("r_flux", C.c_int32), ("r_dedupe", C.c_int32), ("r_assoc", C.c_int32), ("n_forget", C.c_int32),
         ("T_ring", C.c_int32), ("n_cand_max", C.c_int32), ("max_det", C.c_int32), ("n_lanes", C.c_int32),
+        ("n_back", C.c_int32),
     ]
 
 

@@ -387,6 +387,61 @@ k_append(float* __restrict__ ring, long long* __restrict__ meta_t, unsigned long
   }
 }
 
+// O11, backward fill: one warp per active position; a slot born at t gets, for every cached
+// frame tau in [t - n_back, t - 1] whose ring column still belongs to tau, the O9 flux of that frame at its
+// pixel.  Thread 0 of the grid then labels the cache entry that the caller overwrites with frame t next.
+struct BackfillArgs {
+  float* ring; const long long* meta_t; const long long* born; int T_ring, B, Dy, Dx, r, n_back;
+  const int32_t* slots; const int32_t* pix; const int32_t* n;
+  const float* cache; const uint8_t* cache_ok; long long* cache_t; const uint8_t* W; long long t;
+};
+
+__global__ void __launch_bounds__(256)
+k_backfill(const BackfillArgs a) {
+  const int lane = threadIdx.x & 31;
+  const int wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+  const int cnt = *a.n;
+  const long long N = (long long)a.Dy * a.Dx;
+  for (int i = wid; i < cnt; i += nw) {
+    const int s = a.slots[i];
+    if (a.born[s] != a.t) continue;
+    const int pix = a.pix[i];
+    const int y = pix / a.Dx, x = pix - y * a.Dx;
+    for (int e = 0; e < a.n_back; ++e) {
+      const long long tau = a.cache_t[e];
+      if (tau < 0 || tau < a.t - a.n_back || tau >= a.t) continue;
+      const int col = (int)(tau % a.T_ring);
+      if (a.meta_t[col] != tau) continue;                 // the ring has moved on: that column is a newer frame's
+      const uint8_t* ok = a.cache_ok + (long long)e * (a.B + 1);
+      const bool frame_ok = ok[a.B] != 0;
+      for (int b = lane; b < a.B; b += 32) {
+        float best = 0.f;
+        if (frame_ok && ok[b]) {
+          const float* X = a.cache + ((long long)e * a.B + b) * N;
+          bool any = false;
+          for (int j = -a.r; j <= a.r; ++j) {
+            const int yy = y + j;
+            if (yy < 0 || yy >= a.Dy) continue;
+            for (int k = -a.r; k <= a.r; ++k) {
+              const int xx = x + k;
+              if (xx < 0 || xx >= a.Dx) continue;
+              const long long q = (long long)yy * a.Dx + xx;
+              if (!a.W[q]) continue;
+              const float v = __ldg(X + q);
+              if (!any || v > best) { best = v; any = true; }
+            }
+          }
+          if (!any) best = 0.f;
+        }
+        a.ring[((long long)s * a.T_ring + col) * a.B + b] = best;
+      }
+    }
+  }
+}
+
+// labels cache entry e with frame t (after the copies that fill it were enqueued)
+__global__ void k_cache_label(long long* cache_t, int e, long long t) { cache_t[e] = t; }
+
 __global__ void __launch_bounds__(256)
 k_get_dynspec(const float* __restrict__ ring, const long long* __restrict__ meta_t, int T_ring, int B, int slot,
               long long t_last, float* __restrict__ out) {
@@ -472,6 +527,23 @@ int lpf_launch_append(lpf_ctx* c, const int32_t* d_slots, const int32_t* d_n, co
   const lpf_params& p = c->p;
   LPF_KLAUNCH(c, KID_APPEND, st, k_append<<<c->n_sm, 256, 0, st>>>(
       c->ring, c->meta_t, c->meta_ok, c->born, p.T_ring, p.B, d_slots, d_n, d_flux, d_band_ok, t));
+  return LPF_OK;
+}
+
+int lpf_launch_backfill(lpf_ctx* c, const int32_t* d_slots, const int32_t* d_pix, const int32_t* d_n, const float* d_cube,
+                        const uint8_t* d_band_ok, long long t, cudaStream_t st) {
+  const lpf_params& p = c->p;
+  BackfillArgs a{};
+  a.ring = c->ring; a.meta_t = c->meta_t; a.born = c->born; a.T_ring = p.T_ring; a.B = p.B; a.Dy = p.Dy; a.Dx = p.Dx;
+  a.r = p.r_flux; a.n_back = p.n_back; a.slots = d_slots; a.pix = d_pix; a.n = d_n;
+  a.cache = c->cube_cache; a.cache_ok = c->cache_ok; a.cache_t = c->cache_t; a.W = c->W; a.t = t;
+  LPF_KLAUNCH(c, KID_BACKFILL, st, k_backfill<<<c->n_sm, 256, 0, st>>>(a));
+  // frame t replaces the oldest cached frame (t - n_back), which the kernel above was the last to need
+  const int e = (int)(t % p.n_back);
+  const size_t cube_elems = (size_t)p.B * c->N;
+  LPF_CUDA(cudaMemcpyAsync(c->cube_cache + (size_t)e * cube_elems, d_cube, cube_elems * sizeof(float), cudaMemcpyDeviceToDevice, st));
+  LPF_CUDA(cudaMemcpyAsync(c->cache_ok + (size_t)e * (p.B + 1), d_band_ok, (size_t)p.B + 1, cudaMemcpyDeviceToDevice, st));
+  LPF_KLAUNCH(c, KID_MISC, st, k_cache_label<<<1, 1, 0, st>>>(c->cache_t, e, t));
   return LPF_OK;
 }
 

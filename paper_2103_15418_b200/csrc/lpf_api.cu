@@ -71,6 +71,7 @@ int check_params(const lpf_params* p) {
   if (p->n_iter < 1 || p->n_iter > 255) return LPF_E_ARG;
   if (p->r_flux < 0 || p->r_flux > 8 || p->r_dedupe < 0 || p->r_dedupe > 8 || p->r_assoc < 0 || p->r_assoc > 8) return LPF_E_ARG;
   if (p->n_forget < 1 || p->T_ring < 1 || p->n_cand_max < 1 || p->max_det < 1 || p->n_lanes < 1 || p->n_lanes > 64) return LPF_E_ARG;
+  if (p->n_back < 0 || p->n_back > 64) return LPF_E_ARG;
   if (!(p->eps_rel >= 0) || !(p->qc_tau > 0) || !(p->qc_clip > 0)) return LPF_E_ARG;
   return LPF_OK;
 }
@@ -197,6 +198,12 @@ int lpf_create(lpf_ctx** out, const lpf_params* p, const uint8_t* d_valid_mask) 
   TRYC(dalloc(&c->ring, nc * p->T_ring * p->B));
   TRYC(dalloc(&c->meta_t, (size_t)p->T_ring)); TRYC(dalloc(&c->meta_ok, (size_t)p->T_ring));
   TRYC(dalloc(&c->counters, 8));
+  if (p->n_back > 0) {
+    TRYC(dalloc(&c->cube_cache, (size_t)p->n_back * p->B * N));
+    TRYC(dalloc(&c->cache_ok, (size_t)p->n_back * (p->B + 1)));
+    TRYC(dalloc(&c->cache_t, (size_t)p->n_back));
+    CUDAC(cudaMemset(c->cache_t, 0xff, (size_t)p->n_back * 8));   // -1
+  }
   CUDAC(cudaMemset(c->active, 0, nc)); CUDAC(cudaMemset(c->forced, 0, nc));
   CUDAC(cudaMemset(c->cpix, 0, nc * 4)); CUDAC(cudaMemset(c->miss, 0, nc * 4));
   CUDAC(cudaMemset(c->born, 0xff, nc * 8));       // -1
@@ -222,7 +229,8 @@ int lpf_destroy(lpf_ctx* c) {
   cudaDeviceSynchronize();
   for (auto& L : c->lanes) free_lane(L);
   void* ptrs[] = {c->W, c->norm_mf, c->norm_bg, c->active, c->forced, c->cpix, c->miss, c->born, c->matched_t,
-                  c->slotmap, c->free_list, c->ring, c->meta_t, c->meta_ok, c->counters};
+                  c->slotmap, c->free_list, c->ring, c->meta_t, c->meta_ok, c->counters, c->cube_cache, c->cache_ok,
+                  c->cache_t};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (c->chain_ev) cudaEventDestroy(c->chain_ev);
   lpf_fused_plan_free(c->fused);
@@ -293,6 +301,7 @@ int lpf_process_frame(lpf_ctx* c, int lane, const float* d_cube, int64_t t, void
   TRY(lpf_launch_associate(c, L.upos, L.nu, L.band_ok, (long long)t, L.cand_idx, L.act_slots, L.act_pix, L.npos, st));
   TRY(lpf_launch_measure_flux(c, d_cube, L.band_ok, L.act_pix, L.npos, L.flux, st));
   TRY(lpf_launch_append(c, L.act_slots, L.npos, L.flux, L.band_ok, (long long)t, st));
+  if (c->p.n_back > 0) TRY(lpf_launch_backfill(c, L.act_slots, L.act_pix, L.npos, d_cube, L.band_ok, (long long)t, st));   // O11
   LPF_CUDA(cudaEventRecord(c->chain_ev, st));
   c->chain_valid = true;
   return LPF_OK;
@@ -367,7 +376,7 @@ int lpf_get_counters(lpf_ctx* c, int64_t* h_out) {
 static const char* const kKernelNames[KID_COUNT] = {
     "qc_pass1", "qc_pass2", "qc_verdict", "sum_plane", "conv_mf", "conv_c", "conv_s", "conv_den", "threshold_peaks",
     "fused_detect", "dedupe_scatter", "dedupe_select", "dedupe_sort", "assoc_match", "assoc_update", "measure_flux",
-    "append_dynspec", "misc"};
+    "append_dynspec", "backfill", "misc"};
 
 int lpf_profile_begin(lpf_ctx* c) {
   if (!c) return LPF_E_ARG;

@@ -78,6 +78,10 @@ struct lpf_ctx {
   long long* meta_t = nullptr; // [T_ring]
   unsigned long long* meta_ok = nullptr;
   int32_t* counters = nullptr; // [0] dropped records, [1] dropped detections, [2] active candidates
+  // backward fill (O11): the last n_back cubes, their verdicts and time steps
+  float* cube_cache = nullptr;      // [n_back][B][N]
+  uint8_t* cache_ok = nullptr;      // [n_back][B + 1]
+  long long* cache_t = nullptr;     // [n_back], -1 = empty
   cudaEvent_t chain_ev = nullptr;
   bool chain_valid = false;
   int64_t launches = 0;
@@ -103,7 +107,7 @@ int lpf_cuda_fail(cudaError_t e, const char* what);
 enum LpfKernelId {
   KID_QC_PASS1 = 0, KID_QC_PASS2, KID_QC_VERDICT, KID_SUM_PLANE, KID_CONV_MF, KID_CONV_C, KID_CONV_S,
   KID_CONV_DEN, KID_THRESHOLD, KID_FUSED_DETECT, KID_DEDUPE_SCATTER, KID_DEDUPE_SELECT, KID_DEDUPE_SORT,
-  KID_ASSOC_MATCH, KID_ASSOC_UPDATE, KID_MEASURE_FLUX, KID_APPEND, KID_MISC, KID_COUNT
+  KID_ASSOC_MATCH, KID_ASSOC_UPDATE, KID_MEASURE_FLUX, KID_APPEND, KID_BACKFILL, KID_MISC, KID_COUNT
 };
 void lpf_prof_pre(lpf_ctx* c, int kid, cudaStream_t st);
 void lpf_prof_post(lpf_ctx* c, cudaStream_t st);
@@ -147,6 +151,8 @@ int lpf_launch_measure_flux(lpf_ctx* c, const float* d_cube, const uint8_t* d_ba
                             const int32_t* d_npos, float* d_flux, cudaStream_t st);
 int lpf_launch_append(lpf_ctx* c, const int32_t* d_slots, const int32_t* d_n, const float* d_flux,
                       const uint8_t* d_band_ok, long long t, cudaStream_t st);
+int lpf_launch_backfill(lpf_ctx* c, const int32_t* d_slots, const int32_t* d_pix, const int32_t* d_n, const float* d_cube,
+                        const uint8_t* d_band_ok, long long t, cudaStream_t st);
 int lpf_launch_get_dynspec(lpf_ctx* c, int slot, long long t_last, float* d_out, cudaStream_t st);
 int lpf_launch_fill_nan(lpf_ctx* c, float* d, int64_t n, cudaStream_t st);
 int lpf_launch_fill_i32(lpf_ctx* c, int32_t* d, int64_t n, int32_t v, cudaStream_t st);

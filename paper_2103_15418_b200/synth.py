@@ -139,6 +139,7 @@ def default_params(cfg: int, bg: str = "box", n_iter: int = 1) -> dict:
         n_cand_max={1: 64, 2: 2048, 3: 8192, 4: 32768, 5: 32768}[cfg],
         max_det={1: 1024, 2: 16384, 3: 131072, 4: 524288, 5: 524288}[cfg],
         n_lanes=c.n_lanes,
+        n_back=0,
     )
     return p
 

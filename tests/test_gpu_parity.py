@@ -420,3 +420,38 @@ def test_config3_bench_launch_configuration(torch_cuda):
         assert np.allclose(a["snr"], b["snr"], rtol=1e-4, atol=1e-5) and np.allclose(a["f"], b["f"], rtol=1e-4, atol=1e-5)
         assert np.allclose(v["stats"], views[t]["stats"], rtol=1e-6, atol=1e-6, equal_nan=True)
     seq.close(); lpf.close()
+
+
+@pytest.mark.parametrize("T_ring,n_back", [(128, 8), (6, 12)])
+def test_backward_fill(torch_cuda, T_ring, n_back):
+    """O11: slots created at t are back-filled from the device cache of the last n_back cubes.
+    Every active slot's dynamic spectrum must equal the oracle's bit for bit, including the pre-birth columns,
+    with a rejected band in one cached frame and with a ring shorter than the cache."""
+    torch = torch_cuda
+    s, p, lpf = _make(2, torch, T_ring=T_ring, n_back=n_back)
+    pipe = O.OraclePipeline(p, s.mask, direct=False)
+    n = 26
+    for t in range(n):
+        cube = s.frame(t)
+        if t == 9:
+            cube = cube.copy(); cube[3, 5, 5] = np.nan          # band 3 rejected in this frame
+        o = pipe.step(cube, t)
+        lpf.process_frame(torch.from_numpy(cube).cuda(), t)
+        g = lpf.frame_view(0)
+        assert np.array_equal(g["band_ok"], o["band_ok"]) and np.array_equal(g["upos"], o["upos"])
+        assert np.array_equal(g["cand_idx"], o["cand_idx"]) and np.array_equal(g["act_slots"], o["act_slots"])
+    tb = pipe.table
+    act = np.flatnonzero(tb.active)
+    late = [int(sl) for sl in act if tb.born[sl] > 2]            # born late enough to have something to back-fill
+    assert len(late) >= 2
+    n_pre = 0
+    for sl in act:
+        a = lpf.get_dynspec(int(sl), n - 1).cpu().numpy(); b = tb.dynspec(int(sl), n - 1)
+        assert np.array_equal(np.isnan(a), np.isnan(b)), int(sl)
+        assert np.array_equal(a[~np.isnan(a)], b[~np.isnan(b)]), int(sl)
+        if tb.born[sl] > 2:
+            k = T_ring - 1 - (n - 1 - int(tb.born[sl]))         # column of the birth frame (newest frame is last)
+            if k >= 1:
+                n_pre += int(not np.isnan(b[:, k - 1]).any())
+    assert n_pre >= 1                                             # the build-up columns are really there
+    lpf.close()
