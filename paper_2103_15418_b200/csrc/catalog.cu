@@ -391,7 +391,7 @@ k_append(float* __restrict__ ring, long long* __restrict__ meta_t, unsigned long
 // frame tau in [t - n_back, t - 1] whose ring column still belongs to tau, the O9 flux of that frame at its
 // pixel.  Thread 0 of the grid then labels the cache entry that the caller overwrites with frame t next.
 struct BackfillArgs {
-  float* ring; const long long* meta_t; const long long* born; int T_ring, B, Dy, Dx, r, n_back;
+  float* ring; const long long* meta_t; const long long* born; int T_ring, B, Dy, Dx, r, n_back, depth;
   const int32_t* slots; const int32_t* pix; const int32_t* n;
   const float* cache; const uint8_t* cache_ok; long long* cache_t; const uint8_t* W; long long t;
 };
@@ -402,13 +402,15 @@ k_backfill(const BackfillArgs a) {
   const int wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
   const int cnt = *a.n;
   const long long N = (long long)a.Dy * a.Dx;
-  for (int i = wid; i < cnt; i += nw) {
+  // one warp per (active position, cache entry): the few new slots' loads do not queue up behind each other
+  for (long long job = wid; job < (long long)cnt * a.depth; job += nw) {
+    const int i = (int)(job / a.depth), e = (int)(job - (long long)i * a.depth);
     const int s = a.slots[i];
-    if (a.born[s] != a.t) continue;
+    const long long tau = a.cache_t[e];
     const int pix = a.pix[i];
+    if (a.born[s] != a.t) continue;
     const int y = pix / a.Dx, x = pix - y * a.Dx;
-    for (int e = 0; e < a.n_back; ++e) {
-      const long long tau = a.cache_t[e];
+    {
       if (tau < 0 || tau < a.t - a.n_back || tau >= a.t) continue;
       const int col = (int)(tau % a.T_ring);
       if (a.meta_t[col] != tau) continue;                 // the ring has moved on: that column is a newer frame's
@@ -535,11 +537,18 @@ int lpf_launch_backfill(lpf_ctx* c, const int32_t* d_slots, const int32_t* d_pix
   const lpf_params& p = c->p;
   BackfillArgs a{};
   a.ring = c->ring; a.meta_t = c->meta_t; a.born = c->born; a.T_ring = p.T_ring; a.B = p.B; a.Dy = p.Dy; a.Dx = p.Dx;
-  a.r = p.r_flux; a.n_back = p.n_back; a.slots = d_slots; a.pix = d_pix; a.n = d_n;
+  a.r = p.r_flux; a.n_back = p.n_back; a.depth = p.n_back + p.n_lanes; a.slots = d_slots; a.pix = d_pix; a.n = d_n;
   a.cache = c->cube_cache; a.cache_ok = c->cache_ok; a.cache_t = c->cache_t; a.W = c->W; a.t = t;
-  LPF_KLAUNCH(c, KID_BACKFILL, st, k_backfill<<<c->n_sm, 256, 0, st>>>(a));
-  // frame t replaces the oldest cached frame (t - n_back), which the kernel above was the last to need
-  const int e = (int)(t % p.n_back);
+  LPF_KLAUNCH(c, KID_BACKFILL, st, k_backfill<<<c->n_sm * 2, 256, 0, st>>>(a));
+  return LPF_OK;
+}
+
+// Frame t joins the cache.  The cache holds n_back + n_lanes entries, so the entry that frame t overwrites
+// (frame t - n_back - n_lanes) is older than anything a frame still in flight on another lane back-fills from:
+// the copy needs no ordering against the other lanes and overlaps the lane's own detection kernel.
+int lpf_launch_cache_store(lpf_ctx* c, const float* d_cube, const uint8_t* d_band_ok, long long t, cudaStream_t st) {
+  const lpf_params& p = c->p;
+  const int e = (int)(t % (p.n_back + p.n_lanes));
   const size_t cube_elems = (size_t)p.B * c->N;
   LPF_CUDA(cudaMemcpyAsync(c->cube_cache + (size_t)e * cube_elems, d_cube, cube_elems * sizeof(float), cudaMemcpyDeviceToDevice, st));
   LPF_CUDA(cudaMemcpyAsync(c->cache_ok + (size_t)e * (p.B + 1), d_band_ok, (size_t)p.B + 1, cudaMemcpyDeviceToDevice, st));

@@ -199,10 +199,11 @@ int lpf_create(lpf_ctx** out, const lpf_params* p, const uint8_t* d_valid_mask) 
   TRYC(dalloc(&c->meta_t, (size_t)p->T_ring)); TRYC(dalloc(&c->meta_ok, (size_t)p->T_ring));
   TRYC(dalloc(&c->counters, 8));
   if (p->n_back > 0) {
-    TRYC(dalloc(&c->cube_cache, (size_t)p->n_back * p->B * N));
-    TRYC(dalloc(&c->cache_ok, (size_t)p->n_back * (p->B + 1)));
-    TRYC(dalloc(&c->cache_t, (size_t)p->n_back));
-    CUDAC(cudaMemset(c->cache_t, 0xff, (size_t)p->n_back * 8));   // -1
+    const size_t depth = (size_t)p->n_back + p->n_lanes;
+    TRYC(dalloc(&c->cube_cache, depth * p->B * N));
+    TRYC(dalloc(&c->cache_ok, depth * (p->B + 1)));
+    TRYC(dalloc(&c->cache_t, depth));
+    CUDAC(cudaMemset(c->cache_t, 0xff, depth * 8));   // -1
   }
   CUDAC(cudaMemset(c->active, 0, nc)); CUDAC(cudaMemset(c->forced, 0, nc));
   CUDAC(cudaMemset(c->cpix, 0, nc * 4)); CUDAC(cudaMemset(c->miss, 0, nc * 4));
@@ -294,6 +295,7 @@ int lpf_process_frame(lpf_ctx* c, int lane, const float* d_cube, int64_t t, void
   cudaStream_t st = (cudaStream_t)stream;
   LpfLane& L = c->lanes[lane];
   TRY(lpf_launch_qc_sum(c, L, d_cube, L.stats, L.band_ok, L.ndets, st));      // S1-S3, one kernel per pass over the cube
+  if (c->p.n_back > 0) TRY(lpf_launch_cache_store(c, d_cube, L.band_ok, (long long)t, st));   // O11: the frame joins the cache
   TRY(lpf_launch_detect(c, L, d_cube, L.band_ok, L.dets, L.ndets, true, st));
   TRY(lpf_launch_dedupe(c, L, L.dets, L.ndets, L.upos, L.uplane, L.usnr, L.nu, st));
   // the candidate table and the rings are shared by all lanes: order the chain across streams

@@ -79,9 +79,9 @@ struct lpf_ctx {
   unsigned long long* meta_ok = nullptr;
   int32_t* counters = nullptr; // [0] dropped records, [1] dropped detections, [2] active candidates
   // backward fill (O11): the last n_back cubes, their verdicts and time steps
-  float* cube_cache = nullptr;      // [n_back][B][N]
-  uint8_t* cache_ok = nullptr;      // [n_back][B + 1]
-  long long* cache_t = nullptr;     // [n_back], -1 = empty
+  float* cube_cache = nullptr;      // [n_back + n_lanes][B][N]
+  uint8_t* cache_ok = nullptr;      // [n_back + n_lanes][B + 1]
+  long long* cache_t = nullptr;     // [n_back + n_lanes], -1 = empty
   cudaEvent_t chain_ev = nullptr;
   bool chain_valid = false;
   int64_t launches = 0;
@@ -153,6 +153,7 @@ int lpf_launch_append(lpf_ctx* c, const int32_t* d_slots, const int32_t* d_n, co
                       const uint8_t* d_band_ok, long long t, cudaStream_t st);
 int lpf_launch_backfill(lpf_ctx* c, const int32_t* d_slots, const int32_t* d_pix, const int32_t* d_n, const float* d_cube,
                         const uint8_t* d_band_ok, long long t, cudaStream_t st);
+int lpf_launch_cache_store(lpf_ctx* c, const float* d_cube, const uint8_t* d_band_ok, long long t, cudaStream_t st);
 int lpf_launch_get_dynspec(lpf_ctx* c, int slot, long long t_last, float* d_out, cudaStream_t st);
 int lpf_launch_fill_nan(lpf_ctx* c, float* d, int64_t n, cudaStream_t st);
 int lpf_launch_fill_i32(lpf_ctx* c, int32_t* d, int64_t n, int32_t v, cudaStream_t st);

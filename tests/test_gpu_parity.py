@@ -455,3 +455,31 @@ def test_backward_fill(torch_cuda, T_ring, n_back):
                 n_pre += int(not np.isnan(b[:, k - 1]).any())
     assert n_pre >= 1                                             # the build-up columns are really there
     lpf.close()
+
+
+def test_backward_fill_with_lanes_in_flight(torch_cuda):
+    """O11 with four frames in flight: the cache holds n_back + n_lanes cubes, so a lane's early copy into the
+    cache never overwrites a cube that a frame still in flight on another lane back-fills from."""
+    torch = torch_cuda
+    L, n_back, n = 4, 3, 24
+    s, p, lpf = _make(2, torch, T_ring=32, n_back=n_back, n_lanes=L)
+    pipe = O.OraclePipeline(p, s.mask, direct=False)
+    streams = [torch.cuda.Stream() for _ in range(L)]
+    cubes = [s.frame(t) for t in range(n)]
+    dcubes = [torch.from_numpy(c).cuda() for c in cubes]
+    torch.cuda.synchronize()
+    for t0 in range(0, n, L):
+        for k in range(L):
+            lpf.process_frame(dcubes[t0 + k], t0 + k, lane=k, stream=streams[k])
+        torch.cuda.synchronize()
+        for k in range(L):
+            o = pipe.step(cubes[t0 + k], t0 + k)
+            g = lpf.frame_view(k)
+            assert np.array_equal(g["upos"], o["upos"]) and np.array_equal(g["cand_idx"], o["cand_idx"])
+            assert np.array_equal(g["act_slots"], o["act_slots"]) and np.array_equal(g["flux"], o["flux"])
+    tb = pipe.table
+    for sl in np.flatnonzero(tb.active):
+        a = lpf.get_dynspec(int(sl), n - 1).cpu().numpy(); b = tb.dynspec(int(sl), n - 1)
+        assert np.array_equal(np.isnan(a), np.isnan(b)), int(sl)
+        assert np.array_equal(a[~np.isnan(a)], b[~np.isnan(b)]), int(sl)
+    lpf.close()
