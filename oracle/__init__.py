@@ -150,6 +150,51 @@ def measure_flux(cube, band_ok, W, pos, r_flux: int) -> np.ndarray:
     return out
 
 
+class RunningQC:
+    """O12, per-pixel running quality control (eq. A.2; R22).
+
+    State per band and pixel: running mean m and variance v of the image stream (Welford 1962 while the band
+    has fewer than `window` updates, exponentially weighted after that, Finch 2009), and the number of
+    updates n_b.  For a frame: zeta = (x - m) / sqrt(v) (eq. A.2) at every valid pixel of every band with
+    n_b >= warm; the band is discarded when more than `nmax` pixels have |zeta| > thr (nmax = 0: the
+    paper's "if zeta exceeds a threshold").  The test comes before the update, and only bands that survive
+    both eq. A.1 and eq. A.2 update their state.  The test is a floating-point decision, so it is taken in
+    float32 with the kernel's operation order (each operation rounded once, no fused multiply-add):
+    d = x - m;  exceeds  <=>  d*d > thr^2 * v;  update: a = 1/min(n_b + 1, window), m += a*d,
+    v = (1 - a) * (v + (a*d)*d).
+    """
+
+    def __init__(self, B: int, Dy: int, Dx: int, thr: float, nmax: int, window: int, warm: int):
+        self.thr2 = np.float32(np.float32(thr) * np.float32(thr)); self.nmax = int(nmax)
+        self.window = int(window); self.warm = int(warm)
+        self.m = np.zeros((B, Dy, Dx), np.float32); self.v = np.zeros((B, Dy, Dx), np.float32)
+        self.n = np.zeros(B, np.int32)
+
+    def step(self, cube, W, band_ok):
+        """band_ok: [B+1] after eq. A.1.  Returns (counts [B] int32, band_ok' [B+1])."""
+        cube = np.asarray(cube, np.float32)
+        B = cube.shape[0]
+        ok = np.array(band_ok, np.uint8, copy=True)
+        cnt = np.zeros(B, np.int32)
+        valid = np.ones(cube.shape[1:], bool) if W is None else (np.asarray(W) != 0)
+        for b in range(B):
+            with np.errstate(invalid="ignore", over="ignore"):
+                d = cube[b] - self.m[b]
+                if self.n[b] >= self.warm:
+                    exceeds = (d * d) > (self.thr2 * self.v[b])
+                    cnt[b] = int(np.count_nonzero(exceeds & valid))
+                    if cnt[b] > self.nmax:
+                        ok[b] = 0
+                if ok[b]:
+                    a = np.float32(1.0) / np.float32(min(int(self.n[b]) + 1, self.window))
+                    ad = a * d
+                    self.m[b] = self.m[b] + ad
+                    self.v[b] = (np.float32(1.0) - a) * (self.v[b] + ad * d)
+                    self.n[b] += 1
+        ok[B] = 1 if int(ok[:B].sum()) >= (B + 1) // 2 else 0
+        return cnt, ok
+
+
 class CandidateTable:
     """O8 + O10 state: candidate table and dynamic-spectrum rings."""
 
@@ -218,12 +263,19 @@ class OraclePipeline:
         p = self.p
         self.table = CandidateTable(p["n_cand_max"], p["T_ring"], p["B"], p["Dx"], p["r_assoc"], p["n_forget"])
         self.n_back = int(p.get("n_back", 0))
+        self.rq = None
+        if float(p.get("zeta_thr", 0.0)) > 0:
+            self.rq = RunningQC(p["B"], p["Dy"], p["Dx"], p["zeta_thr"], p.get("zeta_nmax", 0), p.get("zeta_window", 64),
+                                p.get("zeta_warm", 8))
+        self.zeta_cnt = np.zeros(p["B"], np.int32)
         self.history = []   # O11: the last n_back frames as (t, cube, band_ok)
 
     # -- steps ---------------------------------------------------------------
     def cube_qc(self, cube):
         st = band_stats(cube, self.W, self.p["qc_clip"])
         z, ok = qc_verdict(st, self.p["qc_tau"])
+        if self.rq is not None:                       # eq. A.2 after eq. A.1 (O12)
+            self.zeta_cnt, ok = self.rq.step(cube, self.W, ok)
         return np.concatenate([st, z], axis=1), ok  # [B][8], [B+1]
 
     def detect(self, cube, band_ok, keep_planes: bool = False):
@@ -283,5 +335,6 @@ class OraclePipeline:
         flux = measure_flux(cube, ok, self.W, act_p, p["r_flux"])
         self.table.append(act_s, flux, ok, t)
         self.backfill(cube, ok, t)
+        det.update(zeta_cnt=self.zeta_cnt.copy())
         det.update(stats=stats, band_ok=ok, cand_idx=cand, act_slots=act_s, act_pix=act_p, flux=flux)
         return det

@@ -724,3 +724,69 @@ def test_backward_fill_respects_rejected_bands_and_ring_age():
     for tau in (t_d - 2, t_d - 1, t_d):
         want = np.array([cubes[tau][b, y - 1:y + 2, x - 1:x + 2].max() for b in range(B)], np.float32)
         assert np.array_equal(ring[tau % 3], want)
+
+
+# ------------------------------------------------------------------ O12 running per-pixel QC (eq. A.2)
+def test_running_qc_is_welford_then_exponential():
+    import oracle as O
+    rng = np.random.default_rng(11)
+    B, D, Nw = 2, 8, 16
+    rq = O.RunningQC(B, D, D, thr=1e9, nmax=0, window=Nw, warm=4)
+    frames = [(3.0 + 2.0 * rng.standard_normal((B, D, D))).astype(np.float32) for _ in range(Nw)]
+    ok = np.ones(B + 1, np.uint8)
+    for k, f in enumerate(frames):
+        cnt, ok2 = rq.step(f, None, ok)
+        assert ok2.all() and not cnt.any()
+        st = np.stack(frames[:k + 1]).astype(np.float64)
+        # Welford (1962): after k+1 <= window updates the state IS the sample mean and the population variance
+        assert np.allclose(rq.m, st.mean(0), rtol=2e-6, atol=2e-6)
+        assert np.allclose(rq.v, st.var(0), rtol=2e-5, atol=2e-6)
+    assert (rq.n == Nw).all()
+    # Finch (2009): from here on alpha = 1/window; a step of height h is followed as h (1 - (1 - alpha)^k)
+    base = rq.m.copy()
+    h = np.float32(5.0)
+    for k in range(1, 9):
+        rq.step(base + h, None, ok)
+        assert np.allclose(rq.m - base, h * (1.0 - (1.0 - 1.0 / Nw) ** k), rtol=1e-5, atol=1e-5)
+
+
+def test_running_qc_verdict_rules():
+    import oracle as O
+    rng = np.random.default_rng(12)
+    B, D = 4, 16
+    W = np.ones((D, D), np.uint8); W[0, :] = 0
+    mk = lambda: rng.standard_normal((B, D, D)).astype(np.float32)
+    rq = O.RunningQC(B, D, D, thr=15.0, nmax=0, window=32, warm=8)
+    ok = np.ones(B + 1, np.uint8)
+    for t in range(8):
+        f = mk()
+        if t == 3:
+            f[1, 5, 5] = 1e4                      # before the warm-up is over nothing is tested
+        cnt, o = rq.step(f, W, ok)
+        assert o.all() and not cnt.any()
+    for _ in range(20):
+        rq.step(mk(), W, ok)                      # let the spike of t = 3 decay out of band 1's variance
+    f = mk(); f[2, 7, 9] += 200.0; f[3, 0, 4] += 200.0      # a spike at a valid pixel, one at a masked pixel
+    before = (rq.m.copy(), rq.v.copy(), rq.n.copy())
+    cnt, o = rq.step(f, W, ok)
+    assert cnt.tolist() == [0, 0, 1, 0] and o.tolist() == [1, 1, 0, 1, 1]
+    # the discarded band keeps its state (test before update, update only accepted bands); the others moved on
+    assert np.array_equal(rq.m[2], before[0][2]) and np.array_equal(rq.v[2], before[1][2]) and rq.n[2] == before[2][2]
+    assert not np.array_equal(rq.m[0], before[0][0]) and rq.n[0] == before[2][0] + 1
+    # count rule: with nmax = 1 the same frame passes; bands rejected by eq. A.1 are neither tested away nor updated
+    rq2 = O.RunningQC(B, D, D, thr=15.0, nmax=1, window=32, warm=8)
+    for _ in range(10):
+        rq2.step(mk(), W, ok)
+    f = mk(); f[2, 7, 9] += 200.0
+    cnt, o = rq2.step(f, W, ok)
+    assert cnt[2] == 1 and o.all()
+    a1 = np.array([1, 0, 0, 1, 1], np.uint8)     # two bands already rejected by eq. A.1
+    n0 = rq2.n.copy()
+    cnt, o = rq2.step(mk(), W, a1)
+    assert o.tolist() == [1, 0, 0, 1, 1] and (rq2.n - n0).tolist() == [1, 0, 0, 1]
+    f = mk(); f[0, 3, 3] += 500.0
+    cnt, o = rq2.step(f, W, a1)                   # one spike: passes (nmax = 1)
+    assert o[0] == 1
+    f = mk(); f[0, 8, 8] += 500.0; f[0, 9, 2] += 500.0
+    cnt, o = rq2.step(f, W, a1)
+    assert cnt[0] == 2 and o.tolist() == [0, 0, 0, 1, 0]       # one accepted band of four: the frame is rejected
