@@ -157,6 +157,8 @@ def run_ours(args):
     p = synth.default_params(cfg, bg=args.bg, n_iter=args.n_iter)
     p["n_lanes"] = args.lanes
     p["n_back"] = args.n_back
+    if args.zeta > 0:
+        p.update(zeta_thr=args.zeta, zeta_nmax=8, zeta_window=64, zeta_warm=16)
     B, D = p["B"], p["Dy"]
     N = D * D
     cube_bytes = 4 * B * N
@@ -299,7 +301,7 @@ def run_ours(args):
         "metric": METRIC, "value": frames_s, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": s.c.name, "cube": [B, D, D], "bg_kernel": args.bg, "n_iter": args.n_iter, "lanes": lanes, "n_back": args.n_back,
+        "config": {"workload": s.c.name, "cube": [B, D, D], "bg_kernel": args.bg, "n_iter": args.n_iter, "lanes": lanes, "n_back": args.n_back, "zeta_thr": args.zeta,
                    "pool_frames": n_pool, "pool_bytes": n_pool * cube_bytes,
                    "l2": "inputs larger than L2 (pool cycled, %d MB)" % (n_pool * cube_bytes >> 20),
                    "parallelism": "independent streams per GPU, no data-path collective" if world > 1 else "1 GPU"},
@@ -398,6 +400,8 @@ def main():
     ap.add_argument("--pool", type=int, default=16)
     ap.add_argument("--n-back", dest="n_back", type=int, default=0,
                     help="backward fill from a device cache of the last n cubes (SURVEY 8(f1)); 0 = off (headline)")
+    ap.add_argument("--zeta", type=float, default=0.0,
+                    help="threshold of the per-pixel running QC of eq. A.2 (SURVEY 8(f2)); 0 = off (headline)")
     ap.add_argument("--e2e-steps", type=int, default=64)
     ap.add_argument("--e2e-lanes", dest="e2e_lanes", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")

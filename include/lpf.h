@@ -78,6 +78,11 @@ typedef struct {
   int32_t n_lanes;          /* frames in flight */
   int32_t n_back;           /* backward fill: a slot created at t also gets the fluxes of the last n_back
                              * cubes, which lpf_process_frame then keeps in a device cache; 0 = off, <= 64 */
+  float zeta_thr;           /* eq. A.2: per-pixel running mean / variance of every band; a band with more
+                             * than zeta_nmax valid pixels at |x - mean| > zeta_thr * sqrt(var) is discarded; 0 = off */
+  int32_t zeta_nmax;        /* 0 = the paper's "if zeta exceeds a threshold" */
+  int32_t zeta_window;      /* Welford up to this many updates, exponentially weighted (alpha = 1/window) after */
+  int32_t zeta_warm;        /* no test before a band has had this many updates */
 } lpf_params;
 
 /* One peak (eq. 7: p = q and y) of one plane.  24 bytes. */
@@ -106,6 +111,7 @@ typedef struct {
   const int32_t* d_act_pix;  /* [npos] their pixels */
   const int32_t* d_npos;     /* [1] */
   const float* d_flux;       /* [npos][B] */
+  const int32_t* d_zeta_cnt; /* [B] pixels over the eq. A.2 threshold in this frame (zeros when the test is off) */
 } lpf_frame_view;
 
 /* Host-side result sizes / pointers for lpf_process_frame_host (all HOST memory, caller-owned). */

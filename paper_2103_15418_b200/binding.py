@@ -30,13 +30,14 @@ class LpfParams(C.Structure):
         ("r_flux", C.c_int32), ("r_dedupe", C.c_int32), ("r_assoc", C.c_int32), ("n_forget", C.c_int32),
         ("T_ring", C.c_int32), ("n_cand_max", C.c_int32), ("max_det", C.c_int32), ("n_lanes", C.c_int32),
         ("n_back", C.c_int32),
+        ("zeta_thr", C.c_float), ("zeta_nmax", C.c_int32), ("zeta_window", C.c_int32), ("zeta_warm", C.c_int32),
     ]
 
 
 class LpfFrameView(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in (
         "d_stats", "d_band_ok", "d_dets", "d_ndets", "d_upos", "d_uplane", "d_usnr", "d_nu", "d_cand_idx",
-        "d_act_slots", "d_act_pix", "d_npos", "d_flux")]
+        "d_act_slots", "d_act_pix", "d_npos", "d_flux", "d_zeta_cnt")]
 
 
 class LpfHostResult(C.Structure):
@@ -245,6 +246,7 @@ class LPF:
             cand_idx=rd(v.d_cand_idx, nu, np.int32),
             act_slots=rd(v.d_act_slots, npos, np.int32), act_pix=rd(v.d_act_pix, npos, np.int32),
             flux=rd(v.d_flux, npos * B, np.float32).reshape(npos, B),
+            zeta_cnt=rd(v.d_zeta_cnt, B, np.int32),
         )
 
     def process_frame_host(self, h_cube, t: int, res: "HostResult", lane: int = 0, stream=None):

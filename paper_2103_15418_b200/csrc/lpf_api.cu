@@ -72,6 +72,8 @@ int check_params(const lpf_params* p) {
   if (p->r_flux < 0 || p->r_flux > 8 || p->r_dedupe < 0 || p->r_dedupe > 8 || p->r_assoc < 0 || p->r_assoc > 8) return LPF_E_ARG;
   if (p->n_forget < 1 || p->T_ring < 1 || p->n_cand_max < 1 || p->max_det < 1 || p->n_lanes < 1 || p->n_lanes > 64) return LPF_E_ARG;
   if (p->n_back < 0 || p->n_back > 64) return LPF_E_ARG;
+  if (!(p->zeta_thr >= 0)) return LPF_E_ARG;
+  if (p->zeta_thr > 0 && (p->zeta_nmax < 0 || p->zeta_window < 1 || p->zeta_warm < 1)) return LPF_E_ARG;
   if (!(p->eps_rel >= 0) || !(p->qc_tau > 0) || !(p->qc_clip > 0)) return LPF_E_ARG;
   return LPF_OK;
 }
@@ -98,6 +100,8 @@ int alloc_lane(lpf_ctx* c, LpfLane& L) {
   TRY(dalloc(&L.tmp_snr, (size_t)p.max_det));
   TRY(dalloc(&L.tmp_n, 1));
   TRY(dalloc(&L.stats, (size_t)p.B * LPF_STATS_PER_BAND));
+  TRY(dalloc(&L.zeta_cnt, (size_t)p.B));
+  LPF_CUDA(cudaMemset(L.zeta_cnt, 0, (size_t)p.B * sizeof(int32_t)));
   TRY(dalloc(&L.band_ok, (size_t)p.B + 1));
   TRY(dalloc(&L.dets, (size_t)p.max_det));
   TRY(dalloc(&L.ndets, 1));
@@ -120,7 +124,7 @@ int alloc_lane(lpf_ctx* c, LpfLane& L) {
 void free_lane(LpfLane& L) {
   void* ptrs[] = {L.qc_part1, L.qc_part2, L.qc_band_clip, L.qc_counter, L.sum_plane, L.dirty, L.F, L.C, L.S, L.Y, L.normp, L.M, L.tmp_pos, L.tmp_plane,
                   L.tmp_snr, L.tmp_n, L.stats, L.band_ok, L.dets, L.ndets, L.upos, L.uplane, L.usnr, L.nu,
-                  L.cand_idx, L.act_slots, L.act_pix, L.npos, L.flux, L.cube};
+                  L.cand_idx, L.act_slots, L.act_pix, L.npos, L.flux, L.cube, L.zeta_cnt};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (L.h_counts) cudaFreeHost(L.h_counts);
   L = LpfLane();
@@ -198,6 +202,15 @@ int lpf_create(lpf_ctx** out, const lpf_params* p, const uint8_t* d_valid_mask) 
   TRYC(dalloc(&c->ring, nc * p->T_ring * p->B));
   TRYC(dalloc(&c->meta_t, (size_t)p->T_ring)); TRYC(dalloc(&c->meta_ok, (size_t)p->T_ring));
   TRYC(dalloc(&c->counters, 8));
+  if (p->zeta_thr > 0) {
+    TRYC(dalloc(&c->rq_m, 2 * (size_t)p->B * N));
+    TRYC(dalloc(&c->rq_v, 2 * (size_t)p->B * N));
+    TRYC(dalloc(&c->rq_state, 3 * (size_t)p->B + 1));
+    CUDAC(cudaMemset(c->rq_m, 0, 2 * (size_t)p->B * N * sizeof(float)));
+    CUDAC(cudaMemset(c->rq_v, 0, 2 * (size_t)p->B * N * sizeof(float)));
+    CUDAC(cudaMemset(c->rq_state, 0, (3 * (size_t)p->B + 1) * sizeof(int32_t)));
+    CUDAC(cudaEventCreateWithFlags(&c->rq_ev, cudaEventDisableTiming));
+  }
   if (p->n_back > 0) {
     const size_t depth = (size_t)p->n_back + p->n_lanes;
     TRYC(dalloc(&c->cube_cache, depth * p->B * N));
@@ -231,9 +244,10 @@ int lpf_destroy(lpf_ctx* c) {
   for (auto& L : c->lanes) free_lane(L);
   void* ptrs[] = {c->W, c->norm_mf, c->norm_bg, c->active, c->forced, c->cpix, c->miss, c->born, c->matched_t,
                   c->slotmap, c->free_list, c->ring, c->meta_t, c->meta_ok, c->counters, c->cube_cache, c->cache_ok,
-                  c->cache_t};
+                  c->cache_t, c->rq_m, c->rq_v, c->rq_state};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (c->chain_ev) cudaEventDestroy(c->chain_ev);
+  if (c->rq_ev) cudaEventDestroy(c->rq_ev);
   lpf_fused_plan_free(c->fused);
   for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
   delete c;
@@ -316,6 +330,7 @@ int lpf_get_frame_view(lpf_ctx* c, int lane, lpf_frame_view* v) {
   v->d_stats = L.stats; v->d_band_ok = L.band_ok; v->d_dets = L.dets; v->d_ndets = L.ndets;
   v->d_upos = L.upos; v->d_uplane = L.uplane; v->d_usnr = L.usnr; v->d_nu = L.nu; v->d_cand_idx = L.cand_idx;
   v->d_act_slots = L.act_slots; v->d_act_pix = L.act_pix; v->d_npos = L.npos; v->d_flux = L.flux;
+  v->d_zeta_cnt = L.zeta_cnt;
   return LPF_OK;
 }
 
@@ -376,7 +391,7 @@ int lpf_get_counters(lpf_ctx* c, int64_t* h_out) {
 }
 
 static const char* const kKernelNames[KID_COUNT] = {
-    "qc_pass1", "qc_pass2", "qc_verdict", "sum_plane", "conv_mf", "conv_c", "conv_s", "conv_den", "threshold_peaks",
+    "qc_pass1", "qc_pass2", "qc_running", "sum_plane", "conv_mf", "conv_c", "conv_s", "conv_den", "threshold_peaks",
     "fused_detect", "dedupe_scatter", "dedupe_select", "dedupe_sort", "assoc_match", "assoc_update", "measure_flux",
     "append_dynspec", "backfill", "misc"};
 

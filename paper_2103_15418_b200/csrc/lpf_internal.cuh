@@ -48,6 +48,7 @@ struct LpfLane {
   int32_t* npos = nullptr;
   float* flux = nullptr;
   float* cube = nullptr;       // device cube for the *_host entry (lazy)
+  int32_t* zeta_cnt = nullptr; // [B] eq. A.2 counts of the lane's frame
   int32_t* h_counts = nullptr; // pinned [4]
 };
 
@@ -78,6 +79,13 @@ struct lpf_ctx {
   long long* meta_t = nullptr; // [T_ring]
   unsigned long long* meta_ok = nullptr;
   int32_t* counters = nullptr; // [0] dropped records, [1] dropped detections, [2] active candidates
+  // running per-pixel QC (O12, eq. A.2): two copies of the mean / variance images (the update of a frame is written
+  // to the other copy and adopted per band only if the band is accepted), update counts, scratch
+  float* rq_m = nullptr;            // [2][B][N]
+  float* rq_v = nullptr;            // [2][B][N]
+  int32_t* rq_state = nullptr;      // [B] current copy, [B] updates so far, [B] counts of the frame in progress, [1] block counter
+  cudaEvent_t rq_ev = nullptr;      // orders the frames' updates across lanes
+  bool rq_valid = false;
   // backward fill (O11): the last n_back cubes, their verdicts and time steps
   float* cube_cache = nullptr;      // [n_back + n_lanes][B][N]
   uint8_t* cache_ok = nullptr;      // [n_back + n_lanes][B + 1]
@@ -105,7 +113,7 @@ int lpf_cuda_fail(cudaError_t e, const char* what);
 
 // Kernel ids for the optional per-kernel CUDA-event profile (lpf_profile_begin / lpf_profile_end).
 enum LpfKernelId {
-  KID_QC_PASS1 = 0, KID_QC_PASS2, KID_QC_VERDICT, KID_SUM_PLANE, KID_CONV_MF, KID_CONV_C, KID_CONV_S,
+  KID_QC_PASS1 = 0, KID_QC_PASS2, KID_QC_VERDICT /* = the running per-pixel test, eq. A.2 */, KID_SUM_PLANE, KID_CONV_MF, KID_CONV_C, KID_CONV_S,
   KID_CONV_DEN, KID_THRESHOLD, KID_FUSED_DETECT, KID_DEDUPE_SCATTER, KID_DEDUPE_SELECT, KID_DEDUPE_SORT,
   KID_ASSOC_MATCH, KID_ASSOC_UPDATE, KID_MEASURE_FLUX, KID_APPEND, KID_BACKFILL, KID_MISC, KID_COUNT
 };
@@ -128,6 +136,7 @@ int lpf_launch_qc(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, u
 int lpf_launch_qc_sum(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, int32_t* zero_me,
                       cudaStream_t st);
 int lpf_qc2_blocks(const lpf_ctx* c);
+int lpf_launch_qc_running(lpf_ctx* c, LpfLane& L, const float* d_cube, uint8_t* d_band_ok, cudaStream_t st);
 
 int lpf_launch_sum_plane(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, bool want_sum, cudaStream_t st);
 int lpf_launch_detect_general(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok,

@@ -354,6 +354,95 @@ k_qc_pass2(const Qc2Args a) {
   }
 }
 
+// ---- O12: per-pixel running quality control (eq. A.2; R22) -------------------
+// One block per (chunk, band).  zeta = (x - mean) / sqrt(var) is tested as d*d > thr^2 * var with every
+// operation rounded once (no fused multiply-add: the oracle takes the same float32 decision); the Welford /
+// exponentially weighted update of the frame is written to the OTHER copy of the state and adopted per band by
+// the last block, which also folds the verdict into band_ok / frame_ok ("test before update, update only
+// accepted bands").
+struct RqArgs {
+  const float* cube; const uint8_t* W; long long N; int B, nblk;
+  float* m; float* v;            // [2][B][N]
+  int32_t* cur; int32_t* nupd; int32_t* cnt; int32_t* counter;   // [B], [B], [B], [1]
+  float thr2; int nmax, window, warm;
+  uint8_t* band_ok; int32_t* zeta_cnt;
+};
+
+__device__ __forceinline__ void rq_pixel(float x, float m, float v, bool test, float a, float one_m_a, float thr2,
+                                         float& m2, float& v2, int& hits) {
+  const float d = __fsub_rn(x, m);
+  if (test && __fmul_rn(d, d) > __fmul_rn(thr2, v)) ++hits;
+  const float ad = __fmul_rn(a, d);
+  m2 = __fadd_rn(m, ad);
+  v2 = __fmul_rn(one_m_a, __fadd_rn(v, __fmul_rn(ad, d)));
+}
+
+__global__ void __launch_bounds__(QC_THREADS)
+k_qc_running(const RqArgs a) {
+  __shared__ int s_hits[QC_WARPS];
+  const int b = blockIdx.y, nblk = a.nblk;
+  const long long N = a.N;
+  const int cur = a.cur[b], nup = a.nupd[b];
+  const bool tested = nup >= a.warm;
+  const int k = nup + 1 < a.window ? nup + 1 : a.window;
+  const float al = __fdiv_rn(1.0f, (float)k), oma = __fsub_rn(1.0f, al);
+  const float* X = a.cube + (long long)b * N;
+  const float* m0 = a.m + ((long long)cur * a.B + b) * N;
+  const float* v0 = a.v + ((long long)cur * a.B + b) * N;
+  float* m1 = a.m + ((long long)(cur ^ 1) * a.B + b) * N;
+  float* v1 = a.v + ((long long)(cur ^ 1) * a.B + b) * N;
+  const long long n4 = (N + 3) >> 2;
+  const long long per = (n4 + nblk - 1) / nblk;
+  const long long q0 = (long long)blockIdx.x * per;
+  const long long q1 = (q0 + per < n4) ? q0 + per : n4;
+  const bool vec = ((N & 3) == 0) && ((((uintptr_t)a.cube) & 15) == 0);
+  int hits = 0;
+  if (vec) {
+    for (long long q = q0 + threadIdx.x; q < q1; q += QC_THREADS) {
+      const float4 x = __ldg(reinterpret_cast<const float4*>(X) + q);
+      const float4 m = *(reinterpret_cast<const float4*>(m0) + q), v = *(reinterpret_cast<const float4*>(v0) + q);
+      const unsigned wm = __ldg(reinterpret_cast<const unsigned*>(a.W) + q);
+      float4 m2, v2;
+      rq_pixel(x.x, m.x, v.x, tested && (wm & 0x000000ffu), al, oma, a.thr2, m2.x, v2.x, hits);
+      rq_pixel(x.y, m.y, v.y, tested && (wm & 0x0000ff00u), al, oma, a.thr2, m2.y, v2.y, hits);
+      rq_pixel(x.z, m.z, v.z, tested && (wm & 0x00ff0000u), al, oma, a.thr2, m2.z, v2.z, hits);
+      rq_pixel(x.w, m.w, v.w, tested && (wm & 0xff000000u), al, oma, a.thr2, m2.w, v2.w, hits);
+      *(reinterpret_cast<float4*>(m1) + q) = m2; *(reinterpret_cast<float4*>(v1) + q) = v2;
+    }
+  } else {
+    for (long long i = (q0 << 2) + threadIdx.x; i < (q1 << 2) && i < N; i += QC_THREADS) {
+      float m2, v2;
+      rq_pixel(X[i], m0[i], v0[i], tested && a.W[i] != 0, al, oma, a.thr2, m2, v2, hits);
+      m1[i] = m2; v1[i] = v2;
+    }
+  }
+  hits = lpf_warp_sum(hits);
+  if ((threadIdx.x & 31) == 0) s_hits[threadIdx.x >> 5] = hits;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int t = 0;
+    for (int w = 0; w < QC_WARPS; ++w) t += s_hits[w];
+    if (t) atomicAdd(&a.cnt[b], t);
+  }
+  if (!last_block_done(a.counter, gridDim.x * gridDim.y)) return;
+  __shared__ int s_nok;
+  if (threadIdx.x == 0) s_nok = 0;
+  __syncthreads();
+  if (threadIdx.x < a.B) {
+    const int bb = threadIdx.x;
+    const int c = __ldcg(&a.cnt[bb]);
+    const int nu = a.nupd[bb];
+    int ok = a.band_ok[bb];
+    if (nu >= a.warm && c > a.nmax) ok = 0;          // eq. A.2
+    if (ok) { a.cur[bb] ^= 1; a.nupd[bb] = nu + 1; atomicAdd(&s_nok, 1); }
+    a.band_ok[bb] = (uint8_t)ok;
+    a.zeta_cnt[bb] = c;
+    a.cnt[bb] = 0;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) a.band_ok[a.B] = (s_nok >= (a.B + 1) / 2) ? 1 : 0;
+}
+
 }  // namespace
 
 static Qc2Args make_qc2(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, float* d_stats, bool want_sum,
@@ -382,9 +471,30 @@ int lpf_qc2_blocks(const lpf_ctx* c) {
   return (int)(chunks < 1 ? 1 : (chunks < cap ? chunks : cap));
 }
 
+// O12 between the two passes (when zeta_thr > 0).  The state is one recurrence over the frames, so the calls of
+// different lanes are ordered by an event.
+int lpf_launch_qc_running(lpf_ctx* c, LpfLane& L, const float* d_cube, uint8_t* d_band_ok, cudaStream_t st) {
+  const lpf_params& p = c->p;
+  if (!(p.zeta_thr > 0)) return LPF_OK;
+  if (c->rq_valid) LPF_CUDA(cudaStreamWaitEvent(st, c->rq_ev, 0));
+  RqArgs a{};
+  a.cube = d_cube; a.W = c->W; a.N = c->N; a.B = p.B; a.nblk = c->qc_nblk;
+  a.m = c->rq_m; a.v = c->rq_v; a.cur = c->rq_state; a.nupd = c->rq_state + p.B; a.cnt = c->rq_state + 2 * p.B;
+  a.counter = c->rq_state + 3 * p.B;
+  a.thr2 = p.zeta_thr * p.zeta_thr; a.nmax = p.zeta_nmax; a.window = p.zeta_window; a.warm = p.zeta_warm;
+  a.band_ok = d_band_ok; a.zeta_cnt = L.zeta_cnt;
+  const dim3 grid(c->qc_nblk, p.B);
+  LPF_KLAUNCH(c, KID_QC_VERDICT, st, k_qc_running<<<grid, QC_THREADS, 0, st>>>(a));
+  LPF_CUDA(cudaEventRecord(c->rq_ev, st));
+  c->rq_valid = true;
+  return LPF_OK;
+}
+
 // S1 + S2 as the C-ABI's lpf_cube_qc: statistics and verdict only.
 int lpf_launch_qc(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, cudaStream_t st) {
   int rc = qc_launch_pass1(c, L, d_cube, d_stats, d_band_ok, st);
+  if (rc) return rc;
+  rc = lpf_launch_qc_running(c, L, d_cube, d_band_ok, st);
   if (rc) return rc;
   const Qc2Args a = make_qc2(c, L, d_cube, d_band_ok, d_stats, false, nullptr);
   LPF_KLAUNCH(c, KID_QC_PASS2, st, k_qc_pass2<true, false><<<lpf_qc2_blocks(c), QC2_THREADS, 0, st>>>(a));
@@ -396,6 +506,8 @@ int lpf_launch_qc(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, u
 int lpf_launch_qc_sum(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, int32_t* zero_me,
                       cudaStream_t st) {
   int rc = qc_launch_pass1(c, L, d_cube, d_stats, d_band_ok, st);
+  if (rc) return rc;
+  rc = lpf_launch_qc_running(c, L, d_cube, d_band_ok, st);
   if (rc) return rc;
   L.dirty_seq = L.dirty_seq >= 0x7ffffff0 ? 1 : L.dirty_seq + 1;
   const Qc2Args a = make_qc2(c, L, d_cube, d_band_ok, d_stats, c->p.detect_sum_plane != 0, zero_me);

@@ -140,6 +140,7 @@ def default_params(cfg: int, bg: str = "box", n_iter: int = 1) -> dict:
         max_det={1: 1024, 2: 16384, 3: 131072, 4: 524288, 5: 524288}[cfg],
         n_lanes=c.n_lanes,
         n_back=0,
+        zeta_thr=0.0, zeta_nmax=0, zeta_window=64, zeta_warm=16,
     )
     return p
 

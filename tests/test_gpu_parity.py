@@ -483,3 +483,34 @@ def test_backward_fill_with_lanes_in_flight(torch_cuda):
         assert np.array_equal(np.isnan(a), np.isnan(b)), int(sl)
         assert np.array_equal(a[~np.isnan(a)], b[~np.isnan(b)]), int(sl)
     lpf.close()
+
+
+def test_running_pixel_qc(torch_cuda):
+    """O12 (eq. A.2): per-pixel running mean / variance, test before update, update only accepted
+    bands.  Band verdicts and the per-band counts must equal the oracle's exactly in every frame (the decision is
+    taken in float32 with the same operation order on both sides); the rest of the chain follows band_ok."""
+    torch = torch_cuda
+    s, p, lpf = _make(2, torch, zeta_thr=12.0, zeta_nmax=3, zeta_window=16, zeta_warm=8, n_lanes=2)
+    pipe = O.OraclePipeline(p, s.mask, direct=False)
+    rng = np.random.default_rng(4)
+    streams = [torch.cuda.Stream() for _ in range(2)]
+    n_rej = 0
+    for t in range(24):
+        cube = s.frame(t)
+        if t in (12, 13, 19):                              # short-lived local interference in one or two bands
+            cube = cube.copy()
+            for b in ((5,) if t != 13 else (5, 9)):
+                for _ in range(6):
+                    cube[b, rng.integers(10, 240), rng.integers(10, 240)] += 400.0
+        o = pipe.step(cube, t)
+        lpf.process_frame(torch.from_numpy(cube).cuda(), t, lane=t % 2, stream=streams[t % 2])
+        g = lpf.frame_view(t % 2)
+        assert np.array_equal(g["zeta_cnt"], o["zeta_cnt"]), (t, g["zeta_cnt"], o["zeta_cnt"])
+        assert np.array_equal(g["band_ok"], o["band_ok"]), t
+        r = parity.check_frame(g, o, pipe, cube, f"running qc t={t}")
+        assert r["in_sync"]
+        n_rej += int((o["band_ok"][:-1] == 0).sum())
+        if t in (12, 13, 19):
+            assert o["band_ok"][5] == 0 and o["zeta_cnt"][5] >= 6
+    assert n_rej >= 4
+    lpf.close()
