@@ -338,3 +338,39 @@ class OraclePipeline:
         det.update(zeta_cnt=self.zeta_cnt.copy())
         det.update(stats=stats, band_ok=ok, cand_idx=cand, act_slots=act_s, act_pix=act_p, flux=flux)
         return det
+
+
+# ---------------------------------------------------------------------------------------------------
+# O13 / O14: what the parameter-inference network is fed with ("x is a dynamic spectrum that we
+# obtained from the image processing steps"; :197-210 eqs. 19-21, the simulated dispersed pulses it is trained on).
+C_DM = 4148.806  # s MHz^2 cm^3 / pc (eq. 20, :206; R19)
+
+
+def export_dynspec(table: "CandidateTable", slots, t_last: int, sigma=None) -> np.ndarray:
+    """O13 -> [n][B][T_ring] float32: the time-ordered dynamic spectra (O10 view) of the given slots, each band
+    divided by its noise sigma ("A ... in standard deviations of the noise", :208), samples that do not exist
+    (NaN: before birth, rejected columns outside the ring) set to 0."""
+    out = np.zeros((len(slots), table.B, table.T), dtype=np.float32)
+    sg = np.ones(table.B, np.float64) if sigma is None else np.asarray(sigma, np.float64)
+    sg = np.where(sg > 0, sg, 1.0)
+    for i, s in enumerate(slots):
+        ds = table.dynspec(int(s), t_last).astype(np.float64)
+        ds = ds / sg[:, None]
+        out[i] = np.where(np.isnan(ds), 0.0, ds).astype(np.float32)
+    return out
+
+
+def simulate_pulses(theta, nu, nu0: float, T: int, dt: float = 1.0) -> np.ndarray:
+    """O14, eqs. 19-21 -> [n][B][T] float64.  theta rows: (t0 [steps], w [steps], DM [pc/cm^3], A, alpha).
+    t_nu = t0 + C_DM DM (nu^-2 - nu0^-2) / dt  (eq. 20, nu in MHz, dt seconds per step);
+    f = exp[-1/2 ((t - t_nu)/w)^2]  (eq. 19 with the 1/2 that its own "w = 16 <-> FWHM 37.67" implies, R18);
+    I = A (nu/nu0)^alpha f  (eq. 21)."""
+    theta = np.asarray(theta, np.float64).reshape(-1, 5)
+    nu = np.asarray(nu, np.float64)
+    t = np.arange(T, dtype=np.float64)
+    out = np.zeros((theta.shape[0], nu.size, T))
+    for i, (t0, w, dm, A, al) in enumerate(theta):
+        for b, v in enumerate(nu):
+            tn = t0 + C_DM * dm * (v ** -2 - nu0 ** -2) / dt
+            out[i, b] = A * (v / nu0) ** al * np.exp(-0.5 * ((t - tn) / w) ** 2)
+    return out

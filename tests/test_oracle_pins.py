@@ -790,3 +790,41 @@ def test_running_qc_verdict_rules():
     f = mk(); f[0, 8, 8] += 500.0; f[0, 9, 2] += 500.0
     cnt, o = rq2.step(f, W, a1)
     assert cnt[0] == 2 and o.tolist() == [0, 0, 0, 1, 0]       # one accepted band of four: the frame is rejected
+
+
+# ------------------------------------------------------------------ O13 / O14 network input and simulated pulses
+def test_simulated_pulse_closed_forms():
+    """eqs. 19-21: the peak of band nu sits at t0 + delay(nu) with the golden delays of eq. 20, its height is
+    A (nu/nu0)^alpha, the full width at half maximum is 2 sqrt(2 ln 2) w (w = 16 <-> 37.67, :197-199), DM = 0 is
+    undispersed."""
+    import oracle as O
+    nu = np.array([57.0, 58.3671875, 61.7, 63.0671875]); nu0 = 63.1
+    T = 4096
+    th = np.array([[300.0, 16.0, 30.0, 5.0, -2.0], [900.25, 40.0, 0.0, 2.0, 1.5]])
+    I = O.simulate_pulses(th, nu, nu0, T, dt=0.01)            # 10 ms steps: the delays span hundreds of steps
+    gold = {57.0: 7.0487, 58.3671875: 5.2750, 61.7: 1.4347, 63.0671875: 0.0325}   # s, tests/golden/dispersion_delays.txt
+    for b, v in enumerate(nu):
+        tp = int(np.argmax(I[0, b]))
+        assert abs(tp - (300.0 + gold[v] / 0.01)) <= 1.0
+        assert np.isclose(I[0, b].max(), 5.0 * (v / nu0) ** -2.0, rtol=2e-3)
+        above = np.flatnonzero(I[0, b] >= 0.5 * I[0, b].max())
+        assert abs((above[-1] - above[0]) - 37.67) <= 2.0        # sampled at integer steps
+        assert int(np.argmax(I[1, b])) == 900 and np.isclose(I[1, b, 900], 2.0 * (v / nu0) ** 1.5 * np.exp(-0.5 * (0.25 / 40) ** 2))
+    assert np.isclose(O.C_DM * (1000.0 ** -2), 4.148806e-3)   # 4.1488 ms at 1 GHz for DM = 1 (:206)
+
+
+def test_export_dynspec_is_the_ordered_normalised_view():
+    import oracle as O
+    tb = O.CandidateTable(8, 6, 3, 16, 3, 10)
+    slots = tb.add_forced(np.array([5, 40], np.int32))
+    ok = np.ones(4, np.uint8)
+    for t in range(9):                                         # more frames than the ring holds
+        flux = np.array([[t + 0.0, 10 * t + 1.0, 100 * t + 2.0], [-t, -2.0 * t, -3.0 * t]], np.float32)
+        tb.append(slots, flux, ok, t)
+    x = O.export_dynspec(tb, slots, 8, sigma=[1.0, 2.0, 0.0])
+    assert x.shape == (2, 3, 6) and x.dtype == np.float32
+    ts = np.arange(3, 9)                                       # the six newest frames, oldest first
+    assert np.array_equal(x[0, 0], ts) and np.allclose(x[0, 1], (10 * ts + 1) / 2.0) and np.array_equal(x[0, 2], 100 * ts + 2)
+    assert np.array_equal(x[1, 0], -ts)
+    y = O.export_dynspec(tb, slots, 10, sigma=None)            # two frames that do not exist yet: zeros, not NaN
+    assert np.array_equal(y[0, 0], [5, 6, 7, 8, 0, 0])
