@@ -179,6 +179,20 @@ int lpf_append_dynspec(lpf_ctx* ctx, const int32_t* d_slots, const int32_t* d_n,
 /* d_out [B][T_ring], time ordered oldest -> newest, ending at t_last (frequency x time, Fig. 1). */
 int lpf_get_dynspec(lpf_ctx* ctx, int32_t slot, int64_t t_last, float* d_out, void* stream);
 
+/* -- what the parameter-inference network is fed with ------------------------
+ * d_out [n][B][T_ring] float32: the time-ordered dynamic spectra (as lpf_get_dynspec) of the n slots in d_slots,
+ * each band divided by d_sigma[b] (its noise sigma, e.g. column 2 or 5 of the QC statistics; NULL or <= 0: 1),
+ * samples that do not exist (before birth, outside the ring) set to 0 instead of NaN.  A batch (N, 1, B, T). */
+int lpf_export_dynspec(lpf_ctx* ctx, const int32_t* d_slots, int32_t n, int64_t t_last, const float* d_sigma,
+                       float* d_out, void* stream);
+/* Simulated dispersed pulses, eqs. 19-21: for sample i with d_theta[i] = (t0 [steps], w [steps],
+ * DM [pc/cm^3], A, alpha):  t_nu = t0 + 4148.806 s MHz^2 DM (nu^-2 - nu0^-2) / dt_s;
+ * I(t, nu) = A (nu/nu0)^alpha exp[-1/2 ((t - t_nu)/w)^2]  (eq. 19 with the 1/2 its own FWHM implies, R18).
+ * d_out [n][B][T] is overwritten (accumulate = 0) or added to (accumulate != 0: injection into noise or into
+ * exported dynamic spectra).  d_nu [B] in MHz.  No context needed. */
+int lpf_simulate_pulses(int32_t n, int32_t B, int32_t T, const float* d_nu, float nu0, float dt_s, const float* d_theta,
+                        float* d_out, int32_t accumulate, void* stream);
+
 /* -- whole step --------------------------------------------------------------
  * qc -> detect -> associate -> flux -> append for one cube on one lane, results in lane-owned
  * buffers (lpf_frame_view).  Frames on different lanes/streams overlap; the association chain is

@@ -56,6 +56,7 @@ EXPORTS = [
     "lpf_create", "lpf_destroy", "lpf_cube_qc", "lpf_detect_sources", "lpf_associate", "lpf_add_candidates",
     "lpf_measure_flux", "lpf_append_dynspec", "lpf_get_dynspec", "lpf_process_frame", "lpf_get_frame_view",
     "lpf_process_frame_host", "lpf_process_frame_host_begin", "lpf_process_frame_host_end", "lpf_get_counters", "lpf_memcpy_d2h", "lpf_strerror", "lpf_last_cuda_error",
+    "lpf_export_dynspec", "lpf_simulate_pulses",
     "lpf_version", "lpf_get_plan", "lpf_profile_begin", "lpf_profile_end", "lpf_profile_kernel_count", "lpf_profile_kernel_name",
 ]
 
@@ -84,6 +85,8 @@ def load_library(path: Optional[str] = None):
     lib.lpf_measure_flux.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     lib.lpf_append_dynspec.argtypes = [vp, vp, vp, vp, vp, i64, vp]
     lib.lpf_get_dynspec.argtypes = [vp, i32, i64, vp, vp]
+    lib.lpf_export_dynspec.argtypes = [vp, vp, i32, i64, vp, vp, vp]
+    lib.lpf_simulate_pulses.argtypes = [i32, i32, i32, vp, C.c_float, C.c_float, vp, vp, i32, vp]
     lib.lpf_process_frame.argtypes = [vp, C.c_int, vp, i64, vp]
     lib.lpf_get_frame_view.argtypes = [vp, C.c_int, C.POINTER(LpfFrameView)]
     lib.lpf_process_frame_host.argtypes = [vp, C.c_int, vp, i64, C.POINTER(LpfHostResult), vp]
@@ -266,6 +269,15 @@ class LPF:
                "lpf_process_frame_host_end")
         return res
 
+    def export_dynspec(self, slots, t_last: int, sigma=None, stream=None):
+        """[n][B][T_ring] float32 network input: ordered, sigma-normalised, NaN-free dynamic spectra."""
+        import torch
+        n = int(slots.numel())
+        out = torch.empty((n, self.B, self.p["T_ring"]), dtype=torch.float32, device=slots.device)
+        _check(self.lib, self.lib.lpf_export_dynspec(self.h, _ptr(slots), n, t_last, _ptr(sigma), _ptr(out), _stream(stream)),
+               "lpf_export_dynspec")
+        return out
+
     def plan(self) -> dict:
         h = (C.c_int64 * 8)()
         _check(self.lib, self.lib.lpf_get_plan(self.h, h), "lpf_get_plan")
@@ -323,3 +335,16 @@ class HostResult:
     def d2h_bytes(self):
         B = self.stats.shape[0]
         return B * STATS_PER_BAND * 4 + B + 1 + 12 + self.nu * 14 + self.npos * (4 + 4 * B)
+
+
+def simulate_pulses(theta, nu, nu0: float, T: int, dt_s: float = 1.0, out=None, accumulate: bool = False, stream=None):
+    """Simulated dispersed pulses (eqs. 19-21): theta [n][5] = (t0, w, DM, A, alpha), nu [B] MHz -> [n][B][T] (CUDA tensors)."""
+    import torch
+    lib = load_library()
+    n, B = int(theta.shape[0]), int(nu.numel())
+    if out is None:
+        out = torch.empty((n, B, T), dtype=torch.float32, device=theta.device)
+        accumulate = False
+    _check(lib, lib.lpf_simulate_pulses(n, B, T, _ptr(nu), float(nu0), float(dt_s), _ptr(theta), _ptr(out), int(bool(accumulate)),
+                                        _stream(stream)), "lpf_simulate_pulses")
+    return out

@@ -2,6 +2,8 @@
 // (O7-O10.)  All integer / compare work: results are exact.
 #include <math_constants.h>
 
+#include <algorithm>
+
 #include "lpf_internal.cuh"
 
 namespace {
@@ -553,6 +555,69 @@ int lpf_launch_cache_store(lpf_ctx* c, const float* d_cube, const uint8_t* d_ban
   LPF_CUDA(cudaMemcpyAsync(c->cube_cache + (size_t)e * cube_elems, d_cube, cube_elems * sizeof(float), cudaMemcpyDeviceToDevice, st));
   LPF_CUDA(cudaMemcpyAsync(c->cache_ok + (size_t)e * (p.B + 1), d_band_ok, (size_t)p.B + 1, cudaMemcpyDeviceToDevice, st));
   LPF_KLAUNCH(c, KID_MISC, st, k_cache_label<<<1, 1, 0, st>>>(c->cache_t, e, t));
+  return LPF_OK;
+}
+
+// O13: [n][B][T_ring] time-ordered, sigma-normalised, NaN-free dynamic spectra of a list of slots
+__global__ void __launch_bounds__(256)
+k_export_dynspec(const float* __restrict__ ring, const long long* __restrict__ meta_t, int T_ring, int B, int n_cand_max,
+                 const int32_t* __restrict__ slots, int n, long long t_last, const float* __restrict__ sigma, float* __restrict__ out) {
+  const long long per = (long long)B * T_ring, total = per * n;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+    const int is = (int)(i / per);
+    const int r = (int)(i - (long long)is * per);
+    const int b = r / T_ring, j = r - b * T_ring;
+    const int slot = slots[is];
+    float v = 0.f;
+    if (slot >= 0 && slot < n_cand_max) {
+      const long long tt = t_last - T_ring + 1 + j;
+      const int tau = (int)(((tt % T_ring) + T_ring) % T_ring);
+      if (tt >= 0 && meta_t[tau] == tt) {
+        const float x = ring[((long long)slot * T_ring + tau) * B + b];
+        const float sg = sigma ? sigma[b] : 1.f;
+        if (x == x) v = (float)((double)x / (double)(sg > 0.f ? sg : 1.f));
+      }
+    }
+    out[i] = v;
+  }
+}
+
+// O14: eqs. 19-21, one thread per (sample, band, time step)
+__global__ void __launch_bounds__(256)
+k_simulate_pulses(int n, int B, int T, const float* __restrict__ nu, float nu0, float dt_s, const float* __restrict__ theta,
+                  float* __restrict__ out, int accumulate) {
+  const long long per = (long long)B * T, total = per * n;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+    const int is = (int)(i / per);
+    const int r = (int)(i - (long long)is * per);
+    const int b = r / T, j = r - b * T;
+    const float* th = theta + 5 * is;
+    const float t0 = th[0], w = th[1], dm = th[2], A = th[3], al = th[4];
+    const float v = nu[b];
+    const float tn = t0 + 4148.806f * dm * (1.f / (v * v) - 1.f / (nu0 * nu0)) / dt_s;      // eq. 20
+    const float u = ((float)j - tn) / w;
+    const float I = A * powf(v / nu0, al) * expf(-0.5f * u * u);                              // eqs. 19, 21
+    out[i] = accumulate ? out[i] + I : I;
+  }
+}
+
+int lpf_launch_export_dynspec(lpf_ctx* c, const int32_t* d_slots, int n, long long t_last, const float* d_sigma, float* d_out,
+                              cudaStream_t st) {
+  const lpf_params& p = c->p;
+  const long long total = (long long)n * p.B * p.T_ring;
+  const int blocks = (int)std::min<long long>((total + 255) / 256, (long long)c->n_sm * 8);
+  LPF_KLAUNCH(c, KID_MISC, st, k_export_dynspec<<<blocks, 256, 0, st>>>(c->ring, c->meta_t, p.T_ring, p.B, p.n_cand_max, d_slots, n,
+                                                                       t_last, d_sigma, d_out));
+  return LPF_OK;
+}
+
+int lpf_launch_simulate_pulses(int n, int B, int T, const float* d_nu, float nu0, float dt_s, const float* d_theta, float* d_out,
+                               int accumulate, cudaStream_t st) {
+  const long long total = (long long)n * B * T;
+  const int blocks = (int)std::min<long long>((total + 255) / 256, 148LL * 16);
+  k_simulate_pulses<<<blocks, 256, 0, st>>>(n, B, T, d_nu, nu0, dt_s, d_theta, d_out, accumulate);
+  cudaError_t e = cudaPeekAtLastError();
+  if (e != cudaSuccess) return lpf_cuda_fail(e, "k_simulate_pulses");
   return LPF_OK;
 }
 

@@ -303,6 +303,20 @@ int lpf_get_dynspec(lpf_ctx* c, int32_t slot, int64_t t_last, float* d_out, void
   return lpf_launch_get_dynspec(c, slot, (long long)t_last, d_out, (cudaStream_t)stream);
 }
 
+int lpf_export_dynspec(lpf_ctx* c, const int32_t* d_slots, int32_t n, int64_t t_last, const float* d_sigma, float* d_out,
+                       void* stream) {
+  if (!c || n < 0 || (n > 0 && (!d_slots || !d_out))) return LPF_E_ARG;
+  if (n == 0) return LPF_OK;
+  return lpf_launch_export_dynspec(c, d_slots, n, (long long)t_last, d_sigma, d_out, (cudaStream_t)stream);
+}
+
+int lpf_simulate_pulses(int32_t n, int32_t B, int32_t T, const float* d_nu, float nu0, float dt_s, const float* d_theta,
+                        float* d_out, int32_t accumulate, void* stream) {
+  if (n < 0 || B < 1 || T < 1 || !(nu0 > 0) || !(dt_s > 0) || (n > 0 && (!d_nu || !d_theta || !d_out))) return LPF_E_ARG;
+  if (n == 0) return LPF_OK;
+  return lpf_launch_simulate_pulses(n, B, T, d_nu, nu0, dt_s, d_theta, d_out, accumulate, (cudaStream_t)stream);
+}
+
 int lpf_process_frame(lpf_ctx* c, int lane, const float* d_cube, int64_t t, void* stream) {
   TRY(lane_ok(c, lane));
   if (!d_cube || t < 0) return LPF_E_ARG;

@@ -162,6 +162,10 @@ int lpf_launch_append(lpf_ctx* c, const int32_t* d_slots, const int32_t* d_n, co
                       const uint8_t* d_band_ok, long long t, cudaStream_t st);
 int lpf_launch_backfill(lpf_ctx* c, const int32_t* d_slots, const int32_t* d_pix, const int32_t* d_n, const float* d_cube,
                         const uint8_t* d_band_ok, long long t, cudaStream_t st);
+int lpf_launch_export_dynspec(lpf_ctx* c, const int32_t* d_slots, int n, long long t_last, const float* d_sigma, float* d_out,
+                              cudaStream_t st);
+int lpf_launch_simulate_pulses(int n, int B, int T, const float* d_nu, float nu0, float dt_s, const float* d_theta, float* d_out,
+                               int accumulate, cudaStream_t st);
 int lpf_launch_cache_store(lpf_ctx* c, const float* d_cube, const uint8_t* d_band_ok, long long t, cudaStream_t st);
 int lpf_launch_get_dynspec(lpf_ctx* c, int slot, long long t_last, float* d_out, cudaStream_t st);
 int lpf_launch_fill_nan(lpf_ctx* c, float* d, int64_t n, cudaStream_t st);

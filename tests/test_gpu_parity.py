@@ -514,3 +514,43 @@ def test_running_pixel_qc(torch_cuda):
             assert o["band_ok"][5] == 0 and o["zeta_cnt"][5] >= 6
     assert n_rej >= 4
     lpf.close()
+
+
+def test_network_input_export_and_pulse_simulator(torch_cuda):
+    """O13 (batched, ordered, sigma-normalised dynamic spectra, bit-exact) and O14 (eqs. 19-21 pulses,
+    float32 kernel against the float64 oracle) and their combination (injection into exported spectra)."""
+    torch = torch_cuda
+    from paper_2103_15418_b200.binding import simulate_pulses
+    s, p, lpf = _make(2, torch, T_ring=24)
+    pipe = O.OraclePipeline(p, s.mask, direct=False)
+    n = 30
+    for t in range(n):
+        cube = s.frame(t)
+        o = pipe.step(cube, t)
+        lpf.process_frame(torch.from_numpy(cube).cuda(), t)
+    g = lpf.frame_view(0)
+    assert np.array_equal(g["act_slots"], o["act_slots"])
+    slots = o["act_slots"][::3].astype(np.int32)
+    sigma = g["stats"][:, 5].astype(np.float32)               # clipped rms per band
+    for t_last, sg in ((n - 1, sigma), (n + 4, None)):
+        x = lpf.export_dynspec(torch.from_numpy(slots).cuda(), t_last, None if sg is None else torch.from_numpy(sg).cuda())
+        ref = O.export_dynspec(pipe.table, slots, t_last, sg)
+        assert x.shape == ref.shape and np.array_equal(x.cpu().numpy(), ref)
+        assert not np.isnan(ref).any()
+    # simulator
+    rng = np.random.default_rng(8)
+    B, T = p["B"], 24
+    nu = np.array(s.c.nu_mhz if hasattr(s.c, "nu_mhz") else np.linspace(57.0, 63.1, B), np.float32)
+    nu0 = float(nu.max())
+    m = slots.size
+    theta = np.stack([rng.uniform(2, T - 2, m), rng.uniform(0.8, 6, m), rng.uniform(0, 40, m), rng.uniform(0, 8, m),
+                      rng.uniform(-4, 4, m)], 1).astype(np.float32)
+    I = simulate_pulses(torch.from_numpy(theta).cuda(), torch.from_numpy(nu).cuda(), nu0, T, dt_s=1.0).cpu().numpy()
+    ref = O.simulate_pulses(theta.astype(np.float64), nu.astype(np.float64), nu0, T, 1.0)
+    assert np.allclose(I, ref, rtol=2e-4, atol=2e-5 * float(theta[:, 3].max()))
+    # injection into the exported spectra (accumulate)
+    x = lpf.export_dynspec(torch.from_numpy(slots).cuda(), n - 1, torch.from_numpy(sigma).cuda())
+    x0 = x.cpu().numpy().copy()
+    simulate_pulses(torch.from_numpy(theta).cuda(), torch.from_numpy(nu).cuda(), nu0, T, 1.0, out=x, accumulate=True)
+    assert np.allclose(x.cpu().numpy(), x0 + ref, rtol=2e-4, atol=1e-4)
+    lpf.close()
