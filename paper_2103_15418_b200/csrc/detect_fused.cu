@@ -412,8 +412,9 @@ struct Sweep {
     return smem_u32(reinterpret_cast<const float*>(g_sm4) + O_BAR + 2 * stage);
   }
 
-  // the per-iteration barrier of all warps, in two halves (an mbarrier with one arrival per thread)
-  __device__ __forceinline__ void sync_arrive() const { mbar_arrive(bar_addr(XST)); }
+  // the per-iteration barrier of all warps, in two halves (an mbarrier with one arrival per warp: 32 arrivals on
+  // one shared-memory word would serialise)
+  __device__ __forceinline__ void sync_arrive() const { __syncwarp(); if (lane == 0) mbar_arrive(bar_addr(XST)); }
   __device__ __forceinline__ void sync_wait(int b) const { mbar_wait(bar_addr(XST), (uint32_t)b & 1u); }
 
   __device__ __forceinline__ CandCtx cand_ctx() const {
@@ -708,7 +709,7 @@ k_fused_box(const FusedArgs a) {
   if (s.tid == 0) {
 #pragma unroll
     for (int i = 0; i < XST; ++i) mbar_init(s.bar_addr(i), 1);
-    mbar_init(s.bar_addr(XST), NT);
+    mbar_init(s.bar_addr(XST), NT / 32);
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
   asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");   // the zero fill above precedes the bulk copies
