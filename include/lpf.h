@@ -140,7 +140,10 @@ int lpf_destroy(lpf_ctx* ctx);
  * Per band over valid pixels: n, mean b (the paper's b), rms, and after one
  * qc_clip-sigma clip round n_clip, clipped mean, clipped rms; then eq. A.1 z-scores of the mean
  * and of the rms across bands (median / median-absolute-deviation, SE floor; R10-R13);
- * band_ok = |z_mean| <= tau and |z_rms| <= tau; frame_ok = #ok >= ceil(B/2). */
+ * band_ok = |z_mean| <= tau and |z_rms| <= tau; frame_ok = #ok >= ceil(B/2).
+ * With zeta_thr > 0 the per-pixel running test of eq. A.2 (O12) follows: it can discard further bands (frame_ok is
+ * re-evaluated) and advances the running mean / variance images of the bands it accepts, so call it once per cube,
+ * in increasing t (the calls of different lanes are ordered by an event). */
 int lpf_cube_qc(lpf_ctx* ctx, int lane, const float* d_cube, int64_t t, float* d_stats,
                 uint8_t* d_band_ok, void* stream);
 
