@@ -79,10 +79,15 @@ typedef struct {
   int32_t n_back;           /* backward fill: a slot created at t also gets the fluxes of the last n_back
                              * cubes, which lpf_process_frame then keeps in a device cache; 0 = off, <= 64 */
   float zeta_thr;           /* eq. A.2: per-pixel running mean / variance of every band; a band with more
-                             * than zeta_nmax valid pixels at |x - mean| > zeta_thr * sqrt(var) is discarded; 0 = off */
+                             * than zeta_nmax valid pixels (with var > 0) at |x - mean| > zeta_thr * sqrt(var) is discarded; 0 = off */
   int32_t zeta_nmax;        /* 0 = the paper's "if zeta exceeds a threshold" */
   int32_t zeta_window;      /* Welford up to this many updates, exponentially weighted (alpha = 1/window) after */
-  int32_t zeta_warm;        /* no test before a band has had this many updates */
+  int32_t zeta_warm;        /* no test before a band has had this many updates; >= 2 (after one update every variance is 0) */
+  int32_t zeta_reset;       /* a band discarded by eq. A.2 in this many consecutive frames starts over (its running state is
+                             * forgotten: Welford from scratch, untested during the warm-up) -- the way out of a lasting level
+                             * change; 0 = never (a discarded band keeps its state, R22) */
+  int32_t force_general;    /* 1: lpf_detect_sources takes the general multi-kernel path even when the parameter set allows the
+                             * fused single-pass kernel (used by the parity tests to reach both); 0: automatic */
 } lpf_params;
 
 /* One peak (eq. 7: p = q and y) of one plane.  24 bytes. */
@@ -223,8 +228,8 @@ int lpf_get_counters(lpf_ctx* ctx, int64_t* h_out);
 /* Launch plan chosen at lpf_create: h_out[0] = 1 if the fused single-pass detection kernel is in use
  * (box K = 12, k_mf = 3, n_iter = 1, Dx % 4 == 0; otherwise the general multi-kernel path),
  * [1] strip width in columns, [2] threads per CTA, [3] CTAs per plane, [4] dynamic shared memory
- * bytes per CTA, [5] planes, [6] SMs, [7] QC blocks per band.  Setting the environment variable
- * LPF_FORCE_GENERAL=1 before lpf_create selects the general path (used by the parity tests). */
+ * bytes per CTA, [5] planes, [6] SMs, [7] QC blocks per band.  lpf_params.force_general = 1 selects the
+ * general path (used by the parity tests). */
 int lpf_get_plan(lpf_ctx* ctx, int64_t* h_out);
 
 /* Optional per-kernel timing with CUDA events recorded on the launching stream, around every kernel

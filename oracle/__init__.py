@@ -153,22 +153,29 @@ def measure_flux(cube, band_ok, W, pos, r_flux: int) -> np.ndarray:
 class RunningQC:
     """O12, per-pixel running quality control (eq. A.2; R22).
 
-    State per band and pixel: running mean m and variance v of the image stream (Welford 1962 while the band
-    has fewer than `window` updates, exponentially weighted after that, Finch 2009), and the number of
-    updates n_b.  For a frame: zeta = (x - m) / sqrt(v) (eq. A.2) at every valid pixel of every band with
+    State per band and pixel: running mean m and variance v of the image stream -- float32 IMAGES, like the
+    cube itself (:389 "running mean and standard deviation images") -- and the number of updates n_b.
+    Welford (1962) while the band has fewer than `window` updates, exponentially weighted after that
+    (Finch 2009): one recurrence, a = 1/min(n_b + 1, window), d = x - m, m += a d, v = (1 - a)(v + a d^2).
+    For a frame: zeta = (x - m)/sqrt(v) (eq. A.2) at every valid pixel with v > 0 of every band with
     n_b >= warm; the band is discarded when more than `nmax` pixels have |zeta| > thr (nmax = 0: the
     paper's "if zeta exceeds a threshold").  The test comes before the update, and only bands that survive
-    both eq. A.1 and eq. A.2 update their state.  The test is a floating-point decision, so it is taken in
-    float32 with the kernel's operation order (each operation rounded once, no fused multiply-add):
-    d = x - m;  exceeds  <=>  d*d > thr^2 * v;  update: a = 1/min(n_b + 1, window), m += a*d,
-    v = (1 - a) * (v + (a*d)*d).
+    both eq. A.1 and eq. A.2 update their state.  A band discarded by eq. A.2 in `reset` consecutive frames
+    (reset > 0) starts over (n_b = 0: Welford from scratch, untested during the warm-up) -- the way out of a
+    lasting level change.
+
+    All arithmetic is float64 on the float32 state; each new state value is rounded to float32 once.
+    |zeta| > thr is evaluated as d^2 > thr^2 v.  `near[b]` counts the valid pixels whose decision is within
+    2e-4 relative of the threshold (the parity harness accepts a count difference only up to that number).
     """
 
-    def __init__(self, B: int, Dy: int, Dx: int, thr: float, nmax: int, window: int, warm: int):
-        self.thr2 = np.float32(np.float32(thr) * np.float32(thr)); self.nmax = int(nmax)
-        self.window = int(window); self.warm = int(warm)
+    def __init__(self, B: int, Dy: int, Dx: int, thr: float, nmax: int, window: int, warm: int, reset: int = 0):
+        self.thr2 = float(thr) ** 2; self.nmax = int(nmax)
+        self.window = int(window); self.warm = int(warm); self.reset = int(reset)
         self.m = np.zeros((B, Dy, Dx), np.float32); self.v = np.zeros((B, Dy, Dx), np.float32)
         self.n = np.zeros(B, np.int32)
+        self.run = np.zeros(B, np.int32)          # consecutive eq. A.2 discards
+        self.near = np.zeros(B, np.int32)
 
     def step(self, cube, W, band_ok):
         """band_ok: [B+1] after eq. A.1.  Returns (counts [B] int32, band_ok' [B+1])."""
@@ -176,21 +183,31 @@ class RunningQC:
         B = cube.shape[0]
         ok = np.array(band_ok, np.uint8, copy=True)
         cnt = np.zeros(B, np.int32)
+        self.near[:] = 0
         valid = np.ones(cube.shape[1:], bool) if W is None else (np.asarray(W) != 0)
         for b in range(B):
             with np.errstate(invalid="ignore", over="ignore"):
-                d = cube[b] - self.m[b]
+                m = self.m[b].astype(np.float64); v = self.v[b].astype(np.float64)
+                d = cube[b].astype(np.float64) - m
+                a1_ok = bool(ok[b]); discard = False
                 if self.n[b] >= self.warm:
-                    exceeds = (d * d) > (self.thr2 * self.v[b])
-                    cnt[b] = int(np.count_nonzero(exceeds & valid))
-                    if cnt[b] > self.nmax:
-                        ok[b] = 0
+                    lhs = d * d; rhs = self.thr2 * v
+                    tested = valid & (v > 0)
+                    cnt[b] = int(np.count_nonzero((lhs > rhs) & tested))
+                    self.near[b] = int(np.count_nonzero((np.abs(lhs - rhs) <= 2e-4 * rhs) & tested))
+                    discard = cnt[b] > self.nmax
+                if discard:
+                    ok[b] = 0
                 if ok[b]:
-                    a = np.float32(1.0) / np.float32(min(int(self.n[b]) + 1, self.window))
-                    ad = a * d
-                    self.m[b] = self.m[b] + ad
-                    self.v[b] = (np.float32(1.0) - a) * (self.v[b] + ad * d)
+                    a = 1.0 / min(int(self.n[b]) + 1, self.window)
+                    self.m[b] = (m + a * d).astype(np.float32)
+                    self.v[b] = ((1.0 - a) * (v + a * d * d)).astype(np.float32)
                     self.n[b] += 1
+                    self.run[b] = 0
+                elif a1_ok and discard:
+                    self.run[b] += 1
+                    if self.reset > 0 and self.run[b] >= self.reset:
+                        self.m[b] = 0; self.v[b] = 0; self.n[b] = 0; self.run[b] = 0
         ok[B] = 1 if int(ok[:B].sum()) >= (B + 1) // 2 else 0
         return cnt, ok
 
@@ -266,7 +283,7 @@ class OraclePipeline:
         self.rq = None
         if float(p.get("zeta_thr", 0.0)) > 0:
             self.rq = RunningQC(p["B"], p["Dy"], p["Dx"], p["zeta_thr"], p.get("zeta_nmax", 0), p.get("zeta_window", 64),
-                                p.get("zeta_warm", 8))
+                                p.get("zeta_warm", 8), p.get("zeta_reset", 0))
         self.zeta_cnt = np.zeros(p["B"], np.int32)
         self.history = []   # O11: the last n_back frames as (t, cube, band_ok)
 
@@ -335,7 +352,7 @@ class OraclePipeline:
         flux = measure_flux(cube, ok, self.W, act_p, p["r_flux"])
         self.table.append(act_s, flux, ok, t)
         self.backfill(cube, ok, t)
-        det.update(zeta_cnt=self.zeta_cnt.copy())
+        det.update(zeta_cnt=self.zeta_cnt.copy(), zeta_near=(self.rq.near.copy() if self.rq is not None else None))
         det.update(stats=stats, band_ok=ok, cand_idx=cand, act_slots=act_s, act_pix=act_p, flux=flux)
         return det
 

@@ -3,7 +3,7 @@
 //
 // A plain, slow, single-threaded float64 restatement of what the path computes,
 // written from the paper (Ruhe et al., arXiv 2103.15418; /root/reference/PAPER.md)
-// and from the readings listed in DESIGN.md ("Readings", R1..R24).  It shares no
+// and from the readings listed in DESIGN.md ("Readings", R1..R26).  It shares no
 // code with the CUDA path (paper_2103_15418_b200/csrc) and neither includes the
 // other.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
 // --impl reference legs may load this library.
@@ -47,11 +47,11 @@ void orc_band_stats(const float* cube, int B, int Dy, int Dx, const uint8_t* W,
     for (int64_t i = 0; i < N; ++i)
       if (!W || W[i]) { double d = (double)X[i] - mean; ss += d * d; }
     const double rms = std::sqrt(ss / n);
-    // membership of the clip round is a floating-point DECISION: it is taken in the kernel's precision
-    // (float32: |x - (float)mean| <= (float)(qc_clip rms)), reading R25; the moments of the
-    // selected pixels are float64 as everywhere else.
-    const float meanf = (float)mean, thrf = (float)(qc_clip * rms);
-    auto inside = [&](float x) { const float d = x - meanf; return std::fabs(d) <= thrf; };
+    // one clip round, as defined (O1): the pixels with |x - mean| <= qc_clip rms, decided in float64 like
+    // everything else here.  (A float32 implementation may put a pixel that sits within rounding of the
+    // boundary on the other side; the parity harness classifies such pixels by THIS margin and logs them.)
+    const double thr = qc_clip * rms;
+    auto inside = [&](float x) { return std::fabs((double)x - mean) <= thr; };
     double nc = 0, sc = 0;
     for (int64_t i = 0; i < N; ++i)
       if ((!W || W[i]) && inside(X[i])) { nc += 1; sc += (double)X[i]; }

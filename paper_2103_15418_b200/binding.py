@@ -31,6 +31,7 @@ class LpfParams(C.Structure):
         ("T_ring", C.c_int32), ("n_cand_max", C.c_int32), ("max_det", C.c_int32), ("n_lanes", C.c_int32),
         ("n_back", C.c_int32),
         ("zeta_thr", C.c_float), ("zeta_nmax", C.c_int32), ("zeta_window", C.c_int32), ("zeta_warm", C.c_int32),
+        ("zeta_reset", C.c_int32), ("force_general", C.c_int32),
     ]
 
 
@@ -118,7 +119,7 @@ def _check(lib, rc: int, what: str):
 def make_params(p: dict) -> LpfParams:
     s = LpfParams()
     for name, _ in LpfParams._fields_:
-        setattr(s, name, p[name])
+        setattr(s, name, p[name] if name not in ("zeta_reset", "force_general") else p.get(name, 0))
     return s
 
 

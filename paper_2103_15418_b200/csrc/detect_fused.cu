@@ -814,8 +814,7 @@ enum { CL_ANYW = 1,    // some valid pixel among the warp's columns +-4
 int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
   *out = nullptr;
   const lpf_params& p = c->p;
-  const char* force = getenv("LPF_FORCE_GENERAL");
-  if (force && force[0] == '1') return LPF_OK;
+  if (p.force_general) return LPF_OK;
   if (!(p.bg_kernel == 1 && p.k_bg == KBG && p.k_mf == 3 && p.sigma_mf > 0 && p.n_iter == 1 && (p.Dx % 4) == 0 &&
         (p.Dy % 2) == 0 && p.k_max <= 2))
     return LPF_OK;

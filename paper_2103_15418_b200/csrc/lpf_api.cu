@@ -67,13 +67,14 @@ int check_params(const lpf_params* p) {
   if (!(p->kappa > 0) || p->k_max < 0 || p->k_max > 8) return LPF_E_ARG;
   if (p->k_mf < 0 || p->k_mf > LPF_MAX_RADIUS || p->k_bg < 1 || p->k_bg > LPF_MAX_RADIUS) return LPF_E_ARG;
   if (p->bg_kernel != 0 && p->bg_kernel != 1) return LPF_E_ARG;
+  if (p->force_general != 0 && p->force_general != 1) return LPF_E_ARG;
   if (p->bg_kernel == 0 && !(p->s_bg > 0)) return LPF_E_ARG;
   if (p->n_iter < 1 || p->n_iter > 255) return LPF_E_ARG;
   if (p->r_flux < 0 || p->r_flux > 8 || p->r_dedupe < 0 || p->r_dedupe > 8 || p->r_assoc < 0 || p->r_assoc > 8) return LPF_E_ARG;
   if (p->n_forget < 1 || p->T_ring < 1 || p->n_cand_max < 1 || p->max_det < 1 || p->n_lanes < 1 || p->n_lanes > 64) return LPF_E_ARG;
   if (p->n_back < 0 || p->n_back > 64) return LPF_E_ARG;
   if (!(p->zeta_thr >= 0)) return LPF_E_ARG;
-  if (p->zeta_thr > 0 && (p->zeta_nmax < 0 || p->zeta_window < 1 || p->zeta_warm < 1)) return LPF_E_ARG;
+  if (p->zeta_thr > 0 && (p->zeta_nmax < 0 || p->zeta_window < 1 || p->zeta_warm < 2 || p->zeta_reset < 0)) return LPF_E_ARG;
   if (!(p->eps_rel >= 0) || !(p->qc_tau > 0) || !(p->qc_clip > 0)) return LPF_E_ARG;
   return LPF_OK;
 }
@@ -205,10 +206,10 @@ int lpf_create(lpf_ctx** out, const lpf_params* p, const uint8_t* d_valid_mask) 
   if (p->zeta_thr > 0) {
     TRYC(dalloc(&c->rq_m, 2 * (size_t)p->B * N));
     TRYC(dalloc(&c->rq_v, 2 * (size_t)p->B * N));
-    TRYC(dalloc(&c->rq_state, 3 * (size_t)p->B + 1));
+    TRYC(dalloc(&c->rq_state, 4 * (size_t)p->B + 1));
     CUDAC(cudaMemset(c->rq_m, 0, 2 * (size_t)p->B * N * sizeof(float)));
     CUDAC(cudaMemset(c->rq_v, 0, 2 * (size_t)p->B * N * sizeof(float)));
-    CUDAC(cudaMemset(c->rq_state, 0, (3 * (size_t)p->B + 1) * sizeof(int32_t)));
+    CUDAC(cudaMemset(c->rq_state, 0, (4 * (size_t)p->B + 1) * sizeof(int32_t)));
     CUDAC(cudaEventCreateWithFlags(&c->rq_ev, cudaEventDisableTiming));
   }
   if (p->n_back > 0) {

@@ -83,7 +83,7 @@ struct lpf_ctx {
   // to the other copy and adopted per band only if the band is accepted), update counts, scratch
   float* rq_m = nullptr;            // [2][B][N]
   float* rq_v = nullptr;            // [2][B][N]
-  int32_t* rq_state = nullptr;      // [B] current copy, [B] updates so far, [B] counts of the frame in progress, [1] block counter
+  int32_t* rq_state = nullptr;      // [B] current copy, [B] updates so far, [B] counts of the frame in progress, [B] consecutive discards, [1] block counter
   cudaEvent_t rq_ev = nullptr;      // orders the frames' updates across lanes
   bool rq_valid = false;
   // backward fill (O11): the last n_back cubes, their verdicts and time steps

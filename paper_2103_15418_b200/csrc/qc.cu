@@ -355,26 +355,24 @@ k_qc_pass2(const Qc2Args a) {
 }
 
 // ---- O12: per-pixel running quality control (eq. A.2; R22) -------------------
-// One block per (chunk, band).  zeta = (x - mean) / sqrt(var) is tested as d*d > thr^2 * var with every
-// operation rounded once (no fused multiply-add: the oracle takes the same float32 decision); the Welford /
-// exponentially weighted update of the frame is written to the OTHER copy of the state and adopted per band by
-// the last block, which also folds the verdict into band_ok / frame_ok ("test before update, update only
-// accepted bands").
+// One block per (chunk, band).  zeta = (x - mean) / sqrt(var) is tested as d*d > thr^2 * var at valid pixels with
+// var > 0; the Welford / exponentially weighted update of the frame is written to the OTHER copy of the state and
+// adopted per band by the last block, which also folds the verdict into band_ok / frame_ok ("test before update,
+// update only accepted bands") and applies the start-over rule (zeta_reset consecutive discards).
 struct RqArgs {
   const float* cube; const uint8_t* W; long long N; int B, nblk;
   float* m; float* v;            // [2][B][N]
-  int32_t* cur; int32_t* nupd; int32_t* cnt; int32_t* counter;   // [B], [B], [B], [1]
-  float thr2; int nmax, window, warm;
+  int32_t* cur; int32_t* nupd; int32_t* cnt; int32_t* run; int32_t* counter;   // [B], [B], [B], [B], [1]
+  float thr2; int nmax, window, warm, reset;
   uint8_t* band_ok; int32_t* zeta_cnt;
 };
 
 __device__ __forceinline__ void rq_pixel(float x, float m, float v, bool test, float a, float one_m_a, float thr2,
                                          float& m2, float& v2, int& hits) {
-  const float d = __fsub_rn(x, m);
-  if (test && __fmul_rn(d, d) > __fmul_rn(thr2, v)) ++hits;
-  const float ad = __fmul_rn(a, d);
-  m2 = __fadd_rn(m, ad);
-  v2 = __fmul_rn(one_m_a, __fadd_rn(v, __fmul_rn(ad, d)));
+  const float d = x - m;
+  if (test && v > 0.f && d * d > thr2 * v) ++hits;
+  m2 = fmaf(a, d, m);
+  v2 = one_m_a * fmaf(a * d, d, v);
 }
 
 __global__ void __launch_bounds__(QC_THREADS)
@@ -385,7 +383,8 @@ k_qc_running(const RqArgs a) {
   const int cur = a.cur[b], nup = a.nupd[b];
   const bool tested = nup >= a.warm;
   const int k = nup + 1 < a.window ? nup + 1 : a.window;
-  const float al = __fdiv_rn(1.0f, (float)k), oma = __fsub_rn(1.0f, al);
+  const float al = 1.0f / (float)k, oma = 1.0f - al;
+  const bool fresh = nup == 0;       // a band that starts (over): its state counts as zero
   const float* X = a.cube + (long long)b * N;
   const float* m0 = a.m + ((long long)cur * a.B + b) * N;
   const float* v0 = a.v + ((long long)cur * a.B + b) * N;
@@ -400,7 +399,8 @@ k_qc_running(const RqArgs a) {
   if (vec) {
     for (long long q = q0 + threadIdx.x; q < q1; q += QC_THREADS) {
       const float4 x = __ldg(reinterpret_cast<const float4*>(X) + q);
-      const float4 m = *(reinterpret_cast<const float4*>(m0) + q), v = *(reinterpret_cast<const float4*>(v0) + q);
+      float4 m = *(reinterpret_cast<const float4*>(m0) + q), v = *(reinterpret_cast<const float4*>(v0) + q);
+      if (fresh) { m = make_float4(0.f, 0.f, 0.f, 0.f); v = m; }
       const unsigned wm = __ldg(reinterpret_cast<const unsigned*>(a.W) + q);
       float4 m2, v2;
       rq_pixel(x.x, m.x, v.x, tested && (wm & 0x000000ffu), al, oma, a.thr2, m2.x, v2.x, hits);
@@ -412,7 +412,7 @@ k_qc_running(const RqArgs a) {
   } else {
     for (long long i = (q0 << 2) + threadIdx.x; i < (q1 << 2) && i < N; i += QC_THREADS) {
       float m2, v2;
-      rq_pixel(X[i], m0[i], v0[i], tested && a.W[i] != 0, al, oma, a.thr2, m2, v2, hits);
+      rq_pixel(X[i], fresh ? 0.f : m0[i], fresh ? 0.f : v0[i], tested && a.W[i] != 0, al, oma, a.thr2, m2, v2, hits);
       m1[i] = m2; v1[i] = v2;
     }
   }
@@ -432,9 +432,15 @@ k_qc_running(const RqArgs a) {
     const int bb = threadIdx.x;
     const int c = __ldcg(&a.cnt[bb]);
     const int nu = a.nupd[bb];
-    int ok = a.band_ok[bb];
-    if (nu >= a.warm && c > a.nmax) ok = 0;          // eq. A.2
-    if (ok) { a.cur[bb] ^= 1; a.nupd[bb] = nu + 1; atomicAdd(&s_nok, 1); }
+    const int ok_in = a.band_ok[bb];
+    const bool discard = nu >= a.warm && c > a.nmax;          // eq. A.2
+    const int ok = (ok_in && !discard) ? 1 : 0;
+    if (ok) { a.cur[bb] ^= 1; a.nupd[bb] = nu + 1; a.run[bb] = 0; atomicAdd(&s_nok, 1); }
+    else if (ok_in && discard) {
+      const int r = a.run[bb] + 1;
+      if (a.reset > 0 && r >= a.reset) { a.nupd[bb] = 0; a.run[bb] = 0; }   // the band starts over
+      else a.run[bb] = r;
+    }
     a.band_ok[bb] = (uint8_t)ok;
     a.zeta_cnt[bb] = c;
     a.cnt[bb] = 0;
@@ -480,8 +486,8 @@ int lpf_launch_qc_running(lpf_ctx* c, LpfLane& L, const float* d_cube, uint8_t* 
   RqArgs a{};
   a.cube = d_cube; a.W = c->W; a.N = c->N; a.B = p.B; a.nblk = c->qc_nblk;
   a.m = c->rq_m; a.v = c->rq_v; a.cur = c->rq_state; a.nupd = c->rq_state + p.B; a.cnt = c->rq_state + 2 * p.B;
-  a.counter = c->rq_state + 3 * p.B;
-  a.thr2 = p.zeta_thr * p.zeta_thr; a.nmax = p.zeta_nmax; a.window = p.zeta_window; a.warm = p.zeta_warm;
+  a.run = c->rq_state + 3 * p.B; a.counter = c->rq_state + 4 * p.B;
+  a.thr2 = p.zeta_thr * p.zeta_thr; a.nmax = p.zeta_nmax; a.window = p.zeta_window; a.warm = p.zeta_warm; a.reset = p.zeta_reset;
   a.band_ok = d_band_ok; a.zeta_cnt = L.zeta_cnt;
   const dim3 grid(c->qc_nblk, p.B);
   LPF_KLAUNCH(c, KID_QC_VERDICT, st, k_qc_running<<<grid, QC_THREADS, 0, st>>>(a));

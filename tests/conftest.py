@@ -24,3 +24,18 @@ def pytest_collection_modifyitems(config, items):
     for it in items:
         if "gpu" in it.keywords:
             it.add_marker(skip)
+
+
+def pytest_terminal_summary(terminalreporter, exitstatus, config):
+    """north_star: "any near-threshold ties are logged": the parity harness' tie log is written to
+    gpurun_out/ties.json (the folder that comes back from a GPU run) and its size is printed here."""
+    parity = sys.modules.get("parity")
+    if parity is None:
+        return
+    path = os.path.join(ROOT, "gpurun_out", "ties.json")
+    try:
+        kinds = parity.dump_ties(path)
+    except OSError as e:
+        terminalreporter.write_line(f"parity ties: {len(parity.TIES)} (not written: {e})")
+        return
+    terminalreporter.write_line(f"parity ties logged: {len(parity.TIES)} {kinds} -> {path}")

@@ -18,26 +18,47 @@ ATOL_SIGMA = 1e-5
 TIES = []  # (tag, plane, pix, kind, margin)
 
 
-def check_qc(stats_g, ok_g, stats_o, ok_o, tag=""):
+def clip_boundary_pixels(cube, W, stats_o, qc_clip):
+    """Per band: how many valid pixels have the ORACLE's clip-round margin ||x - mean| - qc_clip rms| inside the
+    north_star tolerance (1e-4 relative + 1e-5 absolute, in units of the band rms).  Only those pixels may fall on
+    the other side of the boundary in a float32 evaluation."""
+    cube = np.asarray(cube, np.float32)
+    valid = np.ones(cube.shape[1:], bool) if W is None else (np.asarray(W) != 0)
+    out = np.zeros(cube.shape[0], np.int64)
+    for b in range(cube.shape[0]):
+        mean, rms = stats_o[b, 1], stats_o[b, 2]
+        if not (np.isfinite(mean) and np.isfinite(rms)):
+            continue
+        with np.errstate(invalid="ignore"):
+            marg = np.abs(np.abs(cube[b].astype(np.float64) - mean) - qc_clip * rms)
+            out[b] = int(np.count_nonzero((marg <= (RTOL + ATOL_SIGMA) * rms) & valid))
+    return out
+
+
+def check_qc(stats_g, ok_g, stats_o, ok_o, tag="", cube=None, W=None, qc_clip=3.0):
     stats_g = np.asarray(stats_g, dtype=np.float64)
     assert np.array_equal(np.asarray(ok_g), np.asarray(ok_o)), f"{tag}: band_ok {ok_g} != {ok_o}"
     n = stats_o[:, 0]
     fin = np.isfinite(stats_o[:, 1]) & np.isfinite(stats_o[:, 2])
     assert np.array_equal(stats_g[:, 0], n), f"{tag}: n"
     sig = np.maximum(stats_o[:, 2], 1e-30)
-    # pixels within float32 rounding of the clip boundary mean +- qc_clip rms may fall on either side
-    # (the two sides' means differ in the last bits): each moves the clipped moments by <= one boundary
-    # pixel's worth; they are logged as ties
+    # The clip round is a floating-point set decision: the oracle takes it in float64; a pixel may fall on the other
+    # side in the kernel only if the oracle's own margin is inside the tolerance.  Such pixels are counted from the
+    # cube, bound the difference in n_clip, and every difference is logged as a tie.
     dn = np.abs(stats_g[:, 3] - stats_o[:, 3])
-    assert np.all(dn[fin] <= 2 + 1e-6 * n[fin]), f"{tag}: n_clip {stats_g[:, 3]} vs {stats_o[:, 3]}"
-    for b in np.flatnonzero(dn > 0):
-        TIES.append((tag, int(b), -1, "clip", float(dn[b])))
+    dn[~fin] = 0
+    if dn.any():
+        assert cube is not None, f"{tag}: n_clip differs and no cube was given to classify it"
+        near = clip_boundary_pixels(cube, W, stats_o, qc_clip)
+        assert np.all(dn <= near), f"{tag}: n_clip {stats_g[:, 3]} vs {stats_o[:, 3]}: more than the {near} boundary pixels"
+        for b in np.flatnonzero(dn > 0):
+            TIES.append((tag, int(b), -1, "clip", float(dn[b])))
     nclip = np.maximum(stats_o[:, 3], 1.0)
     for col, name in ((1, "mean"), (2, "rms"), (4, "clipped mean"), (5, "clipped rms")):
         err = np.abs(stats_g[fin, col] - stats_o[fin, col])
         lim = RTOL * np.abs(stats_o[fin, col]) + ATOL_SIGMA * sig[fin]
-        if col >= 4:
-            lim = lim + dn[fin] * 4.0 * sig[fin] * (3.0 if col == 5 else 1.0) / nclip[fin]
+        if col >= 4:      # a boundary pixel (|x - mean| = qc_clip rms) moves the clipped mean by <= qc_clip rms / n_clip
+            lim = lim + dn[fin] * (qc_clip + 1.0) * sig[fin] * (qc_clip if col == 5 else 1.0) / nclip[fin]
         assert np.all(err <= lim), f"{tag}: {name} err {err.max()} lim {lim.min()}"
     # z is (difference of two nearly equal statistics) / SE with SE = rms/sqrt(n): the statistics'
     # own tolerance maps to 1e-5 sqrt(n) absolute in z (DESIGN.md "Tolerances")
@@ -89,7 +110,7 @@ def check_records(rec_g, det_o, pipe, cube, band_ok, tag=""):
     # values on the common set
     common, ig, io = np.intersect1d(key_g, key_o, return_indices=True)
     g, o = rec_g[ig], rec_o[io]
-    assert np.array_equal(g["iter"], o["iter"]) or n_ties > 0, f"{tag}: iter"
+    assert np.array_equal(g["iter"], o["iter"]), f"{tag}: iter"
     sig = np.sqrt(np.maximum(o["s"], 1e-300))
     for name, scale in (("f", sig), ("c", sig), ("snr", np.ones_like(sig))):
         err = np.abs(g[name].astype(np.float64) - o[name])
@@ -131,13 +152,36 @@ def gpu_step_by_calls(lpf, cube_d, t, lane=0):
 
 def check_frame(g: dict, o: dict, pipe, cube, tag=""):
     """Whole-frame comparison of a GPU result dict against the oracle's step() dict."""
-    zerr = check_qc(g["stats"], g["band_ok"], o["stats"], o["band_ok"], tag)
+    zerr = check_qc(g["stats"], g["band_ok"], o["stats"], o["band_ok"], tag, cube=cube, W=pipe.W, qc_clip=pipe.p["qc_clip"])
+    n0 = len(TIES)
     n_ties = check_records(g["rec"], o, pipe, cube, o["band_ok"], tag)
     same_u = check_unique(g["upos"], g["uplane"], g["usnr"], o, tag)
-    assert same_u or n_ties > 0, f"{tag}: unique positions differ without a logged tie: {g['upos']} vs {o['upos']}"
+    if not same_u:
+        # unique positions may differ only around a logged peak tie of THIS frame: every position in the symmetric
+        # difference must lie within r_dedupe of one (a tie adds / removes a record, which can change its neighbours)
+        tie_pix = [tp[2] for tp in TIES[n0:] if tp[3] in ("thr", "max")]
+        assert tie_pix, f"{tag}: unique positions differ without a logged tie: {g['upos']} vs {o['upos']}"
+        Dx, r = pipe.p["Dx"], pipe.p["r_dedupe"]
+        for q in np.setxor1d(g["upos"], o["upos"]):
+            d2 = min((q // Dx - tq // Dx) ** 2 + (q % Dx - tq % Dx) ** 2 for tq in tie_pix)
+            assert d2 <= (2 * r) ** 2, f"{tag}: unique position {q} differs and is not next to a logged tie {tie_pix}"
     if same_u:
         assert np.array_equal(g["cand_idx"], o["cand_idx"]), f"{tag}: cand_idx"
         assert np.array_equal(g["act_slots"], o["act_slots"]), f"{tag}: act_slots"
         assert np.array_equal(g["act_pix"], o["act_pix"]), f"{tag}: act_pix"
         assert g["flux"].shape == o["flux"].shape and np.array_equal(g["flux"], o["flux"]), f"{tag}: flux not bit-exact"
     return dict(zerr=zerr, n_ties=n_ties, in_sync=same_u)
+
+
+def dump_ties(path):
+    """Write the tie log (north_star: "any near-threshold ties are logged")."""
+    import json
+    import os
+    os.makedirs(os.path.dirname(os.path.abspath(path)), exist_ok=True)
+    kinds = {}
+    for t in TIES:
+        kinds[t[3]] = kinds.get(t[3], 0) + 1
+    with open(path, "w") as f:
+        json.dump({"n_ties": len(TIES), "by_kind": kinds,
+                   "ties": [dict(tag=t[0], plane=t[1], pix=t[2], kind=t[3], margin=t[4]) for t in TIES]}, f, indent=1)
+    return kinds

@@ -18,19 +18,15 @@ def torch_cuda():
 
 
 def _make(cfg, torch, **kw):
-    """Context for a config.  general=True forces the multi-kernel general path (LPF_FORCE_GENERAL);
+    """Context for a config.  general=True forces the multi-kernel general path (lpf_params.force_general);
     otherwise box/K=12/n_iter=1 contexts take the fused single-pass kernel."""
-    import os
     from paper_2103_15418_b200.binding import LPF
     s = synth.CubeStream(cfg)
     bg = kw.pop("bg", "box"); n_iter = kw.pop("n_iter", 1); general = kw.pop("general", False)
     p = synth.default_params(cfg, bg=bg, n_iter=n_iter)
     p.update(kw)
-    os.environ["LPF_FORCE_GENERAL"] = "1" if general else "0"
-    try:
-        lpf = LPF(p, s.mask)
-    finally:
-        os.environ["LPF_FORCE_GENERAL"] = "0"
+    p["force_general"] = 1 if general else 0
+    lpf = LPF(p, s.mask)
     want_fused = (not general) and bg == "box" and n_iter == 1 and p["k_bg"] == 12 and p["k_mf"] == 3
     assert lpf.plan()["fused"] == want_fused, lpf.plan()
     return s, p, lpf
@@ -487,8 +483,10 @@ def test_backward_fill_with_lanes_in_flight(torch_cuda):
 
 def test_running_pixel_qc(torch_cuda):
     """O12 (eq. A.2): per-pixel running mean / variance, test before update, update only accepted
-    bands.  Band verdicts and the per-band counts must equal the oracle's exactly in every frame (the decision is
-    taken in float32 with the same operation order on both sides); the rest of the chain follows band_ok."""
+    bands.  The oracle evaluates eq. A.2 in float64 on its float32 state; the per-band counts of the kernel (plain
+    float32) may differ from the oracle's only by pixels whose ORACLE margin |d^2 - thr^2 v| is within 2e-4 relative
+    (oracle's `near` count; every such difference is logged as a tie), the band verdicts must be equal; the rest of
+    the chain follows band_ok.  Also: the start-over rule (zeta_reset) after a lasting level change."""
     torch = torch_cuda
     s, p, lpf = _make(2, torch, zeta_thr=12.0, zeta_nmax=3, zeta_window=16, zeta_warm=8, n_lanes=2)
     pipe = O.OraclePipeline(p, s.mask, direct=False)
@@ -505,7 +503,10 @@ def test_running_pixel_qc(torch_cuda):
         o = pipe.step(cube, t)
         lpf.process_frame(torch.from_numpy(cube).cuda(), t, lane=t % 2, stream=streams[t % 2])
         g = lpf.frame_view(t % 2)
-        assert np.array_equal(g["zeta_cnt"], o["zeta_cnt"]), (t, g["zeta_cnt"], o["zeta_cnt"])
+        dz = np.abs(g["zeta_cnt"].astype(np.int64) - o["zeta_cnt"])
+        assert np.all(dz <= o["zeta_near"]), (t, g["zeta_cnt"], o["zeta_cnt"], o["zeta_near"])
+        for b in np.flatnonzero(dz):
+            parity.TIES.append((f"running qc t={t}", int(b), -1, "zeta", float(dz[b])))
         assert np.array_equal(g["band_ok"], o["band_ok"]), t
         r = parity.check_frame(g, o, pipe, cube, f"running qc t={t}")
         assert r["in_sync"]
@@ -513,6 +514,24 @@ def test_running_pixel_qc(torch_cuda):
         if t in (12, 13, 19):
             assert o["band_ok"][5] == 0 and o["zeta_cnt"][5] >= 6
     assert n_rej >= 4
+    lpf.close()
+    # a lasting local level change in one band (a 3x3 patch 14 sigma brighter from t = 16 on; small enough to pass
+    # eq. A.1): discarded three frames in a row, then the band starts over, is untested during its new warm-up and
+    # comes back for good
+    s, p, lpf = _make(2, torch, zeta_thr=10.0, zeta_nmax=3, zeta_window=16, zeta_warm=12, zeta_reset=3)
+    pipe = O.OraclePipeline(p, s.mask, direct=False)
+    seen = []
+    for t in range(36):
+        cube = s.frame(t)
+        if t >= 16:
+            cube = cube.copy(); cube[7, 100:103, 60:63] += 14.0
+        o = pipe.step(cube, t)
+        lpf.process_frame(torch.from_numpy(cube).cuda(), t)
+        g = lpf.frame_view(0)
+        assert np.all(np.abs(g["zeta_cnt"].astype(np.int64) - o["zeta_cnt"]) <= o["zeta_near"]), t
+        assert np.array_equal(g["band_ok"], o["band_ok"]), t
+        seen.append(int(g["band_ok"][7]))
+    assert seen[:16] == [1] * 16 and seen[16:19] == [0, 0, 0] and seen[19:] == [1] * 17, seen
     lpf.close()
 
 

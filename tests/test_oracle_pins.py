@@ -44,8 +44,7 @@ def test_band_stats_reduce_to_numpy():
         assert st[b, 0] == v.size
         assert abs(st[b, 1] - v.mean()) < 1e-12
         assert abs(st[b, 2] - v.std()) < 1e-12
-        v32 = cube[b][W == 1]   # clip membership is decided in float32 (reading R25)
-        keep = v[np.abs(v32 - np.float32(v.mean())) <= np.float32(3.0 * v.std())]
+        keep = v[np.abs(v - v.mean()) <= 3.0 * v.std()]      # O1: the plain float64 definition
         assert st[b, 3] == keep.size and keep.size < v.size
         assert abs(st[b, 4] - keep.mean()) < 1e-12 and abs(st[b, 5] - keep.std()) < 1e-12
     # no mask == all-ones mask
@@ -790,6 +789,88 @@ def test_running_qc_verdict_rules():
     f = mk(); f[0, 8, 8] += 500.0; f[0, 9, 2] += 500.0
     cnt, o = rq2.step(f, W, a1)
     assert cnt[0] == 2 and o.tolist() == [0, 0, 0, 1, 0]       # one accepted band of four: the frame is rejected
+
+
+def test_running_qc_variance_recurrence_and_stationary_value():
+    """eq. A.2 + R22 written out here in plain float64 NumPy, per pixel, through the Welford phase and far into the
+    exponentially weighted phase: m += a d, v = (1 - a)(v + a d^2), a = 1/min(k, window).  The oracle (float32 state,
+    one rounding per update) must follow it; and for a stationary stream of variance s^2 the recurrence has the
+    closed-form expectations  E[d^2] = 2 s^2/(2 - a),  E[v] = (1 - a) 2 s^2/(2 - a)  (k >> window)."""
+    import oracle as O
+    rng = np.random.default_rng(13)
+    B, D, Nw, sig = 2, 48, 16, 2.5
+    rq = O.RunningQC(B, D, D, thr=1e9, nmax=0, window=Nw, warm=4)
+    ok = np.ones(B + 1, np.uint8)
+    m = np.zeros((B, D, D)); v = np.zeros((B, D, D))
+    vs = []
+    for k in range(1, 12 * Nw + 1):
+        x = (1.0 + sig * rng.standard_normal((B, D, D))).astype(np.float32)
+        rq.step(x, None, ok)
+        a = 1.0 / min(k, Nw)
+        d = x.astype(np.float64) - m
+        m = m + a * d
+        v = (1.0 - a) * (v + a * d * d)
+        if k in (3, Nw, Nw + 1, 2 * Nw, 12 * Nw):
+            assert np.allclose(rq.m, m, rtol=0, atol=3e-5 * sig), k          # float32 state, contractive recurrence
+            assert np.allclose(rq.v, v, rtol=3e-5, atol=1e-6), k
+        if k > 6 * Nw:
+            vs.append(rq.v.astype(np.float64).mean())
+    a = 1.0 / Nw
+    want = (1.0 - a) * 2.0 * sig ** 2 / (2.0 - a)                             # 0.9677 s^2 for window 16
+    assert abs(np.mean(vs) / want - 1.0) < 0.01, (np.mean(vs), want)
+    # the nearest wrong recurrences are 3-7 % away: v = (1-a) v + a d^2 gives 2 s^2/(2-a); plain s^2 is 1.000
+    assert abs(np.mean(vs) / (2.0 * sig ** 2 / (2.0 - a)) - 1.0) > 0.04 and abs(np.mean(vs) / sig ** 2 - 1.0) > 0.02
+
+
+def test_running_qc_zeta_threshold_edge_and_zero_variance():
+    """|zeta| = thr (1 +- 1e-3): after the two frames +1, -1 the state is m = 0, v = 1 exactly (Welford), so a pixel
+    at thr (1 + 1e-3) exceeds and one at thr (1 - 1e-3) does not, either sign; a pixel whose stream was constant so far
+    (v = 0) has no zeta and is not counted."""
+    import oracle as O
+    B, D, thr = 1, 8, 15.0
+    rq = O.RunningQC(B, D, D, thr=thr, nmax=0, window=64, warm=2)
+    ok = np.ones(B + 1, np.uint8)
+    f = np.ones((B, D, D), np.float32); f[0, 7, 7] = 0.0
+    g = -f
+    rq.step(f, None, ok); rq.step(g, None, ok)
+    assert np.array_equal(rq.m[0, :7, :7], np.zeros((7, 7), np.float32)) and np.array_equal(rq.v[0, :7, :7], np.ones((7, 7), np.float32))
+    assert rq.v[0, 7, 7] == 0.0
+    x = np.zeros((B, D, D), np.float32)
+    x[0, 1, 1] = thr * (1 + 1e-3); x[0, 2, 2] = thr * (1 - 1e-3); x[0, 3, 3] = -thr * (1 + 1e-3); x[0, 4, 4] = -thr * (1 - 1e-3)
+    x[0, 7, 7] = 1e6                                     # v = 0 there: not tested
+    cnt, o = rq.step(x, None, ok)
+    assert cnt.tolist() == [2] and o.tolist() == [0, 0]
+    rq2 = O.RunningQC(B, D, D, thr=thr, nmax=2, window=64, warm=2)
+    rq2.step(f, None, ok); rq2.step(g, None, ok)
+    cnt, o = rq2.step(x, None, ok)
+    assert cnt.tolist() == [2] and o.tolist() == [1, 1]      # count rule: 2 > 2 is false
+    W = np.ones((D, D), np.uint8); W[1, 1] = 0
+    rq3 = O.RunningQC(B, D, D, thr=thr, nmax=0, window=64, warm=2)
+    rq3.step(f, W, ok); rq3.step(g, W, ok)
+    assert rq3.step(x, W, ok)[0].tolist() == [1]             # the masked one does not count
+
+
+def test_running_qc_recovers_after_a_lasting_level_change():
+    """R22: a band discarded by eq. A.2 keeps its state, so after a lasting level change it would stay discarded for
+    good; with zeta_reset = 3 it starts over after three consecutive discards and is accepted again after the warm-up."""
+    import oracle as O
+    rng = np.random.default_rng(14)
+    B, D = 2, 16
+    mk = lambda off: (off + rng.standard_normal((B, D, D))).astype(np.float32)
+    ok = np.ones(B + 1, np.uint8)
+    for reset, want_back in ((0, False), (3, True)):
+        rq = O.RunningQC(B, D, D, thr=8.0, nmax=4, window=16, warm=4, reset=reset)
+        for _ in range(12):
+            assert rq.step(mk(0.0), None, ok)[1].all()
+        verdicts = []
+        for k in range(12):
+            f = mk(0.0); f[1] += 100.0                   # band 1 jumps by 100 sigma and stays there
+            verdicts.append(int(rq.step(f, None, ok)[1][1]))
+        if want_back:
+            assert verdicts[:3] == [0, 0, 0] and all(verdicts[3:]), verdicts      # reset after the 3rd, untested warm-up, then fine
+            assert abs(float(rq.m[1].mean()) - 100.0) < 1.0
+        else:
+            assert not any(verdicts)
 
 
 # ------------------------------------------------------------------ O13 / O14 network input and simulated pulses
