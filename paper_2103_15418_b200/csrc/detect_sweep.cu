@@ -188,7 +188,8 @@ struct Lay {
   static constexpr int O_V1 = O_X + XST * RB * XP;
   static constexpr int O_V2 = O_V1 + NV * RB * PV;
   static constexpr int O_FR = O_V2 + NV * RB * PV;
-  static constexpr int O_BAR = O_FR + DF * PF;     // mbarriers, 2 floats each
+  static constexpr int O_FLG = O_FR + DF * PF;     // eq. 6 flags, one byte per thread and row, 32 rows
+  static constexpr int O_BAR = O_FLG + 32 * NG * 32 / 4;     // mbarriers, 2 floats each
   static constexpr int B_FULL_X = 0, B_EMPTY_X = XST, B_FULL_V1 = 2 * XST, B_EMPTY_V1 = B_FULL_V1 + NV,
                        B_FULL_V2 = B_EMPTY_V1 + NV, B_EMPTY_V2 = B_FULL_V2 + NV, N_BAR = B_EMPTY_V2 + NV;
   static constexpr int O_END = O_BAR + 2 * N_BAR;
@@ -429,9 +430,11 @@ struct RoleB {
   const FusedArgs& a;
   const float* icp;        // padded 1/count at the next step's first rho row
   float2 V2[4], E[4];      // running sum of d^2; sum of V2^2 over the rows since the last exact re-sum
+  float2 Fw[6][4];         // the F rows (invalid pixels -inf) of this step and the two before (rotating, 3 phases)
   float4 ic[RB][2];
   Stage sv;                // stage of both rings (V1 consumed, V2 produced: same step index)
   int fr;                  // F-ring slot of this step's first rho row
+  int fq;                  // flag-ring row of rho0 - 2 (the first row whose eq. 6 flags this step settles)
 
   __device__ __forceinline__ RoleB(const Ctx& c_, const FusedArgs& a_) : c(c_), a(a_) {}
 
@@ -443,7 +446,9 @@ struct RoleB {
     icp += RB * c.sx;
   }
 
+  template <int PH3>
   __device__ __forceinline__ void step(int s, unsigned fl) {
+    constexpr int WN = 2 * PH3, WP = 2 * ((PH3 + 2) % 3), WPP = 2 * ((PH3 + 1) % 3);   // window rows: new, previous step, the one before
     const uint32_t w0 = (uint32_t)(RB * s) & (DR - 1);
     const uint32_t t_lag0 = c.tm + PX * ((w0 + 20) & (DR - 1)), t_lag1 = t_lag0 + PX;       // F(rho): w0 + 20 is even
     const uint32_t t_new0 = c.tm + TM_D + PX * w0, t_new1 = t_new0 + PX;
@@ -489,10 +494,37 @@ struct RoleB {
         const int o = L::O_V2 + (sv.s * RB + j) * L::PV + KBG + PX * c.t;
         sts4(o, make_float4(V2[0].x, V2[0].y, V2[1].x, V2[1].y));
         sts4(o + 4, make_float4(V2[2].x, V2[2].y, V2[3].x, V2[3].y));
-        int sl = fr + j; sl = sl >= DF ? sl - DF : sl;
-        const int of = L::O_FR + sl * L::PF + 4 + PX * c.t;
-        sts4(of, make_float4(fm[0].x, fm[0].y, fm[1].x, fm[1].y));
-        sts4(of + 4, make_float4(fm[2].x, fm[2].y, fm[3].x, fm[3].y));
+#pragma unroll
+        for (int p = 0; p < 4; ++p) Fw[WN + j][p] = fm[p];
+      }
+      {   // eq. 6, vertical half, for the two rows of the previous step (centres q = rho0 - 2, rho0 - 1: their windows are
+          // complete now): cm = the column maximum over rows q-k_max .. q+k_max goes to the shared ring (group C compares
+          // it across columns), and one bit per pixel says whether F(q, x) is that maximum (then cm IS F(q, x))
+        const int km = a.k_max;
+        uint8_t* flg = reinterpret_cast<uint8_t*>(reinterpret_cast<float*>(g_sm4) + L::O_FLG);
+#pragma unroll
+        for (int j = 0; j < RB; ++j) {
+          float2 cm[4];
+          unsigned q = 0u;
+#pragma unroll
+          for (int p = 0; p < 4; ++p) {
+            // rows around the centre WP + j: one up / down, two up / down (window slots of the three steps)
+            const float2 ce = Fw[WP + j][p];
+            const float2 u1 = j ? Fw[WP][p] : Fw[WPP + 1][p], d1 = j ? Fw[WN][p] : Fw[WP + 1][p];
+            const float2 u2 = j ? Fw[WPP + 1][p] : Fw[WPP][p], d2 = j ? Fw[WN + 1][p] : Fw[WN][p];
+            float2 x = ce;
+            if (km >= 1) x = make_float2(fmaxf(x.x, fmaxf(u1.x, d1.x)), fmaxf(x.y, fmaxf(u1.y, d1.y)));
+            if (km >= 2) x = make_float2(fmaxf(x.x, fmaxf(u2.x, d2.x)), fmaxf(x.y, fmaxf(u2.y, d2.y)));
+            cm[p] = x;
+            q |= (ce.x >= x.x ? 1u : 0u) << (2 * p);
+            q |= (ce.y >= x.y ? 1u : 0u) << (2 * p + 1);
+          }
+          int sl = fr + j - 2; sl = sl < 0 ? sl + DF : sl;
+          const int of = L::O_FR + sl * L::PF + 4 + PX * c.t;
+          sts4(of, make_float4(cm[0].x, cm[0].y, cm[1].x, cm[1].y));
+          sts4(of + 4, make_float4(cm[2].x, cm[2].y, cm[3].x, cm[3].y));
+          flg[((fq + j) & 31) * (NG * 32) + c.t] = (uint8_t)q;
+        }
       }
       // the roundings V2 has inherited: variance 2^-46/6 * sum of V2^2 over the rows since the last exact re-sum
       float2 tq[4];
@@ -516,6 +548,7 @@ struct RoleB {
     if (c.lane == 0) mbar_arrive(L::bar(L::B_FULL_V2 + sv.s));
     sv.next(NV);
     fr += RB; fr = fr >= DF ? fr - DF : fr;
+    fq += RB;
   }
 
   __device__ __forceinline__ void run() {
@@ -524,54 +557,48 @@ struct RoleB {
       load_ic(f0 & FL_ICR_LD);
     }
     unsigned f0 = ctl<NG>(c, 0), f1 = ctl<NG>(c, 1), f2 = ctl<NG>(c, 2);
-    for (int b = 0; b < c.nb; ++b) {
-      const unsigned f3 = ctl<NG>(c, b + 3);
-      step(b, f0);
-      f0 = f1; f1 = f2; f2 = f3;
+    int b = 0;
+    while (true) {     // the word of step b + 3 takes the place of the one just used
+      step<0>(b, f0); f0 = ctl<NG>(c, b + 3); if (++b >= c.nb) break;
+      step<1>(b, f1); f1 = ctl<NG>(c, b + 3); if (++b >= c.nb) break;
+      step<2>(b, f2); f2 = ctl<NG>(c, b + 3); if (++b >= c.nb) break;
     }
   }
 };
 
 // ---- group C: local spread, eq. 5, and for the hits eq. 6 / eq. 7 ------------------------------------------
-// The warp tests the pixels flagged in `bits` (one byte per lane) one after the other, all lanes together:
-// the owner broadcasts the pixel, 25 lanes fetch one neighbour each from the shared F ring (rows sigma-k_max ..
-// sigma+k_max, invalid pixels and the margins hold -inf) and a vote settles eq. 6; S_eff guard (R8) and eq. 5 in its
-// rounded form on the way.  The records of the warp's row go to the global list with one atomic.
-// o_fr: float index of the F ring; sl: ring slot of row sg; cl: strip column of the lane's first pixel.
-struct Hit8 { float d[8], s[8]; };
-template <int PF>
-__device__ __noinline__ void c_hits(const FusedArgs* ap, int o_fr, int sl, int cl, int sg, int xs, int plane, int lane, unsigned bits,
-                                    const Hit8 h) {
+// The pixels flagged in `bits` (one byte per lane) passed the unguarded eq. 5 and the vertical half of eq. 6 (group B's
+// flag: F is the maximum of its column over the window's rows, so the ring value cm at that pixel IS F).  What is left:
+// the horizontal half, cm(x) >= cm(x + dx) for |dx| <= k_max on the shared ring row (invalid pixels and the margins
+// hold -inf), the S_eff guard (R8) and eq. 5 in its rounded form.  The records of the warp's row go to the global list
+// with one atomic.  row0: float index of the lane's first pixel in the ring row of sigma; cl: its strip column.
+__device__ __noinline__ void c_hits(const FusedArgs* ap, int row0, int cl, int sg, int xs, int plane, int lane, unsigned bits,
+                                    float4 d0, float4 d1, float4 s0, float4 s1) {
   const FusedArgs& a = *ap;
   const int km = a.k_max;
-  const int wdy = lane / 5 - 2, wdx = lane - 5 * (lane / 5) - 2;           // this lane's window offset (lanes 0..24)
-  const bool in_win = lane < 25 && wdy >= -km && wdy <= km && wdx >= -km && wdx <= km;
-  int wr = sl + wdy; wr = wr < 0 ? wr + DF : (wr >= DF ? wr - DF : wr);
-  const int woff = o_fr + 4 + wr * PF + wdx;                                // + strip column of the pixel
-  float fv[8], se[8];
+  float cm[12];                                      // columns -2 .. 9 relative to the lane's first pixel
+  {
+    const float4 q0 = lds4(row0), q1 = lds4(row0 + 4);
+    const float2 ql = *reinterpret_cast<const float2*>(reinterpret_cast<const float*>(g_sm4) + row0 - 2);
+    const float2 qr = *reinterpret_cast<const float2*>(reinterpret_cast<const float*>(g_sm4) + row0 + 8);
+    cm[0] = ql.x; cm[1] = ql.y; cm[2] = q0.x; cm[3] = q0.y; cm[4] = q0.z; cm[5] = q0.w;
+    cm[6] = q1.x; cm[7] = q1.y; cm[8] = q1.z; cm[9] = q1.w; cm[10] = qr.x; cm[11] = qr.y;
+  }
+  const float d[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
+  const float sv[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
   unsigned ok = 0u;
+  float se[8];
 #pragma unroll
   for (int k = 0; k < 8; ++k) {
-    fv[k] = 0.f; se[k] = 1.f;
-    unsigned m = __ballot_sync(0xffffffffu, (bits >> k) & 1u);
-    while (m) {
-      const int src = __ffs(m) - 1;
-      m &= m - 1;
-      const int col = __shfl_sync(0xffffffffu, cl, src) + k;
-      const float d = __shfl_sync(0xffffffffu, h.d[k], src);
-      const float s = __shfl_sync(0xffffffffu, h.s[k], src);
-      const float fn = in_win ? lds1(woff + col) : __int_as_float(0xff800000);
-      const float f = __shfl_sync(0xffffffffu, fn, 12);                      // the pixel itself
-      const float cc = f - d;
-      const float gd = a.eps_rel * fabsf(cc);
-      const float sef = fmaxf(s, gd * gd);
-      const bool pass = d > 0.f && d * d > a.kappa2 * sef;
-      const unsigned bigger = __ballot_sync(0xffffffffu, fn > f);
-      if (lane == src) {
-        fv[k] = f; se[k] = sef;
-        if (pass && bigger == 0u) ok |= 1u << k;
-      }
-    }
+    const float f = cm[k + 2];
+    float nb = __int_as_float(0xff800000);
+    if (km >= 1) nb = fmaxf(cm[k + 1], cm[k + 3]);
+    if (km >= 2) nb = fmaxf(nb, fmaxf(cm[k], cm[k + 4]));
+    const float cc = f - d[k];
+    const float gd = a.eps_rel * fabsf(cc);
+    const float sef = fmaxf(sv[k], gd * gd);
+    se[k] = sef;
+    if (((bits >> k) & 1u) && !(nb > f) && d[k] > 0.f && d[k] * d[k] > a.kappa2 * sef) ok |= 1u << k;
   }
   // append: exclusive prefix of the lanes' counts, one atomic for the warp
   const int n = __popc(ok);
@@ -590,8 +617,8 @@ __device__ __noinline__ void c_hits(const FusedArgs* ap, int o_fr, int sl, int c
     if (idx < a.max_det) {
       uint2* dst = reinterpret_cast<uint2*>(a.dets + idx);
       dst[0] = make_uint2((uint32_t)(sg * a.Dx + xs + cl + k), (uint32_t)(plane & 0xffff) | (1u << 16));   // int16 plane, int16 iter = 1
-      dst[1] = make_uint2(__float_as_uint(fv[k]), __float_as_uint(fv[k] - h.d[k]));
-      dst[2] = make_uint2(__float_as_uint(se[k]), __float_as_uint(h.d[k] / sqrtf(se[k])));
+      dst[1] = make_uint2(__float_as_uint(cm[k + 2]), __float_as_uint(cm[k + 2] - d[k]));
+      dst[2] = make_uint2(__float_as_uint(se[k]), __float_as_uint(d[k] / sqrtf(se[k])));
     } else {
       atomicAdd(&a.counters[0], 1);
     }
@@ -659,13 +686,15 @@ struct RoleC {
 #pragma unroll
           for (int k = 0; k < 8; ++k)
             if (dv[k] > 0.f && mv[k] > 0.f) bits |= 1u << k;
-          bits &= umask;
+          {   // group B's flags of row sigma: the vertical half of eq. 6 (written 10 rows ago)
+            const uint8_t* flg = reinterpret_cast<const uint8_t*>(reinterpret_cast<const float*>(g_sm4) + L::O_FLG);
+            bits &= umask & (unsigned)flg[((RB * s + j + 20) & 31) * (NG * 32) + c.t];
+          }
           if (__any_sync(0xffffffffu, bits != 0u)) {
             int sl = fr + j; sl = sl >= DF ? sl - DF : sl;
-            Hit8 h;
-#pragma unroll
-            for (int p = 0; p < 4; ++p) { h.d[2 * p] = dl[j][p].x; h.d[2 * p + 1] = dl[j][p].y; h.s[2 * p] = S[p].x; h.s[2 * p + 1] = S[p].y; }
-            c_hits<L::PF>(c.a, L::O_FR, sl, PX * c.t, y0 + j - LAG_C, c.xs, c.plane, c.lane, bits, h);
+            c_hits(c.a, L::O_FR + 4 + sl * L::PF + PX * c.t, PX * c.t, y0 + j - LAG_C, c.xs, c.plane, c.lane, bits,
+                          make_float4(dl[j][0].x, dl[j][0].y, dl[j][1].x, dl[j][1].y), make_float4(dl[j][2].x, dl[j][2].y, dl[j][3].x, dl[j][3].y),
+                          make_float4(S[0].x, S[0].y, S[1].x, S[1].y), make_float4(S[2].x, S[2].y, S[3].x, S[3].y));
           }
         }
       }
@@ -785,6 +814,11 @@ k_sweep_box(const FusedArgs a) {
 #pragma unroll
       for (int j = 0; j < RB; ++j) { r.ic[j][0] = zero4(); r.ic[j][1] = zero4(); }
       r.fr = 0;
+      r.fq = 30;                // rho0 - 2 of step 0, modulo the 32 rows of the flag ring
+#pragma unroll
+      for (int i = 0; i < 6; ++i)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) r.Fw[i][q] = splat(__int_as_float(0xff800000));
       r.run();
     } else {
       RoleC<NG> r(c, a);
