@@ -1,31 +1,36 @@
-// S4-S8 fused fast path: matched filter -> local centre -> local spread -> sigma clip -> local
-// maxima -> compaction in ONE pass over each plane, for the headline parameter set
-// (box background K = 12, Gaussian matched filter k_mf = 3, n_iter = 1).
+// S4-S8 fused fast path: matched filter -> local centre -> local spread -> sigma clip in ONE pass over
+// each plane (k_sweep), local maxima + records in a short follow-up over the few survivors (k_peaks), for
+// the headline parameter set (box background K = 12, Gaussian matched filter k_mf = 3, n_iter = 1).
 // (eqs. 2-7; O3-O6 and "Fused detection kernel".)
 //
-// Design (sm_100a).  A CTA owns a column strip (4 columns per thread, up to 1024 columns) and sweeps
-// down a segment of rows, two rows per iteration, as a three-stage software pipeline with ONE
-// block barrier per iteration (the stages of one iteration work on different rows, so their
-// shared-memory exchanges are double buffered and independent):
+// k_sweep (sm_100a).  A CTA owns a column strip (4 columns per thread, 128 per warp) and sweeps down a
+// segment of rows, two rows per iteration, as a three-stage software pipeline with ONE block barrier per
+// iteration (the stages of one iteration work on different rows, so their shared-memory exchanges are
+// double buffered and independent):
 //   A  rows y:        the input rows arrive in shared memory by bulk asynchronous copies (TMA,
-//                     cp.async.bulk + mbarrier) issued three iterations ahead by one thread; every
-//                     thread reads its 4 pixels and both neighbours' with three 128-bit shared loads ->
-//                     horizontal 7-tap matched filter -> vertical 7-tap on a register window (packed
-//                     f32x2) -> F(y-3); 25-row running sum V1 += F(y-3) - F(y-28)
-//   B  rows rho=y-17: horizontal 25-box of V1 (blocked partial sums) x 1/count -> C (eq. 3);
-//                     d = F - C; 25-row running sum V2 += d^2 - d_old^2
-//   C  rows sig=y-31: horizontal 25-box of V2 x 1/count -> S (eq. 4); eq. 5 on d(sig) for the whole
-//                     row with four packed operations and one vote; rows with a hit go out of line:
-//                     exact bits, a cheap in-thread 3x3 pre-filter on the F ring, then the S_eff guard
-//                     (R8), eq. 6 with one neighbour per lane and the eq. 7 record.
-// The 32-row histories of F and d that the running sums and the lagged reads need are private to
-// a thread, so they live in TENSOR MEMORY (tcgen05.st/ld 32x32b.x4, two power-of-two rings of 128
-// columns per thread); shared memory carries only what threads exchange plus a 32-row ring of F for
-// the local-maximum tests.  What a warp has to decide in an iteration (is there input, which
-// normalisers are the interior constants, which stages run) is one 32-bit word of a per-item table
-// built by the host plan.  F, C, d, S never leave the SM.
-// The input is used unmasked when the cube holds exact zeros at every invalid pixel (checked per
-// frame by the sum-plane kernel); otherwise each thread applies W itself (slow, rare).
+//                     cp.async.bulk + mbarrier) issued XST - 1 iterations ahead by thread 0; every thread
+//                     reads its 4 pixels and both neighbours' with three 128-bit shared loads -> horizontal
+//                     7-tap matched filter -> vertical 7-tap on a register window (packed f32x2) -> F(y-3);
+//                     25-row running sum V1 += F(y-3) - F(y-28)
+//   B  rows rho=y-17: horizontal 25-box of V1 (group sums, every window summed afresh) x 1/count -> C
+//                     (eq. 3); d = F - C; 25-row running sum V2 += d^2 - d_old^2
+//   C  rows sig=y-31: horizontal 25-box of V2 x 1/count -> S (eq. 4); eq. 5 on d(sig) for the whole row with
+//                     four packed operations and one vote; a thread with a hit drops the pixels that a
+//                     vertical neighbour of its own columns already beats (F from tensor memory) and appends
+//                     one 48-byte entry {pixel, bits, d[4], S[4]} to the CTA's segment of the hit list.
+// The 32-row histories of F and d that the running sums and the lagged reads need are private to a
+// thread, so they live in TENSOR MEMORY (tcgen05.st/ld 32x32b.x4, two power-of-two rings of 128 columns
+// per thread); shared memory carries only what threads exchange and the input stages.  What a warp has to
+// decide in an iteration (is there input, which normalisers are the interior constants, which stages run)
+// is one 32-bit word of a per-item table built by the host plan.  F, C, d, S never leave the SM.
+// A value far above the plane's noise that leaves a running sum would leave its rounding behind for the
+// rest of the sweep: in that iteration the sum is rebuilt from the ring instead (warp-uniform, rare).
+// The input is used unmasked when the cube holds exact zeros at every invalid pixel (checked per frame by
+// the QC pass); otherwise each thread applies W itself (slow, rare).
+//
+// k_peaks.  One thread per surviving pixel recomputes F on its (2 k_max + 1)^2 neighbourhood from the raw
+// plane with the sweep's own operation order (so the values are the sweep's, bit for bit), applies the
+// S_eff guard (R8), the rounded eq. 5, eq. 6 and writes the eq. 7 record.
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
@@ -43,13 +48,20 @@ constexpr int HALO = 2 * KBG + 3;   // rows of X above the first output row (27)
 constexpr int LAG_B = 3 + KBG + RB;          // rho = y - 17
 constexpr int LAG_C = LAG_B + KBG + RB;      // sig = y - 31
 constexpr int DR = 32;              // depth (rows) of the tensor-memory rings of F and d (power of two)
-constexpr int DRS = 34;             // depth of the shared-memory ring of F: local maxima are tested one iteration late
-constexpr int QCAP = 64;            // queued candidates per iteration (more are tested in place)
-constexpr int SCAP = 32;            // records staged by a helper warp between flushes
-constexpr int NHW = 3;              // helper warps: input producer and candidate tests
-constexpr int XST = 4;              // input staging stages (iterations in flight)
+#ifndef LPF_XST
+#define LPF_XST 16
+#endif
+constexpr int XST = LPF_XST;        // input staging stages (iterations in flight, power of two)
 constexpr int TM_D = 4 * DR;        // first tensor-memory column of the d ring (F ring starts at 0)
 constexpr int PADR = 64;            // zero rows above and below the padded normaliser planes
+constexpr float BIG_SIGMA = 64.f;
+constexpr long long HIT_BUDGET = 1ll << 20;   // entries of the hit list of one frame (48 bytes each)
+#ifndef LPF_EXP_SKIP
+#define LPF_EXP_SKIP 0            // experiment switch (timing only): 1 no stage C, 2 no stage B, 4 no stage A part 2, 8 no stage A part 1
+#endif
+#ifndef LPF_SWEEP_MAXW
+#define LPF_SWEEP_MAXW 1024       // widest column strip of a CTA (1024: 8 warps, 1 CTA per SM; 512: 4 warps, 2 CTAs per SM)
+#endif   // "far above the noise": |value| > BIG_SIGMA x rms of the plane
 
 // per-(iteration, warp) control word
 constexpr unsigned FL_X = 1u;              // stage A has input: rows in the image, something valid near the warp
@@ -65,13 +77,18 @@ constexpr unsigned FL_C1 = 1u << 14;
 
 struct FusedItem { int xs, ux0, ux1, ya, yb, y_start, nb, fl_off; };
 
+// one entry of the hit list: the pixels of one thread and row that pass eq. 5 and the vertical pre-filter
+struct alignas(16) HitRec { int32_t pix0, bits, pad0, pad1; float d[4]; float s[4]; };
+
 struct FusedArgs {
   const float* cube; const float* sum_plane; const uint8_t* band_ok; const uint8_t* W;
   const float* nm_pad; const float* ic_pad;      // [(Dy + 2 PADR)][Dx], zero rows around the image
   const FusedItem* items; const uint32_t* flags;
   const int32_t* dirty; int dirty_seq;           // *dirty == dirty_seq: some invalid pixel of this cube is not an exact zero
-  int B, Dy, Dx, CW, k_max, max_det;
+  const float* big_thr;                          // [B + 1] BIG_SIGMA x rms of each plane
+  int B, Dy, Dx, CW, k_max, max_det, seg_cap, n_items;
   float g0, g1, g2, g3, kappa2, eps_rel, nm_const, ic_const;
+  HitRec* hits; int32_t* hit_cnt;                // [segments][seg_cap], [segments]; segment = plane * items + item
   lpf_det* dets; int32_t* ndets; int32_t* counters;
 };
 
@@ -90,6 +107,7 @@ __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __
 __device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __ffma2_rn(b, make_float2(-1.f, -1.f), a); }
 __device__ __forceinline__ float2 splat(float s) { return make_float2(s, s); }
 __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ float amax4(float2 a, float2 b) { return fmaxf(fmaxf(fabsf(a.x), fabsf(a.y)), fmaxf(fabsf(b.x), fabsf(b.y))); }
 
 // ---- tensor memory as a thread-private scratch ring ---------------------------------------------
 __device__ __forceinline__ void tm_st4(uint32_t taddr, float2 lo, float2 hi) {
@@ -140,203 +158,33 @@ __device__ __forceinline__ float lds1(int i) { return reinterpret_cast<const flo
 __device__ __forceinline__ void sts4(int i, float4 v) { *reinterpret_cast<float4*>(reinterpret_cast<float*>(g_sm4) + i) = v; }
 __device__ __forceinline__ void sts1(int i, float v) { reinterpret_cast<float*>(g_sm4)[i] = v; }
 
-// horizontal 25-box of a row of per-column values, 4 per thread: the six group sums q-3..q+2 give the
-// window of the thread's first column up to one pixel, the other three windows slide.
-// ev: float index of the thread's group q-3 in the value row; et: index of group sum q-3.
-__device__ __forceinline__ void hbox25(int ev, int et, float out[4]) {
+// horizontal 25-box of a row of per-column values, 4 per thread.  The window of the thread's column k is the
+// last 4 - k values of group q-3, the groups q-2 .. q+2 (their sums were exchanged) and the first k + 1 values
+// of group q+3; every window is summed afresh (no sliding: a huge column that leaves would leave its rounding).
+// ev: float index of group q-3 in the value row; et: index of the group sum q-3.
+__device__ __forceinline__ void hbox25(int ev, int et, float2& o01, float2& o23) {
   const float4 L = lds4(ev);        // group q-3
   const float4 R = lds4(ev + 24);   // group q+3
-  const float t0 = lds1(et), t1 = lds1(et + 1), t2 = lds1(et + 2), t3 = lds1(et + 3), t4 = lds1(et + 4), t5 = lds1(et + 5);
-  out[0] = (((t0 + t1) + (t2 + t3)) + (t4 + t5)) + R.x;
-  out[1] = out[0] + (R.y - L.x);
-  out[2] = out[1] + (R.z - L.y);
-  out[3] = out[2] + (R.w - L.z);
+  const float t1 = lds1(et + 1), t2 = lds1(et + 2), t3 = lds1(et + 3), t4 = lds1(et + 4), t5 = lds1(et + 5);
+  const float a5 = ((t1 + t2) + (t3 + t4)) + t5;
+  const float l2 = L.z + L.w, l1 = L.y + l2, l0 = L.x + l1;
+  const float r1 = R.x + R.y, r2 = r1 + R.z, r3 = r2 + R.w;
+  o01 = add2(add2(make_float2(l0, l1), make_float2(R.x, r1)), splat(a5));
+  o23 = add2(add2(make_float2(l2, L.w), make_float2(r2, r3)), splat(a5));
 }
 
-// ---- candidate path ---------------------------------------------------------------------------------
-// Pixels that pass the unguarded eq. 5 are queued by the sweep warps (a few per iteration) and tested one
-// iteration later by a dedicated warp, off the sweep's critical path: S_eff guard (R8), eq. 6 on the
-// shared-memory ring of F, eq. 7 record.  One candidate per lane, up to 32 at a time.
-struct CandCtx {           // what the candidate functions need, by value
-  const FusedArgs* ap;     // kernel arguments (shared-memory copy)
-  int CWP, xs, plane, lane, ring_y0;
-};
-
-__device__ __forceinline__ int ring_slot(int row, int ring_y0) { return (int)((unsigned)(row - ring_y0) % (unsigned)DRS); }
-
-// the test of one candidate by its own lane; returns true when it is a peak (fills f, c, s_eff).
-// KM = k_max at compile time (fully unrolled window, independent shared loads); KM < 0: run-time k_max.
-template <int KM>
-__device__ __forceinline__ bool cand_test_lane(const CandCtx& c, int cl, int sg, float d, float s,
-                                               float& fv, float& cc, float& se) {
-  const FusedArgs& a = *c.ap;
-  const int CWP = c.CWP;
-  const int s0 = ring_slot(sg, c.ring_y0);
-  fv = lds1(s0 * CWP + cl);
-  cc = fv - d;
-  const float gd = a.eps_rel * fabsf(cc);
-  se = fmaxf(s, gd * gd);
-  if (!(d > 0.f && d * d > a.kappa2 * se)) return false;
-  const int km = KM >= 0 ? KM : a.k_max;
-  bool bigger = false, zero_wins = false;       // a neighbour with F = 0 > fv: masked or not?  (rare: asks W)
-#pragma unroll
-  for (int dy = -km; dy <= km; ++dy) {
-    const int yy = sg + dy;
-    int sl = s0 + dy;
-    sl = sl < 0 ? sl + DRS : (sl >= DRS ? sl - DRS : sl);
-    const bool row_in = yy >= 0 && yy < a.Dy;
-#pragma unroll
-    for (int dx = -km; dx <= km; ++dx) {
-      const int c2 = cl + dx;
-      const bool in = row_in && c2 >= 0 && c2 < CWP && c.xs + c2 < a.Dx;
-      const float fn = in ? lds1(sl * CWP + c2) : fv;
-      bigger = bigger || (fn > fv && fn != 0.f);
-      zero_wins = zero_wins || (fn > fv && fn == 0.f);
-    }
+// sum over the 23 ring rows before slot w (rows k = 1 .. 23 back), of the values (sq = 0) or their squares
+__device__ __noinline__ float4 ring_sum23(uint32_t ring, int w, int sq) {
+  float2 a0 = splat(0.f), a1 = splat(0.f);
+  for (int k = 1; k <= 23; ++k) {
+    float2 lo, hi;
+    tm_ld4(ring + 4u * (uint32_t)((w - k) & (DR - 1)), lo, hi);
+    tm_wait_ld();
+    tm_use(lo, hi);
+    if (sq) { a0 = fma2(lo, lo, a0); a1 = fma2(hi, hi, a1); }
+    else { a0 = add2(a0, lo); a1 = add2(a1, hi); }
   }
-  if (bigger) return false;
-  if (zero_wins) {
-    for (int dy = -km; dy <= km; ++dy)
-      for (int dx = -km; dx <= km; ++dx) {
-        const int yy = sg + dy, c2 = cl + dx, xn = c.xs + c2;
-        if (yy < 0 || yy >= a.Dy || c2 < 0 || c2 >= CWP || xn >= a.Dx) continue;
-        if (lds1(ring_slot(yy, c.ring_y0) * CWP + c2) > fv && a.W[(long long)yy * a.Dx + xn] != 0) return false;
-      }
-  }
-  return true;
-}
-
-__device__ __forceinline__ bool cand_test_any(const CandCtx& c, int cl, int sg, float d, float s, float& fv, float& cc, float& se) {
-  const int km = c.ap->k_max;
-  if (km == 2) return cand_test_lane<2>(c, cl, sg, d, s, fv, cc, se);
-  if (km == 1) return cand_test_lane<1>(c, cl, sg, d, s, fv, cc, se);
-  return cand_test_lane<-1>(c, cl, sg, d, s, fv, cc, se);
-}
-
-// staged records (shared memory, 8 words each, n of them at float index o_st) -> global list, one atomic
-__device__ __noinline__ void cand_flush(const FusedArgs* ap, int o_st, int lane, int n) {
-  if (n <= 0) return;
-  int base = 0;
-  if (lane == 0) base = atomicAdd(ap->ndets, n);
-  base = __shfl_sync(0xffffffffu, base, 0);
-  for (int i = lane; i < n; i += 32) {
-    const uint2* r = reinterpret_cast<const uint2*>(reinterpret_cast<const uint32_t*>(g_sm4) + o_st + i * 8);
-    const int idx = base + i;
-    if (idx < ap->max_det) {
-      uint2* dst = reinterpret_cast<uint2*>(ap->dets + idx);
-      uint2 r2 = r[2];
-      r2.y = __float_as_uint(__uint_as_float(r2.y) / sqrtf(__uint_as_float(r2.x)));
-      dst[0] = r[0]; dst[1] = r[1]; dst[2] = r2;
-    } else {
-      atomicAdd(&ap->counters[0], 1);
-    }
-  }
-  __syncwarp();
-}
-
-// lanes with ok stage their records at o_st (nst staged so far, room for SCAP); returns the new count
-__device__ __forceinline__ int cand_stage(const CandCtx& c, int o_st, int nst, bool ok, int cl, int sg, float d, float fv, float cc, float se) {
-  const FusedArgs& a = *c.ap;
-  const unsigned m = __ballot_sync(0xffffffffu, ok);
-  if (!m) return nst;
-  if (nst + __popc(m) > SCAP) { cand_flush(c.ap, o_st, c.lane, nst); nst = 0; }
-  if (ok) {
-    uint32_t* r = reinterpret_cast<uint32_t*>(g_sm4) + o_st + (nst + __popc(m & ((1u << c.lane) - 1u))) * 8;
-    r[0] = (uint32_t)(sg * a.Dx + c.xs + cl);
-    r[1] = (uint32_t)(c.plane & 0xffff) | (1u << 16);        // int16 plane, int16 iter = 1
-    r[2] = __float_as_uint(fv); r[3] = __float_as_uint(cc); r[4] = __float_as_uint(se);
-    r[5] = __float_as_uint(d);                               // snr = d / sqrt(s_eff) is taken at flush time
-  }
-  __syncwarp();
-  return nst + __popc(m);
-}
-
-// k_max = 2: five lanes per candidate, one window row each (six candidates per warp and pass).  e0: the
-// warp's first entry of this pass.  Queue entry: {col | slot << 16, row, d, s}, slot = the row's place in
-// the F ring.  Written for a short dependent chain: all six shared loads leave together.
-struct CandK { float kappa2, eps_rel; int Dy, Dx; const uint8_t* W; };
-__device__ __forceinline__ int cand_pass5(const CandCtx& c, const CandK& k, int o_q, int n, int e0, int o_st, int nst) {
-  const int CWP = c.CWP;
-  const int g = (c.lane * 13) >> 6, r = c.lane - 5 * g;        // lane / 5, lane % 5 (lanes 30, 31: g = 6, idle)
-  const int e = e0 + g;
-  const bool act = g < 6 && e < n;
-  const float4 q = lds4(o_q + 4 * (act ? e : 0));
-  const int cs = __float_as_int(q.x), cl = cs & 0xffff, s0 = cs >> 16, sg = __float_as_int(q.y);
-  const float d = q.z;
-  int sl = s0 + r - 2;
-  sl = sl < 0 ? sl + DRS : (sl >= DRS ? sl - DRS : sl);
-  const int yy = sg + r - 2;
-  const int rb = sl * CWP;
-  const float fv = lds1(s0 * CWP + cl);
-  float fn[5];
-#pragma unroll
-  for (int dx = 0; dx < 5; ++dx) {
-    int c2 = cl + dx - 2;
-    c2 = c2 < 0 ? 0 : (c2 >= CWP ? CWP - 1 : c2);
-    fn[dx] = lds1(rb + c2);
-  }
-  const float cc = fv - d;
-  const float gd = k.eps_rel * fabsf(cc);
-  const float se = fmaxf(q.w, gd * gd);
-  const bool pass = act && d > 0.f && d * d > k.kappa2 * se;
-  const bool row_in = pass && yy >= 0 && yy < k.Dy;
-  bool bigger = false;
-#pragma unroll
-  for (int dx = 0; dx < 5; ++dx) {
-    const int c2 = cl + dx - 2, xn = c.xs + c2;
-    const bool in = row_in && c2 >= 0 && c2 < CWP && xn < k.Dx;
-    // masked pixels hold F = 0 in the ring: W is consulted only when such a zero would win
-    if (in && fn[dx] > fv) bigger = bigger || (fn[dx] != 0.f) || (k.W[(long long)yy * k.Dx + xn] != 0);
-  }
-  const unsigned ball = __ballot_sync(0xffffffffu, bigger);
-  const bool ok = pass && r == 0 && ((ball >> (5 * g)) & 31u) == 0u;
-  return cand_stage(c, o_st, nst, ok, cl, sg, d, fv, cc, se);
-}
-
-// the queue of one iteration, n entries {col, row, d, s} at float index o_q: the share of helper warp hw of nh
-__device__ __noinline__ int cand_consume(CandCtx c, int o_q, int n, int hw, int nh, int o_st, int nst) {
-  for (int e0 = 32 * hw; e0 < n; e0 += 32 * nh) {
-    const int e = e0 + c.lane;
-    bool ok = false;
-    int cl = 0, sg = 0; float d = 0.f, fv = 0.f, cc = 0.f, se = 1.f;
-    if (e < n) {
-      const float4 q = lds4(o_q + 4 * e);
-      cl = __float_as_int(q.x) & 0xffff; sg = __float_as_int(q.y); d = q.z;
-      ok = cand_test_any(c, cl, sg, d, q.w, fv, cc, se);
-    }
-    nst = cand_stage(c, o_st, nst, ok, cl, sg, d, fv, cc, se);
-  }
-  return nst;
-}
-
-// a sweep warp whose candidates did not fit the queue (rare: a row full of bright pixels) tests them itself
-// and appends the records straight to the global list
-__device__ __noinline__ void cand_in_place(CandCtx c, unsigned bits, int col0, int sg, float4 dv, float4 sv) {
-  const FusedArgs& a = *c.ap;
-  const float d[4] = {dv.x, dv.y, dv.z, dv.w};
-  const float s[4] = {sv.x, sv.y, sv.z, sv.w};
-#pragma unroll
-  for (int k = 0; k < 4; ++k) {
-    float fv = 0.f, cc = 0.f, se = 1.f;
-    bool ok = false;
-    if ((bits >> k) & 1u) ok = cand_test_lane<-1>(c, col0 + k, sg, d[k], s[k], fv, cc, se);
-    const unsigned m = __ballot_sync(0xffffffffu, ok);
-    if (!m) continue;
-    int base = 0;
-    if (c.lane == 0) base = atomicAdd(a.ndets, __popc(m));
-    base = __shfl_sync(0xffffffffu, base, 0);
-    if (ok) {
-      const int idx = base + __popc(m & ((1u << c.lane) - 1u));
-      if (idx < a.max_det) {
-        uint2* dst = reinterpret_cast<uint2*>(a.dets + idx);
-        dst[0] = make_uint2((uint32_t)(sg * a.Dx + c.xs + col0 + k), (uint32_t)(c.plane & 0xffff) | (1u << 16));
-        dst[1] = make_uint2(__float_as_uint(fv), __float_as_uint(cc));
-        dst[2] = make_uint2(__float_as_uint(se), __float_as_uint(d[k] / sqrtf(se)));
-      } else {
-        atomicAdd(&a.counters[0], 1);
-      }
-    }
-  }
+  return make_float4(a0.x, a0.y, a1.x, a1.y);
 }
 
 // the slow input path: a cube with something other than an exact zero at an invalid pixel; x0: column of v.l.x
@@ -359,46 +207,49 @@ struct Planes {            // normaliser values of non-interior cells, loaded on
   float4 nm[RB], icr[RB], ics[RB];
 };
 
+// the control word of an interior iteration: input, all three stages, every normaliser the interior constant
+constexpr unsigned FL_FAST = FL_X | FL_DO_B | FL_C0 | FL_C1;
+
 template <int NW>
 struct Sweep {
+  static constexpr int NT = NW * 32;
   static constexpr int CWP = NW * 128;             // shared-memory row pitch: the CTA's full width
   static constexpr int XP = CWP + 8;               // staged input row: 4 columns of margin on both sides
   static constexpr int PEV = CWP + 2 * KBG, PET = NW * 32 + 8;
-  static constexpr int O_RING = 0;
-  static constexpr int O_X = DRS * CWP;
+  static constexpr int O_X = 0;
   static constexpr int O_EV1 = O_X + XST * RB * XP;
   static constexpr int O_EV2 = O_EV1 + 2 * RB * PEV;
   static constexpr int O_ET1 = O_EV2 + 2 * RB * PEV;
   static constexpr int O_ET2 = O_ET1 + 2 * RB * PET;
-  static constexpr int O_Q = O_ET2 + 2 * RB * PET;       // candidate queues, [2][QCAP] x {col, row, d, s}
-  static constexpr int O_QN = O_Q + 2 * QCAP * 4;        // their lengths, one word per iteration mod 4
-  static constexpr int O_ST = O_QN + 4;                  // staged records of the helper warps, [NHW][SCAP] x 8 words
-  static constexpr int O_BAR = O_ST + NHW * SCAP * 8;    // XST mbarriers (8 bytes each)
-  static constexpr int O_FL = O_BAR + 2 * XST + 2;       // end of the layout (XST input barriers + the iteration barrier)
+  static constexpr int O_BAR = O_ET2 + 2 * RB * PET;     // XST input barriers + the iteration barrier (8 bytes each)
+  static constexpr int O_NH = O_BAR + 2 * XST + 2;       // entries in the CTA's hit segment so far
+  static constexpr int O_FL = O_NH + 2;                  // end of the layout
   // ---- constants of the thread -----------------------------------------------------------------
   const FusedArgs& a;
-  const FusedArgs* a_sh;   // the same arguments in shared memory (for the out-of-line candidate path)
+  const FusedArgs* a_sh;   // the same arguments in shared memory (for the out-of-line paths)
   int xs, plane, tid, lane, warp;
   const uint32_t* flp;     // this warp's control words, [nb] with stride NW
-  int sx;                  // row stride of the plane pointers (0 for lanes outside the strip)
   bool col_in, dirty;
   unsigned umask;
   uint32_t tm;             // tensor-memory address of the thread's column 0
+  float big;               // |F| or |d| above this: the running sums are rebuilt when it leaves
+  HitRec* seg;             // the CTA's segment of the hit list
+  const float* nm0;        // padded norm_mf / 1/count at (row 0 of the image, the thread's first column); the zero row
+  const float* ic0;        //   of a padded plane for lanes outside the strip (sx = 0)
+  int sx;
   // producer (thread 0)
   const float* xrow0;      // X at (y_start, first copied column)
   uint32_t x_dst0;         // shared address of that column in stage 0, row 0
   uint32_t row_bytes;
-  int nb;
+  int nb, ys;
   // ---- running state -----------------------------------------------------------------------------
-  const float* nmp;        // padded norm_mf at the next iteration's first F row
-  const float* icrp;       // padded 1/count at the next iteration's first rho row
-  const float* icsp;       // padded 1/count at the next iteration's first sigma row
   int y0;                  // first input row of the current iteration
-  int ring_y0;             // the row that sits in slot 0 of the rings
-  int ws;                  // slot of this iteration's first F row in the shared-memory ring
-  float2 hw[8][2];         // horizontally filtered rows (rotating; static indices per phase)
+  float2 hn[RB][2];        // horizontally filtered input rows of the coming iteration
+  float2 acc[6][2];        // vertical matched filter: the partial sums of the next six F rows
   float2 V1[2], V2[2];     // vertical running sums
-  Planes pl;               // normalisers of the coming rows: each plane is reloaded right after its use
+  Planes pl;               // normalisers of the coming rows (edge cells only)
+  // tensor-memory values of the coming iteration, loaded while the CTA sits in the barrier
+  float2 fold[RB][2], flag[RB][2], dold[RB][2], dlag[RB][2], fs[4][2];
 
   __device__ __forceinline__ Sweep(const FusedArgs& a_) : a(a_) {}
 
@@ -412,23 +263,16 @@ struct Sweep {
     return smem_u32(reinterpret_cast<const float*>(g_sm4) + O_BAR + 2 * stage);
   }
 
-  // the per-iteration barrier of all warps, in two halves (an mbarrier with one arrival per warp: 32 arrivals on
-  // one shared-memory word would serialise)
+  // the per-iteration barrier of all warps, in two halves (an mbarrier with one arrival per warp)
   __device__ __forceinline__ void sync_arrive() const { __syncwarp(); if (lane == 0) mbar_arrive(bar_addr(XST)); }
   __device__ __forceinline__ void sync_wait(int b) const { mbar_wait(bar_addr(XST), (uint32_t)b & 1u); }
 
-  __device__ __forceinline__ CandCtx cand_ctx() const {
-    CandCtx c;
-    c.ap = a_sh; c.CWP = CWP; c.xs = xs; c.plane = plane; c.lane = lane; c.ring_y0 = ring_y0;
-    return c;
-  }
-
   // thread 0: the two input rows of iteration bb into stage bb mod XST (a plain arrival when they lie outside the image)
-  __device__ __forceinline__ void issue_rows(int bb, int ys) {
+  __device__ __forceinline__ void issue_rows(int bb) {
     const int st = bb & (XST - 1);
     const uint32_t bar = bar_addr(st);
     const int y = ys + RB * bb;
-    if (bb >= XST) mbar_wait(bar, (uint32_t)((bb >> 2) - 1) & 1u);   // its previous phase (complete unless no warp waited for it)
+    if (bb >= XST) mbar_wait(bar, (uint32_t)((bb / XST) - 1) & 1u);   // its previous phase (complete unless no warp waited for it)
     if (y >= 0 && y + RB <= a.Dy) {
       mbar_expect_tx(bar, RB * row_bytes);
       const float* src = xrow0 + (long long)RB * bb * a.Dx;
@@ -440,29 +284,23 @@ struct Sweep {
     }
   }
 
-  __device__ __forceinline__ void load_nm(unsigned on) {
-    if (on) { pl.nm[0] = ldg4_pinned(nmp); pl.nm[1] = ldg4_pinned(nmp + sx); }
-    nmp += RB * sx;
-  }
-  __device__ __forceinline__ void load_icr(unsigned on) {
-    if (on) { pl.icr[0] = ldg4_pinned(icrp); pl.icr[1] = ldg4_pinned(icrp + sx); }
-    icrp += RB * sx;
-  }
-  __device__ __forceinline__ void load_ics(unsigned on) {
-    if (on) { pl.ics[0] = ldg4_pinned(icsp); pl.ics[1] = ldg4_pinned(icsp + sx); }
-    icsp += RB * sx;
+  // the normaliser rows of an edge cell; row: first image row wanted
+  __device__ __forceinline__ void load_rows(const float* p0, int row, float4 (&dst)[RB]) {
+    const float* p = p0 + (long long)(row + PADR) * sx;
+#pragma unroll
+    for (int j = 0; j < RB; ++j) dst[j] = ldg4_pinned(p + (long long)j * sx);
   }
 
-  // Stage A, part 1 for iteration bn (PH = bn mod 4): staged input rows -> horizontal matched filter -> hw.
-  // It touches only the input stages and registers, so it runs in the shadow of the previous iteration's
-  // barrier (between the arrival and the wait).  yn: first input row of iteration bn.
-  template <int PH>
+  // Stage A, part 1 for iteration bn: staged input rows -> horizontal matched filter -> hn.  It touches only the
+  // input stages and registers, so it runs in the shadow of the previous iteration's barrier (between the
+  // arrival and the wait).  yn: first input row of iteration bn.
   __device__ __forceinline__ void stage_a1(int bn, unsigned fl, int yn) {
-    if (fl & FL_X) {
-      mbar_wait(bar_addr(PH), (uint32_t)(bn >> 2) & 1u);
+    if ((fl & FL_X) && !(LPF_EXP_SKIP & 8)) {
+      const int st = bn & (XST - 1);
+      mbar_wait(bar_addr(st), (uint32_t)(bn / XST) & 1u);
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
-        const int xr = O_X + (PH * RB + j) * XP + 4 * tid;
+        const int xr = O_X + (st * RB + j) * XP + 4 * tid;
         float4 l = lds4(xr), m = lds4(xr + 4), r = lds4(xr + 8);
         if (dirty) {
           Row12 v; v.l = l; v.m = m; v.r = r;
@@ -474,53 +312,101 @@ struct Sweep {
 #pragma unroll
         for (int k = 0; k < 4; ++k)
           h[k] = fmaf(a.g0, wv[k + 3], fmaf(a.g1, wv[k + 2] + wv[k + 4], fmaf(a.g2, wv[k + 1] + wv[k + 5], a.g3 * (wv[k] + wv[k + 6]))));
-        hw[(2 * PH + 6 + j) & 7][0] = make_float2(h[0], h[1]);
-        hw[(2 * PH + 6 + j) & 7][1] = make_float2(h[2], h[3]);
+        hn[j][0] = make_float2(h[0], h[1]);
+        hn[j][1] = make_float2(h[2], h[3]);
       }
     } else {
 #pragma unroll
-      for (int j = 0; j < RB; ++j) { hw[(2 * PH + 6 + j) & 7][0] = splat(0.f); hw[(2 * PH + 6 + j) & 7][1] = splat(0.f); }
+      for (int j = 0; j < RB; ++j) { hn[j][0] = splat(0.f); hn[j][1] = splat(0.f); }
     }
-
   }
 
-  // One iteration: rows y0, y0+1 enter stage A; PH = iteration index mod 4 fixes the register rotation
-  // and the staging stage.  fl: this iteration's control word.
-  template <int PH>
-  __device__ __forceinline__ void iteration(int b, unsigned fl, unsigned fl_next) {
-    constexpr int buf = PH & 1, pbuf = buf ^ 1;
-    const float2 g0 = splat(a.g0), g1 = splat(a.g1), g2 = splat(a.g2), g3 = splat(a.g3);
-    const int w = (RB * b) & (DR - 1);                       // ring slot of this iteration's first row (even)
-    const uint32_t t_old0 = tm + 4u * (uint32_t)((w + 7) & (DR - 1)), t_old1 = tm + 4u * (uint32_t)((w + 8) & (DR - 1));
-    const uint32_t t_lag0 = tm + 4u * (uint32_t)((w + 18) & (DR - 1)), t_lag1 = t_lag0 + 4u;   // w + 18 is even: no wrap in between
-    const uint32_t t_new0 = tm + 4u * (uint32_t)w, t_new1 = t_new0 + 4u;
-
-    // ---- tensor-memory reads: F(fr - 25), F(rho), d(rho - 25), d(sigma) ---------------------------------
-    float2 fold[RB][2], flag[RB][2], dold[RB][2], dlag[RB][2];
-    tm_ld4(t_old0, fold[0][0], fold[0][1]); tm_ld4(t_old1, fold[1][0], fold[1][1]);
-
-
-    tm_wait_ld();
+  // pixels of the thread's own 3 x 4 block (rows sigma - 1 .. sigma + 1) that some valid neighbour inside the
+  // (2 KM + 1)^2 window already beats: F >= 0 and a neighbour above it (a positive F belongs to a valid pixel;
+  // a neighbour at 0 may be a masked one, which eq. 6 skips, so nothing is decided against an F < 0 here)
+  template <int KM>
+  __device__ __forceinline__ unsigned beaten(const float (&fu)[4], const float (&fc)[4], const float (&fd)[4]) const {
+    float cm[4], vm[4];
 #pragma unroll
-    for (int j = 0; j < RB; ++j) tm_use(fold[j][0], fold[j][1]);
-    // second batch, for stages B and C: F(rho), d(rho - 25), d(sigma)
+    for (int k = 0; k < 4; ++k) { vm[k] = fmaxf(fu[k], fd[k]); cm[k] = fmaxf(vm[k], fc[k]); }
+    unsigned out = 0u;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      float e = vm[k];
+#pragma unroll
+      for (int kk = 0; kk < 4; ++kk)
+        if (kk != k && kk - k <= KM && k - kk <= KM) e = fmaxf(e, cm[kk]);
+      if (fc[k] >= 0.f && e > fc[k]) out |= 1u << k;
+    }
+    return out;
+  }
+
+  // a thread with eq. 5 hits in sigma row sg: drop what its own block already beats, append the rest as one entry
+  __device__ __forceinline__ void emit_hits(unsigned bits, int sg, float2 d0, float2 d1, float2 s0, float2 s1,
+                                            float2 fu0, float2 fu1, float2 fc0, float2 fc1, float2 fd0, float2 fd1) {
+    if (a.k_max > 0) {
+      const float fu[4] = {fu0.x, fu0.y, fu1.x, fu1.y}, fc[4] = {fc0.x, fc0.y, fc1.x, fc1.y}, fd[4] = {fd0.x, fd0.y, fd1.x, fd1.y};
+      bits &= ~(a.k_max >= 2 ? beaten<2>(fu, fc, fd) : beaten<1>(fu, fc, fd));
+    }
+    if (!bits) return;
+    const int idx = atomicAdd(reinterpret_cast<int*>(g_sm4) + O_NH, 1);
+    if (idx < a.seg_cap) {
+      uint4* dst = reinterpret_cast<uint4*>(seg + idx);
+      dst[0] = make_uint4((uint32_t)(sg * a.Dx + xs + 4 * tid), bits, 0u, 0u);
+      dst[1] = make_uint4(__float_as_uint(d0.x), __float_as_uint(d0.y), __float_as_uint(d1.x), __float_as_uint(d1.y));
+      dst[2] = make_uint4(__float_as_uint(s0.x), __float_as_uint(s0.y), __float_as_uint(s1.x), __float_as_uint(s1.y));
+    }
+  }
+
+  // tensor-memory reads of iteration b: F(fr - 25), F(rho), d(rho - 25), d(sigma), F(sigma - 1 .. sigma + 2).  None of
+  // these rows is written in iteration b - 1, so they are issued before that iteration's barrier.
+  __device__ __forceinline__ void tm_prefetch(int b) {
+    const int w = (RB * b) & (DR - 1);
+    auto slot = [&](int k) -> uint32_t { return tm + 4u * (uint32_t)((w + k) & (DR - 1)); };
+    const uint32_t t_old0 = slot(7), t_old1 = slot(8);       // rows 25 and 24 back
+    const uint32_t t_lag0 = slot(18), t_lag1 = t_lag0 + 4u;  // w + 18 is even: no wrap in between
+    tm_ld4(t_old0, fold[0][0], fold[0][1]); tm_ld4(t_old1, fold[1][0], fold[1][1]);
     tm_ld4(t_lag0, flag[0][0], flag[0][1]); tm_ld4(t_lag1, flag[1][0], flag[1][1]);
     tm_ld4(t_old0 + TM_D, dold[0][0], dold[0][1]); tm_ld4(t_old1 + TM_D, dold[1][0], dold[1][1]);
     tm_ld4(t_lag0 + TM_D, dlag[0][0], dlag[0][1]); tm_ld4(t_lag1 + TM_D, dlag[1][0], dlag[1][1]);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) tm_ld4(slot(3 + k), fs[k][0], fs[k][1]);
+  }
+
+  // One iteration: rows y0, y0+1 enter stage A.  fl: this iteration's control word.  FAST: an interior iteration
+  // (fl = FL_FAST): no flag is looked at, no normaliser plane is loaded.
+  template <bool FAST>
+  __device__ __forceinline__ void iteration(int b, unsigned fl, unsigned fl_next) {
+    const int buf = b & 1, pbuf = buf ^ 1;
+    const float2 g0 = splat(a.g0), g1 = splat(a.g1), g2 = splat(a.g2), g3 = splat(a.g3);
+    const int w = (RB * b) & (DR - 1);                       // ring slot of this iteration's first row (even)
+    const uint32_t t_new0 = tm + 4u * (uint32_t)w, t_new1 = t_new0 + 4u;
+
+    tm_wait_ld();
+#pragma unroll
+    for (int j = 0; j < RB; ++j) { tm_use(fold[j][0], fold[j][1]); tm_use(flag[j][0], flag[j][1]); tm_use(dold[j][0], dold[j][1]); tm_use(dlag[j][0], dlag[j][1]); }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) tm_use(fs[k][0], fs[k][1]);
 
     // ---- stage A, part 2: vertical matched filter -> F(fr), running sum V1, exchange ----------------
-    {
+    // F(fr) = g3 h(fr-3) + g2 h(fr-2) + g1 h(fr-1) + g0 h(fr) + g1 h(fr+1) + g2 h(fr+2) + g3 h(fr+3), summed in that
+    // order: row y adds its term to the six F rows still open and closes F(y - 3) (k_peaks follows the same order)
+    if (!(LPF_EXP_SKIP & 4)) {
       float2 f[RB][2];
 #pragma unroll
       for (int j = 0; j < RB; ++j)
 #pragma unroll
         for (int p = 0; p < 2; ++p) {
-          const float2 h0 = hw[(2 * PH + j + 0) & 7][p], h1 = hw[(2 * PH + j + 1) & 7][p], h2 = hw[(2 * PH + j + 2) & 7][p],
-                       h3 = hw[(2 * PH + j + 3) & 7][p], h4 = hw[(2 * PH + j + 4) & 7][p], h5 = hw[(2 * PH + j + 5) & 7][p],
-                       h6 = hw[(2 * PH + j + 6) & 7][p];
-          f[j][p] = fma2(g0, h3, fma2(g1, add2(h2, h4), fma2(g2, add2(h1, h5), mul2(g3, add2(h0, h6)))));
+          const float2 h = hn[j][p];
+          f[j][p] = fma2(g3, h, acc[0][p]);
+          acc[0][p] = fma2(g2, h, acc[1][p]);
+          acc[1][p] = fma2(g1, h, acc[2][p]);
+          acc[2][p] = fma2(g0, h, acc[3][p]);
+          acc[3][p] = fma2(g1, h, acc[4][p]);
+          acc[4][p] = fma2(g2, h, acc[5][p]);
+          acc[5][p] = mul2(g3, h);
         }
-      if (fl & FL_NM_LD) {
+      if (!FAST && (fl & FL_NM_LD)) {
 #pragma unroll
         for (int j = 0; j < RB; ++j) {
           f[j][0] = mul2(f[j][0], make_float2(pl.nm[j].x, pl.nm[j].y));
@@ -531,173 +417,151 @@ struct Sweep {
 #pragma unroll
         for (int j = 0; j < RB; ++j) { f[j][0] = mul2(f[j][0], c); f[j][1] = mul2(f[j][1], c); }
       }
+      float2 v[RB][2];
+      const float hot = fmaxf(amax4(fold[0][0], fold[0][1]), amax4(fold[1][0], fold[1][1]));
+      if (__any_sync(0xffffffffu, hot > big)) {
+        // something far above the noise leaves the window: rebuild the sums from the ring
+        const float4 s23 = ring_sum23(tm, w, 0);
+        const float2 b0 = make_float2(s23.x, s23.y), b1 = make_float2(s23.z, s23.w);
+        v[0][0] = add2(add2(b0, fold[1][0]), f[0][0]); v[0][1] = add2(add2(b1, fold[1][1]), f[0][1]);
+        v[1][0] = add2(add2(b0, f[0][0]), f[1][0]);    v[1][1] = add2(add2(b1, f[0][1]), f[1][1]);
+      } else {
+        v[0][0] = add2(V1[0], sub2(f[0][0], fold[0][0])); v[0][1] = add2(V1[1], sub2(f[0][1], fold[0][1]));
+        v[1][0] = add2(v[0][0], sub2(f[1][0], fold[1][0])); v[1][1] = add2(v[0][1], sub2(f[1][1], fold[1][1]));
+      }
+      V1[0] = v[1][0]; V1[1] = v[1][1];
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
-        V1[0] = add2(V1[0], sub2(f[j][0], fold[j][0]));
-        V1[1] = add2(V1[1], sub2(f[j][1], fold[j][1]));
         tm_st4(j ? t_new1 : t_new0, f[j][0], f[j][1]);
-        sts4(O_RING + (ws + j) * CWP + 4 * tid, make_float4(f[j][0].x, f[j][0].y, f[j][1].x, f[j][1].y));
-        sts4(O_EV1 + (buf * RB + j) * PEV + KBG + 4 * tid, make_float4(V1[0].x, V1[0].y, V1[1].x, V1[1].y));
-        const float2 ts = add2(V1[0], V1[1]);
+        sts4(O_EV1 + (buf * RB + j) * PEV + KBG + 4 * tid, make_float4(v[j][0].x, v[j][0].y, v[j][1].x, v[j][1].y));
+        const float2 ts = add2(v[j][0], v[j][1]);
         sts1(O_ET1 + (buf * RB + j) * PET + 3 + tid, ts.x + ts.y);
       }
     }
-
-    load_nm(fl & FL_NM_PF);                          // the next iteration's norm_mf rows
-    tm_wait_ld();
-#pragma unroll
-    for (int j = 0; j < RB; ++j) { tm_use(flag[j][0], flag[j][1]); tm_use(dold[j][0], dold[j][1]); tm_use(dlag[j][0], dlag[j][1]); }
+    if (!FAST && (fl & FL_NM_PF)) load_rows(nm0, y0 + RB - 3, pl.nm);           // the next iteration's norm_mf rows
 
     // ---- stage B: C = box(V1) / count at rho ; d = F - C ; running sum V2 of d^2 ---------------------
-    if (fl & FL_DO_B) {
+    if ((FAST || (fl & FL_DO_B)) && !(LPF_EXP_SKIP & 2)) {
       float2 dd[RB][2];
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
-        float bx[4];
-        hbox25(O_EV1 + (pbuf * RB + j) * PEV + 4 * tid, O_ET1 + (pbuf * RB + j) * PET + tid, bx);
+        float2 b01, b23;
+        hbox25(O_EV1 + (pbuf * RB + j) * PEV + 4 * tid, O_ET1 + (pbuf * RB + j) * PET + tid, b01, b23);
         float2 ic0, ic1;
-        if (fl & FL_ICR_LD) { ic0 = make_float2(pl.icr[j].x, pl.icr[j].y); ic1 = make_float2(pl.icr[j].z, pl.icr[j].w); }
+        if (!FAST && (fl & FL_ICR_LD)) { ic0 = make_float2(pl.icr[j].x, pl.icr[j].y); ic1 = make_float2(pl.icr[j].z, pl.icr[j].w); }
         else { ic0 = splat(a.ic_const); ic1 = ic0; }
-        dd[j][0] = fma2(make_float2(-bx[0], -bx[1]), ic0, flag[j][0]);     // d = F - box * (1/count)
-        dd[j][1] = fma2(make_float2(-bx[2], -bx[3]), ic1, flag[j][1]);
+        dd[j][0] = fma2(neg2(b01), ic0, flag[j][0]);     // d = F - box * (1/count)
+        dd[j][1] = fma2(neg2(b23), ic1, flag[j][1]);
       }
+      float2 v[RB][2];
+      const float hot = fmaxf(amax4(dold[0][0], dold[0][1]), amax4(dold[1][0], dold[1][1]));
+      if (__any_sync(0xffffffffu, hot > big)) {
+        const float4 s23 = ring_sum23(tm + TM_D, w, 1);
+        const float2 b0 = make_float2(s23.x, s23.y), b1 = make_float2(s23.z, s23.w);
+        const float2 q0 = fma2(dd[0][0], dd[0][0], b0), q1 = fma2(dd[0][1], dd[0][1], b1);
+        v[0][0] = fma2(dold[1][0], dold[1][0], q0); v[0][1] = fma2(dold[1][1], dold[1][1], q1);
+        v[1][0] = fma2(dd[1][0], dd[1][0], q0);     v[1][1] = fma2(dd[1][1], dd[1][1], q1);
+      } else {
+        v[0][0] = fma2(neg2(dold[0][0]), dold[0][0], fma2(dd[0][0], dd[0][0], V2[0]));
+        v[0][1] = fma2(neg2(dold[0][1]), dold[0][1], fma2(dd[0][1], dd[0][1], V2[1]));
+        v[1][0] = fma2(neg2(dold[1][0]), dold[1][0], fma2(dd[1][0], dd[1][0], v[0][0]));
+        v[1][1] = fma2(neg2(dold[1][1]), dold[1][1], fma2(dd[1][1], dd[1][1], v[0][1]));
+      }
+      V2[0] = v[1][0]; V2[1] = v[1][1];
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
-        V2[0] = fma2(neg2(dold[j][0]), dold[j][0], fma2(dd[j][0], dd[j][0], V2[0]));
-        V2[1] = fma2(neg2(dold[j][1]), dold[j][1], fma2(dd[j][1], dd[j][1], V2[1]));
         tm_st4((j ? t_new1 : t_new0) + TM_D, dd[j][0], dd[j][1]);
-        sts4(O_EV2 + (buf * RB + j) * PEV + KBG + 4 * tid, make_float4(V2[0].x, V2[0].y, V2[1].x, V2[1].y));
-        const float2 ts = add2(V2[0], V2[1]);
+        sts4(O_EV2 + (buf * RB + j) * PEV + KBG + 4 * tid, make_float4(v[j][0].x, v[j][0].y, v[j][1].x, v[j][1].y));
+        const float2 ts = add2(v[j][0], v[j][1]);
         sts1(O_ET2 + (buf * RB + j) * PET + 3 + tid, ts.x + ts.y);
       }
     }
+    if (!FAST && (fl & FL_ICR_PF)) load_rows(ic0, y0 + RB - LAG_B, pl.icr);
 
-    load_icr(fl & FL_ICR_PF);
-
-    // ---- stage C: S = box(V2) / count at sigma ; eq. 5 for the row ; candidates ------------------------
-    if (fl & (FL_C0 | FL_C1)) {
+    // ---- stage C: S = box(V2) / count at sigma ; eq. 5 for the row ; hits ------------------------------
+    if ((FAST || (fl & (FL_C0 | FL_C1))) && !(LPF_EXP_SKIP & 1)) {
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
-        if (!(fl & (FL_C0 << j))) continue;          // uniform
-        float bx[4];
-        hbox25(O_EV2 + (pbuf * RB + j) * PEV + 4 * tid, O_ET2 + (pbuf * RB + j) * PET + tid, bx);
+        if (!FAST && !(fl & (FL_C0 << j))) continue;          // uniform
+        float2 b01, b23;
+        hbox25(O_EV2 + (pbuf * RB + j) * PEV + 4 * tid, O_ET2 + (pbuf * RB + j) * PET + tid, b01, b23);
         float2 ic0, ic1;
-        if (fl & FL_ICS_LD) { ic0 = make_float2(pl.ics[j].x, pl.ics[j].y); ic1 = make_float2(pl.ics[j].z, pl.ics[j].w); }
+        if (!FAST && (fl & FL_ICS_LD)) { ic0 = make_float2(pl.ics[j].x, pl.ics[j].y); ic1 = make_float2(pl.ics[j].z, pl.ics[j].w); }
         else { ic0 = splat(a.ic_const); ic1 = ic0; }
-        const float2 s0 = mul2(make_float2(bx[0], bx[1]), ic0), s1 = mul2(make_float2(bx[2], bx[3]), ic1);
+        const float2 s0 = mul2(b01, ic0), s1 = mul2(b23, ic1);
         const float2 k0 = mul2(s0, splat(a.kappa2)), k1 = mul2(s1, splat(a.kappa2));
-        // d^2 - kappa^2 S > 0 somewhere in the warp's row?  (the sign of the difference is exact)
+        // d^2 - kappa^2 S > 0 somewhere in the thread's pixels?  (the sign of the difference is exact; k_peaks
+        // applies the guarded, rounded test)
         const float2 m0 = fma2(dlag[j][0], dlag[j][0], neg2(k0)), m1 = fma2(dlag[j][1], dlag[j][1], neg2(k1));
         const float mm = fmaxf(fmaxf(m0.x, m0.y), fmaxf(m1.x, m1.y));
-        if (__any_sync(0xffffffffu, mm > 0.f)) {
-          // exact bits (the sign of m is that of d^2 - kappa^2 S), then the queue of this iteration
-          const float dv[4] = {dlag[j][0].x, dlag[j][0].y, dlag[j][1].x, dlag[j][1].y};
-          const float mv[4] = {m0.x, m0.y, m1.x, m1.y};
+        if (mm > 0.f) {
           unsigned bits = 0u;
-#pragma unroll
-          for (int k = 0; k < 4; ++k)
-            if (dv[k] > 0.f && mv[k] > 0.f) bits |= 1u << k;
+          if (dlag[j][0].x > 0.f && m0.x > 0.f) bits |= 1u;
+          if (dlag[j][0].y > 0.f && m0.y > 0.f) bits |= 2u;
+          if (dlag[j][1].x > 0.f && m1.x > 0.f) bits |= 4u;
+          if (dlag[j][1].y > 0.f && m1.y > 0.f) bits |= 8u;
           bits &= umask;
-          const float sv[4] = {s0.x, s0.y, s1.x, s1.y};
-          const int sg = y0 + j - LAG_C;
-          int sslot = ws + j - (LAG_C - 3);                    // ring slot of row sigma (this iteration's F row j: ws + j)
-          sslot = sslot < 0 ? sslot + DRS : sslot;
-          if (bits) {
-            int pos = atomicAdd(reinterpret_cast<int*>(g_sm4) + O_QN + (b & 3), __popc(bits));
-#pragma unroll
-            for (int k = 0; k < 4; ++k)
-              if (((bits >> k) & 1u) && pos < QCAP) {
-                sts4(O_Q + (buf * QCAP + pos) * 4, make_float4(__int_as_float((4 * tid + k) | (sslot << 16)), __int_as_float(sg), dv[k], sv[k]));
-                ++pos; bits &= ~(1u << k);
-              }
-          }
-          if (__any_sync(0xffffffffu, bits != 0u))     // queue full
-            cand_in_place(cand_ctx(), bits, 4 * tid, sg, make_float4(dv[0], dv[1], dv[2], dv[3]), make_float4(sv[0], sv[1], sv[2], sv[3]));
+          if (bits)
+            emit_hits(bits, y0 + j - LAG_C, dlag[j][0], dlag[j][1], s0, s1, fs[j][0], fs[j][1], fs[j + 1][0], fs[j + 1][1],
+                      fs[j + 2][0], fs[j + 2][1]);
         }
       }
     }
-    load_ics(fl & FL_ICS_PF);
-    ws = ws + RB >= DRS ? ws + RB - DRS : ws + RB;
+    if (!FAST && (fl & FL_ICS_PF)) load_rows(ic0, y0 + RB - LAG_C, pl.ics);
     y0 += RB;
-    tm_wait_st();
+    tm_prefetch(b + 1);
     // split barrier: arrive, filter the next iteration's input rows while the slower warps finish, wait
     sync_arrive();
-    stage_a1<(PH + 1) & 3>(b + 1, fl_next, y0);
+    stage_a1(b + 1, fl_next, y0);
     sync_wait(b);
-  }
-
-  // the helper warps: helper 0 feeds the input stages (bulk copies three iterations ahead); all of them test
-  // what the sweep warps queued in the previous iteration.  Same barriers as run().
-  __device__ __forceinline__ void run_helper(int ys) {
-    int* qn = reinterpret_cast<int*>(g_sm4) + O_QN;
-    const int hw = warp - NW;
-    const int o_st = O_ST + hw * SCAP * 8;
-    int nst = 0;
-    const CandCtx cc = cand_ctx();
-    CandK ck; ck.kappa2 = a.kappa2; ck.eps_rel = a.eps_rel; ck.Dy = a.Dy; ck.Dx = a.Dx; ck.W = a.W;
-    const bool km2 = a.k_max == 2;
-    for (int b = 0; b <= nb; ++b) {
-      if (hw == NHW - 1 && lane == 0) {
-        if (b + XST - 1 < nb) issue_rows(b + XST - 1, ys);     // their stage was read in iteration b - 1
-        qn[(b + 1) & 3] = 0;                                   // next iteration's counter (last read in b - 2)
-      }
-      if (b > 0) {
-        const int n = min(qn[(b - 1) & 3], QCAP);
-        if (n > 0) {
-          const int o_q = O_Q + ((b - 1) & 1) * QCAP * 4;
-          if (km2) { for (int e0 = 6 * hw; e0 < n; e0 += 6 * NHW) nst = cand_pass5(cc, ck, o_q, n, e0, o_st, nst); }
-          else nst = cand_consume(cc, o_q, n, hw, NHW, o_st, nst);
-        }
-      }
-      if (b < nb) { sync_arrive(); sync_wait(b); }
-    }
-    cand_flush(a_sh, o_st, lane, nst);
-    if (hw == NHW - 1 && lane == 0)                   // no bulk copy may be in flight when the CTA leaves
-      for (int bb = nb > XST ? nb - XST : 0; bb < nb; ++bb) mbar_wait(bar_addr(bb & (XST - 1)), (uint32_t)(bb >> 2) & 1u);
+    tm_wait_st();
+    // every warp has read the input stage of iteration b: thread 0 refills it
+    if (tid == 0 && b + XST < nb) issue_rows(b + XST);
   }
 
   __device__ __forceinline__ void run() {
-    {
-      const unsigned f0 = ctl(0);
-      load_nm(f0 & FL_NM_LD); load_icr(f0 & FL_ICR_LD); load_ics(f0 & FL_ICS_LD);
-    }
-    int b = 0;
     unsigned f0 = ctl(0), f1 = ctl(1), f2 = ctl(2);
-    stage_a1<0>(0, f0, y0);
-    while (true) {
-      unsigned f3 = ctl(b + 3);
-      iteration<0>(b, f0, f1); if (++b >= nb) break;
-      f0 = ctl(b + 3);
-      iteration<1>(b, f1, f2); if (++b >= nb) break;
-      f1 = ctl(b + 3);
-      iteration<2>(b, f2, f3); if (++b >= nb) break;
-      f2 = ctl(b + 3);
-      iteration<3>(b, f3, f0); if (++b >= nb) break;
+    if (f0 & FL_NM_LD) load_rows(nm0, y0 - 3, pl.nm);
+    if (f0 & FL_ICR_LD) load_rows(ic0, y0 - LAG_B, pl.icr);
+    if (f0 & FL_ICS_LD) load_rows(ic0, y0 - LAG_C, pl.ics);
+    tm_prefetch(0);
+    stage_a1(0, f0, y0);
+    for (int b = 0; b < nb; ++b) {
+      const unsigned f3 = ctl(b + 3);
+      if (f0 == FL_FAST) iteration<true>(b, f0, f1);
+      else iteration<false>(b, f0, f1);
+      f0 = f1; f1 = f2; f2 = f3;
     }
+    tm_wait_ld();        // the reads issued for an iteration past the end
   }
 };
 
 template <int NW>
-__global__ void __launch_bounds__(NW * 32 + NHW * 32, 1)
-k_fused_box(const FusedArgs a) {
+__global__ void __launch_bounds__(NW * 32, NW > 4 ? 1 : 2)
+k_sweep(const FusedArgs a) {
   __shared__ uint32_t s_tmem;
   __shared__ FusedArgs s_args;
   constexpr int TM_COLS = NW > 4 ? 512 : 256;
   using SW = Sweep<NW>;
   const int p = blockIdx.y;
-  if (!a.band_ok[a.B]) return;
-  if (p < a.B && !a.band_ok[p]) return;
+  const int segi = p * gridDim.x + blockIdx.x;
+  if (!a.band_ok[a.B] || (p < a.B && !a.band_ok[p])) {
+    if (threadIdx.x == 0) a.hit_cnt[segi] = 0;
+    return;
+  }
 
   SW s(a);
   const FusedItem it = a.items[blockIdx.x];
   s.a_sh = &s_args;
   s.tid = threadIdx.x; s.lane = threadIdx.x & 31; s.warp = threadIdx.x >> 5; s.plane = p; s.xs = it.xs;
-  s.nb = it.nb;
+  s.nb = it.nb; s.ys = it.y_start;
   s.dirty = *a.dirty == a.dirty_seq;
+  s.big = a.big_thr[p];
+  s.seg = a.hits + (long long)segi * a.seg_cap;
   if (s.tid == 0) s_args = a;
-  constexpr int NT = NW * 32 + NHW * 32;    // NW sweep warps and the helper warps
+  constexpr int NT = SW::NT;
   for (int i = s.tid; i < (SW::O_FL >> 2); i += NT) g_sm4[i] = zero4();
-  s.flp = a.flags + it.fl_off + (s.warp < NW ? s.warp : 0);
+  s.flp = a.flags + it.fl_off + s.warp;
   if (s.warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n"
                  ::"l"((uint64_t)__cvta_generic_to_shared(&s_tmem)), "n"(TM_COLS));
@@ -709,23 +573,20 @@ k_fused_box(const FusedArgs a) {
   if (s.tid == 0) {
 #pragma unroll
     for (int i = 0; i < XST; ++i) mbar_init(s.bar_addr(i), 1);
-    mbar_init(s.bar_addr(XST), NT / 32);
+    mbar_init(s.bar_addr(XST), NW);
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
   asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");   // the zero fill above precedes the bulk copies
   const uint32_t tm_base = s_tmem;
   // warp w reaches the 32 lanes (w mod 4) * 32 ...; warps w and w+4 share them on different columns
   s.tm = tm_base + ((uint32_t)((s.warp & 3) * 32) << 16) + (uint32_t)(s.warp >> 2) * 256u;
-  const bool sweeper = s.warp < NW;
-  if (sweeper) {
-    for (int i = 0; i < 2 * DR; ++i) tm_st4(s.tm + 4 * i, splat(0.f), splat(0.f));
-    tm_wait_st();
-  }
+  for (int i = 0; i < 2 * DR; ++i) tm_st4(s.tm + 4 * i, splat(0.f), splat(0.f));
+  tm_wait_st();
 
   const long long N = (long long)a.Dy * a.Dx;
   const float* X = (p < a.B) ? a.cube + (long long)p * N : a.sum_plane;
   const int x = it.xs + 4 * s.tid;
-  s.col_in = sweeper && 4 * s.tid < a.CW && x < a.Dx;
+  s.col_in = 4 * s.tid < a.CW && x < a.Dx;
   s.umask = 0u;
 #pragma unroll
   for (int k = 0; k < 4; ++k)
@@ -740,30 +601,172 @@ k_fused_box(const FusedArgs a) {
   }
   if (s.col_in) {
     s.sx = a.Dx;
-    s.nmp = a.nm_pad + (long long)(it.y_start - 3 + PADR) * a.Dx + x;
-    s.icrp = a.ic_pad + (long long)(it.y_start - LAG_B + PADR) * a.Dx + x;
-    s.icsp = a.ic_pad + (long long)(it.y_start - LAG_C + PADR) * a.Dx + x;
+    s.nm0 = a.nm_pad + x; s.ic0 = a.ic_pad + x;
   } else {              // lanes outside the strip read the zero row of a padded plane, over and over
     s.sx = 0;
-    s.nmp = a.nm_pad; s.icrp = a.nm_pad; s.icsp = a.nm_pad;
+    s.nm0 = a.nm_pad; s.ic0 = a.nm_pad;
   }
 #pragma unroll
-  for (int i = 0; i < 8; ++i) { s.hw[i][0] = splat(0.f); s.hw[i][1] = splat(0.f); }
+  for (int i = 0; i < 6; ++i) { s.acc[i][0] = splat(0.f); s.acc[i][1] = splat(0.f); }
   s.V1[0] = s.V1[1] = s.V2[0] = s.V2[1] = splat(0.f);
 #pragma unroll
-    for (int j = 0; j < RB; ++j) { s.pl.nm[j] = zero4(); s.pl.icr[j] = zero4(); s.pl.ics[j] = zero4(); }
-  s.ring_y0 = it.y_start - 3; s.ws = 0;
+  for (int j = 0; j < RB; ++j) { s.pl.nm[j] = zero4(); s.pl.icr[j] = zero4(); s.pl.ics[j] = zero4(); }
   __syncthreads();
-  if (s.tid == (NW + NHW - 1) * 32)
-    for (int bb = 0; bb < XST - 1 && bb < it.nb; ++bb) s.issue_rows(bb, it.y_start);
+  if (s.tid == 0)
+    for (int bb = 0; bb < XST && bb < it.nb; ++bb) s.issue_rows(bb);
 
-  if (sweeper) s.run(); else s.run_helper(it.y_start);
+  s.run();
 
+  if (s.tid == 0)                   // no bulk copy may be in flight when the CTA leaves
+    for (int bb = it.nb > XST ? it.nb - XST : 0; bb < it.nb; ++bb) mbar_wait(s.bar_addr(bb & (XST - 1)), (uint32_t)(bb / XST) & 1u);
   tm_wait_st();
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
   __syncthreads();
+  if (s.tid == 0) {
+    const int n = reinterpret_cast<const int*>(g_sm4)[SW::O_NH];
+    a.hit_cnt[segi] = n < a.seg_cap ? n : a.seg_cap;
+    if (n > a.seg_cap) atomicAdd(&a.counters[0], n - a.seg_cap);
+#ifdef LPF_DEBUG_HITS
+    atomicAdd(&a.counters[1], n);
+#endif
+  }
   if (s.warp == 0)
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tm_base), "n"(TM_COLS));
+}
+
+// ---- eq. 6 / eq. 7 on the survivors ------------------------------------------------------------------------------
+// One THREAD per surviving pixel (the cheapest form in instructions; the kernel is short on parallelism, not on issue
+// slots, and shares the SMs with the other lanes' kernels).  F at the pixels of its (2 KM + 1)^2 neighbourhood is
+// recomputed from the plane with the sweep's operation order: horizontal 7 taps as nested fused multiply-adds,
+// vertical 7 taps oldest row first, x norm_mf - the values are the sweep's, bit for bit.  X counts as 0 outside the
+// image and at invalid pixels (the cube holds exact zeros there, or W is applied when it does not: MASKED).
+template <int KM, bool MASKED>
+__device__ __forceinline__ bool peak_test(const FusedArgs& a, const float* __restrict__ X, int y, int x, float d, float s,
+                                          float& fv, float& cc, float& se) {
+  constexpr int NR = 2 * KM + 7, NC = 2 * KM + 1;
+  float h[NR][NC];
+#pragma unroll
+  for (int r = 0; r < NR; ++r) {
+    const int yy = y - KM - 3 + r;
+    float xv[NC + 6];
+#pragma unroll
+    for (int c = 0; c < NC + 6; ++c) {
+      const int xx = x - KM - 3 + c;
+      const bool in = yy >= 0 && yy < a.Dy && xx >= 0 && xx < a.Dx;
+      const long long q = (long long)yy * a.Dx + xx;
+      xv[c] = (in && (!MASKED || a.W[q] != 0)) ? X[q] : 0.f;
+    }
+#pragma unroll
+    for (int c = 0; c < NC; ++c)
+      h[r][c] = fmaf(a.g0, xv[c + 3], fmaf(a.g1, xv[c + 2] + xv[c + 4], fmaf(a.g2, xv[c + 1] + xv[c + 5], a.g3 * (xv[c] + xv[c + 6]))));
+  }
+  auto F = [&](int dy, int dx) -> float {   // F at (y + dy, x + dx), |dy|, |dx| <= KM; 0 at an invalid pixel (norm_mf = 0)
+    const int r = dy + KM, c = dx + KM;
+    float v = a.g3 * h[r][c];          // the sweep's order: oldest row first, one fused multiply-add per row
+    v = fmaf(a.g2, h[r + 1][c], v); v = fmaf(a.g1, h[r + 2][c], v); v = fmaf(a.g0, h[r + 3][c], v);
+    v = fmaf(a.g1, h[r + 4][c], v); v = fmaf(a.g2, h[r + 5][c], v); v = fmaf(a.g3, h[r + 6][c], v);
+    return v * a.nm_pad[(long long)(y + dy + PADR) * a.Dx + x + dx];
+  };
+  fv = F(0, 0);
+  cc = fv - d;
+  const float gd = a.eps_rel * fabsf(cc);
+  se = fmaxf(s, gd * gd);
+  if (!(d > 0.f && d * d > a.kappa2 * se)) return false;
+  bool bigger = false;
+#pragma unroll
+  for (int dy = -KM; dy <= KM; ++dy)
+#pragma unroll
+    for (int dx = -KM; dx <= KM; ++dx) {
+      if (dy == 0 && dx == 0) continue;
+      const int yy = y + dy, xx = x + dx;
+      if (yy < 0 || yy >= a.Dy || xx < 0 || xx >= a.Dx) continue;
+      const float fn = F(dy, dx);
+      // a neighbour at 0 above a negative F: masked (skipped by eq. 6) or a valid pixel that happens to hold 0?
+      if (fn > fv && (fn != 0.f || a.W[(long long)yy * a.Dx + xx] != 0)) bigger = true;
+    }
+  return !bigger;
+}
+
+template <bool MASKED>
+__device__ __forceinline__ bool peak_test_km(const FusedArgs& a, const float* __restrict__ X, int y, int x, float d, float s,
+                                             float& fv, float& cc, float& se) {
+  return a.k_max == 2 ? peak_test<2, MASKED>(a, X, y, x, d, s, fv, cc, se)
+       : a.k_max == 1 ? peak_test<1, MASKED>(a, X, y, x, d, s, fv, cc, se)
+                      : peak_test<0, MASKED>(a, X, y, x, d, s, fv, cc, se);
+}
+
+// grid (split, segments): the blocks of a segment share its entries.  A warp takes 32 entries at a time, spreads
+// their surviving pixels over its lanes through shared memory (one pixel per lane and round) and appends the peaks
+// with one atomic per round.
+__global__ void __launch_bounds__(128)
+k_peaks(const FusedArgs a) {
+  __shared__ int s_pix[4][128];
+  __shared__ float s_d[4][128], s_s[4][128];
+  const int segi = blockIdx.y;
+  const int p = segi / a.n_items;
+  const int n = a.hit_cnt[segi];
+  if ((int)(blockIdx.x * blockDim.x) >= n) return;
+  const bool masked = *a.dirty == a.dirty_seq;
+  const long long N = (long long)a.Dy * a.Dx;
+  const float* X = (p < a.B) ? a.cube + (long long)p * N : a.sum_plane;
+  const HitRec* seg = a.hits + (long long)segi * a.seg_cap;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int i0 = blockIdx.x * blockDim.x; i0 < n; i0 += gridDim.x * blockDim.x) {
+    const int i = i0 + threadIdx.x;
+    int bits = 0, pix0 = 0;
+    uint4 r1 = make_uint4(0u, 0u, 0u, 0u), r2 = r1;
+    if (i < n) {
+      const uint4* r = reinterpret_cast<const uint4*>(seg + i);
+      const uint4 r0 = r[0];
+      r1 = r[1]; r2 = r[2];
+      pix0 = (int)r0.x; bits = (int)r0.y & 15;
+    }
+    // exclusive prefix of the pixel counts over the warp
+    const int cnt = __popc(bits);
+    int pre = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pre, o); if (lane >= o) pre += v; }
+    const int total = __shfl_sync(0xffffffffu, pre, 31);
+    pre -= cnt;
+    __syncwarp();
+    {
+      const uint32_t dk[4] = {r1.x, r1.y, r1.z, r1.w}, sk[4] = {r2.x, r2.y, r2.z, r2.w};
+      int o = pre;
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if ((bits >> k) & 1) { s_pix[warp][o] = pix0 + k; s_d[warp][o] = __uint_as_float(dk[k]); s_s[warp][o] = __uint_as_float(sk[k]); ++o; }
+    }
+    __syncwarp();
+    for (int j0 = 0; j0 < total; j0 += 32) {
+      const int j = j0 + lane;
+      bool ok = false;
+      int pix = 0;
+      float d = 0.f, fv = 0.f, cc = 0.f, se = 1.f;
+      if (j < total) {
+        pix = s_pix[warp][j]; d = s_d[warp][j];
+        const float sj = s_s[warp][j];
+        const int y = pix / a.Dx, x = pix - y * a.Dx;
+        ok = masked ? peak_test_km<true>(a, X, y, x, d, sj, fv, cc, se) : peak_test_km<false>(a, X, y, x, d, sj, fv, cc, se);
+      }
+      const unsigned m = __ballot_sync(0xffffffffu, ok);
+      if (!m) continue;
+      int base = 0;
+      if (lane == 0) base = atomicAdd(a.ndets, __popc(m));
+      base = __shfl_sync(0xffffffffu, base, 0);
+      if (ok) {
+        const int idx = base + __popc(m & ((1u << lane) - 1u));
+        if (idx < a.max_det) {
+          uint2* dst = reinterpret_cast<uint2*>(a.dets + idx);
+          dst[0] = make_uint2((uint32_t)pix, (uint32_t)(p & 0xffff) | (1u << 16));        // int16 plane, int16 iter = 1
+          dst[1] = make_uint2(__float_as_uint(fv), __float_as_uint(cc));
+          dst[2] = make_uint2(__float_as_uint(se), __float_as_uint(d / sqrtf(se)));
+        } else {
+          atomicAdd(&a.counters[0], 1);
+        }
+      }
+    }
+    __syncwarp();
+  }
 }
 
 }  // namespace
@@ -773,7 +776,7 @@ k_fused_box(const FusedArgs a) {
 // the per-(iteration, warp) control words of every item, zero-padded normaliser planes.
 struct LpfFusedPlan {
   bool ok = false;
-  int CW = 0, NW = 0, threads = 0, n_items = 0;
+  int CW = 0, NW = 0, threads = 0, n_items = 0, seg_cap = 0;
   size_t smem = 0;
   float nm_const = 1.f, ic_const = 1.f / 625.f;
   FusedItem* d_items = nullptr;
@@ -782,17 +785,16 @@ struct LpfFusedPlan {
   float* d_ic_pad = nullptr;
 };
 
-static size_t fused_smem_bytes(int NW, int max_nb) {
+static size_t fused_smem_bytes(int NW) {
   const int CWP = NW * 128, XP = CWP + 8, PEV = CWP + 2 * KBG, PET = NW * 32 + 8;
-  const size_t nfl = (size_t)DRS * CWP + (size_t)XST * RB * XP + 4 * RB * PEV + 4 * RB * PET + 2 * QCAP * 4 + 4 + NHW * SCAP * 8 + 2 * XST + 2;
-  (void)max_nb;                 // the control words stay in global memory
+  const size_t nfl = (size_t)XST * RB * XP + 4 * RB * PEV + 4 * RB * PET + 2 * XST + 2 + 2;
   return nfl * sizeof(float) + 16;
 }
 
 template <int NW>
 static cudaError_t fused_launch_t(const FusedArgs& a, dim3 grid, size_t smem, cudaStream_t st, bool set_attr) {
-  if (set_attr) return cudaFuncSetAttribute(k_fused_box<NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  k_fused_box<NW><<<grid, NW * 32 + NHW * 32, smem, st>>>(a);
+  if (set_attr) return cudaFuncSetAttribute(k_sweep<NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  k_sweep<NW><<<grid, NW * 32, smem, st>>>(a);
   return cudaSuccess;
 }
 
@@ -864,7 +866,7 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
       cw = std::max(cw, xe - it.xs);
       strips.push_back(it);
     }
-    if (cw <= 1024) { n_strips = (int)strips.size(); CW = cw; }
+    if (cw <= LPF_SWEEP_MAXW) { n_strips = (int)strips.size(); CW = cw; }
   }
   if (!n_strips) return LPF_OK;
   int NW = 1;
@@ -979,8 +981,14 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
   static_assert((FL_NM_LD << 3) == FL_NM_PF && (FL_ICR_LD << 3) == FL_ICR_PF && (FL_ICS_LD << 3) == FL_ICS_PF, "flag layout");
 
   LpfFusedPlan* pl = new LpfFusedPlan();
-  pl->CW = CW; pl->NW = NW; pl->threads = NW * 32 + NHW * 32; pl->n_items = (int)ditems.size();
-  pl->smem = fused_smem_bytes(NW, max_nb);
+  pl->CW = CW; pl->NW = NW; pl->threads = NW * 32; pl->n_items = (int)ditems.size();
+  pl->smem = fused_smem_bytes(NW);
+  (void)max_nb;
+  if ((long long)pl->n_items * c->n_planes > 65535) { delete pl; return LPF_OK; }   // grid.y of k_peaks
+  {   // the hit list: HIT_BUDGET entries shared evenly by the (item, plane) segments
+    const long long nseg = (long long)pl->n_items * c->n_planes;
+    pl->seg_cap = (int)std::max<long long>(256, HIT_BUDGET / std::max<long long>(1, nseg));
+  }
   int dev = 0; cudaGetDevice(&dev);
   int max_smem = 0;
   cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
@@ -1027,22 +1035,60 @@ int lpf_fused_plan_info(const LpfFusedPlan* pl, int* cw, int* threads, int* n_it
   return 1;
 }
 
+// rms-like scale of every plane for a cube whose QC statistics the caller kept to itself (lpf_detect_sources
+// alone): sqrt(sum x^2 / n) over valid pixels x BIG_SIGMA.  One block per plane.
+namespace {
+__global__ void __launch_bounds__(1024)
+k_big_thr(const float* __restrict__ cube, const float* __restrict__ sum_plane, const uint8_t* __restrict__ W, long long N, int B,
+          float* __restrict__ big_thr) {
+  __shared__ double s2[32], sn[32];
+  const int p = blockIdx.x;
+  const float* X = p < B ? cube + (long long)p * N : sum_plane;
+  double a2 = 0, an = 0;
+  for (long long i = threadIdx.x; i < N; i += blockDim.x)
+    if (W[i]) { const float x = X[i]; a2 += (double)x * x; an += 1.0; }
+  a2 = lpf_warp_sum(a2); an = lpf_warp_sum(an);
+  if ((threadIdx.x & 31) == 0) { s2[threadIdx.x >> 5] = a2; sn[threadIdx.x >> 5] = an; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t2 = 0, tn = 0;
+    for (int w = 0; w < 32; ++w) { t2 += s2[w]; tn += sn[w]; }
+    big_thr[p] = tn > 0 ? BIG_SIGMA * (float)sqrt(t2 / tn) : 0.f;
+  }
+}
+}  // namespace
+
+void lpf_fused_hit_sizes(const LpfFusedPlan* pl, int n_planes, long long* hit_bytes, long long* n_seg) {
+  *n_seg = (long long)pl->n_items * n_planes;
+  *hit_bytes = *n_seg * pl->seg_cap * (long long)sizeof(HitRec);
+}
+
+float lpf_fused_big_sigma(void) { return BIG_SIGMA; }
+
 int lpf_launch_detect_fused(lpf_ctx* c, LpfFusedPlan* pl, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok,
                             lpf_det* d_dets, int32_t* d_ndets, bool sum_done, cudaStream_t st) {
   const lpf_params& p = c->p;
-  if (!sum_done) {     // the chained frame call has done both in its second QC pass
+  if (!sum_done) {     // the chained frame call has done all of this in its QC passes
     LPF_CUDA(cudaMemsetAsync(d_ndets, 0, sizeof(int32_t), st));
     int rc = lpf_launch_sum_plane(c, L, d_cube, d_band_ok, p.detect_sum_plane != 0, st);   // + the exact-zero check
     if (rc) return rc;
+    LPF_KLAUNCH(c, KID_MISC, st, k_big_thr<<<c->n_planes, 1024, 0, st>>>(d_cube, L.sum_plane, c->W, c->N, p.B, L.big_thr));
   }
   FusedArgs a{};
   a.cube = d_cube; a.sum_plane = L.sum_plane; a.band_ok = d_band_ok; a.W = c->W;
   a.nm_pad = pl->d_nm_pad; a.ic_pad = pl->d_ic_pad; a.items = pl->d_items; a.flags = pl->d_flags; a.dirty = L.dirty; a.dirty_seq = L.dirty_seq;
-  a.B = p.B; a.Dy = p.Dy; a.Dx = p.Dx; a.CW = pl->CW; a.k_max = p.k_max; a.max_det = p.max_det;
+  a.big_thr = L.big_thr;
+  a.B = p.B; a.Dy = p.Dy; a.Dx = p.Dx; a.CW = pl->CW; a.k_max = p.k_max; a.max_det = p.max_det; a.seg_cap = pl->seg_cap; a.n_items = pl->n_items;
   a.g0 = c->g_mf.g[3]; a.g1 = c->g_mf.g[2]; a.g2 = c->g_mf.g[1]; a.g3 = c->g_mf.g[0];
   a.kappa2 = p.kappa * p.kappa; a.eps_rel = p.eps_rel; a.nm_const = pl->nm_const; a.ic_const = pl->ic_const;
+  a.hits = reinterpret_cast<HitRec*>(L.hits); a.hit_cnt = L.hit_cnt;
   a.dets = d_dets; a.ndets = d_ndets; a.counters = c->counters;
   const dim3 grid(pl->n_items, c->n_planes);
   LPF_KLAUNCH(c, KID_FUSED_DETECT, st, fused_dispatch(pl->NW, a, grid, pl->smem, st, false));
+  {   // enough blocks per segment to cover the GPU a few times over; a block leaves at once when its share is empty
+    const int nseg = pl->n_items * c->n_planes;
+    const int split = std::max(1, std::min(64, (8 * c->n_sm + nseg - 1) / nseg));
+    LPF_KLAUNCH(c, KID_PEAKS, st, k_peaks<<<dim3(split, nseg), 128, 0, st>>>(a));
+  }
   return LPF_OK;
 }

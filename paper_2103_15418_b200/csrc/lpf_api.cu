@@ -1,4 +1,5 @@
 // C-ABI entry points (include/lpf.h): argument checks, context life cycle, step chaining.
+#include <algorithm>
 #include <climits>
 #include <cmath>
 #include <cstdio>
@@ -82,8 +83,11 @@ int check_params(const lpf_params* p) {
 int alloc_lane(lpf_ctx* c, LpfLane& L) {
   const lpf_params& p = c->p;
   const size_t N = (size_t)c->N, P = (size_t)p.B + 1;
-  TRY(dalloc(&L.qc_part1, (size_t)p.B * c->qc_nblk * 3));
-  TRY(dalloc(&L.qc_part2, (size_t)lpf_qc2_blocks(c) * p.B * 3));
+  TRY(dalloc(&L.qc_part1, (size_t)p.B * std::max(c->qc_nblk, lpf_qs_blocks(c)) * 3));
+  TRY(dalloc(&L.qc_part2, (size_t)std::max(lpf_qc2_blocks(c), lpf_qs_blocks(c)) * p.B * 3));
+  TRY(dalloc(&L.qc_mom, (size_t)p.B * 3));
+  TRY(dalloc(&L.dirty_b, (size_t)p.B));
+  LPF_CUDA(cudaMemset(L.dirty_b, 0, (size_t)p.B * sizeof(int32_t)));
   TRY(dalloc(&L.qc_band_clip, (size_t)p.B * 2));
   TRY(dalloc(&L.qc_counter, 2));
   LPF_CUDA(cudaMemset(L.qc_counter, 0, 2 * sizeof(int32_t)));
@@ -101,6 +105,14 @@ int alloc_lane(lpf_ctx* c, LpfLane& L) {
   TRY(dalloc(&L.tmp_snr, (size_t)p.max_det));
   TRY(dalloc(&L.tmp_n, 1));
   TRY(dalloc(&L.stats, (size_t)p.B * LPF_STATS_PER_BAND));
+  TRY(dalloc(&L.big_thr, (size_t)p.B + 1));
+  if (c->fused) {
+    long long hb = 0, ns = 0;
+    lpf_fused_hit_sizes(c->fused, c->n_planes, &hb, &ns);
+    TRY(dalloc(reinterpret_cast<char**>(&L.hits), (size_t)hb));
+    TRY(dalloc(&L.hit_cnt, (size_t)ns));
+    LPF_CUDA(cudaMemset(L.hit_cnt, 0, (size_t)ns * sizeof(int32_t)));
+  }
   TRY(dalloc(&L.zeta_cnt, (size_t)p.B));
   LPF_CUDA(cudaMemset(L.zeta_cnt, 0, (size_t)p.B * sizeof(int32_t)));
   TRY(dalloc(&L.band_ok, (size_t)p.B + 1));
@@ -125,7 +137,7 @@ int alloc_lane(lpf_ctx* c, LpfLane& L) {
 void free_lane(LpfLane& L) {
   void* ptrs[] = {L.qc_part1, L.qc_part2, L.qc_band_clip, L.qc_counter, L.sum_plane, L.dirty, L.F, L.C, L.S, L.Y, L.normp, L.M, L.tmp_pos, L.tmp_plane,
                   L.tmp_snr, L.tmp_n, L.stats, L.band_ok, L.dets, L.ndets, L.upos, L.uplane, L.usnr, L.nu,
-                  L.cand_idx, L.act_slots, L.act_pix, L.npos, L.flux, L.cube, L.zeta_cnt};
+                  L.cand_idx, L.act_slots, L.act_pix, L.npos, L.flux, L.cube, L.zeta_cnt, L.hits, L.hit_cnt, L.big_thr, L.dirty_b, L.qc_mom};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (L.h_counts) cudaFreeHost(L.h_counts);
   L = LpfLane();
@@ -408,7 +420,7 @@ int lpf_get_counters(lpf_ctx* c, int64_t* h_out) {
 static const char* const kKernelNames[KID_COUNT] = {
     "qc_pass1", "qc_pass2", "qc_running", "sum_plane", "conv_mf", "conv_c", "conv_s", "conv_den", "threshold_peaks",
     "fused_detect", "dedupe_scatter", "dedupe_select", "dedupe_sort", "assoc_match", "assoc_update", "measure_flux",
-    "append_dynspec", "backfill", "misc"};
+    "append_dynspec", "backfill", "misc", "peaks", "qc_verdict", "qc_clip_finish"};
 
 int lpf_profile_begin(lpf_ctx* c) {
   if (!c) return LPF_E_ARG;

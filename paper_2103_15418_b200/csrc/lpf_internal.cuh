@@ -20,9 +20,11 @@ struct LpfLane {
   double* qc_part2 = nullptr;  // [blocks of pass 2][B][3]  clipped
   float* qc_band_clip = nullptr;   // [B][2] centre, half width of the clip round
   int32_t* qc_counter = nullptr;   // [2] last-block counters of the two passes
+  double* qc_mom = nullptr;        // [B][3] finished sums of the streaming QC
   float* sum_plane = nullptr;  // [N]
   int32_t* dirty = nullptr;    // [1] == dirty_seq: the cube of the current frame needs masking (detect_general.cu k_sum_plane)
   int32_t dirty_seq = 0;
+  int32_t* dirty_b = nullptr;  // [B] == dirty_seq: that band is not an exact zero at some invalid pixel (streaming QC)
   float* F = nullptr;          // [(B+1)][N] matched-filtered planes (general path)
   float* C = nullptr;          // [(B+1)][N]
   float* S = nullptr;          // [(B+1)][N]
@@ -49,6 +51,9 @@ struct LpfLane {
   float* flux = nullptr;
   float* cube = nullptr;       // device cube for the *_host entry (lazy)
   int32_t* zeta_cnt = nullptr; // [B] eq. A.2 counts of the lane's frame
+  void* hits = nullptr;        // fused path: the hit list of the frame, [segments][seg_cap] entries (detect_fused.cu)
+  int32_t* hit_cnt = nullptr;  // [segments]
+  float* big_thr = nullptr;    // [B + 1] 'far above the noise' level of every plane (64 x rms)
   int32_t* h_counts = nullptr; // pinned [4]
 };
 
@@ -115,7 +120,7 @@ int lpf_cuda_fail(cudaError_t e, const char* what);
 enum LpfKernelId {
   KID_QC_PASS1 = 0, KID_QC_PASS2, KID_QC_VERDICT /* = the running per-pixel test, eq. A.2 */, KID_SUM_PLANE, KID_CONV_MF, KID_CONV_C, KID_CONV_S,
   KID_CONV_DEN, KID_THRESHOLD, KID_FUSED_DETECT, KID_DEDUPE_SCATTER, KID_DEDUPE_SELECT, KID_DEDUPE_SORT,
-  KID_ASSOC_MATCH, KID_ASSOC_UPDATE, KID_MEASURE_FLUX, KID_APPEND, KID_BACKFILL, KID_MISC, KID_COUNT
+  KID_ASSOC_MATCH, KID_ASSOC_UPDATE, KID_MEASURE_FLUX, KID_APPEND, KID_BACKFILL, KID_MISC, KID_PEAKS, KID_QC_VERDICT1, KID_QC_CLIPFIN, KID_COUNT
 };
 void lpf_prof_pre(lpf_ctx* c, int kid, cudaStream_t st);
 void lpf_prof_post(lpf_ctx* c, cudaStream_t st);
@@ -136,6 +141,7 @@ int lpf_launch_qc(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, u
 int lpf_launch_qc_sum(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, int32_t* zero_me,
                       cudaStream_t st);
 int lpf_qc2_blocks(const lpf_ctx* c);
+int lpf_qs_blocks(const lpf_ctx* c);
 int lpf_launch_qc_running(lpf_ctx* c, LpfLane& L, const float* d_cube, uint8_t* d_band_ok, cudaStream_t st);
 
 int lpf_launch_sum_plane(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, bool want_sum, cudaStream_t st);
@@ -144,6 +150,8 @@ int lpf_launch_detect_general(lpf_ctx* c, LpfLane& L, const float* d_cube, const
 int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out);
 void lpf_fused_plan_free(LpfFusedPlan* pl);
 int lpf_fused_plan_info(const LpfFusedPlan* pl, int* cw, int* threads, int* n_items, long long* smem);
+void lpf_fused_hit_sizes(const LpfFusedPlan* pl, int n_planes, long long* hit_bytes, long long* n_seg);
+float lpf_fused_big_sigma(void);
 int lpf_launch_detect_fused(lpf_ctx* c, LpfFusedPlan* pl, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok,
                             lpf_det* d_dets, int32_t* d_ndets, bool sum_done, cudaStream_t st);
 int lpf_launch_detect(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, lpf_det* d_dets,

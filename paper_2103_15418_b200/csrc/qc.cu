@@ -1,16 +1,21 @@
 // S1 + S2 (+ S3): quality control (App. A, eq. A.1; O1, O2) and the sum plane.
 //
-// Pass 1 streams the cube once with 128-bit loads and accumulates, per band over valid pixels, n,
-// sum(x - p) and sum(x - p)^2 about a per-band pivot p (the band's first valid pixel): fp32 over
-// runs of <= 16 values, float64 across runs, warp-shuffle + shared-memory block reduction, one
-// partial per block.  The LAST block to finish (a device-wide counter) finishes the moments and
-// evaluates eq. A.1 across bands (median, MAD, SE floor) for the mean vector and the rms vector:
-// band_ok, frame_ok, and the centre / half width of the clip round.
-// Pass 2 reads the cube a second time, all bands of a pixel group together, and does up to three
-// things with that one read: the moments of the pixels inside the one qc_clip-sigma clip round
-// (O1), the sum plane X_B = sum of the accepted bands (O4, S3) and the check that every invalid
-// pixel of the accepted bands holds an exact zero (then W X = X and the fused detection kernel
-// reads the cube unmasked).  Its last block finishes the clipped moments.
+// The streaming form (a 16-byte aligned cube with N a multiple of 4: every shaped configuration):
+//   k_qc_moments  reads the cube ONCE, all bands of a group of 4 pixels in one thread (loads of the next four
+//                 bands in flight while four are consumed), and takes three things from that read: per band over
+//                 valid pixels sum(x - p) and sum(x - p)^2 about a pivot p (the band's first valid pixel; packed
+//                 fp32 per thread - a thread sees a few dozen values - then float64), the sum plane of ALL bands
+//                 (O4, S3: speculative - the verdict is not known yet, and 19 frames in 20 reject nothing) and,
+//                 per band, whether some invalid pixel holds anything but an exact zero.
+//   k_qc_verdict  one block: finishes the moments, eq. A.1 across bands (median, MAD, SE floor) for the mean
+//                 vector and the rms vector -> band_ok, frame_ok, the centre / half width of the clip round, the
+//                 "far above the noise" level of every plane, and whether the accepted bands are clean outside
+//                 the mask (then W X = X and the fused detection kernel reads the cube unmasked).
+//   k_qc_clip     second read of the cube: the moments of the pixels inside the one qc_clip-sigma clip round
+//                 (O1); when a band was rejected it also rebuilds the sum plane from the accepted bands.
+//   k_qc_clip_finish  one block: the clipped mean / rms.
+// The generic form (any alignment) keeps the two older kernels, whose last block does the finishing:
+// k_qc_pass1 (per-band moments + verdict) and k_qc_pass2 (clip round, sum plane, exact-zero check).
 #include "lpf_internal.cuh"
 
 namespace {
@@ -56,22 +61,34 @@ struct QcArgs {
   float* stats;           // [B][8]
   uint8_t* band_ok;       // [B + 1]
   float* band_clip;       // [B][2] centre and half width of the clip round
+  float* big_thr;         // [B + 1] big_sigma x rms of every plane (the sum plane: of the accepted bands, in quadrature)
+  float big_sigma;
   int32_t* counter;
 };
 
 // eq. A.1 for all bands, by one block of QC_THREADS threads.
-__device__ void qc_verdict(const QcArgs& a) {
+__device__ void qc_verdict(const QcArgs& a, const double* mom = nullptr /* [B][3] n, sum, sum of squares: skips the partials */) {
   __shared__ double s_mean[LPF_MAX_BANDS], s_rms[LPF_MAX_BANDS], s_n[LPF_MAX_BANDS], s_sorted[LPF_MAX_BANDS], s_dev[LPF_MAX_BANDS];
   __shared__ int s_fin[LPF_MAX_BANDS];
   __shared__ int s_nfin, s_nok;
+  __shared__ float s_var_ok;
   const int B = a.B, nblk = a.nblk;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   // finish pass 1: warp w takes bands w, w + 8, ...; lanes share the partials of a band
   for (int b = warp; b < B; b += QC_WARPS) {
     double n = 0, s1 = 0, s2 = 0;
-    for (int i = lane; i < nblk; i += 32) {
-      const double* q = a.part1 + ((long long)b * nblk + i) * 3;
-      n += __ldcg(q); s1 += __ldcg(q + 1); s2 += __ldcg(q + 2);
+    if (mom) { if (lane == 0) { n = __ldcg(mom + 3 * b); s1 = __ldcg(mom + 3 * b + 1); s2 = __ldcg(mom + 3 * b + 2); } }
+    else for (int i0 = 0; i0 < nblk; i0 += 32 * 10) {      // thirty independent loads per lane and round (one round up to 320 blocks)
+      double v[10][3];
+#pragma unroll
+      for (int u = 0; u < 10; ++u) {
+        const int i = i0 + 32 * u + lane;
+        const double* q = a.part1 + ((long long)b * nblk + (i < nblk ? i : 0)) * 3;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) v[u][k] = i < nblk ? __ldcg(q + k) : 0.0;
+      }
+#pragma unroll
+      for (int u = 0; u < 10; ++u) { n += v[u][0]; s1 += v[u][1]; s2 += v[u][2]; }
     }
     n = lpf_warp_sum(n); s1 = lpf_warp_sum(s1); s2 = lpf_warp_sum(s2);
     if (lane == 0) {
@@ -87,7 +104,7 @@ __device__ void qc_verdict(const QcArgs& a) {
       s_fin[b] = (n > 0 && isfinite(mean) && isfinite(rms)) ? 1 : 0;
     }
   }
-  if (threadIdx.x == 0) { s_nfin = 0; s_nok = 0; }
+  if (threadIdx.x == 0) { s_nfin = 0; s_nok = 0; s_var_ok = 0.f; }
   __syncthreads();
   const int b = threadIdx.x;
   const double n = b < B ? s_n[b] : 0.0, mean = b < B ? s_mean[b] : 0.0, rms = b < B ? s_rms[b] : 0.0;
@@ -128,7 +145,7 @@ __device__ void qc_verdict(const QcArgs& a) {
     zm = den_m > 0 ? num_m / den_m : (num_m == 0 ? 0.0 : (num_m > 0 ? INFINITY : -INFINITY));
     zr = den_r > 0 ? num_r / den_r : (num_r == 0 ? 0.0 : (num_r > 0 ? INFINITY : -INFINITY));
     ok = (fabs(zm) <= (double)a.tau && fabs(zr) <= (double)a.tau) ? 1 : 0;
-    if (ok) atomicAdd(&s_nok, 1);
+    if (ok) { atomicAdd(&s_nok, 1); atomicAdd(&s_var_ok, (float)(rms * rms)); }
   }
   __syncthreads();
   if (b < B) {
@@ -138,8 +155,12 @@ __device__ void qc_verdict(const QcArgs& a) {
     a.band_ok[b] = (uint8_t)ok;
     a.band_clip[2 * b] = (float)mean;                          // the clip round is decided in float32 (R25)
     a.band_clip[2 * b + 1] = (float)((double)a.qc_clip * rms);
+    a.big_thr[b] = a.big_sigma * (float)rms;
   }
-  if (threadIdx.x == 0) a.band_ok[B] = (s_nok >= (B + 1) / 2) ? 1 : 0;
+  if (threadIdx.x == 0) {
+    a.band_ok[B] = (s_nok >= (B + 1) / 2) ? 1 : 0;
+    a.big_thr[B] = a.big_sigma * sqrtf(s_var_ok);
+  }
 }
 
 __global__ void __launch_bounds__(QC_THREADS)
@@ -212,6 +233,38 @@ struct Qc2Args {
   int32_t* zero_me;        // a counter this kernel resets (the record count of the frame), or null
   int32_t* counter;
 };
+
+// the clipped moments from the per-block partials [nblk][B][3]: warp w takes bands w, w + nwarps, ...
+__device__ void clip_finish(const double* part2, int nblk, int B, const float* band_clip, float* stats) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  for (int b = warp; b < B; b += nw) {
+    double nc = 0, c1 = 0, c2 = 0;
+    for (int i0 = 0; i0 < nblk; i0 += 32 * 10) {      // thirty independent loads per lane and round
+      double v[10][3];
+#pragma unroll
+      for (int u = 0; u < 10; ++u) {
+        const int i = i0 + 32 * u + lane;
+        const double* r = part2 + ((long long)(i < nblk ? i : 0) * B + b) * 3;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) v[u][k] = i < nblk ? __ldcg(r + k) : 0.0;
+      }
+#pragma unroll
+      for (int u = 0; u < 10; ++u) { nc += v[u][0]; c1 += v[u][1]; c2 += v[u][2]; }
+    }
+    nc = lpf_warp_sum(nc); c1 = lpf_warp_sum(c1); c2 = lpf_warp_sum(c2);
+    if (lane == 0) {
+      double cmean = 0, crms = 0;
+      if (nc > 0) {
+        const double k1 = c1 / nc;
+        cmean = (double)band_clip[2 * b] + k1;         // the clip pass is centred on the fp32 mean
+        const double cv = c2 / nc - k1 * k1;
+        crms = sqrt(cv > 0 ? cv : 0.0);
+      }
+      float* o = stats + LPF_STATS_PER_BAND * b;
+      o[3] = (float)nc; o[4] = (float)cmean; o[5] = (float)crms;
+    }
+  }
+}
 
 // CLIP: the clipped moments of every band; SUM: the sum plane of the accepted bands + the exact-zero check.
 template <bool CLIP, bool SUM>
@@ -332,25 +385,281 @@ k_qc_pass2(const Qc2Args a) {
     a.part2[((long long)blockIdx.x * B + b) * 3 + k] = t;
   }
   if (!last_block_done(a.counter, gridDim.x)) return;
-  // the clipped moments: warp w takes bands w, w + 8, ...
-  for (int b = warp; b < B; b += QC2_WARPS) {
-    double nc = 0, c1 = 0, c2 = 0;
-    for (int i = lane; i < (int)gridDim.x; i += 32) {
-      const double* r = a.part2 + ((long long)i * B + b) * 3;
-      nc += __ldcg(r); c1 += __ldcg(r + 1); c2 += __ldcg(r + 2);
+  clip_finish(a.part2, (int)gridDim.x, B, a.band_clip, a.stats);
+}
+
+// ---- the streaming form -------------------------------------------------------------------------------------------
+#ifndef LPF_QS_THREADS
+#define LPF_QS_THREADS 256
+#endif
+#ifndef LPF_QS_BLOCKS
+#define LPF_QS_BLOCKS 2
+#endif
+constexpr int QS_THREADS = LPF_QS_THREADS;     // LPF_QS_BLOCKS blocks per SM; a thread owns one group of 4 pixels at a time, all bands
+constexpr int QS_WARPS = QS_THREADS / 32;
+constexpr int QS_BG = 16;           // bands of one register-resident group
+
+__device__ __forceinline__ float2 q_add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 q_fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+
+struct QsArgs {
+  const float* cube; const uint8_t* W; long long N; int first_valid, B;
+  double* part1;          // [B][gridDim.x][3]
+  float* sum_out;         // [N] or null
+  int32_t* dirty_b; int seq;   // [B] == seq: the band holds something other than an exact zero at an invalid pixel
+};
+
+// 16-byte asynchronous copies global -> shared (LDGSTS): the bytes in flight are not held in registers.  A thread
+// owns one 16-byte slot per band of the group; slot b is refilled for the thread's next pixel group as soon as it
+// has been consumed, one commit group per copy, so "at most QS_BG - 1 groups pending" means "slot b has landed".
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+constexpr size_t QS_SMEM = (size_t)QS_BG * QS_THREADS * sizeof(float4);   // 64 KB
+
+__global__ void __launch_bounds__(QS_THREADS, LPF_QS_BLOCKS)
+k_qc_moments(const QsArgs a) {
+  extern __shared__ float4 qs_slots[];     // [QS_BG][QS_THREADS]
+  __shared__ float s_piv[LPF_MAX_BANDS];
+  __shared__ double s_red[QS_WARPS][QS_BG][2];
+  __shared__ double s_n[QS_WARPS];
+  const int B = a.B, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long N = a.N, n4 = N >> 2;
+  for (int b = threadIdx.x; b < B; b += QS_THREADS) s_piv[b] = a.cube[(long long)b * N + a.first_valid];
+  __syncthreads();
+  const long long per = (n4 + gridDim.x - 1) / gridDim.x;
+  const long long q0 = (long long)blockIdx.x * per, q1 = q0 + per < n4 ? q0 + per : n4;
+  const float4* X4 = reinterpret_cast<const float4*>(a.cube);
+  const bool want_sum = a.sum_out != nullptr;
+  const uint32_t slot0 = (uint32_t)__cvta_generic_to_shared(qs_slots + threadIdx.x);
+
+  for (int g0 = 0; g0 < B; g0 += QS_BG) {
+    float2 f1[QS_BG], f2[QS_BG];
+#pragma unroll
+    for (int b = 0; b < QS_BG; ++b) { f1[b] = make_float2(0.f, 0.f); f2[b] = f1[b]; }
+    unsigned dirt = 0u;            // one bit per band of the group
+    int nval = 0;
+    long long q = q0 + threadIdx.x;
+    bool has = q < q1;
+#pragma unroll
+    for (int b = 0; b < QS_BG; ++b) {
+      if (has && g0 + b < B) cp_async16(slot0 + (uint32_t)(b * QS_THREADS * sizeof(float4)), X4 + (long long)(g0 + b) * n4 + q);
+      cp_commit();
     }
-    nc = lpf_warp_sum(nc); c1 = lpf_warp_sum(c1); c2 = lpf_warp_sum(c2);
-    if (lane == 0) {
-      double cmean = 0, crms = 0;
-      if (nc > 0) {
-        const double k1 = c1 / nc;
-        cmean = (double)s_clip[b][0] + k1;             // pass 2 is centred on the fp32 mean
-        const double cv = c2 / nc - k1 * k1;
-        crms = sqrt(cv > 0 ? cv : 0.0);
+    unsigned wm = has ? __ldg(reinterpret_cast<const unsigned*>(a.W) + q) : 0u;
+    while (has) {
+      const long long qn = q + QS_THREADS;
+      const bool hasn = qn < q1;
+      const unsigned wmn = hasn ? __ldg(reinterpret_cast<const unsigned*>(a.W) + qn) : 0u;
+      nval += __popc(wm & 0x01010101u);
+      const unsigned inv = ~(wm * 0xffu);      // 0xff in the bytes of the invalid pixels (W is 0 / 1); 0: none
+      float2 s01 = make_float2(0.f, 0.f), s23 = s01;
+      if (g0 > 0 && want_sum) { const float4 sp = reinterpret_cast<const float4*>(a.sum_out)[q]; s01 = make_float2(sp.x, sp.y); s23 = make_float2(sp.z, sp.w); }
+#pragma unroll
+      for (int b = 0; b < QS_BG; ++b) {
+        cp_wait<QS_BG - 1>();
+        const bool live = g0 + b < B;
+        const float4 x = live ? qs_slots[b * QS_THREADS + threadIdx.x] : make_float4(0.f, 0.f, 0.f, 0.f);
+        const float2 x01 = make_float2(x.x, x.y), x23 = make_float2(x.z, x.w);
+        const float np = -s_piv[live ? g0 + b : 0];
+        float2 t01 = q_add2(x01, make_float2(np, np)), t23 = q_add2(x23, make_float2(np, np));
+        if (inv) {     // a group with invalid pixels: they count as 0 whatever they hold (NaN and Inf included)
+          if (inv & 0x000000ffu) t01.x = 0.f;
+          if (inv & 0x0000ff00u) t01.y = 0.f;
+          if (inv & 0x00ff0000u) t23.x = 0.f;
+          if (inv & 0xff000000u) t23.y = 0.f;
+          const unsigned nz = ((__float_as_uint(x.x) << 1) != 0u && (inv & 0x000000ffu)) |
+                              ((__float_as_uint(x.y) << 1) != 0u && (inv & 0x0000ff00u)) |
+                              ((__float_as_uint(x.z) << 1) != 0u && (inv & 0x00ff0000u)) |
+                              ((__float_as_uint(x.w) << 1) != 0u && (inv & 0xff000000u));
+          dirt |= nz << b;
+        }
+        f1[b] = q_add2(f1[b], q_add2(t01, t23));
+        f2[b] = q_fma2(t01, t01, q_fma2(t23, t23, f2[b]));
+        s01 = q_add2(s01, x01); s23 = q_add2(s23, x23);
+        if (hasn && live) cp_async16(slot0 + (uint32_t)(b * QS_THREADS * sizeof(float4)), X4 + (long long)(g0 + b) * n4 + qn);
+        cp_commit();
       }
-      float* o = a.stats + LPF_STATS_PER_BAND * b;
-      o[3] = (float)nc; o[4] = (float)cmean; o[5] = (float)crms;
+      if (want_sum) reinterpret_cast<float4*>(a.sum_out)[q] = make_float4(s01.x, s01.y, s23.x, s23.y);
+      q = qn; has = hasn; wm = wmn;
     }
+    cp_wait<0>();
+    // block reduction: fp32 across the warp (a few hundred values), float64 from there on
+#pragma unroll
+    for (int b = 0; b < QS_BG; ++b) {
+      float v1 = f1[b].x + f1[b].y, v2 = f2[b].x + f2[b].y;
+      v1 = lpf_warp_sum(v1); v2 = lpf_warp_sum(v2);
+      if (lane == 0) { s_red[warp][b][0] = (double)v1; s_red[warp][b][1] = (double)v2; }
+      const unsigned any_dirt = __ballot_sync(0xffffffffu, (dirt >> b) & 1u);
+      if (any_dirt && lane == 0 && g0 + b < B) a.dirty_b[g0 + b] = a.seq;
+    }
+    nval = lpf_warp_sum(nval);
+    if (lane == 0) s_n[warp] = (double)nval;
+    __syncthreads();
+    if (threadIdx.x < QS_BG && g0 + threadIdx.x < B) {
+      double t1 = 0, t2 = 0, tn = 0;
+#pragma unroll
+      for (int w = 0; w < QS_WARPS; ++w) { t1 += s_red[w][threadIdx.x][0]; t2 += s_red[w][threadIdx.x][1]; tn += s_n[w]; }
+      double* o = a.part1 + ((long long)(g0 + threadIdx.x) * gridDim.x + blockIdx.x) * 3;
+      o[0] = tn; o[1] = t1; o[2] = t2;
+    }
+    __syncthreads();
+  }
+}
+
+struct QvArgs {
+  QcArgs q;                 // partials [B][nblk][3] and everything the verdict writes
+  const int32_t* dirty_b; int seq; int32_t* dirty;   // -> *dirty = seq when an accepted band is not clean outside the mask
+  int32_t* zero_me;         // a counter this kernel resets (the record count of the frame), or null
+  double* mom;              // [B][3] scratch: the finished sums of every band
+};
+
+// sum of three doubles over the block (QC_THREADS threads); valid in thread 0
+__device__ __forceinline__ void block_sum3(double& a, double& b, double& c) {
+  __shared__ double s_bs[3][QC_WARPS];
+  a = lpf_warp_sum(a); b = lpf_warp_sum(b); c = lpf_warp_sum(c);
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  if (l == 0) { s_bs[0][w] = a; s_bs[1][w] = b; s_bs[2][w] = c; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    a = 0; b = 0; c = 0;
+#pragma unroll
+    for (int i = 0; i < QC_WARPS; ++i) { a += s_bs[0][i]; b += s_bs[1][i]; c += s_bs[2][i]; }
+  }
+}
+
+// one block per band sums that band's partials (one load round); the last block to finish evaluates eq. A.1
+__global__ void __launch_bounds__(QC_THREADS)
+k_qc_verdict(const QvArgs a) {
+  const int b = blockIdx.x, nblk = a.q.nblk;
+  double n = 0, s1 = 0, s2 = 0;
+  for (int i = threadIdx.x; i < nblk; i += QC_THREADS) {
+    const double* q = a.q.part1 + ((long long)b * nblk + i) * 3;
+    n += __ldcg(q); s1 += __ldcg(q + 1); s2 += __ldcg(q + 2);
+  }
+  block_sum3(n, s1, s2);
+  if (threadIdx.x == 0) { a.mom[3 * b] = n; a.mom[3 * b + 1] = s1; a.mom[3 * b + 2] = s2; }
+  if (!last_block_done(a.q.counter, gridDim.x)) return;
+  const int dirt = ((int)threadIdx.x < a.q.B) ? (__ldcg(&a.dirty_b[threadIdx.x]) == a.seq) : 0;   // asked for before the verdict
+  qc_verdict(a.q, a.mom);
+  const bool mine = (int)threadIdx.x < a.q.B && dirt && a.q.band_ok[threadIdx.x];   // band_ok[t] was written by this thread
+  const int bad = __syncthreads_or(mine ? 1 : 0);
+  if (threadIdx.x == 0) {
+    if (bad) *a.dirty = a.seq;
+    if (a.zero_me) *a.zero_me = 0;
+  }
+}
+
+struct QkArgs {
+  const float* cube; const uint8_t* W; const uint8_t* band_ok; long long N; int B;
+  const float* band_clip;  // [B][2]
+  double* part2;           // [gridDim.x][B][3]
+  float* sum_out;          // [N]: rebuilt from the accepted bands when a band was rejected; or null
+};
+
+__global__ void __launch_bounds__(QS_THREADS, LPF_QS_BLOCKS)
+k_qc_clip(const QkArgs a) {
+  extern __shared__ float4 qs_slots[];     // [QS_BG][QS_THREADS]
+  __shared__ float s_c[LPF_MAX_BANDS], s_w[LPF_MAX_BANDS];
+  __shared__ uint8_t s_ok[LPF_MAX_BANDS + 1];
+  __shared__ double s_red[QS_WARPS][QS_BG][3];
+  __shared__ int s_rej;
+  const int B = a.B, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long N = a.N, n4 = N >> 2;
+  if (threadIdx.x == 0) s_rej = 0;
+  __syncthreads();
+  for (int b = threadIdx.x; b <= B; b += QS_THREADS) {
+    s_ok[b] = a.band_ok[b];
+    if (b < B) { s_c[b] = a.band_clip[2 * b]; s_w[b] = a.band_clip[2 * b + 1]; if (!s_ok[b]) s_rej = 1; }
+  }
+  __syncthreads();
+  const bool resum = a.sum_out != nullptr && s_rej != 0 && s_ok[B] != 0;   // a rejected frame has no sum plane
+  const long long per = (n4 + gridDim.x - 1) / gridDim.x;
+  const long long q0 = (long long)blockIdx.x * per, q1 = q0 + per < n4 ? q0 + per : n4;
+  const float4* X4 = reinterpret_cast<const float4*>(a.cube);
+  const uint32_t slot0 = (uint32_t)__cvta_generic_to_shared(qs_slots + threadIdx.x);
+
+  for (int g0 = 0; g0 < B; g0 += QS_BG) {
+    float fn[QS_BG], f1[QS_BG], f2[QS_BG];
+#pragma unroll
+    for (int b = 0; b < QS_BG; ++b) { fn[b] = 0.f; f1[b] = 0.f; f2[b] = 0.f; }
+    long long q = q0 + threadIdx.x;
+    bool has = q < q1;
+#pragma unroll
+    for (int b = 0; b < QS_BG; ++b) {
+      if (has && g0 + b < B) cp_async16(slot0 + (uint32_t)(b * QS_THREADS * sizeof(float4)), X4 + (long long)(g0 + b) * n4 + q);
+      cp_commit();
+    }
+    unsigned wm = has ? __ldg(reinterpret_cast<const unsigned*>(a.W) + q) : 0u;
+    while (has) {
+      const long long qn = q + QS_THREADS;
+      const bool hasn = qn < q1;
+      const unsigned wmn = hasn ? __ldg(reinterpret_cast<const unsigned*>(a.W) + qn) : 0u;
+      const bool vv[4] = {(wm & 0x000000ffu) != 0, (wm & 0x0000ff00u) != 0, (wm & 0x00ff0000u) != 0, (wm & 0xff000000u) != 0};
+      float4 sp = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (resum && g0 > 0) sp = reinterpret_cast<const float4*>(a.sum_out)[q];
+#pragma unroll
+      for (int b = 0; b < QS_BG; ++b) {
+        cp_wait<QS_BG - 1>();
+        const bool live = g0 + b < B;
+        const int bb = live ? g0 + b : 0;
+        const float4 x = live ? qs_slots[b * QS_THREADS + threadIdx.x] : make_float4(0.f, 0.f, 0.f, 0.f);
+        const float c = s_c[bb], w = live ? s_w[bb] : -1.f;
+        const float xv[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const float d = xv[j] - c;
+          const bool take = vv[j] && fabsf(d) <= w;
+          const float dm = take ? d : 0.f;
+          fn[b] += take ? 1.f : 0.f; f1[b] += dm; f2[b] = fmaf(dm, dm, f2[b]);
+        }
+        if (resum && live && s_ok[bb]) { sp.x += x.x; sp.y += x.y; sp.z += x.z; sp.w += x.w; }
+        if (hasn && live) cp_async16(slot0 + (uint32_t)(b * QS_THREADS * sizeof(float4)), X4 + (long long)(g0 + b) * n4 + qn);
+        cp_commit();
+      }
+      if (resum) reinterpret_cast<float4*>(a.sum_out)[q] = sp;
+      q = qn; has = hasn; wm = wmn;
+    }
+    cp_wait<0>();
+#pragma unroll
+    for (int b = 0; b < QS_BG; ++b) {
+      const float vn = lpf_warp_sum(fn[b]), v1 = lpf_warp_sum(f1[b]), v2 = lpf_warp_sum(f2[b]);
+      if (lane == 0) { s_red[warp][b][0] = (double)vn; s_red[warp][b][1] = (double)v1; s_red[warp][b][2] = (double)v2; }
+    }
+    __syncthreads();
+    if (threadIdx.x < QS_BG && g0 + threadIdx.x < B) {
+      double t0 = 0, t1 = 0, t2 = 0;
+#pragma unroll
+      for (int w = 0; w < QS_WARPS; ++w) { t0 += s_red[w][threadIdx.x][0]; t1 += s_red[w][threadIdx.x][1]; t2 += s_red[w][threadIdx.x][2]; }
+      double* o = a.part2 + ((long long)blockIdx.x * B + g0 + threadIdx.x) * 3;
+      o[0] = t0; o[1] = t1; o[2] = t2;
+    }
+    __syncthreads();
+  }
+}
+
+// one block per band: the clipped mean / rms from the per-block partials [nblk][B][3]
+__global__ void __launch_bounds__(QC_THREADS)
+k_qc_clip_finish(const double* part2, int nblk, int B, const float* band_clip, float* stats) {
+  const int b = blockIdx.x;
+  double nc = 0, c1 = 0, c2 = 0;
+  for (int i = threadIdx.x; i < nblk; i += QC_THREADS) {
+    const double* r = part2 + ((long long)i * B + b) * 3;
+    nc += __ldcg(r); c1 += __ldcg(r + 1); c2 += __ldcg(r + 2);
+  }
+  block_sum3(nc, c1, c2);
+  if (threadIdx.x == 0) {
+    double cmean = 0, crms = 0;
+    if (nc > 0) {
+      const double k1 = c1 / nc;
+      cmean = (double)band_clip[2 * b] + k1;         // the clip pass is centred on the fp32 mean
+      const double cv = c2 / nc - k1 * k1;
+      crms = sqrt(cv > 0 ? cv : 0.0);
+    }
+    float* o = stats + LPF_STATS_PER_BAND * b;
+    o[3] = (float)nc; o[4] = (float)cmean; o[5] = (float)crms;
   }
 }
 
@@ -465,7 +774,7 @@ static int qc_launch_pass1(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d
   QcArgs a{};
   a.cube = d_cube; a.W = c->W; a.N = c->N; a.first_valid = c->first_valid; a.B = c->p.B; a.nblk = c->qc_nblk;
   a.part1 = L.qc_part1; a.qc_clip = c->p.qc_clip; a.tau = c->p.qc_tau; a.stats = d_stats; a.band_ok = d_band_ok;
-  a.band_clip = L.qc_band_clip; a.counter = L.qc_counter;
+  a.band_clip = L.qc_band_clip; a.counter = L.qc_counter; a.big_thr = L.big_thr; a.big_sigma = lpf_fused_big_sigma();
   const dim3 grid(c->qc_nblk, c->p.B);
   LPF_KLAUNCH(c, KID_QC_PASS1, st, k_qc_pass1<<<grid, QC_THREADS, 0, st>>>(a));
   return LPF_OK;
@@ -496,8 +805,65 @@ int lpf_launch_qc_running(lpf_ctx* c, LpfLane& L, const float* d_cube, uint8_t* 
   return LPF_OK;
 }
 
+int lpf_qs_blocks(const lpf_ctx* c) {
+  const long long n4 = (c->N + 3) / 4;
+  const long long want = (n4 + QS_THREADS - 1) / QS_THREADS, cap = (long long)LPF_QS_BLOCKS * c->n_sm;
+  return (int)(want < 1 ? 1 : (want < cap ? want : cap));
+}
+
+// 64 KB of dynamic shared memory per block: opt in once per process
+static cudaError_t qs_attr() {
+  static bool done = false;
+  if (done) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(k_qc_moments, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)QS_SMEM);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_qc_clip, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)QS_SMEM);
+  done = e == cudaSuccess;
+  return e;
+}
+
+// the streaming form needs 128-bit loads of every band at the same pixel group
+static bool qc_streaming(const lpf_ctx* c, const float* d_cube) { return (c->N & 3) == 0 && (((uintptr_t)d_cube) & 15) == 0; }
+
+// moments + verdict (+ speculative sum plane, + reset of *zero_me), streaming form
+static int qs_launch_moments(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, bool want_sum,
+                             int32_t* zero_me, cudaStream_t st) {
+  const int nblk = lpf_qs_blocks(c);
+  L.dirty_seq = L.dirty_seq >= 0x7ffffff0 ? 1 : L.dirty_seq + 1;
+  QsArgs m{};
+  m.cube = d_cube; m.W = c->W; m.N = c->N; m.first_valid = c->first_valid; m.B = c->p.B; m.part1 = L.qc_part1;
+  m.sum_out = want_sum ? L.sum_plane : nullptr; m.dirty_b = L.dirty_b; m.seq = L.dirty_seq;
+  LPF_CUDA(qs_attr());
+  LPF_KLAUNCH(c, KID_QC_PASS1, st, k_qc_moments<<<nblk, QS_THREADS, QS_SMEM, st>>>(m));
+  QvArgs v{};
+  v.q.cube = d_cube; v.q.W = c->W; v.q.N = c->N; v.q.first_valid = c->first_valid; v.q.B = c->p.B; v.q.nblk = nblk;
+  v.q.part1 = L.qc_part1; v.q.qc_clip = c->p.qc_clip; v.q.tau = c->p.qc_tau; v.q.stats = d_stats; v.q.band_ok = d_band_ok;
+  v.q.band_clip = L.qc_band_clip; v.q.counter = L.qc_counter; v.q.big_thr = L.big_thr; v.q.big_sigma = lpf_fused_big_sigma();
+  v.dirty_b = L.dirty_b; v.seq = L.dirty_seq; v.dirty = L.dirty; v.zero_me = zero_me; v.mom = L.qc_mom;
+  LPF_KLAUNCH(c, KID_QC_VERDICT1, st, k_qc_verdict<<<c->p.B, QC_THREADS, 0, st>>>(v));
+  return LPF_OK;
+}
+
+static int qs_launch_clip(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, const uint8_t* d_band_ok, bool want_sum,
+                          cudaStream_t st) {
+  const int nblk = lpf_qs_blocks(c);
+  QkArgs k{};
+  k.cube = d_cube; k.W = c->W; k.band_ok = d_band_ok; k.N = c->N; k.B = c->p.B; k.band_clip = L.qc_band_clip; k.part2 = L.qc_part2;
+  k.sum_out = want_sum ? L.sum_plane : nullptr;
+  LPF_CUDA(qs_attr());
+  LPF_KLAUNCH(c, KID_QC_PASS2, st, k_qc_clip<<<nblk, QS_THREADS, QS_SMEM, st>>>(k));
+  LPF_KLAUNCH(c, KID_QC_CLIPFIN, st, k_qc_clip_finish<<<c->p.B, QC_THREADS, 0, st>>>(L.qc_part2, nblk, c->p.B, L.qc_band_clip, d_stats));
+  return LPF_OK;
+}
+
 // S1 + S2 as the C-ABI's lpf_cube_qc: statistics and verdict only.
 int lpf_launch_qc(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, cudaStream_t st) {
+  if (qc_streaming(c, d_cube)) {
+    int rc = qs_launch_moments(c, L, d_cube, d_stats, d_band_ok, false, nullptr, st);
+    if (rc) return rc;
+    rc = lpf_launch_qc_running(c, L, d_cube, d_band_ok, st);
+    if (rc) return rc;
+    return qs_launch_clip(c, L, d_cube, d_stats, d_band_ok, false, st);
+  }
   int rc = qc_launch_pass1(c, L, d_cube, d_stats, d_band_ok, st);
   if (rc) return rc;
   rc = lpf_launch_qc_running(c, L, d_cube, d_band_ok, st);
@@ -507,16 +873,26 @@ int lpf_launch_qc(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, u
   return LPF_OK;
 }
 
-// S1 + S2 + S3 for the chained frame call: the clip round, the sum plane and the exact-zero check share one
-// read of the cube; *zero_me (the frame's record counter) is reset on the way.
+// S1 + S2 + S3 for the chained frame call; *zero_me (the frame's record counter) is reset on the way.
+// Streaming form: the sum plane comes out of the first read of the cube (all bands; the clip pass rebuilds it
+// when the verdict rejected a band).  Generic form: the clip round, the sum plane and the exact-zero check share
+// the second read.
 int lpf_launch_qc_sum(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stats, uint8_t* d_band_ok, int32_t* zero_me,
                       cudaStream_t st) {
+  const bool want_sum = c->p.detect_sum_plane != 0;
+  if (qc_streaming(c, d_cube)) {
+    int rc = qs_launch_moments(c, L, d_cube, d_stats, d_band_ok, want_sum, zero_me, st);
+    if (rc) return rc;
+    rc = lpf_launch_qc_running(c, L, d_cube, d_band_ok, st);
+    if (rc) return rc;
+    return qs_launch_clip(c, L, d_cube, d_stats, d_band_ok, want_sum, st);
+  }
   int rc = qc_launch_pass1(c, L, d_cube, d_stats, d_band_ok, st);
   if (rc) return rc;
   rc = lpf_launch_qc_running(c, L, d_cube, d_band_ok, st);
   if (rc) return rc;
   L.dirty_seq = L.dirty_seq >= 0x7ffffff0 ? 1 : L.dirty_seq + 1;
-  const Qc2Args a = make_qc2(c, L, d_cube, d_band_ok, d_stats, c->p.detect_sum_plane != 0, zero_me);
+  const Qc2Args a = make_qc2(c, L, d_cube, d_band_ok, d_stats, want_sum, zero_me);
   LPF_KLAUNCH(c, KID_QC_PASS2, st, k_qc_pass2<true, true><<<lpf_qc2_blocks(c), QC2_THREADS, 0, st>>>(a));
   return LPF_OK;
 }
