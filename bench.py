@@ -61,6 +61,30 @@ def rank_seed(rank: int) -> int:
     return int(rank)
 
 
+def file_sha256(path):
+    import hashlib
+    try:
+        return hashlib.sha256(open(path, "rb").read()).hexdigest()
+    except OSError:
+        return None
+
+
+def traffic_from_profile(kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel`, from the committed `ncu --set full`
+    capture listed in profiles/traffic.json (never measured under the profiler in this run).  The entry names the CSV
+    and the SHA-256 of the kernel source at capture time; a source that has changed since is reported, not hidden."""
+    meta = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        e = json.load(open(meta))[kernel]
+    except Exception:
+        return None, {"source": None, "note": "no committed ncu capture for this kernel (profiles/traffic.json)"}
+    src_now = file_sha256(os.path.join(ROOT, e["kernel_source"]))
+    return float(e["dram_bytes_per_launch"]), {"source": e["csv"], "kernel_source": e["kernel_source"],
+                                               "kernel_source_sha256_at_capture": e["kernel_source_sha256"],
+                                               "kernel_source_unchanged": src_now == e["kernel_source_sha256"],
+                                               "launch_config": e.get("launch_config")}
+
+
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -127,8 +151,8 @@ def kernel_model(name: str, p: dict, n_valid: int):
     P = B + (1 if p["detect_sum_plane"] else 0)
     kmf, kbg = p["k_mf"], p["k_bg"]
     m = {
-        "qc_pass1": (4 * B * N, 6 * B * N),
-        "qc_pass2": (4 * B * N, 6 * B * N),
+        "qc_pass1": (4 * B * N + 4 * N + N, 5 * B * N),     # moments + speculative sum plane: cube once, plane written, mask
+        "qc_pass2": (4 * B * N + N, 6 * B * N),             # clip round: cube once, mask
         "sum_plane": (4 * B * N + 4 * N, B * N),
         "conv_mf": (8 * P * N, 2 * 2 * (2 * kmf + 1) * P * N),
         "conv_c": (8 * P * N, 2 * 2 * (2 * kbg + 1) * P * N),
@@ -192,22 +216,32 @@ def run_ours(args):
     sampler = ClockSampler(local)
     sampler.start()
     run_steps(0, args.warmup)
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
-    l0 = lpf.counters()["launches"]
+    t_next = args.warmup
     ts0 = sampler.mark()
-    ev0, ev1 = run_steps(args.warmup, args.steps)
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
+    # The timed block is EXACTLY args.steps steps between a barrier + synchronize on both sides.  A short block
+    # (< 100 ms: a few pipeline depths, dominated by fill and drain) is repeated and the MEDIAN block is reported
+    # ("median of 5 repeats"); every repeat is bracketed the same way.
+    blocks = []
+    while True:
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        l0 = lpf.counters()["launches"]
+        ev0, ev1 = run_steps(t_next, args.steps)
+        t_next += args.steps
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        b_ms, b_l = reduce_over_ranks(ev0.elapsed_time(ev1), lpf.counters()["launches"] - l0, dev, world)
+        blocks.append((b_ms, b_l))
+        if len(blocks) >= args.repeats or (len(blocks) == 1 and b_ms >= 100.0 and args.repeats_auto):
+            break
     ts1 = sampler.mark()
-    ms = ev0.elapsed_time(ev1)
-    launches = lpf.counters()["launches"] - l0
-    ms, launches = reduce_over_ranks(ms, launches, dev, world)
-    t_next = args.warmup + args.steps
+    blocks.sort()
+    ms, launches = blocks[len(blocks) // 2]
+    repeats = len(blocks)
 
     # keep the GPU under the same load until nvidia-smi has had time to sample it
     tload = time.time()
@@ -242,7 +276,8 @@ def run_ours(args):
         roof = {"bound": "alu", "achieved": tfl, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": tfl / ALU_PEAK_TFLOPS}
     roof.update({"kernel": dom, "us_per_launch": kernels[dom]["us_per_launch"], "share_of_step": kernels[dom]["us_per_step"] / step_kernel_us,
                  "algorithmic_bytes": abytes, "algorithmic_flops": aflops, "hbm_gbs": gbs, "hbm_frac": gbs / hbm_peak,
-                 "peak_source": peak_src, "alu_peak_source": "148 SM x 128 fp32 lanes x 2 x 1.965 GHz", "traffic": args.traffic})
+                 "peak_source": peak_src, "alu_peak_source": "nominal (derived, not measured): 148 SM x 128 fp32 lanes x 2 x 1.965 GHz"})
+    roof["traffic"], roof["traffic_source"] = traffic_from_profile(dom)
 
     frames_s = whole_job_value(world, args.steps, ms)
     step_gbs = cube_bytes * frames_s / 1e9 / world
@@ -299,7 +334,9 @@ def run_ours(args):
 
     out = {
         "metric": METRIC, "value": frames_s, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms / args.steps, "timed_region_ms": ms, "repeats": repeats,
+        "repeat_ms": [round(b[0], 4) for b in blocks], "repeat_rule": "median of the repeated timed blocks (each exactly `steps` steps)",
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": s.c.name, "cube": [B, D, D], "bg_kernel": args.bg, "n_iter": args.n_iter, "lanes": lanes, "n_back": args.n_back, "zeta_thr": args.zeta,
                    "pool_frames": n_pool, "pool_bytes": n_pool * cube_bytes,
@@ -340,29 +377,42 @@ def oracle_step_factory(cfg, bg, n_iter, crop):
 
 
 def cpu_baseline(cfg, args, seconds=12.0):
-    step, frac, name, p = oracle_step_factory(cfg, args.bg, args.n_iter, args.cpu_crop)
+    """The oracle as it stands, one thread, on FULL frames of the workload (>= 3 of them); a crop only
+    when --cpu-crop asks for one."""
+    D = CONFIG_D(cfg)
+    crop = D if args.cpu_crop <= 0 else min(D, args.cpu_crop)
+    step, frac, name, p = oracle_step_factory(cfg, args.bg, args.n_iter, crop)
     step()
     n = 0; t0 = time.perf_counter()
     while True:
         step(); n += 1
         dt = time.perf_counter() - t0
-        if dt >= seconds or n >= 64:
+        if (n >= 3 and dt >= seconds) or n >= 64:
             break
+    what = "full %dx%d frames" % (D, D) if crop == D else "a centred %dx%d crop" % (crop, crop)
     return {"value": n * frac / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": "%d steps of the whole chain on a centred %dx%d crop of %s (all %d bands), float64 oracle "
-                      "(row-then-column form of the window sums), scaled by crop/frame voxels" % (n, p["Dy"], p["Dx"], name, p["B"]),
-            "host_cpus": os.cpu_count()}
+            "sample": "%d steps of the whole chain on %s of %s (all %d bands), float64 oracle (row-then-column form of the "
+                      "window sums)%s" % (n, what, name, p["B"], "" if crop == D else ", scaled by crop/frame voxels"),
+            "seconds": dt, "host_cpus": os.cpu_count()}
 
 
 def run_reference(args):
     rank, world, _ = env_rank()
     if rank != 0:
         return None
-    # bounded sample: the crop is sized so that K steps of the (untuned) oracle end within ~2.5 minutes
-    # (0.46 s per 256x256x16 crop measured on the build container, cost ~ pixels)
-    per_step = 150.0 / max(1, args.steps + min(args.warmup, 3))
-    crop = int(256.0 * (per_step / 0.5) ** 0.5) // 32 * 32
-    crop = max(64, min(512, crop, args.cpu_crop if args.cpu_crop != 256 else 512))
+    # Every step is one FULL frame of the workload when K + W of them end within ~3.5 minutes (6.5 s per 1024x1024x16
+    # frame measured on the build container, cost ~ voxels); otherwise a centred crop sized to that bound.
+    from paper_2103_15418_b200 import synth
+    D = CONFIG_D(args.config)
+    B = synth.default_params(args.config)["B"]
+    n_steps = max(1, args.steps + min(args.warmup, 3))
+    t_full = 6.5 * (B * D * D) / (16.0 * 1024 * 1024)
+    if args.cpu_crop > 0:
+        crop = min(D, args.cpu_crop)
+    elif n_steps * t_full <= 210.0:
+        crop = D
+    else:
+        crop = max(64, min(D, int(D * (210.0 / (n_steps * t_full)) ** 0.5) // 32 * 32))
     step, frac, name, p = oracle_step_factory(args.config, args.bg, args.n_iter, crop)
     for _ in range(min(args.warmup, 3)):
         step()
@@ -371,13 +421,14 @@ def run_reference(args):
         step()
     dt = time.perf_counter() - t0
     v = args.steps * frac / dt
-    sample = ("each step = whole chain on a centred %dx%d crop of %s (all %d bands) with the float64 CPU oracle, "
-              "1 thread; value scaled by crop/frame voxels" % (p["Dy"], p["Dx"], name, p["B"]))
+    what = "a full %dx%d frame" % (D, D) if crop == D else "a centred %dx%d crop" % (crop, crop)
+    sample = ("each step = whole chain on %s of %s (all %d bands) with the float64 CPU oracle, 1 thread%s"
+              % (what, name, p["B"], "" if crop == D else "; value scaled by crop/frame voxels"))
     return {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": name, "cube": [p["B"], CONFIG_D(args.config), CONFIG_D(args.config)], "bg_kernel": args.bg,
-                       "n_iter": args.n_iter},
+            "config": {"workload": name, "cube": [p["B"], D, D], "bg_kernel": args.bg, "n_iter": args.n_iter,
+                       "sample_is_full_frame": crop == D},
             "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
 
@@ -407,10 +458,13 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
-    ap.add_argument("--cpu-crop", type=int, default=256)
-    ap.add_argument("--traffic", type=float, default=68.68e6,
-                    help="dram read+write bytes per launch of the dominant kernel from ncu --set full (profiles/r1_c_fused_v6.md)")
+    ap.add_argument("--cpu-crop", dest="cpu_crop", type=int, default=0, help="0 = full frames; else the oracle runs on a centred crop")
+    ap.add_argument("--repeats", type=int, default=0,
+                    help="timed blocks (each exactly --steps steps); 0 = automatic: 5 when a block is shorter than 100 ms, else 1")
     args = ap.parse_args()
+    args.repeats_auto = args.repeats <= 0
+    if args.repeats_auto:
+        args.repeats = 5
     if args.warmup < 3:
         args.warmup = 3
     out = run_reference(args) if args.impl == "reference" else run_ours(args)

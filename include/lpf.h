@@ -238,6 +238,10 @@ int lpf_get_plan(lpf_ctx* ctx, int64_t* h_out);
  * Used by bench.py for the roofline of the dominant kernel; off by default (no events recorded). */
 int lpf_profile_begin(lpf_ctx* ctx);
 int lpf_profile_end(lpf_ctx* ctx, int32_t* h_count, float* h_ms, int32_t n);
+/* The raw records of the profile in launch order, instead of the per-kernel sums: kernel id, start and end in
+ * milliseconds after the first record's start (a timeline; with several lanes in flight the records overlap).
+ * Ends the profile like lpf_profile_end.  Returns the number of records written (<= n_max), or a negative status. */
+int lpf_profile_timeline(lpf_ctx* ctx, int32_t* h_kid, float* h_t0_ms, float* h_t1_ms, int32_t n_max);
 int lpf_profile_kernel_count(void);
 const char* lpf_profile_kernel_name(int kid);
 

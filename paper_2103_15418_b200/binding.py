@@ -58,7 +58,7 @@ EXPORTS = [
     "lpf_measure_flux", "lpf_append_dynspec", "lpf_get_dynspec", "lpf_process_frame", "lpf_get_frame_view",
     "lpf_process_frame_host", "lpf_process_frame_host_begin", "lpf_process_frame_host_end", "lpf_get_counters", "lpf_memcpy_d2h", "lpf_strerror", "lpf_last_cuda_error",
     "lpf_export_dynspec", "lpf_simulate_pulses",
-    "lpf_version", "lpf_get_plan", "lpf_profile_begin", "lpf_profile_end", "lpf_profile_kernel_count", "lpf_profile_kernel_name",
+    "lpf_version", "lpf_get_plan", "lpf_profile_begin", "lpf_profile_end", "lpf_profile_timeline", "lpf_profile_kernel_count", "lpf_profile_kernel_name",
 ]
 
 
@@ -101,6 +101,7 @@ def load_library(path: Optional[str] = None):
     lib.lpf_get_plan.argtypes = [vp, C.POINTER(i64)]
     lib.lpf_profile_begin.argtypes = [vp]
     lib.lpf_profile_end.argtypes = [vp, vp, vp, i32]
+    lib.lpf_profile_timeline.argtypes = [vp, vp, vp, vp, i32]
     lib.lpf_profile_kernel_name.argtypes = [C.c_int]
     lib.lpf_profile_kernel_name.restype = C.c_char_p
     for n in EXPORTS:
@@ -294,6 +295,14 @@ class LPF:
         cnt = (C.c_int32 * n)(); ms = (C.c_float * n)()
         _check(self.lib, self.lib.lpf_profile_end(self.h, cnt, ms, n), "lpf_profile_end")
         return {self.lib.lpf_profile_kernel_name(i).decode(): (int(cnt[i]), float(ms[i])) for i in range(n) if cnt[i]}
+
+    def profile_timeline(self, n_max: int = 65536):
+        """[(kernel name, start ms, end ms)] of every kernel launched since profile_begin, in launch order."""
+        kid = (C.c_int32 * n_max)(); t0 = (C.c_float * n_max)(); t1 = (C.c_float * n_max)()
+        n = self.lib.lpf_profile_timeline(self.h, kid, t0, t1, n_max)
+        if n < 0:
+            _check(self.lib, n, "lpf_profile_timeline")
+        return [(self.lib.lpf_profile_kernel_name(kid[i]).decode(), float(t0[i]), float(t1[i])) for i in range(n)]
 
     def counters(self) -> dict:
         h = (C.c_int64 * 4)()

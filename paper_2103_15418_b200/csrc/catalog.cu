@@ -113,13 +113,15 @@ k_dedupe_sort(const lpf_det* __restrict__ dets, const int32_t* __restrict__ ndet
 }
 
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(CAT_THREADS)
-k_assoc_match(const int32_t* __restrict__ upos, const int32_t* __restrict__ nu, const uint8_t* __restrict__ band_ok,
-              int B, const int32_t* __restrict__ slotmap, const int32_t* __restrict__ cpix, int Dy, int Dx, int r,
-              long long t, long long* __restrict__ matched_t, int32_t* __restrict__ cand_idx) {
+// nearest active candidate of every unique detection (thread i0, i0 + stride, ...)
+__device__ __forceinline__ void
+assoc_match_body(const int32_t* __restrict__ upos, const int32_t* __restrict__ nu, const uint8_t* __restrict__ band_ok,
+                 int B, const int32_t* __restrict__ slotmap, const int32_t* __restrict__ cpix, int Dy, int Dx, int r,
+                 long long t, long long* __restrict__ matched_t, int32_t* __restrict__ cand_idx, int i0, int stride) {
+  (void)cpix;
   const int n = *nu;
   const bool frame_ok = band_ok[B] != 0;
-  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+  for (int i = i0; i < n; i += stride) {
     int best = -1;
     if (frame_ok) {
       const int pix = upos[i];
@@ -206,8 +208,7 @@ __device__ __forceinline__ int warp_totals_excl(int my_total, int* s_tot /*[33]*
   return pre;
 }
 
-__global__ void __launch_bounds__(1024)
-k_assoc_update(const AssocArgs a) {
+__device__ __forceinline__ void assoc_update_body(const AssocArgs& a) {
   __shared__ int s_warp[33];
   const int T = blockDim.x;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, nw = T >> 5;
@@ -290,6 +291,15 @@ k_assoc_update(const AssocArgs a) {
     ao += __popc(m);
   }
   if (tid == 0) { *a.npos = n_act; a.counters[2] = n_act; }
+}
+
+// S10 in one block: match (every thread takes detections), then the table update.  One launch, no second
+// trip through the block scheduler on the part of a frame that the next frame has to wait for.
+__global__ void __launch_bounds__(1024)
+k_assoc(const AssocArgs a, int Dy, int Dx, int r, long long* matched_t) {
+  assoc_match_body(a.upos, a.nu, a.band_ok, a.B, a.slotmap, a.cpix, Dy, Dx, r, a.t, matched_t, a.cand_idx, threadIdx.x, blockDim.x);
+  __syncthreads();       // matched_t and cand_idx (global) are this block's own writes
+  assoc_update_body(a);
 }
 
 struct AddArgs {
@@ -484,15 +494,13 @@ int lpf_launch_associate(lpf_ctx* c, const int32_t* d_upos, const int32_t* d_nu,
                          long long t, int32_t* d_cand_idx, int32_t* d_act_slots, int32_t* d_act_pix,
                          int32_t* d_npos, cudaStream_t st) {
   const lpf_params& p = c->p;
-  LPF_KLAUNCH(c, KID_ASSOC_MATCH, st, k_assoc_match<<<CAT_BLOCKS, CAT_THREADS, 0, st>>>(
-      d_upos, d_nu, d_band_ok, p.B, c->slotmap, c->cpix, p.Dy, p.Dx, p.r_assoc, t, c->matched_t, d_cand_idx));
   AssocArgs a{};
   a.active = c->active; a.forced = c->forced; a.cpix = c->cpix; a.miss = c->miss; a.born = c->born;
   a.matched_t = c->matched_t; a.slotmap = c->slotmap; a.free_list = c->free_list;
   a.n_cand_max = p.n_cand_max; a.n_forget = p.n_forget;
   a.upos = d_upos; a.nu = d_nu; a.band_ok = d_band_ok; a.B = p.B; a.t = t;
   a.cand_idx = d_cand_idx; a.act_slots = d_act_slots; a.act_pix = d_act_pix; a.npos = d_npos; a.counters = c->counters;
-  LPF_KLAUNCH(c, KID_ASSOC_UPDATE, st, k_assoc_update<<<1, 1024, 0, st>>>(a));
+  LPF_KLAUNCH(c, KID_ASSOC_UPDATE, st, k_assoc<<<1, 1024, 0, st>>>(a, p.Dy, p.Dx, p.r_assoc, c->matched_t));
   return LPF_OK;
 }
 

@@ -884,7 +884,11 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
   // n_lanes frames in flight the kernels of different lanes share the SMs, so each gets its share of them
   // (fewer, longer segments: less warm-up per output row).
   const int n_planes = c->n_planes;
-  const int sm_share = std::max(1, c->n_sm / std::max(1, std::min(p.n_lanes, 4)));   // (more lanes in flight only deepen the queue)
+  int share_div = std::max(1, std::min(p.n_lanes, 4));   // (more lanes in flight only deepen the queue)
+#ifdef LPF_EXP_SHARE_ENV
+  if (const char* e = getenv("LPF_EXP_SHARE")) share_div = std::max(1, atoi(e));
+#endif
+  const int sm_share = std::max(1, c->n_sm / share_div);
   const double warm = 58.0;   // warm-up / drain rows of a segment
   int best_seg = 1; double best_cost = 1e30;
   const int max_rows_strip = (int)(rows_all / n_strips);

@@ -131,6 +131,8 @@ int alloc_lane(lpf_ctx* c, LpfLane& L) {
   LPF_CUDA(cudaMemset(L.nu, 0, sizeof(int32_t)));
   LPF_CUDA(cudaMemset(L.npos, 0, sizeof(int32_t)));
   LPF_CUDA(cudaMallocHost((void**)&L.h_counts, 4 * sizeof(int32_t)));
+  LPF_CUDA(cudaEventCreateWithFlags(&L.ev_pre, cudaEventDisableTiming));
+  LPF_CUDA(cudaEventCreateWithFlags(&L.ev_post, cudaEventDisableTiming));
   return LPF_OK;
 }
 
@@ -140,6 +142,8 @@ void free_lane(LpfLane& L) {
                   L.cand_idx, L.act_slots, L.act_pix, L.npos, L.flux, L.cube, L.zeta_cnt, L.hits, L.hit_cnt, L.big_thr, L.dirty_b, L.qc_mom};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (L.h_counts) cudaFreeHost(L.h_counts);
+  if (L.ev_pre) cudaEventDestroy(L.ev_pre);
+  if (L.ev_post) cudaEventDestroy(L.ev_post);
   L = LpfLane();
 }
 
@@ -240,7 +244,12 @@ int lpf_create(lpf_ctx** out, const lpf_params* p, const uint8_t* d_valid_mask) 
   CUDAC(cudaMemset(c->meta_ok, 0, (size_t)p->T_ring * 8));
   CUDAC(cudaMemset(c->counters, 0, 8 * 4));
   TRYC(lpf_launch_fill_nan(c, c->ring, (int64_t)(nc * p->T_ring * p->B), 0));
-  CUDAC(cudaEventCreateWithFlags(&c->chain_ev, cudaEventDisableTiming));
+  CUDAC(cudaEventCreateWithFlags(&c->ring_ev, cudaEventDisableTiming));
+  {
+    int lo = 0, hi = 0;
+    CUDAC(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+    CUDAC(cudaStreamCreateWithPriority(&c->chain_st, cudaStreamNonBlocking, hi));
+  }
   c->lanes.resize(p->n_lanes);
   for (auto& L : c->lanes) TRYC(alloc_lane(c, L));
   CUDAC(cudaDeviceSynchronize());
@@ -259,7 +268,8 @@ int lpf_destroy(lpf_ctx* c) {
                   c->slotmap, c->free_list, c->ring, c->meta_t, c->meta_ok, c->counters, c->cube_cache, c->cache_ok,
                   c->cache_t, c->rq_m, c->rq_v, c->rq_state};
   for (void* q : ptrs) if (q) cudaFree(q);
-  if (c->chain_ev) cudaEventDestroy(c->chain_ev);
+  if (c->ring_ev) cudaEventDestroy(c->ring_ev);
+  if (c->chain_st) cudaStreamDestroy(c->chain_st);
   if (c->rq_ev) cudaEventDestroy(c->rq_ev);
   lpf_fused_plan_free(c->fused);
   for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
@@ -296,6 +306,7 @@ int lpf_add_candidates(lpf_ctx* c, const int32_t* d_pix, int32_t n, int32_t* d_s
   if (!c || n < 0 || (n > 0 && !d_pix)) return LPF_E_ARG;
   if (n == 0) return LPF_OK;
   if (n > c->p.n_cand_max) return LPF_E_STATE;
+  LPF_CUDA(cudaDeviceSynchronize());      // the table is shared with every frame in flight, on every stream
   return lpf_launch_add_candidates(c, d_pix, n, d_slots_out, (cudaStream_t)stream);
 }
 
@@ -339,14 +350,23 @@ int lpf_process_frame(lpf_ctx* c, int lane, const float* d_cube, int64_t t, void
   if (c->p.n_back > 0) TRY(lpf_launch_cache_store(c, d_cube, L.band_ok, (long long)t, st));   // O11: the frame joins the cache
   TRY(lpf_launch_detect(c, L, d_cube, L.band_ok, L.dets, L.ndets, true, st));
   TRY(lpf_launch_dedupe(c, L, L.dets, L.ndets, L.upos, L.uplane, L.usnr, L.nu, st));
-  // the candidate table and the rings are shared by all lanes: order the chain across streams
-  if (c->chain_valid) LPF_CUDA(cudaStreamWaitEvent(st, c->chain_ev, 0));
-  TRY(lpf_launch_associate(c, L.upos, L.nu, L.band_ok, (long long)t, L.cand_idx, L.act_slots, L.act_pix, L.npos, st));
+  // The candidate table and the rings are shared by all lanes.  The association steps of all frames run, in frame
+  // order, on ONE stream of the context (highest priority: a single block per frame that the next frame waits for
+  // must not queue behind the other lanes' grids); the lane's stream hands over after its duplicate filter and
+  // takes over again for the flux measurement.  The ring steps are ordered across lanes by an event (a slot born
+  // at t is blanked by the append of frame t, which must not follow the append of frame t + 1); they do not hold
+  // up the association of frame t + 1.
+  LPF_CUDA(cudaEventRecord(L.ev_pre, st));
+  LPF_CUDA(cudaStreamWaitEvent(c->chain_st, L.ev_pre, 0));
+  TRY(lpf_launch_associate(c, L.upos, L.nu, L.band_ok, (long long)t, L.cand_idx, L.act_slots, L.act_pix, L.npos, c->chain_st));
+  LPF_CUDA(cudaEventRecord(L.ev_post, c->chain_st));
+  LPF_CUDA(cudaStreamWaitEvent(st, L.ev_post, 0));
   TRY(lpf_launch_measure_flux(c, d_cube, L.band_ok, L.act_pix, L.npos, L.flux, st));
+  if (c->ring_valid) LPF_CUDA(cudaStreamWaitEvent(st, c->ring_ev, 0));
   TRY(lpf_launch_append(c, L.act_slots, L.npos, L.flux, L.band_ok, (long long)t, st));
   if (c->p.n_back > 0) TRY(lpf_launch_backfill(c, L.act_slots, L.act_pix, L.npos, d_cube, L.band_ok, (long long)t, st));   // O11
-  LPF_CUDA(cudaEventRecord(c->chain_ev, st));
-  c->chain_valid = true;
+  LPF_CUDA(cudaEventRecord(c->ring_ev, st));
+  c->ring_valid = true;
   return LPF_OK;
 }
 
@@ -444,6 +464,23 @@ int lpf_profile_end(lpf_ctx* c, int32_t* h_count, float* h_ms, int32_t n) {
   c->prof_recs.clear();
   c->prof_pool_used = 0;
   return LPF_OK;
+}
+
+int lpf_profile_timeline(lpf_ctx* c, int32_t* h_kid, float* h_t0_ms, float* h_t1_ms, int32_t n_max) {
+  if (!c || !h_kid || !h_t0_ms || !h_t1_ms || n_max < 0) return LPF_E_ARG;
+  c->prof_on = false;
+  LPF_CUDA(cudaDeviceSynchronize());
+  int n = 0;
+  for (const auto& r : c->prof_recs) {
+    if (n >= n_max) break;
+    float a = 0.f, b = 0.f;
+    LPF_CUDA(cudaEventElapsedTime(&a, c->prof_recs.front().e0, r.e0));
+    LPF_CUDA(cudaEventElapsedTime(&b, c->prof_recs.front().e0, r.e1));
+    h_kid[n] = r.kid; h_t0_ms[n] = a; h_t1_ms[n] = b; ++n;
+  }
+  c->prof_recs.clear();
+  c->prof_pool_used = 0;
+  return n;
 }
 
 int lpf_get_plan(lpf_ctx* c, int64_t* h_out) {

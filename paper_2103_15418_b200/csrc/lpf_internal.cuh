@@ -55,6 +55,7 @@ struct LpfLane {
   int32_t* hit_cnt = nullptr;  // [segments]
   float* big_thr = nullptr;    // [B + 1] 'far above the noise' level of every plane (64 x rms)
   int32_t* h_counts = nullptr; // pinned [4]
+  cudaEvent_t ev_pre = nullptr, ev_post = nullptr;   // hand-over to / from the context's association stream
 };
 
 struct LpfFusedPlan;  // detect_fused.cu
@@ -95,8 +96,9 @@ struct lpf_ctx {
   float* cube_cache = nullptr;      // [n_back + n_lanes][B][N]
   uint8_t* cache_ok = nullptr;      // [n_back + n_lanes][B + 1]
   long long* cache_t = nullptr;     // [n_back + n_lanes], -1 = empty
-  cudaEvent_t chain_ev = nullptr;
-  bool chain_valid = false;
+  cudaStream_t chain_st = nullptr;  // the association steps of all frames, in frame order (highest priority)
+  cudaEvent_t ring_ev = nullptr;    // after the ring steps (append, backward fill) of the latest frame
+  bool ring_valid = false;
   int64_t launches = 0;
   std::vector<LpfLane> lanes;
   // per-kernel profile

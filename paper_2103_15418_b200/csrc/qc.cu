@@ -417,7 +417,102 @@ __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
 }
 __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+// keep a value in its register (the compiler would otherwise rebuild it from its inputs at every use)
+__device__ __forceinline__ void pin(float& v) { asm volatile("" : "+f"(v)); }
+__device__ __forceinline__ void pin(unsigned& v) { asm volatile("" : "+r"(v)); }
+__device__ __forceinline__ void pin(const char*& v) { asm volatile("" : "+l"(v)); }
 constexpr size_t QS_SMEM = (size_t)QS_BG * QS_THREADS * sizeof(float4);   // 64 KB
+
+// one group of <= QS_BG bands over the block's pixel groups [q0, q1); FULL: all QS_BG bands exist
+template <bool FULL>
+__device__ __forceinline__ void qs_moments_group(const QsArgs& a, int g0, long long q0, long long q1, const float* s_piv,
+                                                 double (*s_red)[QS_BG][2], double* s_n, float4* qs_slots) {
+  const int B = a.B, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long n4 = a.N >> 2;
+  const long long sb = n4 * (long long)sizeof(float4);           // bytes from a band to the next at the same pixel group
+  const bool want_sum = a.sum_out != nullptr;
+  const uint32_t slot0 = (uint32_t)__cvta_generic_to_shared(qs_slots + threadIdx.x);
+  constexpr uint32_t SLOT = QS_THREADS * sizeof(float4);
+  float2 f1[QS_BG], f2[QS_BG];
+#pragma unroll
+  for (int b = 0; b < QS_BG; ++b) { f1[b] = make_float2(0.f, 0.f); f2[b] = f1[b]; }
+  unsigned dirt = 0u;            // one bit per band of the group
+  int nval = 0;
+  long long q = q0 + threadIdx.x;
+  bool has = q < q1;
+  {
+    const char* pb = reinterpret_cast<const char*>(a.cube) + ((long long)g0 * n4 + q) * (long long)sizeof(float4);
+#pragma unroll
+    for (int b = 0; b < QS_BG; ++b) {
+      if (has && (FULL || g0 + b < B)) cp_async16(slot0 + b * SLOT, pb);
+      cp_commit();
+      pb += sb; pin(pb);
+    }
+  }
+  unsigned wm = has ? __ldg(reinterpret_cast<const unsigned*>(a.W) + q) : 0u;
+  while (has) {
+    const long long qn = q + QS_THREADS;
+    const bool hasn = qn < q1;
+    const unsigned wmn = hasn ? __ldg(reinterpret_cast<const unsigned*>(a.W) + qn) : 0u;
+    nval += __popc(wm & 0x01010101u);
+    const bool edge = (wm & 0x01010101u) != 0x01010101u;          // some invalid pixel in the group
+    // per pixel: all ones where valid (keeps the value), 0x7fffffff where invalid (|x| != 0 there = not clean)
+    const unsigned k0 = (wm & 0x000000ffu) ? 0xffffffffu : 0u, k1 = (wm & 0x0000ff00u) ? 0xffffffffu : 0u,
+                   k2 = (wm & 0x00ff0000u) ? 0xffffffffu : 0u, k3 = (wm & 0xff000000u) ? 0xffffffffu : 0u;
+    unsigned kk0 = k0, kk1 = k1, kk2 = k2, kk3 = k3;
+    pin(kk0); pin(kk1); pin(kk2); pin(kk3);
+    float2 s01 = make_float2(0.f, 0.f), s23 = s01;
+    if (g0 > 0 && want_sum) { const float4 sp = reinterpret_cast<const float4*>(a.sum_out)[q]; s01 = make_float2(sp.x, sp.y); s23 = make_float2(sp.z, sp.w); }
+    const char* pb = reinterpret_cast<const char*>(a.cube) + ((long long)g0 * n4 + qn) * (long long)sizeof(float4);
+#pragma unroll
+    for (int b = 0; b < QS_BG; ++b) {
+      cp_wait<QS_BG - 1>();
+      const bool live = FULL || g0 + b < B;
+      const float4 x = live ? qs_slots[b * QS_THREADS + threadIdx.x] : make_float4(0.f, 0.f, 0.f, 0.f);
+      const float2 x01 = make_float2(x.x, x.y), x23 = make_float2(x.z, x.w);
+      const float np = -s_piv[live ? g0 + b : 0];
+      float2 t01 = q_add2(x01, make_float2(np, np)), t23 = q_add2(x23, make_float2(np, np));
+      if (edge) {     // invalid pixels count as 0 whatever they hold (NaN and Inf included)
+        t01.x = __uint_as_float(__float_as_uint(t01.x) & kk0); t01.y = __uint_as_float(__float_as_uint(t01.y) & kk1);
+        t23.x = __uint_as_float(__float_as_uint(t23.x) & kk2); t23.y = __uint_as_float(__float_as_uint(t23.y) & kk3);
+        const unsigned dz = ((__float_as_uint(x.x) & ~kk0) | (__float_as_uint(x.y) & ~kk1) | (__float_as_uint(x.z) & ~kk2) |
+                             (__float_as_uint(x.w) & ~kk3)) & 0x7fffffffu;
+        if (dz) dirt |= 1u << b;
+      }
+      f1[b] = q_add2(f1[b], q_add2(t01, t23));
+      f2[b] = q_fma2(t01, t01, q_fma2(t23, t23, f2[b]));
+      s01 = q_add2(s01, x01); s23 = q_add2(s23, x23);
+      if (hasn && live) cp_async16(slot0 + b * SLOT, pb);
+      cp_commit();
+      pb += sb; pin(pb);
+    }
+    if (want_sum) reinterpret_cast<float4*>(a.sum_out)[q] = make_float4(s01.x, s01.y, s23.x, s23.y);
+    q = qn; has = hasn; wm = wmn;
+  }
+  cp_wait<0>();
+  // block reduction: fp32 across the warp (a few hundred values), float64 from there on
+#pragma unroll
+  for (int b = 0; b < QS_BG; ++b) {
+    float v1 = f1[b].x + f1[b].y, v2 = f2[b].x + f2[b].y;
+    v1 = lpf_warp_sum(v1); v2 = lpf_warp_sum(v2);
+    if (lane == 0) { s_red[warp][b][0] = (double)v1; s_red[warp][b][1] = (double)v2; }
+  }
+  const unsigned any_dirt = __reduce_or_sync(0xffffffffu, dirt);
+  if (any_dirt && lane == 0)
+    for (int b = 0; b < QS_BG; ++b)
+      if (((any_dirt >> b) & 1u) && g0 + b < B) a.dirty_b[g0 + b] = a.seq;
+  nval = lpf_warp_sum(nval);
+  if (lane == 0) s_n[warp] = (double)nval;
+  __syncthreads();
+  if (threadIdx.x < QS_BG && g0 + threadIdx.x < B) {
+    double t1 = 0, t2 = 0, tn = 0;
+#pragma unroll
+    for (int w = 0; w < QS_WARPS; ++w) { t1 += s_red[w][threadIdx.x][0]; t2 += s_red[w][threadIdx.x][1]; tn += s_n[w]; }
+    double* o = a.part1 + ((long long)(g0 + threadIdx.x) * gridDim.x + blockIdx.x) * 3;
+    o[0] = tn; o[1] = t1; o[2] = t2;
+  }
+  __syncthreads();
+}
 
 __global__ void __launch_bounds__(QS_THREADS, LPF_QS_BLOCKS)
 k_qc_moments(const QsArgs a) {
@@ -425,87 +520,15 @@ k_qc_moments(const QsArgs a) {
   __shared__ float s_piv[LPF_MAX_BANDS];
   __shared__ double s_red[QS_WARPS][QS_BG][2];
   __shared__ double s_n[QS_WARPS];
-  const int B = a.B, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int B = a.B;
   const long long N = a.N, n4 = N >> 2;
   for (int b = threadIdx.x; b < B; b += QS_THREADS) s_piv[b] = a.cube[(long long)b * N + a.first_valid];
   __syncthreads();
   const long long per = (n4 + gridDim.x - 1) / gridDim.x;
   const long long q0 = (long long)blockIdx.x * per, q1 = q0 + per < n4 ? q0 + per : n4;
-  const float4* X4 = reinterpret_cast<const float4*>(a.cube);
-  const bool want_sum = a.sum_out != nullptr;
-  const uint32_t slot0 = (uint32_t)__cvta_generic_to_shared(qs_slots + threadIdx.x);
-
   for (int g0 = 0; g0 < B; g0 += QS_BG) {
-    float2 f1[QS_BG], f2[QS_BG];
-#pragma unroll
-    for (int b = 0; b < QS_BG; ++b) { f1[b] = make_float2(0.f, 0.f); f2[b] = f1[b]; }
-    unsigned dirt = 0u;            // one bit per band of the group
-    int nval = 0;
-    long long q = q0 + threadIdx.x;
-    bool has = q < q1;
-#pragma unroll
-    for (int b = 0; b < QS_BG; ++b) {
-      if (has && g0 + b < B) cp_async16(slot0 + (uint32_t)(b * QS_THREADS * sizeof(float4)), X4 + (long long)(g0 + b) * n4 + q);
-      cp_commit();
-    }
-    unsigned wm = has ? __ldg(reinterpret_cast<const unsigned*>(a.W) + q) : 0u;
-    while (has) {
-      const long long qn = q + QS_THREADS;
-      const bool hasn = qn < q1;
-      const unsigned wmn = hasn ? __ldg(reinterpret_cast<const unsigned*>(a.W) + qn) : 0u;
-      nval += __popc(wm & 0x01010101u);
-      const unsigned inv = ~(wm * 0xffu);      // 0xff in the bytes of the invalid pixels (W is 0 / 1); 0: none
-      float2 s01 = make_float2(0.f, 0.f), s23 = s01;
-      if (g0 > 0 && want_sum) { const float4 sp = reinterpret_cast<const float4*>(a.sum_out)[q]; s01 = make_float2(sp.x, sp.y); s23 = make_float2(sp.z, sp.w); }
-#pragma unroll
-      for (int b = 0; b < QS_BG; ++b) {
-        cp_wait<QS_BG - 1>();
-        const bool live = g0 + b < B;
-        const float4 x = live ? qs_slots[b * QS_THREADS + threadIdx.x] : make_float4(0.f, 0.f, 0.f, 0.f);
-        const float2 x01 = make_float2(x.x, x.y), x23 = make_float2(x.z, x.w);
-        const float np = -s_piv[live ? g0 + b : 0];
-        float2 t01 = q_add2(x01, make_float2(np, np)), t23 = q_add2(x23, make_float2(np, np));
-        if (inv) {     // a group with invalid pixels: they count as 0 whatever they hold (NaN and Inf included)
-          if (inv & 0x000000ffu) t01.x = 0.f;
-          if (inv & 0x0000ff00u) t01.y = 0.f;
-          if (inv & 0x00ff0000u) t23.x = 0.f;
-          if (inv & 0xff000000u) t23.y = 0.f;
-          const unsigned nz = ((__float_as_uint(x.x) << 1) != 0u && (inv & 0x000000ffu)) |
-                              ((__float_as_uint(x.y) << 1) != 0u && (inv & 0x0000ff00u)) |
-                              ((__float_as_uint(x.z) << 1) != 0u && (inv & 0x00ff0000u)) |
-                              ((__float_as_uint(x.w) << 1) != 0u && (inv & 0xff000000u));
-          dirt |= nz << b;
-        }
-        f1[b] = q_add2(f1[b], q_add2(t01, t23));
-        f2[b] = q_fma2(t01, t01, q_fma2(t23, t23, f2[b]));
-        s01 = q_add2(s01, x01); s23 = q_add2(s23, x23);
-        if (hasn && live) cp_async16(slot0 + (uint32_t)(b * QS_THREADS * sizeof(float4)), X4 + (long long)(g0 + b) * n4 + qn);
-        cp_commit();
-      }
-      if (want_sum) reinterpret_cast<float4*>(a.sum_out)[q] = make_float4(s01.x, s01.y, s23.x, s23.y);
-      q = qn; has = hasn; wm = wmn;
-    }
-    cp_wait<0>();
-    // block reduction: fp32 across the warp (a few hundred values), float64 from there on
-#pragma unroll
-    for (int b = 0; b < QS_BG; ++b) {
-      float v1 = f1[b].x + f1[b].y, v2 = f2[b].x + f2[b].y;
-      v1 = lpf_warp_sum(v1); v2 = lpf_warp_sum(v2);
-      if (lane == 0) { s_red[warp][b][0] = (double)v1; s_red[warp][b][1] = (double)v2; }
-      const unsigned any_dirt = __ballot_sync(0xffffffffu, (dirt >> b) & 1u);
-      if (any_dirt && lane == 0 && g0 + b < B) a.dirty_b[g0 + b] = a.seq;
-    }
-    nval = lpf_warp_sum(nval);
-    if (lane == 0) s_n[warp] = (double)nval;
-    __syncthreads();
-    if (threadIdx.x < QS_BG && g0 + threadIdx.x < B) {
-      double t1 = 0, t2 = 0, tn = 0;
-#pragma unroll
-      for (int w = 0; w < QS_WARPS; ++w) { t1 += s_red[w][threadIdx.x][0]; t2 += s_red[w][threadIdx.x][1]; tn += s_n[w]; }
-      double* o = a.part1 + ((long long)(g0 + threadIdx.x) * gridDim.x + blockIdx.x) * 3;
-      o[0] = tn; o[1] = t1; o[2] = t2;
-    }
-    __syncthreads();
+    if (g0 + QS_BG <= B) qs_moments_group<true>(a, g0, q0, q1, s_piv, s_red, s_n, qs_slots);
+    else qs_moments_group<false>(a, g0, q0, q1, s_piv, s_red, s_n, qs_slots);
   }
 }
 
@@ -559,6 +582,82 @@ struct QkArgs {
   float* sum_out;          // [N]: rebuilt from the accepted bands when a band was rejected; or null
 };
 
+template <bool FULL, bool RESUM>
+__device__ __forceinline__ void qs_clip_group(const QkArgs& a, int g0, long long q0, long long q1, const float* s_c,
+                                              const float* s_w, const uint8_t* s_ok, double (*s_red)[QS_BG][3], float4* qs_slots) {
+  const int B = a.B, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long n4 = a.N >> 2;
+  const long long sb = n4 * (long long)sizeof(float4);
+  const uint32_t slot0 = (uint32_t)__cvta_generic_to_shared(qs_slots + threadIdx.x);
+  constexpr uint32_t SLOT = QS_THREADS * sizeof(float4);
+  float fn[QS_BG], f1[QS_BG], f2[QS_BG];
+#pragma unroll
+  for (int b = 0; b < QS_BG; ++b) { fn[b] = 0.f; f1[b] = 0.f; f2[b] = 0.f; }
+  long long q = q0 + threadIdx.x;
+  bool has = q < q1;
+  {
+    const char* pb = reinterpret_cast<const char*>(a.cube) + ((long long)g0 * n4 + q) * (long long)sizeof(float4);
+#pragma unroll
+    for (int b = 0; b < QS_BG; ++b) {
+      if (has && (FULL || g0 + b < B)) cp_async16(slot0 + b * SLOT, pb);
+      cp_commit();
+      pb += sb; pin(pb);
+    }
+  }
+  unsigned wm = has ? __ldg(reinterpret_cast<const unsigned*>(a.W) + q) : 0u;
+  while (has) {
+    const long long qn = q + QS_THREADS;
+    const bool hasn = qn < q1;
+    const unsigned wmn = hasn ? __ldg(reinterpret_cast<const unsigned*>(a.W) + qn) : 0u;
+    // an invalid pixel never passes |d| <= w: its half width is -1
+    const float m0 = (wm & 0x000000ffu) ? 0.f : -INFINITY, m1 = (wm & 0x0000ff00u) ? 0.f : -INFINITY,
+                m2 = (wm & 0x00ff0000u) ? 0.f : -INFINITY, m3 = (wm & 0xff000000u) ? 0.f : -INFINITY;
+    float mm0 = m0, mm1 = m1, mm2 = m2, mm3 = m3;
+    pin(mm0); pin(mm1); pin(mm2); pin(mm3);
+    float4 sp = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (RESUM && g0 > 0) sp = reinterpret_cast<const float4*>(a.sum_out)[q];
+    const char* pb = reinterpret_cast<const char*>(a.cube) + ((long long)g0 * n4 + qn) * (long long)sizeof(float4);
+#pragma unroll
+    for (int b = 0; b < QS_BG; ++b) {
+      cp_wait<QS_BG - 1>();
+      const bool live = FULL || g0 + b < B;
+      const int bb = live ? g0 + b : 0;
+      const float4 x = live ? qs_slots[b * QS_THREADS + threadIdx.x] : make_float4(0.f, 0.f, 0.f, 0.f);
+      const float c = s_c[bb], w = live ? s_w[bb] : -1.f;
+      const float xv[4] = {x.x, x.y, x.z, x.w};
+      const float mv[4] = {mm0, mm1, mm2, mm3};
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const float d = xv[j] - c;
+        const bool take = fabsf(d) <= w + mv[j];
+        const float dm = take ? d : 0.f;
+        fn[b] += take ? 1.f : 0.f; f1[b] += dm; f2[b] = fmaf(dm, dm, f2[b]);
+      }
+      if (RESUM && live && s_ok[bb]) { sp.x += x.x; sp.y += x.y; sp.z += x.z; sp.w += x.w; }
+      if (hasn && live) cp_async16(slot0 + b * SLOT, pb);
+      cp_commit();
+      pb += sb; pin(pb);
+    }
+    if (RESUM) reinterpret_cast<float4*>(a.sum_out)[q] = sp;
+    q = qn; has = hasn; wm = wmn;
+  }
+  cp_wait<0>();
+#pragma unroll
+  for (int b = 0; b < QS_BG; ++b) {
+    const float vn = lpf_warp_sum(fn[b]), v1 = lpf_warp_sum(f1[b]), v2 = lpf_warp_sum(f2[b]);
+    if (lane == 0) { s_red[warp][b][0] = (double)vn; s_red[warp][b][1] = (double)v1; s_red[warp][b][2] = (double)v2; }
+  }
+  __syncthreads();
+  if (threadIdx.x < QS_BG && g0 + threadIdx.x < B) {
+    double t0 = 0, t1 = 0, t2 = 0;
+#pragma unroll
+    for (int w = 0; w < QS_WARPS; ++w) { t0 += s_red[w][threadIdx.x][0]; t1 += s_red[w][threadIdx.x][1]; t2 += s_red[w][threadIdx.x][2]; }
+    double* o = a.part2 + ((long long)blockIdx.x * B + g0 + threadIdx.x) * 3;
+    o[0] = t0; o[1] = t1; o[2] = t2;
+  }
+  __syncthreads();
+}
+
 __global__ void __launch_bounds__(QS_THREADS, LPF_QS_BLOCKS)
 k_qc_clip(const QkArgs a) {
   extern __shared__ float4 qs_slots[];     // [QS_BG][QS_THREADS]
@@ -566,8 +665,8 @@ k_qc_clip(const QkArgs a) {
   __shared__ uint8_t s_ok[LPF_MAX_BANDS + 1];
   __shared__ double s_red[QS_WARPS][QS_BG][3];
   __shared__ int s_rej;
-  const int B = a.B, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const long long N = a.N, n4 = N >> 2;
+  const int B = a.B;
+  const long long n4 = a.N >> 2;
   if (threadIdx.x == 0) s_rej = 0;
   __syncthreads();
   for (int b = threadIdx.x; b <= B; b += QS_THREADS) {
@@ -578,65 +677,12 @@ k_qc_clip(const QkArgs a) {
   const bool resum = a.sum_out != nullptr && s_rej != 0 && s_ok[B] != 0;   // a rejected frame has no sum plane
   const long long per = (n4 + gridDim.x - 1) / gridDim.x;
   const long long q0 = (long long)blockIdx.x * per, q1 = q0 + per < n4 ? q0 + per : n4;
-  const float4* X4 = reinterpret_cast<const float4*>(a.cube);
-  const uint32_t slot0 = (uint32_t)__cvta_generic_to_shared(qs_slots + threadIdx.x);
-
   for (int g0 = 0; g0 < B; g0 += QS_BG) {
-    float fn[QS_BG], f1[QS_BG], f2[QS_BG];
-#pragma unroll
-    for (int b = 0; b < QS_BG; ++b) { fn[b] = 0.f; f1[b] = 0.f; f2[b] = 0.f; }
-    long long q = q0 + threadIdx.x;
-    bool has = q < q1;
-#pragma unroll
-    for (int b = 0; b < QS_BG; ++b) {
-      if (has && g0 + b < B) cp_async16(slot0 + (uint32_t)(b * QS_THREADS * sizeof(float4)), X4 + (long long)(g0 + b) * n4 + q);
-      cp_commit();
-    }
-    unsigned wm = has ? __ldg(reinterpret_cast<const unsigned*>(a.W) + q) : 0u;
-    while (has) {
-      const long long qn = q + QS_THREADS;
-      const bool hasn = qn < q1;
-      const unsigned wmn = hasn ? __ldg(reinterpret_cast<const unsigned*>(a.W) + qn) : 0u;
-      const bool vv[4] = {(wm & 0x000000ffu) != 0, (wm & 0x0000ff00u) != 0, (wm & 0x00ff0000u) != 0, (wm & 0xff000000u) != 0};
-      float4 sp = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (resum && g0 > 0) sp = reinterpret_cast<const float4*>(a.sum_out)[q];
-#pragma unroll
-      for (int b = 0; b < QS_BG; ++b) {
-        cp_wait<QS_BG - 1>();
-        const bool live = g0 + b < B;
-        const int bb = live ? g0 + b : 0;
-        const float4 x = live ? qs_slots[b * QS_THREADS + threadIdx.x] : make_float4(0.f, 0.f, 0.f, 0.f);
-        const float c = s_c[bb], w = live ? s_w[bb] : -1.f;
-        const float xv[4] = {x.x, x.y, x.z, x.w};
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const float d = xv[j] - c;
-          const bool take = vv[j] && fabsf(d) <= w;
-          const float dm = take ? d : 0.f;
-          fn[b] += take ? 1.f : 0.f; f1[b] += dm; f2[b] = fmaf(dm, dm, f2[b]);
-        }
-        if (resum && live && s_ok[bb]) { sp.x += x.x; sp.y += x.y; sp.z += x.z; sp.w += x.w; }
-        if (hasn && live) cp_async16(slot0 + (uint32_t)(b * QS_THREADS * sizeof(float4)), X4 + (long long)(g0 + b) * n4 + qn);
-        cp_commit();
-      }
-      if (resum) reinterpret_cast<float4*>(a.sum_out)[q] = sp;
-      q = qn; has = hasn; wm = wmn;
-    }
-    cp_wait<0>();
-#pragma unroll
-    for (int b = 0; b < QS_BG; ++b) {
-      const float vn = lpf_warp_sum(fn[b]), v1 = lpf_warp_sum(f1[b]), v2 = lpf_warp_sum(f2[b]);
-      if (lane == 0) { s_red[warp][b][0] = (double)vn; s_red[warp][b][1] = (double)v1; s_red[warp][b][2] = (double)v2; }
-    }
-    __syncthreads();
-    if (threadIdx.x < QS_BG && g0 + threadIdx.x < B) {
-      double t0 = 0, t1 = 0, t2 = 0;
-#pragma unroll
-      for (int w = 0; w < QS_WARPS; ++w) { t0 += s_red[w][threadIdx.x][0]; t1 += s_red[w][threadIdx.x][1]; t2 += s_red[w][threadIdx.x][2]; }
-      double* o = a.part2 + ((long long)blockIdx.x * B + g0 + threadIdx.x) * 3;
-      o[0] = t0; o[1] = t1; o[2] = t2;
-    }
-    __syncthreads();
+    const bool full = g0 + QS_BG <= B;
+    if (full && !resum) qs_clip_group<true, false>(a, g0, q0, q1, s_c, s_w, s_ok, s_red, qs_slots);
+    else if (full) qs_clip_group<true, true>(a, g0, q0, q1, s_c, s_w, s_ok, s_red, qs_slots);
+    else if (!resum) qs_clip_group<false, false>(a, g0, q0, q1, s_c, s_w, s_ok, s_red, qs_slots);
+    else qs_clip_group<false, true>(a, g0, q0, q1, s_c, s_w, s_ok, s_red, qs_slots);
   }
 }
 
