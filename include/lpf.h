@@ -24,7 +24,8 @@
  *   - lpf_associate / lpf_append_dynspec must be issued in increasing t.  A lane
  *     (0 <= lane < n_lanes) is a set of scratch buffers; two frames in flight at
  *     the same time must use different lanes (BASELINE.json config 4: 4 lanes).
- *   - Return value: 0 = LPF_OK; negative = error (nothing was enqueued).
+ *   - Return value: 0 = LPF_OK; negative = error (nothing was enqueued); positive = warning (LPF_W_CAPACITY,
+ *     reported at the sync points lpf_get_counters and lpf_process_frame_host / _host_end).
  *     Capacity overflow (max_det, n_cand_max) is not undefined behaviour: the list
  *     is truncated and a device counter is incremented (lpf_get_counters).
  *   - There is no CPU fallback: without a CUDA device lpf_create returns
@@ -46,6 +47,8 @@ extern "C" {
 #define LPF_E_CUDA (-2)  /* a CUDA runtime call failed (see lpf_last_cuda_error) */
 #define LPF_E_STATE (-3) /* call order / lane misuse */
 #define LPF_E_NOMEM (-4)
+#define LPF_W_CAPACITY 1  /* positive = warning, the call did its work: a list was truncated (max_det, n_cand_max, the
+                           * hit list of the fused path, or a caller buffer); the dropped entries are counted */
 
 #define LPF_MAX_BANDS 64  /* band_ok bits are kept in one 64-bit word per time step */
 #define LPF_MAX_RADIUS 16 /* k_mf, k_bg <= 16 ; k_max, r_flux, r_dedupe, r_assoc <= 8 */
@@ -215,14 +218,17 @@ int lpf_process_frame_host(lpf_ctx* ctx, int lane, const float* h_cube, int64_t 
 /* The same call in two halves, so that several lanes can be in flight from the host: _begin enqueues the
  * copy in, the chain and the copy out of the counts / statistics on `stream` and returns at once
  * (h_cube and res must stay untouched until _end); _end waits for the stream, copies the variable-length
- * lists (nu, npos known by then) and returns with `res` filled.  One _begin per lane at a time; issue
- * the _begin calls in increasing t. */
+ * lists (nu, npos known by then) and returns with `res` filled (LPF_W_CAPACITY when the frame found more records
+ * than max_det or more entries than cap_u / cap_pos hold: the lists are truncated).  One _begin per lane at a time;
+ * issue the _begin calls in increasing t. */
 int lpf_process_frame_host_begin(lpf_ctx* ctx, int lane, const float* h_cube, int64_t t, lpf_host_result* res,
                                  void* stream);
 int lpf_process_frame_host_end(lpf_ctx* ctx, int lane, lpf_host_result* res, void* stream);
 
-/* h_out[0] = records dropped (max_det), h_out[1] = detections dropped (n_cand_max full),
- * h_out[2] = kernels launched by this context so far, h_out[3] = active candidates.  Synchronises. */
+/* h_out[0] = records dropped (max_det; the fused path's hit list), h_out[1] = detections dropped (n_cand_max full),
+ * h_out[2] = kernels launched by this context so far, h_out[3] = active candidates.  Synchronises.  Returns
+ * LPF_W_CAPACITY when something was dropped since lpf_create (capacity overflow is never undefined behaviour:
+ * the list is truncated and the drop counted). */
 int lpf_get_counters(lpf_ctx* ctx, int64_t* h_out);
 
 /* Launch plan chosen at lpf_create: h_out[0] = 1 if the fused single-pass detection kernel is in use

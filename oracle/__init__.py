@@ -343,11 +343,22 @@ class OraclePipeline:
         if len(self.history) > self.n_back:
             self.history.pop(0)
 
-    def step(self, cube, t: int, keep_planes: bool = False) -> dict:
-        """One frame through the whole path."""
-        p = self.p
+    def front(self, cube, keep_planes: bool = False):
+        """The part of a step that has no memory (QC, per-plane detection, duplicate filter): (stats, band_ok, det).
+        Frames are independent here, so a test harness may evaluate several frames at once and
+        hand each result to step(pre=...).  Not with eq. A.2 on: that state is a recurrence over the frames."""
+        assert self.rq is None, "the running per-pixel QC carries state from frame to frame"
         stats, ok = self.cube_qc(cube)
-        det = self.detect(cube, ok, keep_planes)
+        return stats, ok, self.detect(cube, ok, keep_planes)
+
+    def step(self, cube, t: int, keep_planes: bool = False, pre=None) -> dict:
+        """One frame through the whole path.  pre: the result of front(cube), if it was evaluated beforehand."""
+        p = self.p
+        if pre is not None:
+            stats, ok, det = pre
+        else:
+            stats, ok = self.cube_qc(cube)
+            det = self.detect(cube, ok, keep_planes)
         cand, act_s, act_p = self.table.associate(det["upos"], t, int(ok[p["B"]]))
         flux = measure_flux(cube, ok, self.W, act_p, p["r_flux"])
         self.table.append(act_s, flux, ok, t)

@@ -112,8 +112,12 @@ def load_library(path: Optional[str] = None):
     return lib
 
 
+W_CAPACITY = 1   # positive status = warning: a list was truncated, the call did its work (include/lpf.h)
+
+
 def _check(lib, rc: int, what: str):
-    if rc != 0:
+    """Negative status: raise.  Positive (LPF_W_CAPACITY): a warning, returned to the caller."""
+    if rc < 0:
         raise LpfError(f"{what}: {lib.lpf_strerror(rc).decode()} ({rc}) {lib.lpf_last_cuda_error().decode()}")
 
 
@@ -267,8 +271,9 @@ class LPF:
                "lpf_process_frame_host_begin")
 
     def process_frame_host_end(self, res: "HostResult", lane: int = 0, stream=None):
-        _check(self.lib, self.lib.lpf_process_frame_host_end(self.h, lane, C.byref(res.c), _stream(stream)),
-               "lpf_process_frame_host_end")
+        rc = self.lib.lpf_process_frame_host_end(self.h, lane, C.byref(res.c), _stream(stream))
+        _check(self.lib, rc, "lpf_process_frame_host_end")
+        res.truncated = rc == W_CAPACITY
         return res
 
     def export_dynspec(self, slots, t_last: int, sigma=None, stream=None):
@@ -306,8 +311,10 @@ class LPF:
 
     def counters(self) -> dict:
         h = (C.c_int64 * 4)()
-        _check(self.lib, self.lib.lpf_get_counters(self.h, h), "lpf_get_counters")
-        return dict(dropped_records=int(h[0]), dropped_detections=int(h[1]), launches=int(h[2]), n_active=int(h[3]))
+        rc = self.lib.lpf_get_counters(self.h, h)
+        _check(self.lib, rc, "lpf_get_counters")
+        return dict(dropped_records=int(h[0]), dropped_detections=int(h[1]), launches=int(h[2]), n_active=int(h[3]),
+                    truncated=rc == W_CAPACITY)
 
 
 class HostResult:

@@ -622,7 +622,9 @@ int lpf_launch_export_dynspec(lpf_ctx* c, const int32_t* d_slots, int n, long lo
 int lpf_launch_simulate_pulses(int n, int B, int T, const float* d_nu, float nu0, float dt_s, const float* d_theta, float* d_out,
                                int accumulate, cudaStream_t st) {
   const long long total = (long long)n * B * T;
-  const int blocks = (int)std::min<long long>((total + 255) / 256, 148LL * 16);
+  int dev = 0, n_sm = 148;
+  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  const int blocks = (int)std::min<long long>((total + 255) / 256, (long long)n_sm * 16);
   k_simulate_pulses<<<blocks, 256, 0, st>>>(n, B, T, d_nu, nu0, dt_s, d_theta, d_out, accumulate);
   cudaError_t e = cudaPeekAtLastError();
   if (e != cudaSuccess) return lpf_cuda_fail(e, "k_simulate_pulses");

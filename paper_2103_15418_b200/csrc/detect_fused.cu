@@ -23,8 +23,10 @@
 // per thread); shared memory carries only what threads exchange and the input stages.  What a warp has to
 // decide in an iteration (is there input, which normalisers are the interior constants, which stages run)
 // is one 32-bit word of a per-item table built by the host plan.  F, C, d, S never leave the SM.
-// A value far above the plane's noise that leaves a running sum would leave its rounding behind for the
-// rest of the sweep: in that iteration the sum is rebuilt from the ring instead (warp-uniform, rare).
+// A value far above the noise that leaves a running sum would leave its rounding behind for the rest of the sweep:
+// in that iteration the sum is rebuilt from the ring instead (warp-uniform, rare).  "Far" = BIG_SIGMA x the smaller
+// of the plane's rms (which bright sources inflate) and the square root of the smallest local spread S the thread
+// has produced so far.
 // The input is used unmasked when the cube holds exact zeros at every invalid pixel (checked per frame by
 // the QC pass); otherwise each thread applies W itself (slow, rare).
 //
@@ -232,7 +234,8 @@ struct Sweep {
   bool col_in, dirty;
   unsigned umask;
   uint32_t tm;             // tensor-memory address of the thread's column 0
-  float big;               // |F| or |d| above this: the running sums are rebuilt when it leaves
+  float big2;              // (BIG_SIGMA x rms of the plane)^2: a first bound on "far above the noise"
+  float smin;              // the smallest local spread S this thread has seen (interior rows): the local noise level
   HitRec* seg;             // the CTA's segment of the hit list
   const float* nm0;        // padded norm_mf / 1/count at (row 0 of the image, the thread's first column); the zero row
   const float* ic0;        //   of a padded plane for lanes outside the strip (sx = 0)
@@ -419,7 +422,8 @@ struct Sweep {
       }
       float2 v[RB][2];
       const float hot = fmaxf(amax4(fold[0][0], fold[0][1]), amax4(fold[1][0], fold[1][1]));
-      if (__any_sync(0xffffffffu, hot > big)) {
+      const float far2 = fminf(big2, (BIG_SIGMA * BIG_SIGMA) * smin);       // |value| > BIG_SIGMA x noise, squared
+      if (__any_sync(0xffffffffu, hot * hot > far2)) {
         // something far above the noise leaves the window: rebuild the sums from the ring
         const float4 s23 = ring_sum23(tm, w, 0);
         const float2 b0 = make_float2(s23.x, s23.y), b1 = make_float2(s23.z, s23.w);
@@ -455,7 +459,8 @@ struct Sweep {
       }
       float2 v[RB][2];
       const float hot = fmaxf(amax4(dold[0][0], dold[0][1]), amax4(dold[1][0], dold[1][1]));
-      if (__any_sync(0xffffffffu, hot > big)) {
+      const float far2 = fminf(big2, (BIG_SIGMA * BIG_SIGMA) * smin);
+      if (__any_sync(0xffffffffu, hot * hot > far2)) {
         const float4 s23 = ring_sum23(tm + TM_D, w, 1);
         const float2 b0 = make_float2(s23.x, s23.y), b1 = make_float2(s23.z, s23.w);
         const float2 q0 = fma2(dd[0][0], dd[0][0], b0), q1 = fma2(dd[0][1], dd[0][1], b1);
@@ -489,6 +494,7 @@ struct Sweep {
         if (!FAST && (fl & FL_ICS_LD)) { ic0 = make_float2(pl.ics[j].x, pl.ics[j].y); ic1 = make_float2(pl.ics[j].z, pl.ics[j].w); }
         else { ic0 = splat(a.ic_const); ic1 = ic0; }
         const float2 s0 = mul2(b01, ic0), s1 = mul2(b23, ic1);
+        if (FAST) smin = fmaxf(0.f, fminf(smin, fminf(fminf(s0.x, s0.y), fminf(s1.x, s1.y))));   // every pixel of the row is valid
         const float2 k0 = mul2(s0, splat(a.kappa2)), k1 = mul2(s1, splat(a.kappa2));
         // d^2 - kappa^2 S > 0 somewhere in the thread's pixels?  (the sign of the difference is exact; k_peaks
         // applies the guarded, rounded test)
@@ -556,7 +562,8 @@ k_sweep(const FusedArgs a) {
   s.tid = threadIdx.x; s.lane = threadIdx.x & 31; s.warp = threadIdx.x >> 5; s.plane = p; s.xs = it.xs;
   s.nb = it.nb; s.ys = it.y_start;
   s.dirty = *a.dirty == a.dirty_seq;
-  s.big = a.big_thr[p];
+  { const float bg = a.big_thr[p]; s.big2 = bg * bg; }
+  s.smin = INFINITY;
   s.seg = a.hits + (long long)segi * a.seg_cap;
   if (s.tid == 0) s_args = a;
   constexpr int NT = SW::NT;
@@ -884,11 +891,8 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
   // n_lanes frames in flight the kernels of different lanes share the SMs, so each gets its share of them
   // (fewer, longer segments: less warm-up per output row).
   const int n_planes = c->n_planes;
-  int share_div = std::max(1, std::min(p.n_lanes, 4));   // (more lanes in flight only deepen the queue)
-#ifdef LPF_EXP_SHARE_ENV
-  if (const char* e = getenv("LPF_EXP_SHARE")) share_div = std::max(1, atoi(e));
-#endif
-  const int sm_share = std::max(1, c->n_sm / share_div);
+  const int sm_share = std::max(1, c->n_sm / std::max(1, std::min(p.n_lanes, 4)));   // (more lanes in flight only deepen the queue;
+                                                                                         // measured: 2 segments per plane beat 1 and 4)
   const double warm = 58.0;   // warm-up / drain rows of a segment
   int best_seg = 1; double best_cost = 1e30;
   const int max_rows_strip = (int)(rows_all / n_strips);

@@ -82,7 +82,7 @@ int check_params(const lpf_params* p) {
 
 int alloc_lane(lpf_ctx* c, LpfLane& L) {
   const lpf_params& p = c->p;
-  const size_t N = (size_t)c->N, P = (size_t)p.B + 1;
+  const size_t N = (size_t)c->N;
   TRY(dalloc(&L.qc_part1, (size_t)p.B * std::max(c->qc_nblk, lpf_qs_blocks(c)) * 3));
   TRY(dalloc(&L.qc_part2, (size_t)std::max(lpf_qc2_blocks(c), lpf_qs_blocks(c)) * p.B * 3));
   TRY(dalloc(&L.qc_mom, (size_t)p.B * 3));
@@ -94,10 +94,7 @@ int alloc_lane(lpf_ctx* c, LpfLane& L) {
   TRY(dalloc(&L.sum_plane, N));
   TRY(dalloc(&L.dirty, 1));
   LPF_CUDA(cudaMemset(L.dirty, 0, sizeof(int32_t)));
-  TRY(dalloc(&L.F, P * N));
-  TRY(dalloc(&L.C, P * N));
-  TRY(dalloc(&L.S, P * N));
-  if (p.n_iter > 1) { TRY(dalloc(&L.Y, P * N)); TRY(dalloc(&L.normp, P * N)); }
+  if (!c->fused) TRY(lpf_ensure_general_scratch(c, L));   // with the fused path planned: on first use (a misaligned cube)
   TRY(dalloc(&L.M, N));
   LPF_CUDA(cudaMemset(L.M, 0, N * sizeof(unsigned long long)));
   TRY(dalloc(&L.tmp_pos, (size_t)p.max_det));
@@ -136,6 +133,22 @@ int alloc_lane(lpf_ctx* c, LpfLane& L) {
   return LPF_OK;
 }
 
+}  // namespace
+
+// F, C, S (+ Y, per-plane normalisers for n_iter > 1) of the general multi-kernel path: 3 (B + 1) N floats per lane
+int lpf_ensure_general_scratch(lpf_ctx* c, LpfLane& L) {
+  if (L.F) return LPF_OK;
+  const lpf_params& p = c->p;
+  const size_t N = (size_t)c->N, P = (size_t)p.B + 1;
+  TRY(dalloc(&L.F, P * N));
+  TRY(dalloc(&L.C, P * N));
+  TRY(dalloc(&L.S, P * N));
+  if (p.n_iter > 1) { TRY(dalloc(&L.Y, P * N)); TRY(dalloc(&L.normp, P * N)); }
+  return LPF_OK;
+}
+
+namespace {
+
 void free_lane(LpfLane& L) {
   void* ptrs[] = {L.qc_part1, L.qc_part2, L.qc_band_clip, L.qc_counter, L.sum_plane, L.dirty, L.F, L.C, L.S, L.Y, L.normp, L.M, L.tmp_pos, L.tmp_plane,
                   L.tmp_snr, L.tmp_n, L.stats, L.band_ok, L.dets, L.ndets, L.upos, L.uplane, L.usnr, L.nu,
@@ -155,6 +168,7 @@ int lpf_launch_detect(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t
   // the fused kernel fetches rows with 16-byte bulk copies: a misaligned cube takes the general path
   if (c->fused && (((uintptr_t)d_cube) & 15) == 0)
     return lpf_launch_detect_fused(c, c->fused, L, d_cube, d_band_ok, d_dets, d_ndets, sum_done, st);
+  TRY(lpf_ensure_general_scratch(c, L));
   return lpf_launch_detect_general(c, L, d_cube, d_band_ok, d_dets, d_ndets, sum_done, st);
 }
 
@@ -407,8 +421,10 @@ int lpf_process_frame_host_end(lpf_ctx* c, int lane, lpf_host_result* res, void*
   const lpf_params& p = c->p;
   LPF_CUDA(cudaStreamSynchronize(st));
   res->nu = L.h_counts[0]; res->npos = L.h_counts[1]; res->ndets = L.h_counts[2];
-  const size_t nu = (size_t)(res->nu < res->cap_u ? res->nu : res->cap_u);
-  const size_t np = (size_t)(res->npos < res->cap_pos ? res->npos : res->cap_pos);
+  const int cap_u = res->cap_u > 0 ? res->cap_u : 0, cap_pos = res->cap_pos > 0 ? res->cap_pos : 0;
+  const size_t nu = (size_t)(res->nu < cap_u ? res->nu : cap_u);
+  const size_t np = (size_t)(res->npos < cap_pos ? res->npos : cap_pos);
+  const bool truncated = res->ndets > p.max_det || res->nu > cap_u || res->npos > cap_pos;
   if (nu) {
     if (res->h_upos) LPF_CUDA(cudaMemcpyAsync(res->h_upos, L.upos, nu * 4, cudaMemcpyDeviceToHost, st));
     if (res->h_uplane) LPF_CUDA(cudaMemcpyAsync(res->h_uplane, L.uplane, nu * 2, cudaMemcpyDeviceToHost, st));
@@ -420,7 +436,7 @@ int lpf_process_frame_host_end(lpf_ctx* c, int lane, lpf_host_result* res, void*
     if (res->h_flux) LPF_CUDA(cudaMemcpyAsync(res->h_flux, L.flux, np * p.B * 4, cudaMemcpyDeviceToHost, st));
   }
   LPF_CUDA(cudaStreamSynchronize(st));
-  return LPF_OK;
+  return truncated ? LPF_W_CAPACITY : LPF_OK;
 }
 
 int lpf_process_frame_host(lpf_ctx* c, int lane, const float* h_cube, int64_t t, lpf_host_result* res, void* stream) {
@@ -434,7 +450,7 @@ int lpf_get_counters(lpf_ctx* c, int64_t* h_out) {
   LPF_CUDA(cudaDeviceSynchronize());
   LPF_CUDA(cudaMemcpy(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost));
   h_out[0] = h[0]; h_out[1] = h[1]; h_out[2] = c->launches; h_out[3] = h[2];
-  return LPF_OK;
+  return (h[0] > 0 || h[1] > 0) ? LPF_W_CAPACITY : LPF_OK;
 }
 
 static const char* const kKernelNames[KID_COUNT] = {
@@ -508,6 +524,7 @@ const char* lpf_strerror(int code) {
     case LPF_E_CUDA: return "CUDA runtime error";
     case LPF_E_STATE: return "bad state (call order, capacity)";
     case LPF_E_NOMEM: return "out of device memory";
+    case LPF_W_CAPACITY: return "warning: a list was truncated (capacity); the dropped entries are counted";
     default: return "unknown";
   }
 }

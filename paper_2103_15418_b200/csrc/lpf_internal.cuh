@@ -158,6 +158,7 @@ int lpf_launch_detect_fused(lpf_ctx* c, LpfFusedPlan* pl, LpfLane& L, const floa
                             lpf_det* d_dets, int32_t* d_ndets, bool sum_done, cudaStream_t st);
 int lpf_launch_detect(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, lpf_det* d_dets,
                       int32_t* d_ndets, bool sum_done, cudaStream_t st);
+int lpf_ensure_general_scratch(lpf_ctx* c, LpfLane& L);
 int lpf_launch_static_norm(lpf_ctx* c, const LpfTaps& g, float* d_norm, float* d_tmp, cudaStream_t st);
 
 int lpf_launch_dedupe(lpf_ctx* c, LpfLane& L, const lpf_det* d_dets, const int32_t* d_ndets, int32_t* d_upos,

@@ -32,6 +32,12 @@ def pytest_terminal_summary(terminalreporter, exitstatus, config):
     parity = sys.modules.get("parity")
     if parity is None:
         return
+    try:
+        import torch
+        if not torch.cuda.is_available():
+            return          # the CPU suite compares nothing with the CUDA path: it leaves a GPU run's log alone
+    except Exception:
+        return
     path = os.path.join(ROOT, "gpurun_out", "ties.json")
     try:
         kinds = parity.dump_ties(path)

@@ -18,6 +18,11 @@ def lib():
     return binding.load_library()
 
 
+def binding_w_capacity():
+    from paper_2103_15418_b200 import binding
+    return binding.W_CAPACITY
+
+
 def declared_functions():
     src = open(HEADER).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
@@ -51,6 +56,11 @@ def test_struct_layouts_match_header(tmp_path):
 def test_version_and_errors_without_gpu(lib):
     assert lib.lpf_version() >= 100
     assert lib.lpf_strerror(0) == b"ok" and b"argument" in lib.lpf_strerror(-1)
+    # the positive status of SURVEY 8(b) "Errors": a truncated list is a warning, not an error
+    hdr = open(HEADER).read()
+    assert re.search(r"#define\s+LPF_W_CAPACITY\s+1\b", hdr) and binding_w_capacity() == 1
+    assert b"truncated" in lib.lpf_strerror(1)
+    assert "force_general" in hdr and "getenv" not in open(os.path.join(ROOT, "paper_2103_15418_b200", "csrc", "detect_fused.cu")).read()
     # bad parameters are rejected before any CUDA call
     from paper_2103_15418_b200 import binding, synth
     p = synth.default_params(1); p["B"] = 0

@@ -255,7 +255,8 @@ def test_edge_cases(torch_cuda):
     p2 = synth.default_params(1); p2["max_det"] = 2; p2["kappa"] = 1.0
     lpf = LPF(p2, None)
     g = parity.gpu_step_by_calls(lpf, torch.from_numpy(s.frame(0)).cuda(), 0)
-    assert g["ndets"] > 2 and len(g["rec"]) == 2 and lpf.counters()["dropped_records"] == g["ndets"] - 2
+    cnt = lpf.counters()
+    assert g["ndets"] > 2 and len(g["rec"]) == 2 and cnt["dropped_records"] == g["ndets"] - 2 and cnt["truncated"]   # LPF_W_CAPACITY
     lpf.close()
     # argument errors
     bad = synth.default_params(1); bad["k_bg"] = 40
@@ -344,6 +345,41 @@ def test_fused_kernel_special_paths(torch_cuda):
     lpf2.process_frame(mis, 0)
     assert parity.check_frame(lpf2.frame_view(0), o2, pipe2, cube, "misaligned cube")["in_sync"]
     lpf.close(); lpf2.close()
+
+
+def test_fused_very_bright_sources(torch_cuda):
+    """Sources at 1e3 and 1e4 sigma (A-team sources in real AARTFAAC images) in the fused sweep: its float32 running
+    sums must not keep the rounding they made while such a value was inside the window (the kernel rebuilds a sum
+    from its ring when a value far above the noise leaves it), so C, S and the detections BELOW and BESIDE the bright
+    sources still meet the float64 oracle within the tolerance."""
+    torch = torch_cuda
+    from paper_2103_15418_b200.binding import LPF
+    rng = np.random.default_rng(77)
+    B, D = 4, 384
+    p = synth.default_params(2); p.update(B=B, Dy=D, Dx=D)
+    yy, xx = np.mgrid[0:D, 0:D]
+
+    def src(y, x, a):
+        return (a * np.exp(-0.5 * ((yy - y) ** 2 + (xx - x) ** 2) / 0.85 ** 2)).astype(np.float32)
+
+    base = np.zeros((D, D), np.float32)
+    base += src(90, 100, 1.0e3) + src(200, 250, 1.0e4) + src(60, 300, 3.0e3)
+    # ordinary sources where a left-over of the bright ones would show: in the rows after they leave the 25-row
+    # windows, in their columns and a little beside them, and far away
+    for (y, x, a) in [(118, 100, 9.0), (131, 104, 12.0), (150, 92, 8.0), (229, 250, 10.0), (245, 262, 14.0), (262, 236, 9.0),
+                      (300, 250, 7.0), (90, 140, 11.0), (200, 290, 9.0), (95, 300, 8.0), (330, 60, 10.0), (20, 20, 12.0)]:
+        base += src(y, x, a)
+    lpf = LPF(p, None)
+    assert lpf.plan()["fused"]
+    pipe = O.OraclePipeline(p, None, direct=False)
+    for t in range(2):
+        cube = (base[None] + rng.standard_normal((B, D, D))).astype(np.float32)
+        o = pipe.step(cube, t)
+        lpf.process_frame(torch.from_numpy(cube).cuda(), t)
+        g = lpf.frame_view(0)
+        r = parity.check_frame(g, o, pipe, cube, f"bright t={t}")
+        assert r["in_sync"] and g["upos"].size >= 12
+    lpf.close()
 
 
 def test_host_entry_point_pipelined(torch_cuda):
