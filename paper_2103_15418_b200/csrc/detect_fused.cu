@@ -23,10 +23,11 @@
 // per thread); shared memory carries only what threads exchange and the input stages.  What a warp has to
 // decide in an iteration (is there input, which normalisers are the interior constants, which stages run)
 // is one 32-bit word of a per-item table built by the host plan.  F, C, d, S never leave the SM.
-// A value far above the noise that leaves a running sum would leave its rounding behind for the rest of the sweep:
-// in that iteration the sum is rebuilt from the ring instead (warp-uniform, rare).  "Far" = BIG_SIGMA x the smaller
-// of the plane's rms (which bright sources inflate) and the square root of the smallest local spread S the thread
-// has produced so far.
+// A term far above the rest that leaves a running sum leaves the rounding made in its presence behind for the rest
+// of the sweep: the sum is then rebuilt from the ring (warp-uniform, rare).  V2 (sums of squares) is rebuilt when it
+// has fallen below 1/FAR_RATIO of the largest value it held since it was last exact; V1 (signed) when an F above
+// BIG_SIGMA x the plane's rms leaves it (its rounding reaches C divided by 625: only sources of thousands of sigma
+// matter there).
 // The input is used unmasked when the cube holds exact zeros at every invalid pixel (checked per frame by
 // the QC pass); otherwise each thread applies W itself (slow, rare).
 //
@@ -56,7 +57,10 @@ constexpr int DR = 32;              // depth (rows) of the tensor-memory rings o
 constexpr int XST = LPF_XST;        // input staging stages (iterations in flight, power of two)
 constexpr int TM_D = 4 * DR;        // first tensor-memory column of the d ring (F ring starts at 0)
 constexpr int PADR = 64;            // zero rows above and below the padded normaliser planes
-constexpr float BIG_SIGMA = 64.f;
+constexpr float BIG_SIGMA = 64.f;   // V1: "far above the noise" = |F| > BIG_SIGMA x rms of the plane
+constexpr float FAR_RATIO = 4096.f; // V2 is rebuilt when it has fallen below 1/FAR_RATIO of the largest value it held since it was last exact:
+                                    // the rounding left in a column is ~1e-7 x that value, and a box of 25 columns holds 3-5 such columns,
+                                    // so S keeps ~1e-4 relative; ordinary sources (tens of sigma) never get there
 constexpr long long HIT_BUDGET = 1ll << 20;   // entries of the hit list of one frame (48 bytes each)
 #ifndef LPF_EXP_SKIP
 #define LPF_EXP_SKIP 0            // experiment switch (timing only): 1 no stage C, 2 no stage B, 4 no stage A part 2, 8 no stage A part 1
@@ -175,10 +179,10 @@ __device__ __forceinline__ void hbox25(int ev, int et, float2& o01, float2& o23)
   o23 = add2(add2(make_float2(l2, L.w), make_float2(r2, r3)), splat(a5));
 }
 
-// sum over the 23 ring rows before slot w (rows k = 1 .. 23 back), of the values (sq = 0) or their squares
-__device__ __noinline__ float4 ring_sum23(uint32_t ring, int w, int sq) {
+// sum over the n ring rows before slot w (rows k = 1 .. n back), of the values (sq = 0) or their squares
+__device__ __noinline__ float4 ring_sum(uint32_t ring, int w, int n, int sq) {
   float2 a0 = splat(0.f), a1 = splat(0.f);
-  for (int k = 1; k <= 23; ++k) {
+  for (int k = 1; k <= n; ++k) {
     float2 lo, hi;
     tm_ld4(ring + 4u * (uint32_t)((w - k) & (DR - 1)), lo, hi);
     tm_wait_ld();
@@ -234,8 +238,9 @@ struct Sweep {
   bool col_in, dirty;
   unsigned umask;
   uint32_t tm;             // tensor-memory address of the thread's column 0
-  float big2;              // (BIG_SIGMA x rms of the plane)^2: a first bound on "far above the noise"
-  float smin;              // the smallest local spread S this thread has seen (interior rows): the local noise level
+  float big2;              // (BIG_SIGMA x rms of the plane)^2: an F above this leaves its rounding in V1
+  float2 vmax[2];          // the largest V2 since V2 was last rebuilt from the ring
+  bool want_fix2;          // this thread saw V2 fall far below vmax at the end of the last stage B
   HitRec* seg;             // the CTA's segment of the hit list
   const float* nm0;        // padded norm_mf / 1/count at (row 0 of the image, the thread's first column); the zero row
   const float* ic0;        //   of a padded plane for lanes outside the strip (sx = 0)
@@ -379,17 +384,11 @@ struct Sweep {
   // One iteration: rows y0, y0+1 enter stage A.  fl: this iteration's control word.  FAST: an interior iteration
   // (fl = FL_FAST): no flag is looked at, no normaliser plane is loaded.
   template <bool FAST>
-  __device__ __forceinline__ void iteration(int b, unsigned fl, unsigned fl_next) {
+  __device__ __forceinline__ void iteration(int b, unsigned fl, unsigned fl_next, bool fix1, bool fix2) {
     const int buf = b & 1, pbuf = buf ^ 1;
     const float2 g0 = splat(a.g0), g1 = splat(a.g1), g2 = splat(a.g2), g3 = splat(a.g3);
     const int w = (RB * b) & (DR - 1);                       // ring slot of this iteration's first row (even)
     const uint32_t t_new0 = tm + 4u * (uint32_t)w, t_new1 = t_new0 + 4u;
-
-    tm_wait_ld();
-#pragma unroll
-    for (int j = 0; j < RB; ++j) { tm_use(fold[j][0], fold[j][1]); tm_use(flag[j][0], flag[j][1]); tm_use(dold[j][0], dold[j][1]); tm_use(dlag[j][0], dlag[j][1]); }
-#pragma unroll
-    for (int k = 0; k < 4; ++k) tm_use(fs[k][0], fs[k][1]);
 
     // ---- stage A, part 2: vertical matched filter -> F(fr), running sum V1, exchange ----------------
     // F(fr) = g3 h(fr-3) + g2 h(fr-2) + g1 h(fr-1) + g0 h(fr) + g1 h(fr+1) + g2 h(fr+2) + g3 h(fr+3), summed in that
@@ -421,11 +420,9 @@ struct Sweep {
         for (int j = 0; j < RB; ++j) { f[j][0] = mul2(f[j][0], c); f[j][1] = mul2(f[j][1], c); }
       }
       float2 v[RB][2];
-      const float hot = fmaxf(amax4(fold[0][0], fold[0][1]), amax4(fold[1][0], fold[1][1]));
-      const float far2 = fminf(big2, (BIG_SIGMA * BIG_SIGMA) * smin);       // |value| > BIG_SIGMA x noise, squared
-      if (__any_sync(0xffffffffu, hot * hot > far2)) {
+      if (!FAST && fix1) {
         // something far above the noise leaves the window: rebuild the sums from the ring
-        const float4 s23 = ring_sum23(tm, w, 0);
+        const float4 s23 = ring_sum(tm, w, 23, 0);
         const float2 b0 = make_float2(s23.x, s23.y), b1 = make_float2(s23.z, s23.w);
         v[0][0] = add2(add2(b0, fold[1][0]), f[0][0]); v[0][1] = add2(add2(b1, fold[1][1]), f[0][1]);
         v[1][0] = add2(add2(b0, f[0][0]), f[1][0]);    v[1][1] = add2(add2(b1, f[0][1]), f[1][1]);
@@ -457,22 +454,36 @@ struct Sweep {
         dd[j][0] = fma2(neg2(b01), ic0, flag[j][0]);     // d = F - box * (1/count)
         dd[j][1] = fma2(neg2(b23), ic1, flag[j][1]);
       }
-      float2 v[RB][2];
-      const float hot = fmaxf(amax4(dold[0][0], dold[0][1]), amax4(dold[1][0], dold[1][1]));
-      const float far2 = fminf(big2, (BIG_SIGMA * BIG_SIGMA) * smin);
-      if (__any_sync(0xffffffffu, hot * hot > far2)) {
-        const float4 s23 = ring_sum23(tm + TM_D, w, 1);
-        const float2 b0 = make_float2(s23.x, s23.y), b1 = make_float2(s23.z, s23.w);
-        const float2 q0 = fma2(dd[0][0], dd[0][0], b0), q1 = fma2(dd[0][1], dd[0][1], b1);
-        v[0][0] = fma2(dold[1][0], dold[1][0], q0); v[0][1] = fma2(dold[1][1], dold[1][1], q1);
-        v[1][0] = fma2(dd[1][0], dd[1][0], q0);     v[1][1] = fma2(dd[1][1], dd[1][1], q1);
-      } else {
-        v[0][0] = fma2(neg2(dold[0][0]), dold[0][0], fma2(dd[0][0], dd[0][0], V2[0]));
-        v[0][1] = fma2(neg2(dold[0][1]), dold[0][1], fma2(dd[0][1], dd[0][1], V2[1]));
-        v[1][0] = fma2(neg2(dold[1][0]), dold[1][0], fma2(dd[1][0], dd[1][0], v[0][0]));
-        v[1][1] = fma2(neg2(dold[1][1]), dold[1][1], fma2(dd[1][1], dd[1][1], v[0][1]));
+      if (!FAST && fix2) {
+        // V2 had fallen far below what it held since it was last exact (seen at the end of the previous iteration):
+        // the roundings made in the presence of the large terms are now a visible part of it.  Rebuild it from the
+        // ring (the 25 rows up to the previous iteration's last; warp-uniform, rare) before it is used again.
+        const float4 s25 = ring_sum(tm + TM_D, w, 25, 1);
+        V2[0] = make_float2(s25.x, s25.y); V2[1] = make_float2(s25.z, s25.w);
+        vmax[0] = V2[0]; vmax[1] = V2[1];
       }
+      float2 v[RB][2];
+      v[0][0] = fma2(neg2(dold[0][0]), dold[0][0], fma2(dd[0][0], dd[0][0], V2[0]));
+      v[0][1] = fma2(neg2(dold[0][1]), dold[0][1], fma2(dd[0][1], dd[0][1], V2[1]));
+      v[1][0] = fma2(neg2(dold[1][0]), dold[1][0], fma2(dd[1][0], dd[1][0], v[0][0]));
+      v[1][1] = fma2(neg2(dold[1][1]), dold[1][1], fma2(dd[1][1], dd[1][1], v[0][1]));
+      vmax[0] = make_float2(fmaxf(vmax[0].x, v[1][0].x), fmaxf(vmax[0].y, v[1][0].y));
+      vmax[1] = make_float2(fmaxf(vmax[1].x, v[1][1].x), fmaxf(vmax[1].y, v[1][1].y));
       V2[0] = v[1][0]; V2[1] = v[1][1];
+      {
+        // has V2 fallen below 1 / FAR_RATIO of the largest value it held since it was last exact?  Where the sweep
+        // leaves the valid region a column's sum falls to (a rounding of) zero, which is no error worth a rebuild:
+        // a column counts only while its own pixel of this row is valid (its 1/count is not 0).
+        const float2 r = splat(FAR_RATIO);
+        float2 e0 = fma2(V2[0], r, neg2(vmax[0])), e1 = fma2(V2[1], r, neg2(vmax[1]));
+        if (!FAST && (fl & FL_ICR_LD)) {
+          if (pl.icr[1].x == 0.f) e0.x = 0.f;
+          if (pl.icr[1].y == 0.f) e0.y = 0.f;
+          if (pl.icr[1].z == 0.f) e1.x = 0.f;
+          if (pl.icr[1].w == 0.f) e1.y = 0.f;
+        }
+        want_fix2 = fminf(fminf(e0.x, e0.y), fminf(e1.x, e1.y)) < 0.f;
+      }
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
         tm_st4((j ? t_new1 : t_new0) + TM_D, dd[j][0], dd[j][1]);
@@ -494,7 +505,6 @@ struct Sweep {
         if (!FAST && (fl & FL_ICS_LD)) { ic0 = make_float2(pl.ics[j].x, pl.ics[j].y); ic1 = make_float2(pl.ics[j].z, pl.ics[j].w); }
         else { ic0 = splat(a.ic_const); ic1 = ic0; }
         const float2 s0 = mul2(b01, ic0), s1 = mul2(b23, ic1);
-        if (FAST) smin = fmaxf(0.f, fminf(smin, fminf(fminf(s0.x, s0.y), fminf(s1.x, s1.y))));   // every pixel of the row is valid
         const float2 k0 = mul2(s0, splat(a.kappa2)), k1 = mul2(s1, splat(a.kappa2));
         // d^2 - kappa^2 S > 0 somewhere in the thread's pixels?  (the sign of the difference is exact; k_peaks
         // applies the guarded, rounded test)
@@ -534,8 +544,19 @@ struct Sweep {
     stage_a1(0, f0, y0);
     for (int b = 0; b < nb; ++b) {
       const unsigned f3 = ctl(b + 3);
-      if (f0 == FL_FAST) iteration<true>(b, f0, f1);
-      else iteration<false>(b, f0, f1);
+      tm_wait_ld();
+#pragma unroll
+      for (int j = 0; j < RB; ++j) { tm_use(fold[j][0], fold[j][1]); tm_use(flag[j][0], flag[j][1]); tm_use(dold[j][0], dold[j][1]); tm_use(dlag[j][0], dlag[j][1]); }
+#pragma unroll
+      for (int k = 0; k < 4; ++k) tm_use(fs[k][0], fs[k][1]);
+      // the two rare repairs of the running sums live in the slow form of the iteration only: the interior form
+      // has no call in it
+      const float hot = fmaxf(amax4(fold[0][0], fold[0][1]), amax4(fold[1][0], fold[1][1]));
+      const bool fix1 = __any_sync(0xffffffffu, hot * hot > big2);
+      const bool fix2 = __any_sync(0xffffffffu, want_fix2);
+      want_fix2 = false;
+      if (f0 == FL_FAST && !fix1 && !fix2) iteration<true>(b, f0, f1, false, false);
+      else iteration<false>(b, f0, f1, fix1, fix2);
       f0 = f1; f1 = f2; f2 = f3;
     }
     tm_wait_ld();        // the reads issued for an iteration past the end
@@ -563,7 +584,8 @@ k_sweep(const FusedArgs a) {
   s.nb = it.nb; s.ys = it.y_start;
   s.dirty = *a.dirty == a.dirty_seq;
   { const float bg = a.big_thr[p]; s.big2 = bg * bg; }
-  s.smin = INFINITY;
+  s.vmax[0] = s.vmax[1] = splat(0.f);
+  s.want_fix2 = false;
   s.seg = a.hits + (long long)segi * a.seg_cap;
   if (s.tid == 0) s_args = a;
   constexpr int NT = SW::NT;
