@@ -341,9 +341,10 @@ k_ring_nan_slots(float* __restrict__ ring, const int32_t* __restrict__ free_list
 
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-k_measure_flux(const float* __restrict__ cube, const uint8_t* __restrict__ band_ok, const uint8_t* __restrict__ W,
-               int B, int Dy, int Dx, int r, const int32_t* __restrict__ pos, const int32_t* __restrict__ npos,
-               float* __restrict__ flux) {
+k_measure_flux(const LpfFrameDesc* __restrict__ fd, const float* __restrict__ cube_arg, const uint8_t* __restrict__ band_ok,
+               const uint8_t* __restrict__ W, int B, int Dy, int Dx, int r, const int32_t* __restrict__ pos,
+               const int32_t* __restrict__ npos, float* __restrict__ flux) {
+  const float* __restrict__ cube = fd ? fd->cube : cube_arg;
   const long long N = (long long)Dy * Dx;
   const long long total = (long long)(*npos) * B;
   const bool frame_ok = band_ok[B] != 0;
@@ -377,7 +378,9 @@ k_measure_flux(const float* __restrict__ cube, const uint8_t* __restrict__ band_
 __global__ void __launch_bounds__(256)
 k_append(float* __restrict__ ring, long long* __restrict__ meta_t, unsigned long long* __restrict__ meta_ok,
          const long long* __restrict__ born, int T_ring, int B, const int32_t* __restrict__ slots,
-         const int32_t* __restrict__ n, const float* __restrict__ flux, const uint8_t* __restrict__ band_ok, long long t) {
+         const int32_t* __restrict__ n, const float* __restrict__ flux, const uint8_t* __restrict__ band_ok, long long t_arg,
+         const LpfFrameDesc* __restrict__ fd) {
+  const long long t = fd ? fd->t : t_arg;
   const int tau = (int)(t % T_ring);
   const int lane = threadIdx.x & 31;
   const int wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
@@ -530,7 +533,7 @@ int lpf_launch_measure_flux(lpf_ctx* c, const float* d_cube, const uint8_t* d_ba
                             const int32_t* d_npos, float* d_flux, cudaStream_t st) {
   const lpf_params& p = c->p;
   LPF_KLAUNCH(c, KID_MEASURE_FLUX, st, k_measure_flux<<<c->n_sm * 2, 256, 0, st>>>(
-      d_cube, d_band_ok, c->W, p.B, p.Dy, p.Dx, p.r_flux, d_pos, d_npos, d_flux));
+      c->cap_fd, d_cube, d_band_ok, c->W, p.B, p.Dy, p.Dx, p.r_flux, d_pos, d_npos, d_flux));
   return LPF_OK;
 }
 
@@ -538,7 +541,7 @@ int lpf_launch_append(lpf_ctx* c, const int32_t* d_slots, const int32_t* d_n, co
                       const uint8_t* d_band_ok, long long t, cudaStream_t st) {
   const lpf_params& p = c->p;
   LPF_KLAUNCH(c, KID_APPEND, st, k_append<<<c->n_sm, 256, 0, st>>>(
-      c->ring, c->meta_t, c->meta_ok, c->born, p.T_ring, p.B, d_slots, d_n, d_flux, d_band_ok, t));
+      c->ring, c->meta_t, c->meta_ok, c->born, p.T_ring, p.B, d_slots, d_n, d_flux, d_band_ok, t, c->cap_fd));
   return LPF_OK;
 }
 

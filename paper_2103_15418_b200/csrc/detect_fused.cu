@@ -87,6 +87,7 @@ struct FusedItem { int xs, ux0, ux1, ya, yb, y_start, nb, fl_off; };
 struct alignas(16) HitRec { int32_t pix0, bits, pad0, pad1; float d[4]; float s[4]; };
 
 struct FusedArgs {
+  const LpfFrameDesc* fd;                        // non-null: cube and dirty_seq come from the frame descriptor
   const float* cube; const float* sum_plane; const uint8_t* band_ok; const uint8_t* W;
   const float* nm_pad; const float* ic_pad;      // [(Dy + 2 PADR)][Dx], zero rows around the image
   const FusedItem* items; const uint32_t* flags;
@@ -582,7 +583,7 @@ k_sweep(const FusedArgs a) {
   s.a_sh = &s_args;
   s.tid = threadIdx.x; s.lane = threadIdx.x & 31; s.warp = threadIdx.x >> 5; s.plane = p; s.xs = it.xs;
   s.nb = it.nb; s.ys = it.y_start;
-  s.dirty = *a.dirty == a.dirty_seq;
+  s.dirty = *a.dirty == (a.fd ? a.fd->seq : a.dirty_seq);
   { const float bg = a.big_thr[p]; s.big2 = bg * bg; }
   s.vmax[0] = s.vmax[1] = splat(0.f);
   s.want_fix2 = false;
@@ -613,7 +614,7 @@ k_sweep(const FusedArgs a) {
   tm_wait_st();
 
   const long long N = (long long)a.Dy * a.Dx;
-  const float* X = (p < a.B) ? a.cube + (long long)p * N : a.sum_plane;
+  const float* X = (p < a.B) ? (a.fd ? a.fd->cube : a.cube) + (long long)p * N : a.sum_plane;
   const int x = it.xs + 4 * s.tid;
   s.col_in = 4 * s.tid < a.CW && x < a.Dx;
   s.umask = 0u;
@@ -735,9 +736,9 @@ k_peaks(const FusedArgs a) {
   const int p = segi / a.n_items;
   const int n = a.hit_cnt[segi];
   if ((int)(blockIdx.x * blockDim.x) >= n) return;
-  const bool masked = *a.dirty == a.dirty_seq;
+  const bool masked = *a.dirty == (a.fd ? a.fd->seq : a.dirty_seq);
   const long long N = (long long)a.Dy * a.Dx;
-  const float* X = (p < a.B) ? a.cube + (long long)p * N : a.sum_plane;
+  const float* X = (p < a.B) ? (a.fd ? a.fd->cube : a.cube) + (long long)p * N : a.sum_plane;
   const HitRec* seg = a.hits + (long long)segi * a.seg_cap;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int i0 = blockIdx.x * blockDim.x; i0 < n; i0 += gridDim.x * blockDim.x) {
@@ -913,7 +914,8 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
   // n_lanes frames in flight the kernels of different lanes share the SMs, so each gets its share of them
   // (fewer, longer segments: less warm-up per output row).
   const int n_planes = c->n_planes;
-  const int sm_share = std::max(1, c->n_sm / std::max(1, std::min(p.n_lanes, 4)));   // (more lanes in flight only deepen the queue;
+  const int cta_per_sm = NW > 4 ? 1 : 2;      // k_sweep's launch bounds
+  const int sm_share = std::max(1, cta_per_sm * c->n_sm / std::max(1, std::min(p.n_lanes, 4)));   // (more lanes in flight only deepen the queue;
                                                                                          // measured: 2 segments per plane beat 1 and 4)
   const double warm = 58.0;   // warm-up / drain rows of a segment
   int best_seg = 1; double best_cost = 1e30;
@@ -1105,7 +1107,7 @@ int lpf_launch_detect_fused(lpf_ctx* c, LpfFusedPlan* pl, LpfLane& L, const floa
     LPF_KLAUNCH(c, KID_MISC, st, k_big_thr<<<c->n_planes, 1024, 0, st>>>(d_cube, L.sum_plane, c->W, c->N, p.B, L.big_thr));
   }
   FusedArgs a{};
-  a.cube = d_cube; a.sum_plane = L.sum_plane; a.band_ok = d_band_ok; a.W = c->W;
+  a.fd = c->cap_fd; a.cube = d_cube; a.sum_plane = L.sum_plane; a.band_ok = d_band_ok; a.W = c->W;
   a.nm_pad = pl->d_nm_pad; a.ic_pad = pl->d_ic_pad; a.items = pl->d_items; a.flags = pl->d_flags; a.dirty = L.dirty; a.dirty_seq = L.dirty_seq;
   a.big_thr = L.big_thr;
   a.B = p.B; a.Dy = p.Dy; a.Dx = p.Dx; a.CW = pl->CW; a.k_max = p.k_max; a.max_det = p.max_det; a.seg_cap = pl->seg_cap; a.n_items = pl->n_items;

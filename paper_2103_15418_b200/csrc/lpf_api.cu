@@ -128,6 +128,7 @@ int alloc_lane(lpf_ctx* c, LpfLane& L) {
   LPF_CUDA(cudaMemset(L.nu, 0, sizeof(int32_t)));
   LPF_CUDA(cudaMemset(L.npos, 0, sizeof(int32_t)));
   LPF_CUDA(cudaMallocHost((void**)&L.h_counts, 4 * sizeof(int32_t)));
+  TRY(dalloc(&L.fdesc, 1));
   LPF_CUDA(cudaEventCreateWithFlags(&L.ev_pre, cudaEventDisableTiming));
   LPF_CUDA(cudaEventCreateWithFlags(&L.ev_post, cudaEventDisableTiming));
   return LPF_OK;
@@ -155,6 +156,10 @@ void free_lane(LpfLane& L) {
                   L.cand_idx, L.act_slots, L.act_pix, L.npos, L.flux, L.cube, L.zeta_cnt, L.hits, L.hit_cnt, L.big_thr, L.dirty_b, L.qc_mom};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (L.h_counts) cudaFreeHost(L.h_counts);
+  if (L.gx_a) cudaGraphExecDestroy(L.gx_a);
+  if (L.gx_b) cudaGraphExecDestroy(L.gx_b);
+  if (L.g_a) cudaGraphDestroy(L.g_a);
+  if (L.fdesc) cudaFree(L.fdesc);
   if (L.ev_pre) cudaEventDestroy(L.ev_pre);
   if (L.ev_post) cudaEventDestroy(L.ev_post);
   L = LpfLane();
@@ -173,6 +178,65 @@ int lpf_launch_detect(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t
 }
 
 namespace {
+
+// first node of a lane's graph: the one node whose parameters change from launch to launch
+__global__ void k_set_frame(LpfFrameDesc* fd, const float* cube, long long t, int seq) {
+  fd->cube = cube; fd->t = t; fd->seq = seq; fd->pad = 0;
+}
+
+int seq_of(long long t) { return (int)(t % 0x3ffffff0LL) + 1; }
+
+// The frame chain of a lane without its association step (which runs on the context's own stream): graph A =
+// set_frame, QC, detection, duplicate filter; graph B = flux, append.  Captured once per lane on the context's
+// capture stream; every pointer in it is lane- or context-owned, what changes per frame comes through the descriptor.
+int build_lane_graphs(lpf_ctx* c, LpfLane& L, const float* d_cube, long long t) {
+  cudaStream_t cs = c->cap_st;
+  cudaGraph_t ga = nullptr, gb = nullptr;
+  const int64_t launches0 = c->launches;
+  c->cap_fd = L.fdesc;
+  int rc = LPF_OK;
+  cudaError_t e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
+  if (e == cudaSuccess) {
+    k_set_frame<<<1, 1, 0, cs>>>(L.fdesc, d_cube, t, seq_of(t));
+    c->launches++;
+    rc = lpf_launch_qc_sum(c, L, d_cube, L.stats, L.band_ok, L.ndets, cs);
+    if (!rc) rc = lpf_launch_detect(c, L, d_cube, L.band_ok, L.dets, L.ndets, true, cs);
+    if (!rc) rc = lpf_launch_dedupe(c, L, L.dets, L.ndets, L.upos, L.uplane, L.usnr, L.nu, cs);
+    e = cudaStreamEndCapture(cs, &ga);
+  }
+  L.g_nodes_a = (int)(c->launches - launches0);
+  const int64_t launches1 = c->launches;
+  if (e == cudaSuccess && !rc) {
+    e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
+    if (e == cudaSuccess) {
+      rc = lpf_launch_measure_flux(c, d_cube, L.band_ok, L.act_pix, L.npos, L.flux, cs);
+      if (!rc) rc = lpf_launch_append(c, L.act_slots, L.npos, L.flux, L.band_ok, t, cs);
+      e = cudaStreamEndCapture(cs, &gb);
+    }
+  }
+  L.g_nodes_b = (int)(c->launches - launches1);
+  c->launches = launches0;          // nothing has been launched yet
+  c->cap_fd = nullptr;
+  if (e == cudaSuccess && !rc) e = cudaGraphInstantiate(&L.gx_a, ga, 0);
+  if (e == cudaSuccess && !rc) e = cudaGraphInstantiate(&L.gx_b, gb, 0);
+  if (e == cudaSuccess && !rc) {     // the descriptor node: the only root of graph A
+    size_t n = 1;
+    cudaGraphNode_t root = nullptr;
+    e = cudaGraphGetRootNodes(ga, &root, &n);
+    if (e == cudaSuccess && n >= 1) L.gnode_set = root; else if (e == cudaSuccess) e = cudaErrorUnknown;
+  }
+  if (gb) cudaGraphDestroy(gb);
+  if (e != cudaSuccess || rc) {
+    (void)cudaGetLastError();
+    if (ga) cudaGraphDestroy(ga);
+    if (L.gx_a) { cudaGraphExecDestroy(L.gx_a); L.gx_a = nullptr; }
+    if (L.gx_b) { cudaGraphExecDestroy(L.gx_b); L.gx_b = nullptr; }
+    L.g_failed = true;
+    return rc ? rc : LPF_OK;         // the direct path serves the lane
+  }
+  L.g_a = ga;                        // the descriptor node's handle belongs to this graph: it lives as long as the lane
+  return LPF_OK;
+}
 
 int lane_ok(lpf_ctx* c, int lane) { return (c && lane >= 0 && lane < (int)c->lanes.size()) ? LPF_OK : LPF_E_ARG; }
 
@@ -259,10 +323,12 @@ int lpf_create(lpf_ctx** out, const lpf_params* p, const uint8_t* d_valid_mask) 
   CUDAC(cudaMemset(c->counters, 0, 8 * 4));
   TRYC(lpf_launch_fill_nan(c, c->ring, (int64_t)(nc * p->T_ring * p->B), 0));
   CUDAC(cudaEventCreateWithFlags(&c->ring_ev, cudaEventDisableTiming));
+  TRYC(lpf_qc_prepare());
   {
     int lo = 0, hi = 0;
     CUDAC(cudaDeviceGetStreamPriorityRange(&lo, &hi));
     CUDAC(cudaStreamCreateWithPriority(&c->chain_st, cudaStreamNonBlocking, hi));
+    CUDAC(cudaStreamCreateWithFlags(&c->cap_st, cudaStreamNonBlocking));
   }
   c->lanes.resize(p->n_lanes);
   for (auto& L : c->lanes) TRYC(alloc_lane(c, L));
@@ -284,6 +350,7 @@ int lpf_destroy(lpf_ctx* c) {
   for (void* q : ptrs) if (q) cudaFree(q);
   if (c->ring_ev) cudaEventDestroy(c->ring_ev);
   if (c->chain_st) cudaStreamDestroy(c->chain_st);
+  if (c->cap_st) cudaStreamDestroy(c->cap_st);
   if (c->rq_ev) cudaEventDestroy(c->rq_ev);
   lpf_fused_plan_free(c->fused);
   for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
@@ -360,10 +427,33 @@ int lpf_process_frame(lpf_ctx* c, int lane, const float* d_cube, int64_t t, void
   if (!d_cube || t < 0) return LPF_E_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   LpfLane& L = c->lanes[lane];
-  TRY(lpf_launch_qc_sum(c, L, d_cube, L.stats, L.band_ok, L.ndets, st));      // S1-S3, one kernel per pass over the cube
-  if (c->p.n_back > 0) TRY(lpf_launch_cache_store(c, d_cube, L.band_ok, (long long)t, st));   // O11: the frame joins the cache
-  TRY(lpf_launch_detect(c, L, d_cube, L.band_ok, L.dets, L.ndets, true, st));
-  TRY(lpf_launch_dedupe(c, L, L.dets, L.ndets, L.upos, L.uplane, L.usnr, L.nu, st));
+  // The lane's chain as two CUDA graphs around the association step: one launch instead of nine, one instead of
+  // two (a frame then costs the host a third of the time, which is what fills the pipeline after a pause).  For
+  // the configuration the graphs were captured for: the fused detection path on an aligned cube, no running
+  // per-pixel QC (its state is ordered across lanes by an event), no backward fill (a device-to-device copy of the
+  // cube whose source changes per frame), no per-kernel profile.
+  const bool graphable = c->fused && (((uintptr_t)d_cube) & 15) == 0 && (c->N & 3) == 0 && !(c->p.zeta_thr > 0) &&
+                         c->p.n_back == 0 && !c->prof_on && !L.g_failed;
+  if (graphable && !L.gx_a) TRY(build_lane_graphs(c, L, d_cube, (long long)t));
+  const bool use_graph = graphable && L.gx_a && L.gx_b;
+  if (use_graph) {
+    LpfFrameDesc* fd = L.fdesc;
+    const float* cube = d_cube;
+    long long tt = (long long)t;
+    int seq = seq_of(tt);
+    void* kargs[4] = {&fd, &cube, &tt, &seq};
+    cudaKernelNodeParams kp{};
+    kp.func = (void*)k_set_frame; kp.gridDim = dim3(1); kp.blockDim = dim3(1); kp.sharedMemBytes = 0;
+    kp.kernelParams = kargs; kp.extra = nullptr;
+    LPF_CUDA(cudaGraphExecKernelNodeSetParams(L.gx_a, L.gnode_set, &kp));
+    LPF_CUDA(cudaGraphLaunch(L.gx_a, st));
+    c->launches += L.g_nodes_a;
+  } else {
+    TRY(lpf_launch_qc_sum(c, L, d_cube, L.stats, L.band_ok, L.ndets, st));      // S1-S3
+    if (c->p.n_back > 0) TRY(lpf_launch_cache_store(c, d_cube, L.band_ok, (long long)t, st));   // O11: the frame joins the cache
+    TRY(lpf_launch_detect(c, L, d_cube, L.band_ok, L.dets, L.ndets, true, st));
+    TRY(lpf_launch_dedupe(c, L, L.dets, L.ndets, L.upos, L.uplane, L.usnr, L.nu, st));
+  }
   // The candidate table and the rings are shared by all lanes.  The association steps of all frames run, in frame
   // order, on ONE stream of the context (highest priority: a single block per frame that the next frame waits for
   // must not queue behind the other lanes' grids); the lane's stream hands over after its duplicate filter and
@@ -375,10 +465,15 @@ int lpf_process_frame(lpf_ctx* c, int lane, const float* d_cube, int64_t t, void
   TRY(lpf_launch_associate(c, L.upos, L.nu, L.band_ok, (long long)t, L.cand_idx, L.act_slots, L.act_pix, L.npos, c->chain_st));
   LPF_CUDA(cudaEventRecord(L.ev_post, c->chain_st));
   LPF_CUDA(cudaStreamWaitEvent(st, L.ev_post, 0));
-  TRY(lpf_launch_measure_flux(c, d_cube, L.band_ok, L.act_pix, L.npos, L.flux, st));
   if (c->ring_valid) LPF_CUDA(cudaStreamWaitEvent(st, c->ring_ev, 0));
-  TRY(lpf_launch_append(c, L.act_slots, L.npos, L.flux, L.band_ok, (long long)t, st));
-  if (c->p.n_back > 0) TRY(lpf_launch_backfill(c, L.act_slots, L.act_pix, L.npos, d_cube, L.band_ok, (long long)t, st));   // O11
+  if (use_graph) {
+    LPF_CUDA(cudaGraphLaunch(L.gx_b, st));
+    c->launches += L.g_nodes_b;
+  } else {
+    TRY(lpf_launch_measure_flux(c, d_cube, L.band_ok, L.act_pix, L.npos, L.flux, st));
+    TRY(lpf_launch_append(c, L.act_slots, L.npos, L.flux, L.band_ok, (long long)t, st));
+    if (c->p.n_back > 0) TRY(lpf_launch_backfill(c, L.act_slots, L.act_pix, L.npos, d_cube, L.band_ok, (long long)t, st));   // O11
+  }
   LPF_CUDA(cudaEventRecord(c->ring_ev, st));
   c->ring_valid = true;
   return LPF_OK;

@@ -14,6 +14,11 @@ struct LpfTaps {
   float g[LPF_NTAPS];
 };
 
+// What changes from one frame to the next on a lane.  With the lane's frame chain captured in CUDA graphs the kernels
+// read it from device memory (written by the first node of the graph, the one node whose parameters are updated per
+// launch); launched directly they get the same values in their arguments (fd = null).
+struct LpfFrameDesc { const float* cube; long long t; int32_t seq; int32_t pad; };
+
 // Scratch and owned outputs of one frame in flight.
 struct LpfLane {
   double* qc_part1 = nullptr;  // [B][nblk][3]  n, sum(x-p), sum(x-p)^2
@@ -56,6 +61,13 @@ struct LpfLane {
   float* big_thr = nullptr;    // [B + 1] 'far above the noise' level of every plane (64 x rms)
   int32_t* h_counts = nullptr; // pinned [4]
   cudaEvent_t ev_pre = nullptr, ev_post = nullptr;   // hand-over to / from the context's association stream
+  // the lane's frame chain as two CUDA graphs (before / after the association step), built on first use
+  LpfFrameDesc* fdesc = nullptr;       // device
+  cudaGraph_t g_a = nullptr;
+  cudaGraphExec_t gx_a = nullptr, gx_b = nullptr;
+  cudaGraphNode_t gnode_set = nullptr; // the k_set_frame node of gx_a
+  int g_nodes_a = 0, g_nodes_b = 0;
+  bool g_failed = false;               // capture was refused once: the lane launches its kernels directly
 };
 
 struct LpfFusedPlan;  // detect_fused.cu
@@ -96,6 +108,8 @@ struct lpf_ctx {
   float* cube_cache = nullptr;      // [n_back + n_lanes][B][N]
   uint8_t* cache_ok = nullptr;      // [n_back + n_lanes][B + 1]
   long long* cache_t = nullptr;     // [n_back + n_lanes], -1 = empty
+  cudaStream_t cap_st = nullptr;    // stream the lanes' graphs are captured on
+  const LpfFrameDesc* cap_fd = nullptr;   // non-null while a capture is in progress: the launchers point the kernels at it
   cudaStream_t chain_st = nullptr;  // the association steps of all frames, in frame order (highest priority)
   cudaEvent_t ring_ev = nullptr;    // after the ring steps (append, backward fill) of the latest frame
   bool ring_valid = false;
@@ -144,6 +158,7 @@ int lpf_launch_qc_sum(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stat
                       cudaStream_t st);
 int lpf_qc2_blocks(const lpf_ctx* c);
 int lpf_qs_blocks(const lpf_ctx* c);
+int lpf_qc_prepare(void);
 int lpf_launch_qc_running(lpf_ctx* c, LpfLane& L, const float* d_cube, uint8_t* d_band_ok, cudaStream_t st);
 
 int lpf_launch_sum_plane(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, bool want_sum, cudaStream_t st);

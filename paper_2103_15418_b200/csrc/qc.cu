@@ -55,6 +55,7 @@ __device__ __forceinline__ bool last_block_done(int32_t* counter, int total) {
 }
 
 struct QcArgs {
+  const LpfFrameDesc* fd;   // non-null: cube comes from the frame descriptor
   const float* cube; const uint8_t* W; long long N; int first_valid, B, nblk;
   double* part1;          // [B][nblk][3]
   float qc_clip, tau;
@@ -403,6 +404,7 @@ __device__ __forceinline__ float2 q_add2(float2 a, float2 b) { return __fadd2_rn
 __device__ __forceinline__ float2 q_fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
 
 struct QsArgs {
+  const LpfFrameDesc* fd;   // non-null: cube and seq come from the frame descriptor
   const float* cube; const uint8_t* W; long long N; int first_valid, B;
   double* part1;          // [B][gridDim.x][3]
   float* sum_out;         // [N] or null
@@ -515,7 +517,9 @@ __device__ __forceinline__ void qs_moments_group(const QsArgs& a, int g0, long l
 }
 
 __global__ void __launch_bounds__(QS_THREADS, LPF_QS_BLOCKS)
-k_qc_moments(const QsArgs a) {
+k_qc_moments(const QsArgs a_in) {
+  QsArgs a = a_in;
+  if (a.fd) { a.cube = a.fd->cube; a.seq = a.fd->seq; }
   extern __shared__ float4 qs_slots[];     // [QS_BG][QS_THREADS]
   __shared__ float s_piv[LPF_MAX_BANDS];
   __shared__ double s_red[QS_WARPS][QS_BG][2];
@@ -555,7 +559,9 @@ __device__ __forceinline__ void block_sum3(double& a, double& b, double& c) {
 
 // one block per band sums that band's partials (one load round); the last block to finish evaluates eq. A.1
 __global__ void __launch_bounds__(QC_THREADS)
-k_qc_verdict(const QvArgs a) {
+k_qc_verdict(const QvArgs a_in) {
+  QvArgs a = a_in;
+  if (a.q.fd) { a.q.cube = a.q.fd->cube; a.seq = a.q.fd->seq; }
   const int b = blockIdx.x, nblk = a.q.nblk;
   double n = 0, s1 = 0, s2 = 0;
   for (int i = threadIdx.x; i < nblk; i += QC_THREADS) {
@@ -576,6 +582,7 @@ k_qc_verdict(const QvArgs a) {
 }
 
 struct QkArgs {
+  const LpfFrameDesc* fd;
   const float* cube; const uint8_t* W; const uint8_t* band_ok; long long N; int B;
   const float* band_clip;  // [B][2]
   double* part2;           // [gridDim.x][B][3]
@@ -659,7 +666,9 @@ __device__ __forceinline__ void qs_clip_group(const QkArgs& a, int g0, long long
 }
 
 __global__ void __launch_bounds__(QS_THREADS, LPF_QS_BLOCKS)
-k_qc_clip(const QkArgs a) {
+k_qc_clip(const QkArgs a_in) {
+  QkArgs a = a_in;
+  if (a.fd) a.cube = a.fd->cube;
   extern __shared__ float4 qs_slots[];     // [QS_BG][QS_THREADS]
   __shared__ float s_c[LPF_MAX_BANDS], s_w[LPF_MAX_BANDS];
   __shared__ uint8_t s_ok[LPF_MAX_BANDS + 1];
@@ -867,6 +876,12 @@ static cudaError_t qs_attr() {
   return e;
 }
 
+// the kernel attributes, once per process, outside any stream capture (lpf_create)
+int lpf_qc_prepare(void) {
+  LPF_CUDA(qs_attr());
+  return LPF_OK;
+}
+
 // the streaming form needs 128-bit loads of every band at the same pixel group
 static bool qc_streaming(const lpf_ctx* c, const float* d_cube) { return (c->N & 3) == 0 && (((uintptr_t)d_cube) & 15) == 0; }
 
@@ -876,12 +891,12 @@ static int qs_launch_moments(lpf_ctx* c, LpfLane& L, const float* d_cube, float*
   const int nblk = lpf_qs_blocks(c);
   L.dirty_seq = L.dirty_seq >= 0x7ffffff0 ? 1 : L.dirty_seq + 1;
   QsArgs m{};
-  m.cube = d_cube; m.W = c->W; m.N = c->N; m.first_valid = c->first_valid; m.B = c->p.B; m.part1 = L.qc_part1;
+  m.fd = c->cap_fd; m.cube = d_cube; m.W = c->W; m.N = c->N; m.first_valid = c->first_valid; m.B = c->p.B; m.part1 = L.qc_part1;
   m.sum_out = want_sum ? L.sum_plane : nullptr; m.dirty_b = L.dirty_b; m.seq = L.dirty_seq;
   LPF_CUDA(qs_attr());
   LPF_KLAUNCH(c, KID_QC_PASS1, st, k_qc_moments<<<nblk, QS_THREADS, QS_SMEM, st>>>(m));
   QvArgs v{};
-  v.q.cube = d_cube; v.q.W = c->W; v.q.N = c->N; v.q.first_valid = c->first_valid; v.q.B = c->p.B; v.q.nblk = nblk;
+  v.q.fd = c->cap_fd; v.q.cube = d_cube; v.q.W = c->W; v.q.N = c->N; v.q.first_valid = c->first_valid; v.q.B = c->p.B; v.q.nblk = nblk;
   v.q.part1 = L.qc_part1; v.q.qc_clip = c->p.qc_clip; v.q.tau = c->p.qc_tau; v.q.stats = d_stats; v.q.band_ok = d_band_ok;
   v.q.band_clip = L.qc_band_clip; v.q.counter = L.qc_counter; v.q.big_thr = L.big_thr; v.q.big_sigma = lpf_fused_big_sigma();
   v.dirty_b = L.dirty_b; v.seq = L.dirty_seq; v.dirty = L.dirty; v.zero_me = zero_me; v.mom = L.qc_mom;
@@ -893,7 +908,7 @@ static int qs_launch_clip(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_
                           cudaStream_t st) {
   const int nblk = lpf_qs_blocks(c);
   QkArgs k{};
-  k.cube = d_cube; k.W = c->W; k.band_ok = d_band_ok; k.N = c->N; k.B = c->p.B; k.band_clip = L.qc_band_clip; k.part2 = L.qc_part2;
+  k.fd = c->cap_fd; k.cube = d_cube; k.W = c->W; k.band_ok = d_band_ok; k.N = c->N; k.B = c->p.B; k.band_clip = L.qc_band_clip; k.part2 = L.qc_part2;
   k.sum_out = want_sum ? L.sum_plane : nullptr;
   LPF_CUDA(qs_attr());
   LPF_KLAUNCH(c, KID_QC_PASS2, st, k_qc_clip<<<nblk, QS_THREADS, QS_SMEM, st>>>(k));
