@@ -496,30 +496,36 @@ struct Sweep {
     if (!FAST && (fl & FL_ICR_PF)) load_rows(ic0, y0 + RB - LAG_B, pl.icr);
 
     // ---- stage C: S = box(V2) / count at sigma ; eq. 5 for the row ; hits ------------------------------
+    // (both rows' arithmetic first, in one block with stages A2 and B for the instruction scheduler; then the hits)
     if ((FAST || (fl & (FL_C0 | FL_C1))) && !(LPF_EXP_SKIP & 1)) {
+      float2 s0[RB], s1[RB], m0[RB], m1[RB];
+      float mm[RB];
 #pragma unroll
       for (int j = 0; j < RB; ++j) {
-        if (!FAST && !(fl & (FL_C0 << j))) continue;          // uniform
         float2 b01, b23;
         hbox25(O_EV2 + (pbuf * RB + j) * PEV + 4 * tid, O_ET2 + (pbuf * RB + j) * PET + tid, b01, b23);
         float2 ic0, ic1;
         if (!FAST && (fl & FL_ICS_LD)) { ic0 = make_float2(pl.ics[j].x, pl.ics[j].y); ic1 = make_float2(pl.ics[j].z, pl.ics[j].w); }
         else { ic0 = splat(a.ic_const); ic1 = ic0; }
-        const float2 s0 = mul2(b01, ic0), s1 = mul2(b23, ic1);
-        const float2 k0 = mul2(s0, splat(a.kappa2)), k1 = mul2(s1, splat(a.kappa2));
+        s0[j] = mul2(b01, ic0); s1[j] = mul2(b23, ic1);
+        const float2 k0 = mul2(s0[j], splat(a.kappa2)), k1 = mul2(s1[j], splat(a.kappa2));
         // d^2 - kappa^2 S > 0 somewhere in the thread's pixels?  (the sign of the difference is exact; k_peaks
         // applies the guarded, rounded test)
-        const float2 m0 = fma2(dlag[j][0], dlag[j][0], neg2(k0)), m1 = fma2(dlag[j][1], dlag[j][1], neg2(k1));
-        const float mm = fmaxf(fmaxf(m0.x, m0.y), fmaxf(m1.x, m1.y));
-        if (mm > 0.f) {
+        m0[j] = fma2(dlag[j][0], dlag[j][0], neg2(k0)); m1[j] = fma2(dlag[j][1], dlag[j][1], neg2(k1));
+        mm[j] = fmaxf(fmaxf(m0[j].x, m0[j].y), fmaxf(m1[j].x, m1[j].y));
+        if (!FAST && !(fl & (FL_C0 << j))) mm[j] = -1.f;      // not an output row of this item
+      }
+#pragma unroll
+      for (int j = 0; j < RB; ++j) {
+        if (mm[j] > 0.f) {
           unsigned bits = 0u;
-          if (dlag[j][0].x > 0.f && m0.x > 0.f) bits |= 1u;
-          if (dlag[j][0].y > 0.f && m0.y > 0.f) bits |= 2u;
-          if (dlag[j][1].x > 0.f && m1.x > 0.f) bits |= 4u;
-          if (dlag[j][1].y > 0.f && m1.y > 0.f) bits |= 8u;
+          if (dlag[j][0].x > 0.f && m0[j].x > 0.f) bits |= 1u;
+          if (dlag[j][0].y > 0.f && m0[j].y > 0.f) bits |= 2u;
+          if (dlag[j][1].x > 0.f && m1[j].x > 0.f) bits |= 4u;
+          if (dlag[j][1].y > 0.f && m1[j].y > 0.f) bits |= 8u;
           bits &= umask;
           if (bits)
-            emit_hits(bits, y0 + j - LAG_C, dlag[j][0], dlag[j][1], s0, s1, fs[j][0], fs[j][1], fs[j + 1][0], fs[j + 1][1],
+            emit_hits(bits, y0 + j - LAG_C, dlag[j][0], dlag[j][1], s0[j], s1[j], fs[j][0], fs[j][1], fs[j + 1][0], fs[j + 1][1],
                       fs[j + 2][0], fs[j + 2][1]);
         }
       }
@@ -532,8 +538,6 @@ struct Sweep {
     stage_a1(b + 1, fl_next, y0);
     sync_wait(b);
     tm_wait_st();
-    // every warp has read the input stage of iteration b: thread 0 refills it
-    if (tid == 0 && b + XST < nb) issue_rows(b + XST);
   }
 
   __device__ __forceinline__ void run() {
@@ -553,11 +557,14 @@ struct Sweep {
       // the two rare repairs of the running sums live in the slow form of the iteration only: the interior form
       // has no call in it
       const float hot = fmaxf(amax4(fold[0][0], fold[0][1]), amax4(fold[1][0], fold[1][1]));
-      const bool fix1 = __any_sync(0xffffffffu, hot * hot > big2);
-      const bool fix2 = __any_sync(0xffffffffu, want_fix2);
-      want_fix2 = false;
-      if (f0 == FL_FAST && !fix1 && !fix2) iteration<true>(b, f0, f1, false, false);
-      else iteration<false>(b, f0, f1, fix1, fix2);
+      const bool h1 = hot * hot > big2;
+      if (f0 == FL_FAST && !__any_sync(0xffffffffu, h1 || want_fix2)) {
+        iteration<true>(b, f0, f1, false, false);
+      } else {
+        const bool fix1 = __any_sync(0xffffffffu, h1), fix2 = __any_sync(0xffffffffu, want_fix2);
+        want_fix2 = false;
+        iteration<false>(b, f0, f1, fix1, fix2);
+      }
       f0 = f1; f1 = f2; f2 = f3;
     }
     tm_wait_ld();        // the reads issued for an iteration past the end
@@ -565,7 +572,7 @@ struct Sweep {
 };
 
 template <int NW>
-__global__ void __launch_bounds__(NW * 32, NW > 4 ? 1 : 2)
+__global__ void __launch_bounds__(NW * 32 + 32, NW > 4 ? 1 : 2)
 k_sweep(const FusedArgs a) {
   __shared__ uint32_t s_tmem;
   __shared__ FusedArgs s_args;
@@ -589,9 +596,10 @@ k_sweep(const FusedArgs a) {
   s.want_fix2 = false;
   s.seg = a.hits + (long long)segi * a.seg_cap;
   if (s.tid == 0) s_args = a;
-  constexpr int NT = SW::NT;
-  for (int i = s.tid; i < (SW::O_FL >> 2); i += NT) g_sm4[i] = zero4();
-  s.flp = a.flags + it.fl_off + s.warp;
+  constexpr int NT = SW::NT + 32;           // NW sweep warps + the input warp
+  for (int i = s.tid; i < ((SW::O_FL + 3) >> 2); i += NT) g_sm4[i] = zero4();
+  const bool sweeper = s.warp < NW;
+  s.flp = a.flags + it.fl_off + (sweeper ? s.warp : 0);
   if (s.warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n"
                  ::"l"((uint64_t)__cvta_generic_to_shared(&s_tmem)), "n"(TM_COLS));
@@ -603,20 +611,22 @@ k_sweep(const FusedArgs a) {
   if (s.tid == 0) {
 #pragma unroll
     for (int i = 0; i < XST; ++i) mbar_init(s.bar_addr(i), 1);
-    mbar_init(s.bar_addr(XST), NW);
+    mbar_init(s.bar_addr(XST), NW + 1);       // one arrival per sweep warp + the input warp's
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
   asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");   // the zero fill above precedes the bulk copies
   const uint32_t tm_base = s_tmem;
   // warp w reaches the 32 lanes (w mod 4) * 32 ...; warps w and w+4 share them on different columns
   s.tm = tm_base + ((uint32_t)((s.warp & 3) * 32) << 16) + (uint32_t)(s.warp >> 2) * 256u;
-  for (int i = 0; i < 2 * DR; ++i) tm_st4(s.tm + 4 * i, splat(0.f), splat(0.f));
-  tm_wait_st();
+  if (sweeper) {
+    for (int i = 0; i < 2 * DR; ++i) tm_st4(s.tm + 4 * i, splat(0.f), splat(0.f));
+    tm_wait_st();
+  }
 
   const long long N = (long long)a.Dy * a.Dx;
   const float* X = (p < a.B) ? (a.fd ? a.fd->cube : a.cube) + (long long)p * N : a.sum_plane;
   const int x = it.xs + 4 * s.tid;
-  s.col_in = 4 * s.tid < a.CW && x < a.Dx;
+  s.col_in = sweeper && 4 * s.tid < a.CW && x < a.Dx;
   s.umask = 0u;
 #pragma unroll
   for (int k = 0; k < 4; ++k)
@@ -642,14 +652,22 @@ k_sweep(const FusedArgs a) {
 #pragma unroll
   for (int j = 0; j < RB; ++j) { s.pl.nm[j] = zero4(); s.pl.icr[j] = zero4(); s.pl.ics[j] = zero4(); }
   __syncthreads();
-  if (s.tid == 0)
+  if (sweeper) {
+    s.run();
+    tm_wait_st();
+  } else if (s.lane == 0) {
+    // the input warp: one thread keeps the 16-stage ring of input rows full.  It takes part in the iteration barrier
+    // (its arrival is always early), so it learns that every sweep warp has read the stage of iteration b the moment
+    // the barrier of b completes, and its copies never sit on a sweep warp's path.
     for (int bb = 0; bb < XST && bb < it.nb; ++bb) s.issue_rows(bb);
-
-  s.run();
-
-  if (s.tid == 0)                   // no bulk copy may be in flight when the CTA leaves
+    for (int b = 0; b < it.nb; ++b) {
+      mbar_arrive(s.bar_addr(XST));
+      s.sync_wait(b);
+      if (b + XST < it.nb) s.issue_rows(b + XST);
+    }
+    // no bulk copy may be in flight when the CTA leaves
     for (int bb = it.nb > XST ? it.nb - XST : 0; bb < it.nb; ++bb) mbar_wait(s.bar_addr(bb & (XST - 1)), (uint32_t)(bb / XST) & 1u);
-  tm_wait_st();
+  }
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
   __syncthreads();
   if (s.tid == 0) {
@@ -824,7 +842,7 @@ static size_t fused_smem_bytes(int NW) {
 template <int NW>
 static cudaError_t fused_launch_t(const FusedArgs& a, dim3 grid, size_t smem, cudaStream_t st, bool set_attr) {
   if (set_attr) return cudaFuncSetAttribute(k_sweep<NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  k_sweep<NW><<<grid, NW * 32, smem, st>>>(a);
+  k_sweep<NW><<<grid, NW * 32 + 32, smem, st>>>(a);
   return cudaSuccess;
 }
 
@@ -1013,7 +1031,7 @@ int lpf_fused_plan(lpf_ctx* c, const uint8_t* hW, LpfFusedPlan** out) {
   static_assert((FL_NM_LD << 3) == FL_NM_PF && (FL_ICR_LD << 3) == FL_ICR_PF && (FL_ICS_LD << 3) == FL_ICS_PF, "flag layout");
 
   LpfFusedPlan* pl = new LpfFusedPlan();
-  pl->CW = CW; pl->NW = NW; pl->threads = NW * 32; pl->n_items = (int)ditems.size();
+  pl->CW = CW; pl->NW = NW; pl->threads = NW * 32 + 32; pl->n_items = (int)ditems.size();
   pl->smem = fused_smem_bytes(NW);
   (void)max_nb;
   if ((long long)pl->n_items * c->n_planes > 65535) { delete pl; return LPF_OK; }   // grid.y of k_peaks
