@@ -206,8 +206,14 @@ int lpf_simulate_pulses(int32_t n, int32_t B, int32_t T, const float* d_nu, floa
 
 /* -- whole step --------------------------------------------------------------
  * qc -> detect -> associate -> flux -> append for one cube on one lane, results in lane-owned
- * buffers (lpf_frame_view).  Frames on different lanes/streams overlap; the association chain is
- * ordered across lanes with an event.  Issue in increasing t. */
+ * buffers (lpf_frame_view).  Frames on different lanes / streams overlap.  Contract: issue the calls in increasing t;
+ * one stream per lane (a lane's buffers are reused by its next frame in stream order); with n_lanes lanes use them
+ * round robin (the backward-fill cache holds n_back + n_lanes cubes: a lane that runs more than n_lanes frames ahead
+ * of another would overwrite a cube that a frame in flight still needs).  Across lanes the context orders two
+ * things itself: the association steps (all frames, in frame order, on a stream of its own) and the ring steps (an
+ * event).  On the fused path with an aligned cube, no eq. A.2 and no backward fill, the lane's kernels are launched
+ * as two CUDA graphs built at the lane's first frame; d_cube and t may change freely from call to call.
+ * lpf_add_candidates synchronises the device (the table is shared with every frame in flight). */
 int lpf_process_frame(lpf_ctx* ctx, int lane, const float* d_cube, int64_t t, void* stream);
 int lpf_get_frame_view(lpf_ctx* ctx, int lane, lpf_frame_view* out);
 
