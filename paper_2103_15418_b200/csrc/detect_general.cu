@@ -147,12 +147,204 @@ k_sepconv(const ConvArgs a) {
   }
 }
 
+// ---- the wide form: radius 3 (matched filter), 12 or 16 on images whose rows are whole float4 groups ---------------
+// A 128 x 64 output tile (halo amplification 1.9 instead of 3 at radius 16).  Staging: a thread loads the same float4
+// group of two tile rows half a tile apart (mask word, values, for the spread also C: all loads of a round issued
+// before the first is used) and stores the two rows interleaved, so that one 128-bit shared load in the row pass
+// gives two ready f32x2 pairs (lanes <-> consecutive row pairs, pitch chosen for conflict-free 128-bit loads).  The
+// column pass pairs two neighbouring columns.  Both passes are packed FFMA2 with the taps applied in the same order
+// as in k_sepconv, so the two forms give the same bits.  RL: the halo staged (a multiple of 4 >= R: groups stay
+// aligned).
+constexpr int WTX = 128, WTY = 64, WPIN = 162, WPT = 132, WU = 4;
+
+template <int MODE>
+__device__ __forceinline__ float4 wide_value(float4 v, float4 cv, unsigned w) {
+  if (MODE == MODE_DEN) v = make_float4(1.f, 1.f, 1.f, 1.f);
+  if (MODE == MODE_S) {
+    const float d0 = v.x - cv.x, d1 = v.y - cv.y, d2 = v.z - cv.z, d3 = v.w - cv.w;
+    v = make_float4(d0 * d0, d1 * d1, d2 * d2, d3 * d3);
+  }
+  if (!(w & 0x000000ffu)) v.x = 0.f;      // selects, not products: an invalid pixel may hold anything
+  if (!(w & 0x0000ff00u)) v.y = 0.f;
+  if (!(w & 0x00ff0000u)) v.z = 0.f;
+  if (!(w & 0xff000000u)) v.w = 0.f;
+  return v;
+}
+
+__device__ __forceinline__ unsigned wide_mask(unsigned w, unsigned yy) {     // W and not Y, per byte
+  if (yy & 0x000000ffu) w &= ~0x000000ffu;
+  if (yy & 0x0000ff00u) w &= ~0x0000ff00u;
+  if (yy & 0x00ff0000u) w &= ~0x00ff0000u;
+  if (yy & 0xff000000u) w &= ~0xff000000u;
+  return w;
+}
+
+template <int MODE, int R, int RL>
+__global__ void __launch_bounds__(CT, 2)
+k_sepconv_wide(const ConvArgs a) {
+  extern __shared__ float4 sm4[];
+  constexpr int TYH = WTY + 2 * RL, NG = (WTX + 2 * RL) / 4, HALF = TYH / 2, OFF = RL - R;
+  static_assert(RL % 4 == 0 && RL >= R && RL <= 16 && 4 * NG <= WPIN, "wide form: staged halo");
+  float* s_in = reinterpret_cast<float*>(sm4);      // [HALF][WPIN] pairs: (row r, row r + HALF)
+  float* s_tmp = s_in + TYH * WPIN;                 // [TYH][WPT]
+  const int p = blockIdx.z;
+  if (!plane_active(a.band_ok, a.B, p)) return;
+  const long long N = (long long)a.Dy * a.Dx;
+  const float* src_p = nullptr;
+  if (MODE == MODE_MF) src_p = (p < a.B) ? a.src + (long long)p * N : a.src_sum;
+  else if (MODE != MODE_DEN) src_p = a.src + (long long)p * N;
+  const float* C_p = (MODE == MODE_S) ? a.Cpl + (long long)p * N : nullptr;
+  const uint8_t* Y_p = (a.Y && MODE != MODE_MF) ? a.Y + (long long)p * N : nullptr;
+  const int x0 = blockIdx.x * WTX, y0 = blockIdx.y * WTY;
+
+  // staging: items (row pair, group), WU items per round
+  for (int i0 = threadIdx.x; i0 < HALF * NG; i0 += WU * CT) {
+    unsigned w[WU][2];
+    float4 v[WU][2], cv[WU][2];
+    long long q[WU][2];
+    bool in[WU][2];
+#pragma unroll
+    for (int u = 0; u < WU; ++u) {
+      const int i = i0 + u * CT;
+      const int r = i / NG, g = i - r * NG;
+      const int x = x0 - RL + 4 * g;
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int y = y0 - RL + r + h * HALF;
+        in[u][h] = i < HALF * NG && y >= 0 && y < a.Dy && x >= 0 && x < a.Dx;   // Dx % 4 == 0: a group is inside or outside as a whole
+        q[u][h] = in[u][h] ? (long long)y * a.Dx + x : 0;
+        w[u][h] = in[u][h] ? __ldg(reinterpret_cast<const unsigned*>(a.W + q[u][h])) : 0u;
+      }
+    }
+    if (Y_p) {
+#pragma unroll
+      for (int u = 0; u < WU; ++u)
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+          if (in[u][h]) w[u][h] = wide_mask(w[u][h], *reinterpret_cast<const unsigned*>(Y_p + q[u][h]));
+    }
+#pragma unroll
+    for (int u = 0; u < WU; ++u)
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        v[u][h] = make_float4(0.f, 0.f, 0.f, 0.f); cv[u][h] = v[u][h];
+        if (MODE != MODE_DEN && in[u][h]) v[u][h] = *reinterpret_cast<const float4*>(src_p + q[u][h]);
+        if (MODE == MODE_S && in[u][h]) cv[u][h] = *reinterpret_cast<const float4*>(C_p + q[u][h]);
+      }
+#pragma unroll
+    for (int u = 0; u < WU; ++u) {
+      const int i = i0 + u * CT;
+      if (i < HALF * NG) {
+        const int r = i / NG, g = i - r * NG;
+        const float4 va = wide_value<MODE>(v[u][0], cv[u][0], w[u][0]), vb = wide_value<MODE>(v[u][1], cv[u][1], w[u][1]);
+        float4* dst = reinterpret_cast<float4*>(s_in + 2 * (r * WPIN + 4 * g));
+        dst[0] = make_float4(va.x, vb.x, va.y, vb.y);
+        dst[1] = make_float4(va.z, vb.z, va.w, vb.w);
+      }
+    }
+  }
+  __syncthreads();
+
+  // row pass: an item = rows (r, r + HALF) x 8 output columns
+  for (int it = threadIdx.x; it < HALF * (WTX / 8); it += CT) {
+    const int r = it % HALF, cg = it / HALF;
+    const float* rp = s_in + 2 * (r * WPIN + cg * 8 + OFF);
+    float2 v[8 + 2 * R];
+    if (OFF % 2 == 0) {
+#pragma unroll
+      for (int i = 0; i < (8 + 2 * R) / 2; ++i) {
+        const float4 x2 = reinterpret_cast<const float4*>(rp)[i];
+        v[2 * i] = make_float2(x2.x, x2.y); v[2 * i + 1] = make_float2(x2.z, x2.w);
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < 8 + 2 * R; ++i) v[i] = reinterpret_cast<const float2*>(rp)[i];
+    }
+    float2 acc[8];
+#pragma unroll
+    for (int o = 0; o < 8; ++o) {
+      acc[o] = make_float2(0.f, 0.f);
+#pragma unroll
+      for (int i = 0; i <= 2 * R; ++i) acc[o] = __ffma2_rn(make_float2(a.g.g[i], a.g.g[i]), v[o + i], acc[o]);
+    }
+    float4* oa = reinterpret_cast<float4*>(s_tmp + r * WPT + cg * 8);
+    float4* ob = reinterpret_cast<float4*>(s_tmp + (r + HALF) * WPT + cg * 8);
+    oa[0] = make_float4(acc[0].x, acc[1].x, acc[2].x, acc[3].x); oa[1] = make_float4(acc[4].x, acc[5].x, acc[6].x, acc[7].x);
+    ob[0] = make_float4(acc[0].y, acc[1].y, acc[2].y, acc[3].y); ob[1] = make_float4(acc[4].y, acc[5].y, acc[6].y, acc[7].y);
+  }
+  __syncthreads();
+
+  // column pass: a thread = columns (2 cp, 2 cp + 1) x 16 output rows, in two blocks of 8
+  {
+    const int cp = threadIdx.x % (WTX / 2), rg = threadIdx.x / (WTX / 2);   // rg in 0..3
+    const int x = x0 + 2 * cp;
+#pragma unroll 1
+    for (int blk = 0; blk < 2; ++blk) {
+      const int ry = rg * 16 + blk * 8;
+      const float* col = s_tmp + (ry + OFF) * WPT + 2 * cp;
+      float2 v[8 + 2 * R];
+#pragma unroll
+      for (int j = 0; j < 8 + 2 * R; ++j) v[j] = *reinterpret_cast<const float2*>(col + j * WPT);
+      float2 acc[8];
+#pragma unroll
+      for (int o = 0; o < 8; ++o) {
+        acc[o] = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int j = 0; j <= 2 * R; ++j) acc[o] = __ffma2_rn(make_float2(a.g.g[j], a.g.g[j]), v[o + j], acc[o]);
+      }
+      if (x < a.Dx) {
+#pragma unroll
+        for (int o = 0; o < 8; ++o) {
+          const int y = y0 + ry + o;
+          if (y >= a.Dy) break;
+          const long long q = (long long)y * a.Dx + x;
+          float2 r;
+          if (MODE == MODE_DEN) {
+            const uint8_t w0 = a.W[q], w1 = a.W[q + 1];
+            r.x = (w0 && acc[o].x > 0.f) ? 1.0f / acc[o].x : 0.f;
+            r.y = (w1 && acc[o].y > 0.f) ? 1.0f / acc[o].y : 0.f;
+          } else {
+            const float2 nm = *reinterpret_cast<const float2*>(a.norm + (a.norm_per_plane ? (long long)p * N + q : q));
+            r.x = acc[o].x * nm.x; r.y = acc[o].y * nm.y;
+          }
+          *reinterpret_cast<float2*>(a.out + ((MODE == MODE_DEN && !a.band_ok) ? q : (long long)p * N + q)) = r;
+        }
+      }
+    }
+  }
+}
+
+template <int R> struct WideHalo { static constexpr int RL = (R + 3) / 4 * 4; };
+
+template <int MODE, int R>
+cudaError_t sepconv_wide_attr() {
+  constexpr int RL = WideHalo<R>::RL;
+  constexpr size_t smem = (size_t)(WTY + 2 * RL) * (WPIN + WPT) * sizeof(float);
+  return cudaFuncSetAttribute(k_sepconv_wide<MODE, R, RL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+}
+
+template <int MODE, int R>
+int launch_sepconv_wide(lpf_ctx* c, int kid, const ConvArgs& a, cudaStream_t st) {
+  constexpr int RL = WideHalo<R>::RL;
+  constexpr size_t smem = (size_t)(WTY + 2 * RL) * (WPIN + WPT) * sizeof(float);
+  const dim3 grid((a.Dx + WTX - 1) / WTX, (a.Dy + WTY - 1) / WTY, a.n_planes);
+  LPF_KLAUNCH(c, kid, st, k_sepconv_wide<MODE, R, RL><<<grid, CT, smem, st>>>(a));
+  return LPF_OK;
+}
+
 template <int MODE>
 int launch_sepconv(lpf_ctx* c, const ConvArgs& a, cudaStream_t st) {
   const int R = a.g.R;
+  const int kid = MODE == MODE_MF ? KID_CONV_MF : MODE == MODE_C ? KID_CONV_C : MODE == MODE_S ? KID_CONV_S : KID_CONV_DEN;
+  // the wide form loads 128 bits at a time: rows of whole groups, and a caller's cube on a 16-byte boundary
+  const bool al16 = (reinterpret_cast<uintptr_t>(a.src) & 15u) == 0 && (reinterpret_cast<uintptr_t>(a.src_sum) & 15u) == 0;
+  if (a.Dx % 4 == 0 && al16) {
+    if (R == 3) return launch_sepconv_wide<MODE, 3>(c, kid, a, st);
+    if (R == 12) return launch_sepconv_wide<MODE, 12>(c, kid, a, st);
+    if (R == 16) return launch_sepconv_wide<MODE, 16>(c, kid, a, st);
+  }
   const dim3 grid((a.Dx + TX - 1) / TX, (a.Dy + TY - 1) / TY, a.n_planes);
   const size_t smem = (size_t)((TY + 2 * R) * (((TX + 2 * R) | 1) + (TX + 1))) * sizeof(float);
-  const int kid = MODE == MODE_MF ? KID_CONV_MF : MODE == MODE_C ? KID_CONV_C : MODE == MODE_S ? KID_CONV_S : KID_CONV_DEN;
   switch (R) {
     case 3: LPF_KLAUNCH(c, kid, st, k_sepconv<MODE, 3><<<grid, CT, smem, st>>>(a)); break;
     case 12: LPF_KLAUNCH(c, kid, st, k_sepconv<MODE, 12><<<grid, CT, smem, st>>>(a)); break;
@@ -222,7 +414,98 @@ k_threshold_peaks(const ThrArgs a) {
   }
 }
 
+// The same for four pixels per thread (N % 4 == 0, Dx % 4 == 0): 128-bit loads of F, C, S, word loads of W and Y.
+// Eq. 6 is tested by the warp together: for every pixel of the warp that passed eq. 5, lane l looks at neighbour l of
+// the (2 k_max + 1)^2 window (in rounds of 32), so a hit costs the warp a dozen instructions instead of a serial loop.
+__global__ void __launch_bounds__(256)
+k_threshold_peaks4(const ThrArgs a) {
+  const int p = blockIdx.z;
+  if (!plane_active(a.band_ok, a.B, p)) return;
+  const long long N = (long long)a.Dy * a.Dx;
+  const long long pix0 = 4 * ((long long)blockIdx.x * blockDim.x + threadIdx.x);
+  const float* F = a.F + (long long)p * N;
+  const int lane = threadIdx.x & 31;
+  unsigned hits = 0u, peaks = 0u;
+  float f[4] = {0.f, 0.f, 0.f, 0.f}, cc[4] = {0.f, 0.f, 0.f, 0.f}, se[4] = {0.f, 0.f, 0.f, 0.f}, d[4] = {0.f, 0.f, 0.f, 0.f};
+  if (pix0 < N) {
+    unsigned w = *reinterpret_cast<const unsigned*>(a.W + pix0);
+    unsigned yy = 0u;
+    if (a.Y) { yy = *reinterpret_cast<const unsigned*>(a.Y + (long long)p * N + pix0); w = wide_mask(w, yy); }
+    if (w) {
+      const float4 f4 = *reinterpret_cast<const float4*>(F + pix0);
+      const float4 c4 = *reinterpret_cast<const float4*>(a.C + (long long)p * N + pix0);
+      const float4 s4 = *reinterpret_cast<const float4*>(a.S + (long long)p * N + pix0);
+      const float fv[4] = {f4.x, f4.y, f4.z, f4.w}, cv[4] = {c4.x, c4.y, c4.z, c4.w}, sv[4] = {s4.x, s4.y, s4.z, s4.w};
+      unsigned ynew = yy;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        if (!((w >> (8 * k)) & 0xffu)) continue;
+        f[k] = fv[k]; cc[k] = cv[k];
+        d[k] = f[k] - cc[k];
+        const float gd = a.eps_rel * fabsf(cc[k]);
+        se[k] = fmaxf(sv[k], gd * gd);
+        if (d[k] > 0.f && d[k] * d[k] > a.kappa2 * se[k]) { ynew |= (unsigned)(a.iter & 0xff) << (8 * k); hits |= 1u << k; }
+      }
+      if (a.Y && ynew != yy) *reinterpret_cast<unsigned*>(a.Y + (long long)p * N + pix0) = ynew;
+    }
+  }
+  if (!__any_sync(0xffffffffu, hits != 0u)) return;
+  const int side = 2 * a.k_max + 1, nwin = side * side;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    unsigned m = __ballot_sync(0xffffffffu, (hits >> k) & 1u);
+    while (m) {
+      const int src = __ffs(m) - 1;
+      m &= m - 1;
+      const long long pix = __shfl_sync(0xffffffffu, pix0, src) + k;
+      const float fc = __shfl_sync(0xffffffffu, f[k], src);
+      const int y = (int)(pix / a.Dx), x = (int)(pix - (long long)y * a.Dx);
+      bool beaten = false;
+      for (int n0 = 0; n0 < nwin; n0 += 32) {
+        const int n = n0 + lane;
+        if (n < nwin) {
+          const int yq = y + n / side - a.k_max, xx = x + n % side - a.k_max;
+          if (yq >= 0 && yq < a.Dy && xx >= 0 && xx < a.Dx) {
+            const long long q = (long long)yq * a.Dx + xx;
+            beaten = beaten || (a.W[q] && F[q] > fc);
+          }
+        }
+      }
+      if (!__any_sync(0xffffffffu, beaten) && lane == src) peaks |= 1u << k;
+    }
+  }
+  if (!__any_sync(0xffffffffu, peaks != 0u)) return;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const bool peak = (peaks >> k) & 1u;
+    const unsigned m = __ballot_sync(0xffffffffu, peak);
+    if (!m) continue;
+    int base = 0;
+    if (lane == (__ffs(m) - 1)) base = atomicAdd(a.ndets, __popc(m));
+    base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
+    if (peak) {
+      const int idx = base + __popc(m & ((1u << lane) - 1u));
+      if (idx < a.max_det) {
+        lpf_det r;
+        r.pix = (int32_t)(pix0 + k); r.plane = (int16_t)p; r.iter = (int16_t)a.iter;
+        r.f = f[k]; r.c = cc[k]; r.s = se[k]; r.snr = d[k] / sqrtf(se[k]);
+        a.dets[idx] = r;
+      } else {
+        atomicAdd(&a.counters[0], 1);
+      }
+    }
+  }
+}
+
 }  // namespace
+
+// kernel attributes of the wide form, once per process, outside any stream capture (lpf_create)
+int lpf_general_prepare(void) {
+#define LPF_WIDE_ATTR(M) LPF_CUDA((sepconv_wide_attr<M, 3>())); LPF_CUDA((sepconv_wide_attr<M, 12>())); LPF_CUDA((sepconv_wide_attr<M, 16>()));
+  LPF_WIDE_ATTR(MODE_MF) LPF_WIDE_ATTR(MODE_C) LPF_WIDE_ATTR(MODE_S) LPF_WIDE_ATTR(MODE_DEN)
+#undef LPF_WIDE_ATTR
+  return LPF_OK;
+}
 
 // norm = W / (g (*) W) for the static mask (R7).  d_tmp unused (kept for symmetry).
 int lpf_launch_static_norm(lpf_ctx* c, const LpfTaps& g, float* d_norm, float* /*d_tmp*/, cudaStream_t st) {
@@ -269,8 +552,13 @@ int lpf_launch_detect_general(lpf_ctx* c, LpfLane& L, const float* d_cube, const
     t.B = p.B; t.Dy = p.Dy; t.Dx = p.Dx; t.k_max = p.k_max; t.iter = it; t.max_det = p.max_det;
     t.kappa2 = p.kappa * p.kappa; t.eps_rel = p.eps_rel;
     t.dets = d_dets; t.ndets = d_ndets; t.counters = c->counters;
-    const dim3 grid((unsigned)((c->N + 255) / 256), 1, c->n_planes);
-    LPF_KLAUNCH(c, KID_THRESHOLD, st, k_threshold_peaks<<<grid, 256, 0, st>>>(t));
+    if (p.Dx % 4 == 0) {
+      const dim3 grid((unsigned)((c->N / 4 + 255) / 256), 1, c->n_planes);
+      LPF_KLAUNCH(c, KID_THRESHOLD, st, k_threshold_peaks4<<<grid, 256, 0, st>>>(t));
+    } else {
+      const dim3 grid((unsigned)((c->N + 255) / 256), 1, c->n_planes);
+      LPF_KLAUNCH(c, KID_THRESHOLD, st, k_threshold_peaks<<<grid, 256, 0, st>>>(t));
+    }
   }
   return LPF_OK;
 }

@@ -285,6 +285,7 @@ int lpf_create(lpf_ctx** out, const lpf_params* p, const uint8_t* d_valid_mask) 
     if (dirty) CUDAC(cudaMemcpy(c->W, hW.data(), N, cudaMemcpyHostToDevice));
     TRYC(dalloc(&c->norm_mf, N));
     TRYC(dalloc(&c->norm_bg, N));
+    TRYC(lpf_general_prepare());
     TRYC(lpf_launch_static_norm(c, c->g_mf, c->norm_mf, nullptr, 0));
     TRYC(lpf_launch_static_norm(c, c->g_bg, c->norm_bg, nullptr, 0));
     TRYC(lpf_fused_plan(c, hW.data(), &c->fused));   // reads norm_mf back for its interior constant

@@ -159,6 +159,7 @@ int lpf_launch_qc_sum(lpf_ctx* c, LpfLane& L, const float* d_cube, float* d_stat
 int lpf_qc2_blocks(const lpf_ctx* c);
 int lpf_qs_blocks(const lpf_ctx* c);
 int lpf_qc_prepare(void);
+int lpf_general_prepare(void);
 int lpf_launch_qc_running(lpf_ctx* c, LpfLane& L, const float* d_cube, uint8_t* d_band_ok, cudaStream_t st);
 
 int lpf_launch_sum_plane(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint8_t* d_band_ok, bool want_sum, cudaStream_t st);
