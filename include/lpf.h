@@ -173,7 +173,8 @@ int lpf_associate(lpf_ctx* ctx, int lane, const int32_t* d_upos, const int32_t* 
                   int32_t* d_act_pix, int32_t* d_npos, void* stream);
 
 /* Pre-load n forced positions (monitored for ever, BASELINE.json config 5) into the lowest free
- * slots; d_slots_out [n] (may be NULL).  Synchronises.  Returns LPF_E_STATE if the table is full. */
+ * slots; d_slots_out [n] (may be NULL).  Synchronises.  Returns LPF_E_STATE if the table is full and LPF_E_ARG if a
+ * position lies outside the image (checked on the device; nothing is added in either case). */
 int lpf_add_candidates(lpf_ctx* ctx, const int32_t* d_pix, int32_t n, int32_t* d_slots_out, void* stream);
 
 /* -- S11: forced peak flux (O9) --------------------------------
@@ -236,6 +237,18 @@ int lpf_process_frame_host_end(lpf_ctx* ctx, int lane, lpf_host_result* res, voi
  * LPF_W_CAPACITY when something was dropped since lpf_create (capacity overflow is never undefined behaviour:
  * the list is truncated and the drop counted). */
 int lpf_get_counters(lpf_ctx* ctx, int64_t* h_out);
+
+/* -- checkpoint / resume (optional; the method is a stream processor) ----------
+ * Everything a context carries from one frame to the next, as one opaque blob in HOST memory: the candidate table
+ * (PAPER.md:108), the dynamic-spectrum rings with their slot metadata, the drop counters, the running per-pixel state
+ * of eq. A.2 and the backward-fill cache of recent cubes.  lpf_state_bytes: size of the blob for this context.
+ * lpf_export_state: synchronises the device, then copies; `bytes` must be >= lpf_state_bytes.  lpf_import_state:
+ * synchronises, checks that the blob was written by a context with identical lpf_params and image size
+ * (LPF_E_ARG otherwise, nothing is changed), then overwrites the state: the next frame continues the exported
+ * stream bit for bit.  The caller owns the buffer. */
+int64_t lpf_state_bytes(const lpf_ctx* ctx);
+int lpf_export_state(lpf_ctx* ctx, void* h_buf, int64_t bytes);
+int lpf_import_state(lpf_ctx* ctx, const void* h_buf, int64_t bytes);
 
 /* Launch plan chosen at lpf_create: h_out[0] = 1 if the fused single-pass detection kernel is in use
  * (box K = 12, k_mf = 3, n_iter = 1, Dx % 4 == 0; otherwise the general multi-kernel path),

@@ -57,7 +57,7 @@ EXPORTS = [
     "lpf_create", "lpf_destroy", "lpf_cube_qc", "lpf_detect_sources", "lpf_associate", "lpf_add_candidates",
     "lpf_measure_flux", "lpf_append_dynspec", "lpf_get_dynspec", "lpf_process_frame", "lpf_get_frame_view",
     "lpf_process_frame_host", "lpf_process_frame_host_begin", "lpf_process_frame_host_end", "lpf_get_counters", "lpf_memcpy_d2h", "lpf_strerror", "lpf_last_cuda_error",
-    "lpf_export_dynspec", "lpf_simulate_pulses",
+    "lpf_export_dynspec", "lpf_simulate_pulses", "lpf_state_bytes", "lpf_export_state", "lpf_import_state",
     "lpf_version", "lpf_get_plan", "lpf_profile_begin", "lpf_profile_end", "lpf_profile_timeline", "lpf_profile_kernel_count", "lpf_profile_kernel_name",
 ]
 
@@ -95,6 +95,9 @@ def load_library(path: Optional[str] = None):
     lib.lpf_process_frame_host_end.argtypes = [vp, C.c_int, C.POINTER(LpfHostResult), vp]
     lib.lpf_get_counters.argtypes = [vp, C.POINTER(i64)]
     lib.lpf_memcpy_d2h.argtypes = [vp, vp, i64]
+    lib.lpf_state_bytes.argtypes = [vp]
+    lib.lpf_export_state.argtypes = [vp, vp, i64]
+    lib.lpf_import_state.argtypes = [vp, vp, i64]
     lib.lpf_strerror.argtypes = [C.c_int]
     lib.lpf_strerror.restype = C.c_char_p
     lib.lpf_last_cuda_error.restype = C.c_char_p
@@ -105,8 +108,9 @@ def load_library(path: Optional[str] = None):
     lib.lpf_profile_kernel_name.argtypes = [C.c_int]
     lib.lpf_profile_kernel_name.restype = C.c_char_p
     for n in EXPORTS:
-        if n not in ("lpf_strerror", "lpf_last_cuda_error", "lpf_profile_kernel_name"):
+        if n not in ("lpf_strerror", "lpf_last_cuda_error", "lpf_profile_kernel_name", "lpf_state_bytes"):
             getattr(lib, n).restype = C.c_int
+    lib.lpf_state_bytes.restype = i64
     if path == LIB_PATH:
         _lib = lib
     return lib
@@ -308,6 +312,19 @@ class LPF:
         if n < 0:
             _check(self.lib, n, "lpf_profile_timeline")
         return [(self.lib.lpf_profile_kernel_name(kid[i]).decode(), float(t0[i]), float(t1[i])) for i in range(n)]
+
+    def export_state(self) -> np.ndarray:
+        """Everything the context carries from frame to frame, as one host blob (lpf_export_state)."""
+        n = int(self.lib.lpf_state_bytes(self.h))
+        if n < 0:
+            _check(self.lib, n, "lpf_state_bytes")
+        buf = np.empty(n, np.uint8)
+        _check(self.lib, self.lib.lpf_export_state(self.h, buf.ctypes.data, n), "lpf_export_state")
+        return buf
+
+    def import_state(self, buf: np.ndarray) -> None:
+        buf = np.ascontiguousarray(buf, dtype=np.uint8)
+        _check(self.lib, self.lib.lpf_import_state(self.h, buf.ctypes.data, buf.nbytes), "lpf_import_state")
 
     def counters(self) -> dict:
         h = (C.c_int64 * 4)()

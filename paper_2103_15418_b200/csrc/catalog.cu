@@ -305,6 +305,8 @@ k_assoc(const AssocArgs a, int Dy, int Dx, int r, long long* matched_t) {
 struct AddArgs {
   uint8_t* active; uint8_t* forced; int32_t* cpix; int32_t* miss; long long* born; int32_t* slotmap;
   int32_t* free_list; int n_cand_max; const int32_t* pix; int n; int32_t* slots_out; int32_t* status;
+  int n_pix;        // pixels of the image: a position outside [0, n_pix) refuses the whole call (status 2)
+  int32_t* n_active; // the context's count of active candidates
 };
 
 __global__ void __launch_bounds__(1024)
@@ -320,13 +322,16 @@ k_add_candidates(const AddArgs a) {
   for (int s = s0; s < s1; ++s) if (!a.active[s]) a.free_list[off++] = s;
   __syncthreads();
   if (n_free < a.n) { if (tid == 0) *a.status = 1; return; }
+  int bad = 0;
+  for (int i = tid; i < a.n; i += T) bad |= (a.pix[i] < 0 || a.pix[i] >= a.n_pix) ? 1 : 0;
+  if (__syncthreads_or(bad)) { if (tid == 0) *a.status = 2; return; }
   for (int i = tid; i < a.n; i += T) {
     const int s = a.free_list[i];
     a.active[s] = 1; a.forced[s] = 1; a.cpix[s] = a.pix[i]; a.miss[s] = 0; a.born[s] = -1;
     atomicMin(reinterpret_cast<unsigned*>(&a.slotmap[a.pix[i]]), (unsigned)s);
     if (a.slots_out) a.slots_out[i] = s;
   }
-  if (tid == 0) *a.status = 0;
+  if (tid == 0) { *a.status = 0; *a.n_active += a.n; }
 }
 
 // NaN rows for freshly added forced slots (slots_out list)
@@ -513,11 +518,12 @@ int lpf_launch_add_candidates(lpf_ctx* c, const int32_t* d_pix, int n, int32_t* 
   AddArgs a{};
   a.active = c->active; a.forced = c->forced; a.cpix = c->cpix; a.miss = c->miss; a.born = c->born;
   a.slotmap = c->slotmap; a.free_list = c->free_list; a.n_cand_max = p.n_cand_max;
-  a.pix = d_pix; a.n = n; a.slots_out = d_slots_out; a.status = d_status;
+  a.pix = d_pix; a.n = n; a.slots_out = d_slots_out; a.status = d_status; a.n_pix = (int)c->N; a.n_active = c->counters + 2;
   LPF_KLAUNCH(c, KID_MISC, st, k_add_candidates<<<1, 1024, 0, st>>>(a));
   int32_t status = -1;
   LPF_CUDA(cudaMemcpyAsync(&status, d_status, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   LPF_CUDA(cudaStreamSynchronize(st));
+  if (status == 2) return LPF_E_ARG;
   if (status != 0) return LPF_E_STATE;
   if (n > 0) {
     const long long per_slot = (long long)p.T_ring * p.B;

@@ -341,6 +341,71 @@ int lpf_create(lpf_ctx** out, const lpf_params* p, const uint8_t* d_valid_mask) 
   return LPF_OK;
 }
 
+// ---- checkpoint / resume ------------------------------------------------------------------------------------------
+namespace {
+struct StateHeader { char magic[8]; int32_t version, params_bytes; int64_t N, total; lpf_params p; };
+struct StateSection { void* d; size_t bytes; };
+
+// the device arrays that persist from frame to frame, in the order they are stored
+std::vector<StateSection> state_sections(const lpf_ctx* c) {
+  const lpf_params& p = c->p;
+  const size_t nc = (size_t)p.n_cand_max, N = (size_t)c->N;
+  std::vector<StateSection> v = {
+      {c->active, nc}, {c->forced, nc}, {c->cpix, nc * 4}, {c->miss, nc * 4}, {c->born, nc * 8}, {c->matched_t, nc * 8},
+      {c->slotmap, N * 4}, {c->ring, nc * p.T_ring * p.B * 4}, {c->meta_t, (size_t)p.T_ring * 8}, {c->meta_ok, (size_t)p.T_ring * 8},
+      {c->counters, 8 * 4}};
+  if (c->rq_m) {
+    v.push_back({c->rq_m, 2 * (size_t)p.B * N * 4}); v.push_back({c->rq_v, 2 * (size_t)p.B * N * 4});
+    v.push_back({c->rq_state, (4 * (size_t)p.B + 1) * 4});
+  }
+  if (c->cube_cache) {
+    const size_t depth = (size_t)p.n_back + p.n_lanes;
+    v.push_back({c->cube_cache, depth * p.B * N * 4}); v.push_back({c->cache_ok, depth * (p.B + 1)});
+    v.push_back({c->cache_t, depth * 8});
+  }
+  return v;
+}
+}  // namespace
+
+int64_t lpf_state_bytes(const lpf_ctx* c) {
+  if (!c) return LPF_E_ARG;
+  size_t n = sizeof(StateHeader);
+  for (const auto& s : state_sections(c)) n += s.bytes;
+  return (int64_t)n;
+}
+
+int lpf_export_state(lpf_ctx* c, void* h_buf, int64_t bytes) {
+  if (!c || !h_buf || bytes < lpf_state_bytes(c)) return LPF_E_ARG;
+  LPF_CUDA(cudaDeviceSynchronize());
+  StateHeader h{};
+  memcpy(h.magic, "LPFSTATE", 8);
+  h.version = 1; h.params_bytes = (int32_t)sizeof(lpf_params); h.N = c->N; h.total = lpf_state_bytes(c); h.p = c->p;
+  char* o = static_cast<char*>(h_buf);
+  memcpy(o, &h, sizeof(h)); o += sizeof(h);
+  for (const auto& s : state_sections(c)) {
+    LPF_CUDA(cudaMemcpy(o, s.d, s.bytes, cudaMemcpyDeviceToHost));
+    o += s.bytes;
+  }
+  return LPF_OK;
+}
+
+int lpf_import_state(lpf_ctx* c, const void* h_buf, int64_t bytes) {
+  if (!c || !h_buf || bytes < (int64_t)sizeof(StateHeader)) return LPF_E_ARG;
+  StateHeader h;
+  memcpy(&h, h_buf, sizeof(h));
+  if (memcmp(h.magic, "LPFSTATE", 8) != 0 || h.version != 1 || h.params_bytes != (int32_t)sizeof(lpf_params) || h.N != c->N ||
+      h.total != lpf_state_bytes(c) || bytes < h.total || memcmp(&h.p, &c->p, sizeof(lpf_params)) != 0)
+    return LPF_E_ARG;
+  LPF_CUDA(cudaDeviceSynchronize());
+  const char* o = static_cast<const char*>(h_buf) + sizeof(h);
+  for (const auto& s : state_sections(c)) {
+    LPF_CUDA(cudaMemcpy(s.d, o, s.bytes, cudaMemcpyHostToDevice));
+    o += s.bytes;
+  }
+  LPF_CUDA(cudaDeviceSynchronize());
+  return LPF_OK;
+}
+
 int lpf_destroy(lpf_ctx* c) {
   if (!c) return LPF_E_ARG;
   cudaDeviceSynchronize();

@@ -262,6 +262,15 @@ def test_edge_cases(torch_cuda):
     bad = synth.default_params(1); bad["k_bg"] = 40
     with pytest.raises(LpfError):
         LPF(bad, None)
+    # a forced position outside the image refuses the whole call on the device; the table stays as it was
+    lpf = LPF(synth.default_params(1), None)
+    n_pix = 64 * 64
+    for wrong in (np.array([5, n_pix], np.int32), np.array([-1, 7], np.int32)):
+        with pytest.raises(LpfError):
+            lpf.add_candidates(wrong)
+    slots = lpf.add_candidates(np.array([5, 7], np.int32)).cpu().numpy()
+    assert slots.tolist() == [0, 1] and lpf.counters()["n_active"] == 2
+    lpf.close()
 
 
 def test_host_entry_point(torch_cuda):
@@ -515,6 +524,55 @@ def test_backward_fill_with_lanes_in_flight(torch_cuda):
         assert np.array_equal(np.isnan(a), np.isnan(b)), int(sl)
         assert np.array_equal(a[~np.isnan(a)], b[~np.isnan(b)]), int(sl)
     lpf.close()
+
+
+def test_checkpoint_resume(torch_cuda):
+    """lpf_export_state / lpf_import_state: a second context that imports the blob written after
+    frame 13 continues the stream bit for bit - against the context that never stopped AND against the oracle that
+    ran all frames (candidate table, rings incl. the backward fill from the cached cubes, eq. A.2 running state).
+    A blob from a context with other parameters is refused."""
+    torch = torch_cuda
+    from paper_2103_15418_b200.binding import LPF, LpfError
+    kw = dict(T_ring=16, n_back=3, zeta_thr=12.0, zeta_nmax=3, zeta_window=16, zeta_warm=8)
+    s, p, lpf_a = _make(2, torch, **kw)
+    pipe = O.OraclePipeline(p, s.mask, direct=False)
+    n0, n1 = 14, 24
+    outs = []
+    for t in range(n0):
+        outs.append(pipe.step(s.frame(t), t))
+        lpf_a.process_frame(torch.from_numpy(s.frame(t)).cuda(), t)
+    blob = lpf_a.export_state()
+    assert blob.nbytes == lpf_a.lib.lpf_state_bytes(lpf_a.h) and bytes(blob[:8]) == b"LPFSTATE"
+    lpf_b = LPF(p, s.mask)
+    lpf_b.import_state(blob)
+    other = dict(p); other["n_forget"] = p["n_forget"] + 1
+    lpf_c = LPF(other, s.mask)
+    with pytest.raises(LpfError):
+        lpf_c.import_state(blob)
+    with pytest.raises(LpfError):
+        lpf_b.import_state(blob[:-8])
+    lpf_c.close()
+    keys = ("band_ok", "upos", "uplane", "cand_idx", "act_slots", "act_pix", "flux")
+    for t in range(n0, n1):
+        cube = s.frame(t)
+        o = pipe.step(cube, t)
+        d = torch.from_numpy(cube).cuda()
+        lpf_a.process_frame(d, t); lpf_b.process_frame(d, t)
+        ga, gb = lpf_a.frame_view(0), lpf_b.frame_view(0)
+        for k in keys:
+            assert np.array_equal(ga[k], gb[k], equal_nan=True), (t, k)
+        assert np.array_equal(gb["upos"], o["upos"]) and np.array_equal(gb["cand_idx"], o["cand_idx"])
+        assert np.array_equal(gb["act_slots"], o["act_slots"]) and np.array_equal(gb["flux"], o["flux"])
+    tb = pipe.table
+    act = np.flatnonzero(tb.active)
+    assert act.size > 10 and any(n0 <= tb.born[sl] < n0 + 3 for sl in act)      # slots back-filled from imported cubes
+    for sl in act:
+        a = lpf_a.get_dynspec(int(sl), n1 - 1).cpu().numpy(); b = lpf_b.get_dynspec(int(sl), n1 - 1).cpu().numpy()
+        ob = tb.dynspec(int(sl), n1 - 1)
+        assert np.array_equal(a, b, equal_nan=True), int(sl)
+        assert np.array_equal(np.isnan(b), np.isnan(ob)) and np.array_equal(b[~np.isnan(b)], ob[~np.isnan(ob)]), int(sl)
+    assert lpf_a.counters()["n_active"] == lpf_b.counters()["n_active"] == act.size
+    lpf_a.close(); lpf_b.close()
 
 
 def test_running_pixel_qc(torch_cuda):
