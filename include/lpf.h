@@ -47,6 +47,7 @@ extern "C" {
 #define LPF_E_CUDA (-2)  /* a CUDA runtime call failed (see lpf_last_cuda_error) */
 #define LPF_E_STATE (-3) /* call order / lane misuse */
 #define LPF_E_NOMEM (-4)
+#define LPF_E_TOO_LARGE (-5) /* the problem exceeds a fixed maximum of the entry point (lpf_last_cuda_error says which) */
 #define LPF_W_CAPACITY 1  /* positive = warning, the call did its work: a list was truncated (max_det, n_cand_max, the
                            * hit list of the fused path, or a caller buffer); the dropped entries are counted */
 
@@ -154,6 +155,19 @@ int lpf_destroy(lpf_ctx* ctx);
  * in increasing t (the calls of different lanes are ordered by an event). */
 int lpf_cube_qc(lpf_ctx* ctx, int lane, const float* d_cube, int64_t t, float* d_stats,
                 uint8_t* d_band_ok, void* stream);
+
+/* The same statistics and eq. A.1 verdict (d_stats, d_band_ok as above; no eq. A.2 step, no lane) for callers that
+ * cannot reach cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it): the call
+ * and everything behind it allocate nothing.  Its scratch (per-block partial sums, clip parameters, two block
+ * counters) is a static device array of LPF_QC_STATIC_BYTES that every GPU which loads the library holds until the
+ * process exits.  Limit: B x (blocks of the two passes) x 24 bytes + 2 KB must fit (every BASELINE.json
+ * configuration does: 1024 x 1024 x 64 needs 0.87 MB); beyond it the call returns LPF_E_TOO_LARGE, launches nothing,
+ * and lpf_last_cuda_error names the sizes.  All calls on a device share the array: calls that overlap on the GPU
+ * (two streams) race; calls on one stream, or ordered by events, do not.  The first call on a device asks the
+ * runtime for the array's device address (cudaGetSymbolAddress): make that call outside a stream capture.
+ * Kernels: the generic k_qc_pass1 / k_qc_pass2 (any alignment of d_cube). */
+#define LPF_QC_STATIC_BYTES (1 << 20)
+int lpf_cube_qc_static(lpf_ctx* ctx, const float* d_cube, float* d_stats, uint8_t* d_band_ok, void* stream);
 
 /* -- S3-S9: detection (eqs. 2-7; O3-O7) -------------------------------------
  * For every accepted plane: F = g_mf (*)_W X; n_iter rounds of C = G (*)_W' F,

@@ -57,7 +57,7 @@ EXPORTS = [
     "lpf_create", "lpf_destroy", "lpf_cube_qc", "lpf_detect_sources", "lpf_associate", "lpf_add_candidates",
     "lpf_measure_flux", "lpf_append_dynspec", "lpf_get_dynspec", "lpf_process_frame", "lpf_get_frame_view",
     "lpf_process_frame_host", "lpf_process_frame_host_begin", "lpf_process_frame_host_end", "lpf_get_counters", "lpf_memcpy_d2h", "lpf_strerror", "lpf_last_cuda_error",
-    "lpf_export_dynspec", "lpf_simulate_pulses", "lpf_state_bytes", "lpf_export_state", "lpf_import_state",
+    "lpf_export_dynspec", "lpf_simulate_pulses", "lpf_state_bytes", "lpf_export_state", "lpf_import_state", "lpf_cube_qc_static",
     "lpf_version", "lpf_get_plan", "lpf_profile_begin", "lpf_profile_end", "lpf_profile_timeline", "lpf_profile_kernel_count", "lpf_profile_kernel_name",
 ]
 
@@ -95,6 +95,7 @@ def load_library(path: Optional[str] = None):
     lib.lpf_process_frame_host_end.argtypes = [vp, C.c_int, C.POINTER(LpfHostResult), vp]
     lib.lpf_get_counters.argtypes = [vp, C.POINTER(i64)]
     lib.lpf_memcpy_d2h.argtypes = [vp, vp, i64]
+    lib.lpf_cube_qc_static.argtypes = [vp, vp, vp, vp, vp]
     lib.lpf_state_bytes.argtypes = [vp]
     lib.lpf_export_state.argtypes = [vp, vp, i64]
     lib.lpf_import_state.argtypes = [vp, vp, i64]
@@ -116,6 +117,7 @@ def load_library(path: Optional[str] = None):
     return lib
 
 
+E_TOO_LARGE = -5   # the problem exceeds a fixed maximum of the entry point (include/lpf.h)
 W_CAPACITY = 1   # positive status = warning: a list was truncated, the call did its work (include/lpf.h)
 
 
@@ -186,6 +188,17 @@ class LPF:
         stats = self._empty((self.B, STATS_PER_BAND), tc.float32)
         ok = self._empty((self.B + 1,), tc.uint8)
         _check(self.lib, self.lib.lpf_cube_qc(self.h, lane, _ptr(cube), t, _ptr(stats), _ptr(ok), _stream(stream)), "lpf_cube_qc")
+        return stats, ok
+
+    def cube_qc_static(self, cube, stats=None, ok=None, stream=None):
+        """lpf_cube_qc_static: the statistics and eq. A.1 verdict with their scratch in the library's static device
+        array; the call allocates nothing when the caller passes `stats` [B][8] float32 and `ok` [B + 1] uint8."""
+        tc = self.torch
+        if stats is None:
+            stats = self._empty((self.B, STATS_PER_BAND), tc.float32)
+        if ok is None:
+            ok = self._empty((self.B + 1,), tc.uint8)
+        _check(self.lib, self.lib.lpf_cube_qc_static(self.h, _ptr(cube), _ptr(stats), _ptr(ok), _stream(stream)), "lpf_cube_qc_static")
         return stats, ok
 
     def detect_sources(self, cube, band_ok, lane: int = 0, stream=None):

@@ -685,6 +685,7 @@ const char* lpf_strerror(int code) {
     case LPF_E_CUDA: return "CUDA runtime error";
     case LPF_E_STATE: return "bad state (call order, capacity)";
     case LPF_E_NOMEM: return "out of device memory";
+    case LPF_E_TOO_LARGE: return "the problem exceeds a fixed maximum of this entry point";
     case LPF_W_CAPACITY: return "warning: a list was truncated (capacity); the dropped entries are counted";
     default: return "unknown";
   }

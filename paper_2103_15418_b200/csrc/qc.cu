@@ -16,6 +16,8 @@
 //   k_qc_clip_finish  one block: the clipped mean / rms.
 // The generic form (any alignment) keeps the two older kernels, whose last block does the finishing:
 // k_qc_pass1 (per-band moments + verdict) and k_qc_pass2 (clip round, sum plane, exact-zero check).
+#include <cstdio>
+
 #include "lpf_internal.cuh"
 
 namespace {
@@ -963,5 +965,71 @@ int lpf_launch_sum_plane(lpf_ctx* c, LpfLane& L, const float* d_cube, const uint
   L.dirty_seq = L.dirty_seq >= 0x7ffffff0 ? 1 : L.dirty_seq + 1;
   const Qc2Args a = make_qc2(c, L, d_cube, d_band_ok, nullptr, want_sum, nullptr);
   LPF_KLAUNCH(c, KID_SUM_PLANE, st, k_qc_pass2<false, true><<<lpf_qc2_blocks(c), QC2_THREADS, 0, st>>>(a));
+  return LPF_OK;
+}
+
+// ---- lpf_cube_qc_static: S1 + S2 with no allocation behind it -------------------------------------------------------
+// For callers that must not (or cannot) reach cudaMalloc: the per-block partial sums, the clip parameters, the noise
+// levels and the two block counters of the generic QC kernels live in ONE file-scope device array instead of a
+// lane's buffers.  Every GPU that loads the library holds LPF_QC_STATIC_BYTES of it until the process exits; every
+// call on a device shares it (calls that overlap on the GPU race) and finds the last call's contents in it (the
+// counters, which must start at zero, are cleared on the stream first; everything else is written before it is read).
+// In host code the array's name is a host-side stand-in, not a device address: the kernels get the address that
+// cudaGetSymbolAddress returns for the current device, asked for once per device.
+static __device__ __align__(256) unsigned char g_qc_static[LPF_QC_STATIC_BYTES];
+
+namespace {
+constexpr size_t QST_COUNTERS = 0;                                       // 2 x int32
+constexpr size_t QST_BAND_CLIP = 256;                                    // [LPF_MAX_BANDS][2] float
+constexpr size_t QST_BIG_THR = 1024;                                     // [LPF_MAX_BANDS + 1] float
+constexpr size_t QST_PART = 2048;                                        // part1 [B][nblk1][3], then part2 [nblk2][B][3], double
+constexpr int QST_MAX_DEV = 64;
+static_assert(QST_BAND_CLIP + LPF_MAX_BANDS * 2 * sizeof(float) <= QST_BIG_THR, "static QC scratch layout");
+static_assert(QST_BIG_THR + (LPF_MAX_BANDS + 1) * sizeof(float) <= QST_PART, "static QC scratch layout");
+
+// device address of g_qc_static on the current device (set-up: the first call on that device)
+int qc_static_base(unsigned char** out) {
+  static unsigned char* base[QST_MAX_DEV] = {};
+  int dev = -1;
+  LPF_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= QST_MAX_DEV) return LPF_E_ARG;
+  if (!base[dev]) {
+    unsigned char* p = nullptr;
+    LPF_CUDA(cudaGetSymbolAddress((void**)&p, g_qc_static));
+    base[dev] = p;
+  }
+  *out = base[dev];
+  return LPF_OK;
+}
+}  // namespace
+
+extern "C" int lpf_cube_qc_static(lpf_ctx* c, const float* d_cube, float* d_stats, uint8_t* d_band_ok, void* stream) {
+  if (!c || !d_cube || !d_stats || !d_band_ok) return LPF_E_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int B = c->p.B, nblk1 = c->qc_nblk, nblk2 = lpf_qc2_blocks(c);
+  const size_t b1 = (size_t)B * nblk1 * 3 * sizeof(double), b2 = (size_t)nblk2 * B * 3 * sizeof(double);
+  const size_t o1 = QST_PART, o2 = (o1 + b1 + 255) & ~(size_t)255, need = o2 + b2;
+  if (need > (size_t)LPF_QC_STATIC_BYTES) {
+    snprintf(g_lpf_cuda_err, sizeof(g_lpf_cuda_err),
+             "lpf_cube_qc_static: B = %d bands x (%d + %d) blocks need %zu bytes of scratch, the static array holds %d "
+             "(LPF_QC_STATIC_BYTES); use lpf_cube_qc", B, nblk1, nblk2, need, (int)LPF_QC_STATIC_BYTES);
+    return LPF_E_TOO_LARGE;
+  }
+  unsigned char* base = nullptr;
+  int rc = qc_static_base(&base);
+  if (rc) return rc;
+  int32_t* counters = reinterpret_cast<int32_t*>(base + QST_COUNTERS);
+  LPF_CUDA(cudaMemsetAsync(counters, 0, 2 * sizeof(int32_t), st));     // a call that was cut short may have left them set
+  QcArgs a{};
+  a.cube = d_cube; a.W = c->W; a.N = c->N; a.first_valid = c->first_valid; a.B = B; a.nblk = nblk1;
+  a.part1 = reinterpret_cast<double*>(base + o1); a.qc_clip = c->p.qc_clip; a.tau = c->p.qc_tau; a.stats = d_stats; a.band_ok = d_band_ok;
+  a.band_clip = reinterpret_cast<float*>(base + QST_BAND_CLIP); a.counter = counters;
+  a.big_thr = reinterpret_cast<float*>(base + QST_BIG_THR); a.big_sigma = lpf_fused_big_sigma();
+  LPF_KLAUNCH(c, KID_QC_PASS1, st, k_qc_pass1<<<dim3(nblk1, B), QC_THREADS, 0, st>>>(a));
+  Qc2Args k{};
+  k.cube = d_cube; k.W = c->W; k.band_ok = d_band_ok; k.N = c->N; k.B = B;
+  k.band_clip = a.band_clip; k.part2 = reinterpret_cast<double*>(base + o2); k.stats = d_stats;
+  k.sum_out = nullptr; k.dirty = nullptr; k.seq = 0; k.zero_me = nullptr; k.counter = counters + 1;
+  LPF_KLAUNCH(c, KID_QC_PASS2, st, k_qc_pass2<true, false><<<nblk2, QC2_THREADS, 0, st>>>(k));
   return LPF_OK;
 }
