@@ -69,7 +69,7 @@ def file_sha256(path):
         return None
 
 
-def traffic_from_profile(kernel: str):
+def traffic_from_profile(kernel: str, workload: str = None, bg: str = None):
     """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel`, from the committed `ncu --set full`
     capture listed in profiles/traffic.json (never measured under the profiler in this run).  The entry names the CSV
     and the SHA-256 of the kernel source at capture time; a source that has changed since is reported, not hidden."""
@@ -78,6 +78,9 @@ def traffic_from_profile(kernel: str):
         e = json.load(open(meta))[kernel]
     except Exception:
         return None, {"source": None, "note": "no committed ncu capture for this kernel (profiles/traffic.json)"}
+    if e.get("workload") and (workload != e["workload"] or (e.get("bg_kernel") and bg != e["bg_kernel"])):
+        return None, {"source": e["csv"], "note": "the committed capture is of workload %s (%s): no per-launch figure for this one"
+                      % (e["workload"], e.get("bg_kernel", "any kernel"))}
     src_now = file_sha256(os.path.join(ROOT, e["kernel_source"]))
     return float(e["dram_bytes_per_launch"]), {"source": e["csv"], "kernel_source": e["kernel_source"],
                                                "kernel_source_sha256_at_capture": e["kernel_source_sha256"],
@@ -277,7 +280,7 @@ def run_ours(args):
     roof.update({"kernel": dom, "us_per_launch": kernels[dom]["us_per_launch"], "share_of_step": kernels[dom]["us_per_step"] / step_kernel_us,
                  "algorithmic_bytes": abytes, "algorithmic_flops": aflops, "hbm_gbs": gbs, "hbm_frac": gbs / hbm_peak,
                  "peak_source": peak_src, "alu_peak_source": "nominal (derived, not measured): 148 SM x 128 fp32 lanes x 2 x 1.965 GHz"})
-    roof["traffic"], roof["traffic_source"] = traffic_from_profile(dom)
+    roof["traffic"], roof["traffic_source"] = traffic_from_profile(dom, s.c.name, args.bg)
 
     frames_s = whole_job_value(world, args.steps, ms)
     step_gbs = cube_bytes * frames_s / 1e9 / world
