@@ -20,6 +20,19 @@ def _free_port():
     return p
 
 
+def _torchrun(args, timeout, attempts=3):
+    """torchrun on a fresh port; the port found free can be taken again before the rendezvous binds it, so a failed
+    rendezvous (not a failed worker) is tried again on another port."""
+    r = None
+    for _ in range(attempts):
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+               "--master-addr", "127.0.0.1", "--master-port", str(_free_port())] + args
+        r = subprocess.run(cmd, capture_output=True, text=True, timeout=timeout, env=dict(os.environ, OMP_NUM_THREADS="1"), cwd=ROOT)
+        if r.returncode == 0 or not any(k in r.stderr for k in ("address already in use", "EADDRINUSE", "Connection refused", "RendezvousConnectionError", "failed to bind", "DistNetworkError")):
+            break
+    return r
+
+
 _WORKER = r"""
 import os, sys, json
 sys.path.insert(0, {root!r})
@@ -35,21 +48,18 @@ cube = s.frame(0)
 out = dict(rank=rank, ms=ms, launches=launches, value=bench.whole_job_value(world, 100, ms),
            checksum=float(cube.astype("float64").sum()))
 dist.barrier()
-print("RESULT " + json.dumps(out), flush=True)
+# one file per rank: two ranks printing to the same pipe can interleave inside a line
+open(os.path.join({out!r}, "rank%d.json" % rank), "w").write(json.dumps(out))
 dist.destroy_process_group()
 """
 
 
 def test_two_ranks_gloo_aggregation(tmp_path):
     script = tmp_path / "worker.py"
-    script.write_text(_WORKER.format(root=ROOT))
-    port = _free_port()
-    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
-           "--master-addr", "127.0.0.1", "--master-port", str(port), str(script)]
-    env = dict(os.environ, OMP_NUM_THREADS="1")
-    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+    script.write_text(_WORKER.format(root=ROOT, out=str(tmp_path)))
+    r = _torchrun([str(script)], timeout=300)
     assert r.returncode == 0, r.stderr[-2000:]
-    res = [json.loads(l.split("RESULT ", 1)[1]) for l in r.stdout.splitlines() if "RESULT " in l]
+    res = [json.loads((tmp_path / f"rank{k}.json").read_text()) for k in range(2)]
     assert sorted(x["rank"] for x in res) == [0, 1]
     for x in res:
         assert x["ms"] == 15.0            # max over ranks
@@ -61,11 +71,8 @@ def test_two_ranks_gloo_aggregation(tmp_path):
 
 def test_reference_arm_runs_on_rank0_only(tmp_path):
     """`bench.py --impl reference` under torchrun: rank 0 alone runs the oracle and prints ONE JSON line."""
-    port = _free_port()
-    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
-           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.join(ROOT, "bench.py"),
-           "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "3", "--config", "1"]
-    r = subprocess.run(cmd, capture_output=True, text=True, timeout=600, env=dict(os.environ, OMP_NUM_THREADS="1"), cwd=ROOT)
+    r = _torchrun([os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "3", "--config", "1"],
+                  timeout=600)
     assert r.returncode == 0, r.stderr[-2000:]
     lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
     assert len(lines) == 1
