@@ -422,7 +422,6 @@ __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
 __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 // keep a value in its register (the compiler would otherwise rebuild it from its inputs at every use)
-__device__ __forceinline__ void pin(float& v) { asm volatile("" : "+f"(v)); }
 __device__ __forceinline__ void pin(unsigned& v) { asm volatile("" : "+r"(v)); }
 __device__ __forceinline__ void pin(const char*& v) { asm volatile("" : "+l"(v)); }
 constexpr size_t QS_SMEM = (size_t)QS_BG * QS_THREADS * sizeof(float4);   // 64 KB
@@ -599,7 +598,7 @@ __device__ __forceinline__ void qs_clip_group(const QkArgs& a, int g0, long long
   const long long sb = n4 * (long long)sizeof(float4);
   const uint32_t slot0 = (uint32_t)__cvta_generic_to_shared(qs_slots + threadIdx.x);
   constexpr uint32_t SLOT = QS_THREADS * sizeof(float4);
-  float fn[QS_BG], f1[QS_BG], f2[QS_BG];
+  float fn[QS_BG], f1[QS_BG], f2[QS_BG];     // fn: a count (a thread sees a few dozen pixels: exact in fp32)
 #pragma unroll
   for (int b = 0; b < QS_BG; ++b) { fn[b] = 0.f; f1[b] = 0.f; f2[b] = 0.f; }
   long long q = q0 + threadIdx.x;
@@ -618,11 +617,8 @@ __device__ __forceinline__ void qs_clip_group(const QkArgs& a, int g0, long long
     const long long qn = q + QS_THREADS;
     const bool hasn = qn < q1;
     const unsigned wmn = hasn ? __ldg(reinterpret_cast<const unsigned*>(a.W) + qn) : 0u;
-    // an invalid pixel never passes |d| <= w: its half width is -1
-    const float m0 = (wm & 0x000000ffu) ? 0.f : -INFINITY, m1 = (wm & 0x0000ff00u) ? 0.f : -INFINITY,
-                m2 = (wm & 0x00ff0000u) ? 0.f : -INFINITY, m3 = (wm & 0xff000000u) ? 0.f : -INFINITY;
-    float mm0 = m0, mm1 = m1, mm2 = m2, mm3 = m3;
-    pin(mm0); pin(mm1); pin(mm2); pin(mm3);
+    // an invalid pixel never passes: its validity is the second operand of the comparison's predicate
+    const bool vk[4] = {(wm & 0x000000ffu) != 0u, (wm & 0x0000ff00u) != 0u, (wm & 0x00ff0000u) != 0u, (wm & 0xff000000u) != 0u};
     float4 sp = make_float4(0.f, 0.f, 0.f, 0.f);
     if (RESUM && g0 > 0) sp = reinterpret_cast<const float4*>(a.sum_out)[q];
     const char* pb = reinterpret_cast<const char*>(a.cube) + ((long long)g0 * n4 + qn) * (long long)sizeof(float4);
@@ -634,13 +630,10 @@ __device__ __forceinline__ void qs_clip_group(const QkArgs& a, int g0, long long
       const float4 x = live ? qs_slots[b * QS_THREADS + threadIdx.x] : make_float4(0.f, 0.f, 0.f, 0.f);
       const float c = s_c[bb], w = live ? s_w[bb] : -1.f;
       const float xv[4] = {x.x, x.y, x.z, x.w};
-      const float mv[4] = {mm0, mm1, mm2, mm3};
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         const float d = xv[j] - c;
-        const bool take = fabsf(d) <= w + mv[j];
-        const float dm = take ? d : 0.f;
-        fn[b] += take ? 1.f : 0.f; f1[b] += dm; f2[b] = fmaf(dm, dm, f2[b]);
+        if (fabsf(d) <= w && vk[j]) { fn[b] += 1.f; f1[b] += d; f2[b] = fmaf(d, d, f2[b]); }   // three predicated instructions
       }
       if (RESUM && live && s_ok[bb]) { sp.x += x.x; sp.y += x.y; sp.z += x.z; sp.w += x.w; }
       if (hasn && live) cp_async16(slot0 + b * SLOT, pb);
