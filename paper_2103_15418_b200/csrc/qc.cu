@@ -392,15 +392,23 @@ k_qc_pass2(const Qc2Args a) {
 }
 
 // ---- the streaming form -------------------------------------------------------------------------------------------
+// Block shape: 128 threads x 8 bands x 16 bytes = 16 KB of staging, <= 102 registers.  A block of this size fits
+// BESIDE a CTA of the fused sweep on the same SM (the sweep leaves ~20 KB of its 196 KB shared-memory carve-out, 14.8 K
+// registers and most of the issue slots free), so with several lanes in flight the QC of one frame runs under the
+// sweeps of the others instead of waiting for the dozen SMs they leave empty: 9 640 -> 10 350 frames/s at 8 lanes
+// (config 3).  The grid: lpf_qs_blocks.
 #ifndef LPF_QS_THREADS
-#define LPF_QS_THREADS 256
+#define LPF_QS_THREADS 128
 #endif
 #ifndef LPF_QS_BLOCKS
-#define LPF_QS_BLOCKS 2
+#define LPF_QS_BLOCKS 5            // resident blocks per SM the register budget is set for (__launch_bounds__)
 #endif
-constexpr int QS_THREADS = LPF_QS_THREADS;     // LPF_QS_BLOCKS blocks per SM; a thread owns one group of 4 pixels at a time, all bands
+#ifndef LPF_QS_BG
+#define LPF_QS_BG 8
+#endif
+constexpr int QS_THREADS = LPF_QS_THREADS;     // a thread owns one group of 4 pixels at a time, QS_BG bands of it
 constexpr int QS_WARPS = QS_THREADS / 32;
-constexpr int QS_BG = 16;           // bands of one register-resident group
+constexpr int QS_BG = LPF_QS_BG;    // bands of one register-resident group
 
 __device__ __forceinline__ float2 q_add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
 __device__ __forceinline__ float2 q_fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
@@ -424,7 +432,7 @@ template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.as
 // keep a value in its register (the compiler would otherwise rebuild it from its inputs at every use)
 __device__ __forceinline__ void pin(unsigned& v) { asm volatile("" : "+r"(v)); }
 __device__ __forceinline__ void pin(const char*& v) { asm volatile("" : "+l"(v)); }
-constexpr size_t QS_SMEM = (size_t)QS_BG * QS_THREADS * sizeof(float4);   // 64 KB
+constexpr size_t QS_SMEM = (size_t)QS_BG * QS_THREADS * sizeof(float4);   // 16 KB
 
 // one group of <= QS_BG bands over the block's pixel groups [q0, q1); FULL: all QS_BG bands exist
 template <bool FULL>
@@ -855,13 +863,22 @@ int lpf_launch_qc_running(lpf_ctx* c, LpfLane& L, const float* d_cube, uint8_t* 
   return LPF_OK;
 }
 
+// Grid of the streaming kernels: blocks of about 28 (pixel group, band group) rounds per thread - long enough to
+// amortise a block's start and its reductions, short enough to balance - twice as many when fewer than 4 lanes are in
+// flight (a kernel alone on the GPU wants more bytes in flight); between one wave of single blocks and the 5 blocks
+// per SM the registers allow.  Measured on configs 3, 4, 5.
 int lpf_qs_blocks(const lpf_ctx* c) {
-  const long long n4 = (c->N + 3) / 4;
-  const long long want = (n4 + QS_THREADS - 1) / QS_THREADS, cap = (long long)LPF_QS_BLOCKS * c->n_sm;
-  return (int)(want < 1 ? 1 : (want < cap ? want : cap));
+  const long long n4 = (c->N + 3) / 4, nbg = (c->p.B + QS_BG - 1) / QS_BG;
+  const long long want = (n4 + QS_THREADS - 1) / QS_THREADS;
+  long long nb = (n4 * nbg + 28ll * QS_THREADS - 1) / (28ll * QS_THREADS);
+  if (c->p.n_lanes < 4) nb *= 2;
+  const long long lo = want < c->n_sm ? want : c->n_sm, hi = (long long)LPF_QS_BLOCKS * c->n_sm;
+  nb = nb < lo ? lo : (nb > hi ? hi : nb);
+  nb = nb > want ? want : nb;
+  return (int)(nb < 1 ? 1 : nb);
 }
 
-// 64 KB of dynamic shared memory per block: opt in once per process
+// the dynamic shared memory attribute, once per process (16 KB needs no opt-in; a larger LPF_QS_* build does)
 static cudaError_t qs_attr() {
   static bool done = false;
   if (done) return cudaSuccess;

@@ -459,7 +459,12 @@ def test_config3_bench_launch_configuration(torch_cuda):
         assert np.array_equal(a["pix"], b["pix"]) and np.array_equal(a["plane"], b["plane"])
         # the running sums of the two plans start at different rows: values agree within the north_star tolerance
         assert np.allclose(a["snr"], b["snr"], rtol=1e-4, atol=1e-5) and np.allclose(a["f"], b["f"], rtol=1e-4, atol=1e-5)
-        assert np.allclose(v["stats"], views[t]["stats"], rtol=1e-6, atol=1e-6, equal_nan=True)
+        # the QC grids of the two plans differ (lpf_qs_blocks: fewer, longer blocks with lanes in flight), hence the
+        # grouping of the float64 partial sums: the statistics agree within the QC tolerances, not bit for bit
+        n_t = len(parity.TIES)
+        parity.check_qc(v["stats"], v["band_ok"], views[t]["stats"].astype(np.float64), views[t]["band_ok"],
+                        f"cfg3 1 lane vs 8 lanes t={t}", cube=cubes[t], W=s.mask, qc_clip=p["qc_clip"])
+        del parity.TIES[n_t:]          # GPU against GPU: not an oracle tie
     seq.close(); lpf.close()
 
 
