@@ -426,30 +426,46 @@ k_threshold_peaks4(const ThrArgs a) {
   const float* F = a.F + (long long)p * N;
   const int lane = threadIdx.x & 31;
   unsigned hits = 0u, peaks = 0u;
-  float f[4] = {0.f, 0.f, 0.f, 0.f}, cc[4] = {0.f, 0.f, 0.f, 0.f}, se[4] = {0.f, 0.f, 0.f, 0.f}, d[4] = {0.f, 0.f, 0.f, 0.f};
+  // eq. 5 for the thread's four pixels without a branch: nothing but the three loaded vectors stays live; the few
+  // threads with a hit work their record values out again below
+  float4 f4 = make_float4(0.f, 0.f, 0.f, 0.f), c4 = f4, s4 = f4;
   if (pix0 < N) {
     unsigned w = *reinterpret_cast<const unsigned*>(a.W + pix0);
     unsigned yy = 0u;
     if (a.Y) { yy = *reinterpret_cast<const unsigned*>(a.Y + (long long)p * N + pix0); w = wide_mask(w, yy); }
     if (w) {
-      const float4 f4 = *reinterpret_cast<const float4*>(F + pix0);
-      const float4 c4 = *reinterpret_cast<const float4*>(a.C + (long long)p * N + pix0);
-      const float4 s4 = *reinterpret_cast<const float4*>(a.S + (long long)p * N + pix0);
+      f4 = *reinterpret_cast<const float4*>(F + pix0);
+      c4 = *reinterpret_cast<const float4*>(a.C + (long long)p * N + pix0);
+      s4 = *reinterpret_cast<const float4*>(a.S + (long long)p * N + pix0);
       const float fv[4] = {f4.x, f4.y, f4.z, f4.w}, cv[4] = {c4.x, c4.y, c4.z, c4.w}, sv[4] = {s4.x, s4.y, s4.z, s4.w};
-      unsigned ynew = yy;
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
-        if (!((w >> (8 * k)) & 0xffu)) continue;
-        f[k] = fv[k]; cc[k] = cv[k];
-        d[k] = f[k] - cc[k];
-        const float gd = a.eps_rel * fabsf(cc[k]);
-        se[k] = fmaxf(sv[k], gd * gd);
-        if (d[k] > 0.f && d[k] * d[k] > a.kappa2 * se[k]) { ynew |= (unsigned)(a.iter & 0xff) << (8 * k); hits |= 1u << k; }
+        const float dk = fv[k] - cv[k];
+        const float gd = a.eps_rel * fabsf(cv[k]);
+        const float sek = fmaxf(sv[k], gd * gd);
+        const bool h = ((w >> (8 * k)) & 0xffu) != 0u && dk > 0.f && dk * dk > a.kappa2 * sek;
+        hits |= h ? (1u << k) : 0u;
       }
-      if (a.Y && ynew != yy) *reinterpret_cast<unsigned*>(a.Y + (long long)p * N + pix0) = ynew;
+      if (a.Y && hits) {
+        unsigned ynew = yy;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) if ((hits >> k) & 1u) ynew |= (unsigned)(a.iter & 0xff) << (8 * k);
+        *reinterpret_cast<unsigned*>(a.Y + (long long)p * N + pix0) = ynew;
+      }
     }
   }
   if (!__any_sync(0xffffffffu, hits != 0u)) return;
+  float f[4], cc[4], se[4], d[4];
+  {
+    const float fv[4] = {f4.x, f4.y, f4.z, f4.w}, cv[4] = {c4.x, c4.y, c4.z, c4.w}, sv[4] = {s4.x, s4.y, s4.z, s4.w};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      f[k] = fv[k]; cc[k] = cv[k];
+      d[k] = f[k] - cc[k];
+      const float gd = a.eps_rel * fabsf(cc[k]);
+      se[k] = fmaxf(sv[k], gd * gd);
+    }
+  }
   const int side = 2 * a.k_max + 1, nwin = side * side;
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
