@@ -155,7 +155,7 @@ k_sepconv(const ConvArgs a) {
 // column pass pairs two neighbouring columns.  Both passes are packed FFMA2 with the taps applied in the same order
 // as in k_sepconv, so the two forms give the same bits.  RL: the halo staged (a multiple of 4 >= R: groups stay
 // aligned).
-constexpr int WTX = 128, WTY = 64, WPIN = 162, WPT = 132, WU = 4;
+constexpr int WTX = 128, WTY = 64, WPIN = 162, WPT = 132;
 
 template <int MODE>
 __device__ __forceinline__ float4 wide_value(float4 v, float4 cv, unsigned w) {
@@ -197,7 +197,11 @@ k_sepconv_wide(const ConvArgs a) {
   const uint8_t* Y_p = (a.Y && MODE != MODE_MF) ? a.Y + (long long)p * N : nullptr;
   const int x0 = blockIdx.x * WTX, y0 = blockIdx.y * WTY;
 
-  // staging: items (row pair, group), WU items per round
+  // staging: items (row pair, group), WU items per round (the spread also holds C: half as many)
+#ifndef LPF_WU_BIG
+#define LPF_WU_BIG 8
+#endif
+  constexpr int WU = (MODE == MODE_S) ? 4 : LPF_WU_BIG;
   for (int i0 = threadIdx.x; i0 < HALF * NG; i0 += WU * CT) {
     unsigned w[WU][2];
     float4 v[WU][2], cv[WU][2];
