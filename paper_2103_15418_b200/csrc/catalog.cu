@@ -214,8 +214,13 @@ __device__ __forceinline__ void assoc_update_body(const AssocArgs& a) {
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, nw = T >> 5;
   const unsigned lt = (1u << lane) - 1u;
   const bool frame_ok = a.band_ok[a.B] != 0;
-  const int spw = ((a.n_cand_max + nw - 1) / nw + 31) & ~31;          // slots per warp, a multiple of 32
-  const int w0 = min(w * spw, a.n_cand_max), w1 = min(w0 + spw, a.n_cand_max);
+  // Slots are handed out lowest first, so the table is dense at the bottom: counters[4] is one more than the highest
+  // slot ever used, everything from there on is free, and the passes below walk only the slots before it (rounded
+  // up to 32) - on the one serial chain of the path this is what the step costs.
+  const int hwm0 = __ldcg(&a.counters[4]);
+  const int n_scan = min(a.n_cand_max, (hwm0 + 31) & ~31);
+  int spw = ((n_scan + nw - 1) / nw + 31) & ~31;          // slots per warp, a multiple of 32
+  int w0 = min(w * spw, n_scan), w1 = min(w0 + spw, n_scan);
   if (frame_ok) {
     // 1. age and retire
     int any_retired = 0;
@@ -241,8 +246,9 @@ __device__ __forceinline__ void assoc_update_body(const AssocArgs& a) {
       const int s = s0 + lane;
       nfree_w += __popc(__ballot_sync(0xffffffffu, s < w1 && !a.active[s]));
     }
-    int n_free;
-    int off = warp_totals_excl(nfree_w, s_warp, n_free);
+    int n_free_low;
+    int off = warp_totals_excl(nfree_w, s_warp, n_free_low);
+    const int n_free = n_free_low + (a.n_cand_max - n_scan);      // every slot from n_scan on is free
     for (int s0 = w0; s0 < w1; s0 += 32) {
       const int s = s0 + lane;
       const bool fr = s < w1 && !a.active[s];
@@ -263,8 +269,9 @@ __device__ __forceinline__ void assoc_update_body(const AssocArgs& a) {
       if (a.cand_idx[i] >= 0) continue;
       const int k = uo++;
       if (k < n_free) {
-        const int s = a.free_list[k];
+        const int s = k < n_free_low ? a.free_list[k] : n_scan + (k - n_free_low);
         const int pix = a.upos[i];
+        if (s >= hwm0) atomicMax(&a.counters[4], s + 1);
         a.active[s] = 1; a.forced[s] = 0; a.cpix[s] = pix; a.miss[s] = 0; a.born[s] = a.t;
         atomicMin(reinterpret_cast<unsigned*>(&a.slotmap[pix]), (unsigned)s);
         a.cand_idx[i] = s;
@@ -274,7 +281,12 @@ __device__ __forceinline__ void assoc_update_body(const AssocArgs& a) {
     }
     __syncthreads();
   }
-  // 5. active list, ascending slot
+  // 5. active list, ascending slot (the slots handed out above may lie beyond n_scan: walk up to the new mark)
+  {
+    const int n_scan1 = min(a.n_cand_max, (__ldcg(&a.counters[4]) + 31) & ~31);      // (after phase 4's block barrier; past L1)
+    spw = ((n_scan1 + nw - 1) / nw + 31) & ~31;
+    w0 = min(w * spw, n_scan1); w1 = min(w0 + spw, n_scan1);
+  }
   int nact_w = 0;
   for (int s0 = w0; s0 < w1; s0 += 32) {
     const int s = s0 + lane;
@@ -307,6 +319,7 @@ struct AddArgs {
   int32_t* free_list; int n_cand_max; const int32_t* pix; int n; int32_t* slots_out; int32_t* status;
   int n_pix;        // pixels of the image: a position outside [0, n_pix) refuses the whole call (status 2)
   int32_t* n_active; // the context's count of active candidates
+  int32_t* hwm;      // one more than the highest slot ever used (k_assoc walks only the slots before it)
 };
 
 __global__ void __launch_bounds__(1024)
@@ -329,6 +342,7 @@ k_add_candidates(const AddArgs a) {
     const int s = a.free_list[i];
     a.active[s] = 1; a.forced[s] = 1; a.cpix[s] = a.pix[i]; a.miss[s] = 0; a.born[s] = -1;
     atomicMin(reinterpret_cast<unsigned*>(&a.slotmap[a.pix[i]]), (unsigned)s);
+    atomicMax(a.hwm, s + 1);
     if (a.slots_out) a.slots_out[i] = s;
   }
   if (tid == 0) { *a.status = 0; *a.n_active += a.n; }
@@ -518,7 +532,7 @@ int lpf_launch_add_candidates(lpf_ctx* c, const int32_t* d_pix, int n, int32_t* 
   AddArgs a{};
   a.active = c->active; a.forced = c->forced; a.cpix = c->cpix; a.miss = c->miss; a.born = c->born;
   a.slotmap = c->slotmap; a.free_list = c->free_list; a.n_cand_max = p.n_cand_max;
-  a.pix = d_pix; a.n = n; a.slots_out = d_slots_out; a.status = d_status; a.n_pix = (int)c->N; a.n_active = c->counters + 2;
+  a.pix = d_pix; a.n = n; a.slots_out = d_slots_out; a.status = d_status; a.n_pix = (int)c->N; a.n_active = c->counters + 2; a.hwm = c->counters + 4;
   LPF_KLAUNCH(c, KID_MISC, st, k_add_candidates<<<1, 1024, 0, st>>>(a));
   int32_t status = -1;
   LPF_CUDA(cudaMemcpyAsync(&status, d_status, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
